@@ -1,0 +1,201 @@
+"""ctypes wrapper around oracle/oracle.c -- the fp64 CPU oracle (TEST INFRASTRUCTURE).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
+may import this package.  It never imports the CUDA package and shares no code with it.
+All arrays are float64, C-contiguous, shape (nz, ny, nx).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("hx", C.c_double), ("hy", C.c_double), ("hz", C.c_double)]
+
+    @property
+    def shape(self):
+        return (self.nz, self.ny, self.nx)
+
+
+def grid(nx, ny, nz, hx, hy=None, hz=None):
+    return Grid(nx, ny, nz, hx, hx if hy is None else hy, hx if hz is None else hz)
+
+
+def build(force=False):
+    """Compile oracle.c with gcc (plain C99, -O2, OpenMP on the outer z loops)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall",
+                               "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_norm2.restype = C.c_double
+        _lib.orc_solve.restype = C.c_int
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    if a is None:
+        return None
+    assert a.dtype == np.float64 and a.flags.c_contiguous
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _bc(bc):
+    return (C.c_int * 6)(*[int(b) for b in bc])
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def num_threads():
+    return lib().orc_num_threads()
+
+
+def set_threads(n):
+    lib().orc_set_threads(int(n))
+
+
+FILTERS = {"lap": 0, "x": 1, "y": 2, "z": 3, "xx": 4, "yy": 5, "zz": 6, "mass": 7}
+
+
+def filter_weights(g, which):
+    """(3,3,3) array indexed [kk+1, jj+1, ii+1] of the nodal filter `which`."""
+    w = np.zeros(27)
+    lib().orc_filter(C.byref(g), FILTERS[which], _p(w))
+    return w.reshape(3, 3, 3)
+
+
+def apply_filter(g, bc, w, field):
+    field = _f64(field); w = _f64(w).reshape(27)
+    y = np.empty(g.shape)
+    lib().orc_apply_filter(C.byref(g), _bc(bc), _p(w), _p(field), _p(y))
+    return y
+
+
+def apply_operator(g, bc, k, x, eq13=False):
+    k = _f64(k); x = _f64(x)
+    y = np.empty(g.shape)
+    fn = lib().orc_apply_operator_eq13 if eq13 else lib().orc_apply_operator
+    fn(C.byref(g), _bc(bc), _p(k), _p(x), _p(y))
+    return y
+
+
+def diagonal(g, k):
+    k = _f64(k)
+    d = np.empty(g.shape)
+    lib().orc_diagonal(C.byref(g), _p(k), _p(d))
+    return d
+
+
+def jacobi_sweep(g, bc, k, x, b, omega):
+    k = _f64(k); x = _f64(x); b = _f64(b)
+    y = np.empty(g.shape)
+    lib().orc_jacobi_sweep(C.byref(g), _bc(bc), _p(k), _p(x), _p(b), C.c_double(omega), _p(y))
+    return y
+
+
+def smooth(g, bc, k, x, b, omega, sweeps):
+    k = _f64(k); b = _f64(b)
+    x = np.array(x, dtype=np.float64, order="C")
+    lib().orc_smooth(C.byref(g), _bc(bc), _p(k), _p(x), _p(b), C.c_double(omega), int(sweeps))
+    return x
+
+
+def residual(g, bc, k, x, b):
+    k = _f64(k); x = _f64(x); b = _f64(b)
+    r = np.empty(g.shape)
+    lib().orc_residual(C.byref(g), _bc(bc), _p(k), _p(x), _p(b), _p(r))
+    return r
+
+
+def restrict(g, rf):
+    rf = _f64(rf)
+    rc = np.empty((g.nz // 2, g.ny // 2, g.nx // 2))
+    lib().orc_restrict(C.byref(g), _p(rf), _p(rc))
+    return rc
+
+
+def prolong_add(g, xc, xf):
+    xc = _f64(xc)
+    xf = np.array(xf, dtype=np.float64, order="C")
+    lib().orc_prolong_add(C.byref(g), _p(xc), _p(xf))
+    return xf
+
+
+def k_from_vof(alpha, rho_l, rho_g):
+    alpha = _f64(alpha)
+    k = np.empty_like(alpha)
+    lib().orc_k_from_vof(C.c_size_t(alpha.size), _p(alpha), C.c_double(rho_l), C.c_double(rho_g), _p(k))
+    return k
+
+
+def vcycle(g, bc, k, x, b, levels, nu_pre=2, nu_post=2, coarse_sweeps=50, omega=2.0 / 3.0):
+    k = _f64(k); b = _f64(b)
+    x = np.array(x, dtype=np.float64, order="C")
+    lib().orc_vcycle(C.byref(g), _bc(bc), _p(k), int(levels), int(nu_pre), int(nu_post), int(coarse_sweeps),
+                     C.c_double(omega), _p(x), _p(b))
+    return x
+
+
+def solve(g, bc, k, x, b, levels, tol, max_cycles, nu_pre=2, nu_post=2, coarse_sweeps=50, omega=2.0 / 3.0):
+    """Returns (x, cycles, relres, history)."""
+    k = _f64(k); b = _f64(b)
+    x = np.array(x, dtype=np.float64, order="C")
+    hist = np.zeros(max(max_cycles, 1))
+    rel = C.c_double(0.0)
+    n = lib().orc_solve(C.byref(g), _bc(bc), _p(k), int(levels), int(nu_pre), int(nu_post), int(coarse_sweeps),
+                        C.c_double(omega), _p(x), _p(b), C.c_double(tol), int(max_cycles), _p(hist), C.byref(rel))
+    return x, n, rel.value, hist[:n]
+
+
+def vof_residual(g, Cf, u, v, w, dt):
+    """Returns (sC, Cnew)."""
+    Cf = _f64(Cf); u = _f64(u); v = _f64(v); w = _f64(w)
+    s = np.empty(g.shape); cn = np.empty(g.shape)
+    lib().orc_vof_residual(C.byref(g), _p(Cf), _p(u), _p(v), _p(w), C.c_double(dt), _p(s), _p(cn))
+    return s, cn
+
+
+def _ptr3(arrs):
+    return (C.c_void_p * 3)(*[a.ctypes.data for a in arrs])
+
+
+def mom_predictor(g, Cf, qh, qn, rho_l, rho_g, mu_l, mu_g, dt):
+    """qh, qn: 3-tuples (u, v, w).  Returns (q_tilde, q_half_new), each a 3-tuple."""
+    Cf = _f64(Cf)
+    qh = [_f64(a) for a in qh]; qn = [_f64(a) for a in qn]
+    qt = [np.empty(g.shape) for _ in range(3)]; qhn = [np.empty(g.shape) for _ in range(3)]
+    lib().orc_mom_predictor(C.byref(g), _p(Cf), _ptr3(qh), _ptr3(qn), C.c_double(rho_l), C.c_double(rho_g),
+                            C.c_double(mu_l), C.c_double(mu_g), C.c_double(dt), _ptr3(qt), _ptr3(qhn))
+    return tuple(qt), tuple(qhn)
+
+
+def pressure_rhs(g, u, v, w, dt):
+    u = _f64(u); v = _f64(v); w = _f64(w)
+    b = np.empty(g.shape)
+    lib().orc_pressure_rhs(C.byref(g), _p(u), _p(v), _p(w), C.c_double(dt), _p(b))
+    return b
+
+
+def project_velocity(g, bc, p, k, dt, u, v, w):
+    p = _f64(p); k = _f64(k)
+    u, v, w = (np.array(a, dtype=np.float64, order="C") for a in (u, v, w))
+    lib().orc_project_velocity(C.byref(g), _bc(bc), _p(p), _p(k), C.c_double(dt), _p(u), _p(v), _p(w))
+    return u, v, w

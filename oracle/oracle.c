@@ -1,0 +1,501 @@
+/*
+ * oracle.c -- plain, slow, fp64 CPU oracle for the multigrid pressure solve and the
+ * explicit stencil residuals of arxiv/paper_2401_06755 (NN4PDEs multiphase flow).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference leg may build, load or call it.  It
+ * shares no code, header, table or constant generator with the CUDA path under
+ * paper_2401_06755_b200/csrc/, and neither includes the other.
+ *
+ * Every function is written as nested loops over (k, j, i) with an explicit ghost()
+ * evaluation of halo values, in the order and notation of the paper.  "P:NNN" is a line
+ * of /root/reference/PAPER.md.  Readings of silent / garbled passages are those of
+ * DESIGN.md ("Readings").
+ *
+ * Parity pins (tests/test_oracle_*.py, -m "not gpu"): Eq. 11's printed weights, the closed
+ * form discrete eigenpair, 2nd-order manufactured solution, symmetry, constant null space,
+ * literal Eq. 13 == collapsed difference form, dense direct solves on <= 8^3, Fourier-mode
+ * Jacobi factors, transfer adjointness, hand-computed VoF cases.
+ * PARITY UNPINNED against the paper (no worked example exists in its text): the transfer
+ * operators / coarse operator (Fig. 5 is an image), the momentum residual without the
+ * missing Eq. 28, and vof_residual beyond its hand-computable special cases.
+ *
+ * Layout: dense, x fastest: idx = i + nx*(j + ny*k); no halo in arrays.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct { int nx, ny, nz; double hx, hy, hz; } orc_grid;
+
+/* boundary codes -> ghost factor s (reading C3):
+ * 0 Neumann (copy, s=+1); 1 Dirichlet zero on the cell face (s=-1); 2 Dirichlet halo value 0 (s=0) */
+static double bc_factor(int code) { return code == 0 ? 1.0 : (code == 1 ? -1.0 : 0.0); }
+
+static const int BC_COPY[6] = {0, 0, 0, 0, 0, 0};
+
+#define IDX(g, i, j, k) ((size_t)(i) + (size_t)(g)->nx * ((size_t)(j) + (size_t)(g)->ny * (size_t)(k)))
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* Halo value of field f at a (possibly out-of-box) index: reflect about the face
+ * (-1 -> 0, n -> n-1) and multiply the face factors; edges and corners reflect
+ * successively so the factors multiply (Fig. 2). */
+static double ghost(const double* f, const orc_grid* g, const int* bc, int i, int j, int k) {
+    double s = 1.0;
+    if (i < 0) { i = -1 - i; s *= bc_factor(bc[0]); } else if (i >= g->nx) { i = 2 * g->nx - 1 - i; s *= bc_factor(bc[1]); }
+    if (j < 0) { j = -1 - j; s *= bc_factor(bc[2]); } else if (j >= g->ny) { j = 2 * g->ny - 1 - j; s *= bc_factor(bc[3]); }
+    if (k < 0) { k = -1 - k; s *= bc_factor(bc[4]); } else if (k >= g->nz) { k = 2 * g->nz - 1 - k; s *= bc_factor(bc[5]); }
+    return s * f[IDX(g, i, j, k)];
+}
+
+/* ------------------------------------------------------------------------------------
+ * Filters (Eqs. 9-11).  All are NODAL, i.e. the
+ * paper's integrated filter divided by m_l = dx dy dz (its own w_ml^-1).
+ * 1-D factors of the trilinear element on a uniform line of spacing d:
+ *   stiffness  K = (1/d) [-1, 2, -1],  consistent mass M = (d/6) [1, 4, 1],
+ *   derivative D = (1/2) [-1, 0, 1]   (int N_i dN_j/dx).
+ * w[(ii+1) + 3*(jj+1) + 9*(kk+1)], ii along x.
+ * which: 0 w_lap = (KMM + MKM + MMK)/m_l     (-Laplacian, positive definite; reading C1)
+ *        1 w_x, 2 w_y, 3 w_z                 (Eq. 11 / m_l)
+ *        4 w_xx, 5 w_yy, 6 w_zz              (the three summands of w_lap)
+ *        7 w_m / m_l                         (consistent mass, MMM / m_l)
+ * ------------------------------------------------------------------------------------ */
+void orc_filter(const orc_grid* g, int which, double* w) {
+    const double h[3] = {g->hx, g->hy, g->hz};
+    double K[3][3], M[3][3], D[3][3];
+    for (int d = 0; d < 3; ++d) {
+        K[d][0] = -1.0 / h[d]; K[d][1] = 2.0 / h[d]; K[d][2] = -1.0 / h[d];
+        M[d][0] = h[d] / 6.0;  M[d][1] = 4.0 * h[d] / 6.0; M[d][2] = h[d] / 6.0;
+        D[d][0] = -0.5;        D[d][1] = 0.0;        D[d][2] = 0.5;
+    }
+    const double ml = h[0] * h[1] * h[2];
+    for (int kk = 0; kk < 3; ++kk)
+        for (int jj = 0; jj < 3; ++jj)
+            for (int ii = 0; ii < 3; ++ii) {
+                const double xx = K[0][ii] * M[1][jj] * M[2][kk];
+                const double yy = M[0][ii] * K[1][jj] * M[2][kk];
+                const double zz = M[0][ii] * M[1][jj] * K[2][kk];
+                double v = 0.0;
+                switch (which) {
+                    case 0: v = xx + yy + zz; break;
+                    case 1: v = D[0][ii] * M[1][jj] * M[2][kk]; break;
+                    case 2: v = M[0][ii] * D[1][jj] * M[2][kk]; break;
+                    case 3: v = M[0][ii] * M[1][jj] * D[2][kk]; break;
+                    case 4: v = xx; break;
+                    case 5: v = yy; break;
+                    case 6: v = zz; break;
+                    case 7: v = M[0][ii] * M[1][jj] * M[2][kk]; break;
+                }
+                w[ii + 3 * jj + 9 * kk] = v / ml;
+            }
+}
+
+/* f(C; w), Eq. 8: y_ijk = sum_{ii,jj,kk} w_{ii,jj,kk} C_{i+ii,j+jj,k+kk}, halo by ghost(). */
+void orc_apply_filter(const orc_grid* g, const int* bc, const double* w, const double* C, double* y) {
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                double s = 0.0;
+                for (int kk = -1; kk <= 1; ++kk)
+                    for (int jj = -1; jj <= 1; ++jj)
+                        for (int ii = -1; ii <= 1; ++ii)
+                            s += w[(ii + 1) + 3 * (jj + 1) + 9 * (kk + 1)] * ghost(C, g, bc, i + ii, j + jj, k + kk);
+                y[IDX(g, i, j, k)] = s;
+            }
+}
+
+/* ------------------------------------------------------------------------------------
+ * Operator y = A x (SURVEY/DESIGN C1, C2).
+ *   kcoef == NULL : y = f(x; w_lap)                                    (Eq. 8 with w_lap)
+ *   kcoef != NULL : y_i = sum_{j != i} (-w_ij) * 1/2 (k_i + k_j) (x_i - x_j)
+ * the exact collapse of Eq. 13 because sum_j w_ij = 0.  Halo of x by the BC
+ * factors, halo of k by copy.  w is any second-derivative filter (w_lap, w_xx...).
+ * ------------------------------------------------------------------------------------ */
+void orc_apply_diffusion(const orc_grid* g, const int* bc, const double* w, const double* kcoef,
+                         const double* x, double* y) {
+    if (!kcoef) { orc_apply_filter(g, bc, w, x, y); return; }
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                const double xi = x[IDX(g, i, j, k)], ki = kcoef[IDX(g, i, j, k)];
+                double s = 0.0;
+                for (int kk = -1; kk <= 1; ++kk)
+                    for (int jj = -1; jj <= 1; ++jj)
+                        for (int ii = -1; ii <= 1; ++ii) {
+                            if (ii == 0 && jj == 0 && kk == 0) continue;
+                            const double wij = w[(ii + 1) + 3 * (jj + 1) + 9 * (kk + 1)];
+                            const double xj = ghost(x, g, bc, i + ii, j + jj, k + kk);
+                            const double kj = ghost(kcoef, g, BC_COPY, i + ii, j + jj, k + kk);
+                            s += (-wij) * 0.5 * (ki + kj) * (xi - xj);
+                        }
+                y[IDX(g, i, j, k)] = s;
+            }
+}
+
+void orc_apply_operator(const orc_grid* g, const int* bc, const double* kcoef, const double* x, double* y) {
+    double w[27];
+    orc_filter(g, 0, w);
+    orc_apply_diffusion(g, bc, w, kcoef, x, y);
+}
+
+/* Literal Eq. 13: 1/2 ( f(k.C; w) + k.f(C; w) - C.f(k; w) ), three stencils.
+ * Halo of the product field k.C is ghost(k)*ghost(C).  Used only to pin the collapsed form. */
+void orc_apply_operator_eq13(const orc_grid* g, const int* bc, const double* kcoef, const double* x, double* y) {
+    double w[27];
+    orc_filter(g, 0, w);
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                double fkc = 0.0, fc = 0.0, fk = 0.0;
+                for (int kk = -1; kk <= 1; ++kk)
+                    for (int jj = -1; jj <= 1; ++jj)
+                        for (int ii = -1; ii <= 1; ++ii) {
+                            const double wij = w[(ii + 1) + 3 * (jj + 1) + 9 * (kk + 1)];
+                            const double xj = ghost(x, g, bc, i + ii, j + jj, k + kk);
+                            const double kj = ghost(kcoef, g, BC_COPY, i + ii, j + jj, k + kk);
+                            fkc += wij * (kj * xj); fc += wij * xj; fk += wij * kj;
+                        }
+                const size_t c = IDX(g, i, j, k);
+                y[c] = 0.5 * (fkc + kcoef[c] * fc - x[c] * fk);
+            }
+}
+
+/* Jacobi "diagonal" (reading C2-2): the centre coefficient of the conv-layer view,
+ * D_i = sum_{j != i} (-w_ij) 1/2 (k_i + k_j) over all 26 positions, ghosts included;
+ * constant coefficient: D = w_000. */
+void orc_diagonal(const orc_grid* g, const double* kcoef, double* D) {
+    double w[27];
+    orc_filter(g, 0, w);
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                if (!kcoef) { D[IDX(g, i, j, k)] = w[13]; continue; }
+                const double ki = kcoef[IDX(g, i, j, k)];
+                double s = 0.0;
+                for (int kk = -1; kk <= 1; ++kk)
+                    for (int jj = -1; jj <= 1; ++jj)
+                        for (int ii = -1; ii <= 1; ++ii) {
+                            if (ii == 0 && jj == 0 && kk == 0) continue;
+                            const double kj = ghost(kcoef, g, BC_COPY, i + ii, j + jj, k + kk);
+                            s += (-w[(ii + 1) + 3 * (jj + 1) + 9 * (kk + 1)]) * 0.5 * (ki + kj);
+                        }
+                D[IDX(g, i, j, k)] = s;
+            }
+}
+
+/* ------------------------------------------------------------------------------------
+ * Weighted Jacobi (reading C4): x' = x + omega (b - A x) / D, every
+ * point from the OLD x (two buffers).  xnew must not alias x.
+ * ------------------------------------------------------------------------------------ */
+void orc_jacobi_sweep(const orc_grid* g, const int* bc, const double* kcoef, const double* x,
+                      const double* b, double omega, double* xnew) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double* Ax = (double*)malloc(n * sizeof(double));
+    double* D = (double*)malloc(n * sizeof(double));
+    orc_apply_operator(g, bc, kcoef, x, Ax);
+    orc_diagonal(g, kcoef, D);
+    for (size_t c = 0; c < n; ++c) xnew[c] = x[c] + omega * (b[c] - Ax[c]) / D[c];
+    free(Ax); free(D);
+}
+
+/* `sweeps` sweeps in place (ping-pong through a scratch copy). */
+void orc_smooth(const orc_grid* g, const int* bc, const double* kcoef, double* x, const double* b,
+                double omega, int sweeps) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double* t = (double*)malloc(n * sizeof(double));
+    for (int s = 0; s < sweeps; ++s) {
+        orc_jacobi_sweep(g, bc, kcoef, x, b, omega, t);
+        memcpy(x, t, n * sizeof(double));
+    }
+    free(t);
+}
+
+void orc_residual(const orc_grid* g, const int* bc, const double* kcoef, const double* x,
+                  const double* b, double* r) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    orc_apply_operator(g, bc, kcoef, x, r);
+    for (size_t c = 0; c < n; ++c) r[c] = b[c] - r[c];
+}
+
+/* ------------------------------------------------------------------------------------
+ * Transfers (Fig. 5 caption P:417; reading C5 -- the paper gives no weights):
+ * restriction = mean of the 8 children (stride-2 2x2x2 filter, weights 1/8);
+ * prolongation = piecewise constant (nearest-neighbour upsampling x2), added to x.
+ * gc is the coarse grid: n/2 in each direction, spacing 2h.
+ * ------------------------------------------------------------------------------------ */
+void orc_coarse_grid(const orc_grid* gf, orc_grid* gc) {
+    gc->nx = gf->nx / 2; gc->ny = gf->ny / 2; gc->nz = gf->nz / 2;
+    gc->hx = 2.0 * gf->hx; gc->hy = 2.0 * gf->hy; gc->hz = 2.0 * gf->hz;
+}
+
+void orc_restrict(const orc_grid* gf, const double* rf, double* rc) {
+    orc_grid gc; orc_coarse_grid(gf, &gc);
+    for (int k = 0; k < gc.nz; ++k)
+        for (int j = 0; j < gc.ny; ++j)
+            for (int i = 0; i < gc.nx; ++i) {
+                double s = 0.0;
+                for (int dk = 0; dk < 2; ++dk)
+                    for (int dj = 0; dj < 2; ++dj)
+                        for (int di = 0; di < 2; ++di)
+                            s += rf[IDX(gf, 2 * i + di, 2 * j + dj, 2 * k + dk)];
+                rc[IDX(&gc, i, j, k)] = 0.125 * s;
+            }
+}
+
+void orc_prolong_add(const orc_grid* gf, const double* xc, double* xf) {
+    orc_grid gc; orc_coarse_grid(gf, &gc);
+    for (int k = 0; k < gf->nz; ++k)
+        for (int j = 0; j < gf->ny; ++j)
+            for (int i = 0; i < gf->nx; ++i)
+                xf[IDX(gf, i, j, k)] += xc[IDX(&gc, i / 2, j / 2, k / 2)];
+}
+
+/* k = 1 / (rho_l alpha + rho_g (1 - alpha)), Eqs. 2 and 19; no clipping (C7). */
+void orc_k_from_vof(size_t n, const double* alpha, double rho_l, double rho_g, double* kcoef) {
+    for (size_t c = 0; c < n; ++c) kcoef[c] = 1.0 / (rho_l * alpha[c] + rho_g * (1.0 - alpha[c]));
+}
+
+/* ------------------------------------------------------------------------------------
+ * V-cycle (Fig. 5; reading C6).  Coarse operators are rediscretised with
+ * spacing 2h and the same BC factors; coarse coefficient = arithmetic mean of the
+ * 8 children.  The coarsest level runs `coarse_sweeps` Jacobi sweeps on the incoming guess.
+ *   vcycle(l,x,b): if coarsest: n_c sweeps; return
+ *                  nu1 sweeps; r = b - A x; b_c = R r; x_c = 0; vcycle(l+1,x_c,b_c);
+ *                  x += P x_c; nu2 sweeps
+ * ------------------------------------------------------------------------------------ */
+void orc_vcycle(const orc_grid* g, const int* bc, const double* kcoef, int levels, int nu_pre, int nu_post,
+                int coarse_sweeps, double omega, double* x, const double* b) {
+    if (levels <= 1) { orc_smooth(g, bc, kcoef, x, b, omega, coarse_sweeps); return; }
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    orc_grid gc; orc_coarse_grid(g, &gc);
+    const size_t nc = (size_t)gc.nx * gc.ny * gc.nz;
+    double* r = (double*)malloc(n * sizeof(double));
+    double* bcz = (double*)malloc(nc * sizeof(double));
+    double* xc = (double*)calloc(nc, sizeof(double));
+    double* kc = kcoef ? (double*)malloc(nc * sizeof(double)) : NULL;
+    if (kcoef) orc_restrict(g, kcoef, kc);
+    orc_smooth(g, bc, kcoef, x, b, omega, nu_pre);
+    orc_residual(g, bc, kcoef, x, b, r);
+    orc_restrict(g, r, bcz);
+    orc_vcycle(&gc, bc, kc, levels - 1, nu_pre, nu_post, coarse_sweeps, omega, xc, bcz);
+    orc_prolong_add(g, xc, x);
+    orc_smooth(g, bc, kcoef, x, b, omega, nu_post);
+    free(r); free(bcz); free(xc); free(kc);
+}
+
+double orc_norm2(size_t n, const double* v) {
+    double s = 0.0;
+    for (size_t c = 0; c < n; ++c) s += v[c] * v[c];
+    return sqrt(s);
+}
+
+/* Repeat V-cycles until ||b - A x||_2 / ||b||_2 < tol (the paper runs a fixed 20; the
+ * tolerance is BASELINE.json's).  history (may be NULL) receives the relative residual after
+ * every cycle (max_cycles entries).  Returns the number of cycles run. */
+int orc_solve(const orc_grid* g, const int* bc, const double* kcoef, int levels, int nu_pre, int nu_post,
+              int coarse_sweeps, double omega, double* x, const double* b, double tol, int max_cycles,
+              double* history, double* relres_out) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double* r = (double*)malloc(n * sizeof(double));
+    const double nb = orc_norm2(n, b);
+    double rel = 0.0;
+    int c = 0;
+    orc_residual(g, bc, kcoef, x, b, r);
+    rel = nb > 0.0 ? orc_norm2(n, r) / nb : 0.0;
+    while (c < max_cycles && !(rel < tol)) {
+        orc_vcycle(g, bc, kcoef, levels, nu_pre, nu_post, coarse_sweeps, omega, x, b);
+        orc_residual(g, bc, kcoef, x, b, r);
+        rel = orc_norm2(n, r) / nb;
+        if (history) history[c] = rel;
+        ++c;
+    }
+    if (relres_out) *relres_out = rel;
+    free(r);
+    return c;
+}
+
+/* ====================================================================================
+ * Explicit stencil residuals that feed the pressure solve.
+ * All derived fields are nodal (divided by m_l); halos of C, of the velocities and of every
+ * derived field are zero-derivative copies (reading C9-iv).
+ * ==================================================================================== */
+
+/* Eqs. 26/27: first residual-based PG diffusion coefficient, p = 1 so
+ * alpha_kabs = 1/(8*2^p) = 1/16, eps_k = 1e-7.  Uniform spacing uses
+ * Eq. 27, otherwise Eq. 26 (reading C9-ii). */
+static double k_abs_pg(const orc_grid* g, double a, double px, double py, double pz) {
+    const double alpha_kabs = 1.0 / 16.0, eps_k = 1e-7;
+    const double s = fabs(px) + fabs(py) + fabs(pz);
+    if (g->hx == g->hy && g->hy == g->hz) return alpha_kabs * g->hx * fabs(a) / (eps_k + s / 3.0);
+    return alpha_kabs * fabs(a) * (g->hx * fabs(px) + g->hy * fabs(py) + g->hz * fabs(pz)) / (eps_k + s * s / 3.0);
+}
+
+/* Gradient by the linear-FE filters (Eq. 11 / m_l) and the advection term q . grad(Psi). */
+static void grad_and_adv(const orc_grid* g, const double* psi, const double* u, const double* v, const double* w,
+                         double* px, double* py, double* pz, double* adv) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wx[27], wy[27], wz[27];
+    orc_filter(g, 1, wx); orc_filter(g, 2, wy); orc_filter(g, 3, wz);
+    orc_apply_filter(g, BC_COPY, wx, psi, px);
+    orc_apply_filter(g, BC_COPY, wy, psi, py);
+    orc_apply_filter(g, BC_COPY, wz, psi, pz);
+    for (size_t c = 0; c < n; ++c) adv[c] = u[c] * px[c] + v[c] * py[c] + w[c] * pz[c];
+}
+
+/* Eq. 29: a = alpha_a f(adv; w_m/m_l - E), alpha_a = 2. */
+static void mixed_mass_residual(const orc_grid* g, const double* adv, double* a) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wm[27];
+    orc_filter(g, 7, wm);
+    wm[13] -= 1.0; /* minus the identity filter E */
+    orc_apply_filter(g, BC_COPY, wm, adv, a);
+    for (size_t c = 0; c < n; ++c) a[c] *= 2.0;
+}
+
+/* vof_residual (reading C9, steps 1-12): sC = nodal s~_C of Eq. 16;
+ * Cnew (may be NULL) = C - dt sC, Eq. 55. */
+void orc_vof_residual(const orc_grid* g, const double* C, const double* u, const double* v, const double* w,
+                      double dt, double* sC, double* Cnew) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    const double Kp = 300.0, Km = 300.0;          /* K+, K-  */
+    const double beta = 0.1, eps_x = 1e-4;        /* Eq. 36 */
+    const double Kcal = 3.0;                      /* Eq. 39 */
+    const double a_min = 1e-4, a_max = 0.05;      /* Eq. 42 */
+    const double hmax = fmax(g->hx, fmax(g->hy, g->hz)), hmin = fmin(g->hx, fmin(g->hy, g->hz));
+    const double k_min = a_min / dt * hmax * hmax, k_max = a_max / dt * hmin * hmin;
+    const double hd[3] = {g->hx, g->hy, g->hz};
+    double* Cx = (double*)malloc(n * sizeof(double)); double* Cy = (double*)malloc(n * sizeof(double));
+    double* Cz = (double*)malloc(n * sizeof(double)); double* adv = (double*)malloc(n * sizeof(double));
+    double* a = (double*)malloc(n * sizeof(double));
+    double* kd[3]; double* diff = (double*)malloc(n * sizeof(double));
+    for (int d = 0; d < 3; ++d) kd[d] = (double*)malloc(n * sizeof(double));
+
+    grad_and_adv(g, C, u, v, w, Cx, Cy, Cz, adv);            /* steps 1-2 */
+    mixed_mass_residual(g, adv, a);                          /* step 3 */
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                const size_t c = IDX(g, i, j, k);
+                const double kabs = k_abs_pg(g, a[c], Cx[c], Cy[c], Cz[c]);          /* step 4 */
+                /* step 5: Eq. 33 + override */
+                const double C0 = C[c];
+                double S[3];
+                S[0] = (C0 - ghost(C, g, BC_COPY, i - 1, j, k)) * (ghost(C, g, BC_COPY, i + 1, j, k) - C0);
+                S[1] = (C0 - ghost(C, g, BC_COPY, i, j - 1, k)) * (ghost(C, g, BC_COPY, i, j + 1, k) - C0);
+                S[2] = (C0 - ghost(C, g, BC_COPY, i, j, k - 1)) * (ghost(C, g, BC_COPY, i, j, k + 1) - C0);
+                if (C0 > 0.95 || C0 < 0.05) S[0] = S[1] = S[2] = -1.0;
+                /* step 7: Eq. 37 */
+                const double g2 = Cx[c] * Cx[c] + Cy[c] * Cy[c] + Cz[c] * Cz[c];
+                const double gq = (u[c] * Cx[c] + v[c] * Cy[c] + w[c] * Cz[c]) / (eps_x + g2);
+                const double us = gq * Cx[c], vs = gq * Cy[c], ws = gq * Cz[c];
+                /* step 8: Eq. 36 */
+                const double kneg = -beta * (u[c] * u[c] + v[c] * v[c] + w[c] * w[c]) /
+                                    (eps_x + g2 * (fabs(us) + fabs(vs) + fabs(ws)) / 3.0);
+                for (int d = 0; d < 3; ++d) {
+                    const double wp = -fmax(-1.0, fmin(0.0, Kp * S[d]));             /* step 6: Eq. 35 */
+                    const double wm = fmin(1.0, fmax(0.0, Km * S[d]));
+                    const double kplus = Kcal * kabs;                                /* step 9: Eq. 39 */
+                    const double kminus = kneg / hd[d];                              /* Eq. 38 */
+                    const double kk = wp * kplus + wm * kminus;                      /* Eq. 40 */
+                    kd[d][c] = fmax(-k_min, fmin(k_max, kk));                        /* step 10: Eq. 41 */
+                }
+            }
+    for (size_t c = 0; c < n; ++c) sC[c] = adv[c];
+    for (int d = 0; d < 3; ++d) {                                                    /* step 11: Eq. 12 collapsed */
+        double wdd[27];
+        orc_filter(g, 4 + d, wdd);
+        orc_apply_diffusion(g, BC_COPY, wdd, kd[d], C, diff);
+        for (size_t c = 0; c < n; ++c) sC[c] += diff[c];
+    }
+    if (Cnew) for (size_t c = 0; c < n; ++c) Cnew[c] = C[c] - dt * sC[c];            /* step 12: Eq. 55 */
+    free(Cx); free(Cy); free(Cz); free(adv); free(a); free(diff);
+    for (int d = 0; d < 3; ++d) free(kd[d]);
+}
+
+/* Momentum advection-diffusion residual and predictor (Eqs. 18, 30-32, 45-46; P:198-220,
+ * 309-319, 433-441; reading C9 "Momentum").  For each component c of the half-level velocity:
+ *   s~_c = rho (q_h . grad c_h) + f^lap(c_h, k_c; w_lap),  k_c = rho min{k_max, k_abs(c_h)} + mu,
+ *   k_max = dx|u_h| + dy|v_h| + dz|w_h| (Eq. 30);  k_square of the lost Eq. 28 is omitted;
+ *   c~ = c_n - dt s~_c / rho (Eq. 45, sigma = 0);  c_half' = (c_n + c~)/2 (Eq. 46).
+ * Pressure-gradient and source terms of Eq. 18 are not part of this residual.
+ * qh/qn/qt/qhn are arrays of 3 component pointers (u, v, w). */
+void orc_mom_predictor(const orc_grid* g, const double* C, const double* const* qh, const double* const* qn,
+                       double rho_l, double rho_g, double mu_l, double mu_g, double dt,
+                       double* const* qt, double* const* qhn) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wl[27];
+    orc_filter(g, 0, wl);
+    double* px = (double*)malloc(n * sizeof(double)); double* py = (double*)malloc(n * sizeof(double));
+    double* pz = (double*)malloc(n * sizeof(double)); double* adv = (double*)malloc(n * sizeof(double));
+    double* a = (double*)malloc(n * sizeof(double)); double* kc = (double*)malloc(n * sizeof(double));
+    double* diff = (double*)malloc(n * sizeof(double));
+    for (int comp = 0; comp < 3; ++comp) {
+        grad_and_adv(g, qh[comp], qh[0], qh[1], qh[2], px, py, pz, adv);
+        mixed_mass_residual(g, adv, a);
+        for (size_t c = 0; c < n; ++c) {
+            const double rho = rho_l * C[c] + rho_g * (1.0 - C[c]);
+            const double mu = mu_l * C[c] + mu_g * (1.0 - C[c]);
+            const double kmax = g->hx * fabs(qh[0][c]) + g->hy * fabs(qh[1][c]) + g->hz * fabs(qh[2][c]);
+            const double kabs = k_abs_pg(g, a[c], px[c], py[c], pz[c]);
+            kc[c] = rho * fmin(kmax, kabs) + mu;
+        }
+        orc_apply_diffusion(g, BC_COPY, wl, kc, qh[comp], diff);
+        for (size_t c = 0; c < n; ++c) {
+            const double rho = rho_l * C[c] + rho_g * (1.0 - C[c]);
+            const double s = rho * adv[c] + diff[c];
+            const double t = qn[comp][c] - dt * s / rho;
+            qt[comp][c] = t;
+            if (qhn) qhn[comp][c] = 0.5 * (qn[comp][c] + t);
+        }
+    }
+    free(px); free(py); free(pz); free(adv); free(a); free(kc); free(diff);
+}
+
+/* Pressure RHS (reading C10; FE divergence structure of Eq. 53):
+ * b = -(1/dt) ( f(u~; w_x) + f(v~; w_y) + f(w~; w_z) ), nodal filters, velocity halos copy. */
+void orc_pressure_rhs(const orc_grid* g, const double* u, const double* v, const double* w, double dt, double* b) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wx[27], wy[27], wz[27];
+    orc_filter(g, 1, wx); orc_filter(g, 2, wy); orc_filter(g, 3, wz);
+    double* t = (double*)malloc(n * sizeof(double));
+    orc_apply_filter(g, BC_COPY, wx, u, b);
+    orc_apply_filter(g, BC_COPY, wy, v, t); for (size_t c = 0; c < n; ++c) b[c] += t[c];
+    orc_apply_filter(g, BC_COPY, wz, w, t); for (size_t c = 0; c < n; ++c) b[c] = -(b[c] + t[c]) / dt;
+    free(t);
+}
+
+/* Velocity projection, Eq. 54 with Eq. 48: q = q~ - dt k . f(p; w_x|y|z),
+ * k = 1/rho; halo of p by the solver's BC factors.  In place on u, v, w. */
+void orc_project_velocity(const orc_grid* g, const int* bc, const double* p, const double* kcoef, double dt,
+                          double* u, double* v, double* w) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wf[27];
+    double* t = (double*)malloc(n * sizeof(double));
+    double* q[3] = {u, v, w};
+    for (int d = 0; d < 3; ++d) {
+        orc_filter(g, 1 + d, wf);
+        orc_apply_filter(g, bc, wf, p, t);
+        for (size_t c = 0; c < n; ++c) q[d][c] -= dt * kcoef[c] * t[c];
+    }
+    free(t);
+}
