@@ -1,0 +1,42 @@
+"""The seeded input generators (workloads/): determinism and the structure DESIGN.md's recipe states."""
+import numpy as np
+
+from workloads import configs, rng
+
+
+def test_rng_is_counter_based_and_stable():
+    a = rng.uniform01(7, 1000)
+    assert np.array_equal(a[100:200], rng.uniform01(7, 200)[100:200])       # value depends on (seed, index) only
+    assert 0.0 < a.min() and a.max() < 1.0 and abs(a.mean() - 0.5) < 0.03
+    # SplitMix64 reference value for counter 0 (state 0 -> first output of the published generator)
+    assert int(rng.splitmix64(np.array([0], dtype=np.uint64))[0]) == 0xE220A8397B1DCDAF
+    n = rng.normal(11, 20000)
+    assert abs(n.mean()) < 0.03 and abs(n.std() - 1.0) < 0.03
+
+
+def test_config1_and_2_fields():
+    w = configs.config1()
+    b = w.fields["b"]
+    assert b.shape == (32, 32, 32) and abs(b.mean()) < 1e-15 and np.abs(b).max() <= 1.05
+    w = configs.config2(n=32, levels=4)
+    a = w.fields["alpha"]
+    assert a.shape == (32, 32, 32) and 0.0 <= a.min() and a.max() <= 1.0
+    # water column: alpha ~ 1 at (x small, z small), ~ 0 elsewhere
+    assert a[2, 5, 2] > 0.99 and a[30, 5, 2] < 0.01 and a[2, 5, 30] < 0.01
+    assert w.bc == (0, 0, 0, 0, 0, 1)
+
+
+def test_bubbles_and_solenoidal_velocity():
+    cs = configs.bubble_centres(4000)
+    assert len(cs) == 4
+    for i in range(4):
+        for j in range(i):
+            assert np.linalg.norm(np.subtract(cs[i], cs[j])) >= 0.14
+    a = configs.bubble_alpha(32, 32, 32, 1 / 32, [(0.5, 0.5, 0.25)], 0.125)
+    assert a[8, 16, 16] < 0.01 and a[28, 16, 16] > 0.99                      # 0 inside the sphere, 1 outside
+    u, v, w = configs.solenoidal_velocity((5001, 5002, 5003), 24, 24, 24, 1 / 24)
+    assert abs(max(np.abs(u).max(), np.abs(v).max(), np.abs(w).max()) - 1.0) < 1e-12
+    h = 1 / 24
+    div = (np.gradient(u, h, axis=2) + np.gradient(v, h, axis=1) + np.gradient(w, h, axis=0))[2:-2, 2:-2, 2:-2]
+    grad = np.abs(np.gradient(u, h, axis=2)).max()
+    assert np.abs(div).max() < 0.2 * grad                                    # analytic curl: divergence-free up to FD error
