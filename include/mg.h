@@ -1,0 +1,159 @@
+/*
+ * mg.h -- C ABI of libmg_b200: the B200 (sm_100a) geometric-multigrid pressure solve and the
+ * explicit stencil residuals of arxiv/paper_2401_06755 (NN4PDEs multiphase flow).
+ *
+ * "P:NNN" cites a line of the paper text.  Readings of silent / garbled passages
+ * ("reading Cn") are listed in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ * ------------------------------
+ *  - Every field is a dense array of nx*ny*nz values, x fastest: idx = i + nx*(j + ny*k),
+ *    cell-centred, WITHOUT halo (the paper's outputs are unpadded).  Halos
+ *    carrying the boundary conditions exist only inside the kernels.
+ *  - Pointers named d_* are DEVICE pointers, 16-byte aligned, owned by the caller; the
+ *    library never frees or reallocates them.  Pointers named h_* are HOST pointers.
+ *    The element type is float (MG_F32) or double (MG_F64) as selected at creation.
+ *  - All work is enqueued on the CUDA stream given at creation (a cudaStream_t passed as
+ *    void*; NULL = the legacy default stream).  Only mg_solve*, *_host and mg_vcycle_timed
+ *    synchronise with the host.
+ *  - Return value: 0 = MG_OK, < 0 = error (nothing useful was computed; mg_last_error()
+ *    describes it), > 0 = non-fatal status of mg_solve.  No exception or abort crosses
+ *    the boundary.  There is no CPU fallback: without a CUDA device every compute call
+ *    returns MG_ECUDA.
+ */
+#ifndef MG_B200_H
+#define MG_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mg_solver mg_solver; /* opaque; owned by the library, freed by mg_destroy */
+
+typedef enum { MG_F32 = 0, MG_F64 = 1 } mg_dtype;
+
+/* Boundary condition of one face = the factor s of the halo rule ghost = s * mirror
+ * (reading C3; Fig. 2 caption P:276); applied at every multigrid level. */
+typedef enum {
+    MG_BC_NEUMANN = 0,       /* s = +1: zero normal derivative, "copying the nearest nodal value" */
+    MG_BC_DIRICHLET = 1,     /* s = -1: zero value ON the cell face (interpolation rule of Fig. 2)  */
+    MG_BC_DIRICHLET_HALO = 2 /* s =  0: halo node set to the value 0 (literal P:256)                        */
+} mg_bc;
+
+typedef struct { int nx, ny, nz; double hx, hy, hz; } mg_grid;
+
+/* V-cycle parameters (the paper gives none: P:43, P:47, P:105 name "Jacobi smoothing" only;
+ * defaults are BASELINE.json config 1): nu_pre, nu_post weighted-Jacobi sweeps, coarse_sweeps
+ * sweeps on the coarsest level from a zero guess, omega the damping.
+ * sweeps_per_pass: how many sweeps one kernel pass may fuse temporally (>= 1; results do not
+ * depend on it beyond rounding order).  mixed_precision (MG_F32 only): mg_solve keeps the
+ * iterate and the fine-grid residual in fp64 around fp32 V-cycles (reading C6/C8). */
+typedef struct {
+    int nu_pre, nu_post, coarse_sweeps, sweeps_per_pass;
+    double omega;
+    int mixed_precision;
+} mg_params;
+
+enum {
+    MG_OK = 0,
+    MG_NOT_CONVERGED = 1, /* mg_solve stopped on max_cycles */
+    MG_STAGNATED = 2,     /* residual ratio > 0.95 for 3 consecutive cycles, or non-finite */
+    MG_EINVAL = -1,       /* NULL or out-of-range argument */
+    MG_ESHAPE = -2,       /* a dimension not divisible by 2^(levels-1), or coarsest dimension < 2 */
+    MG_ECUDA = -3,        /* a CUDA call failed (no device, launch error, ...) */
+    MG_EALLOC = -4        /* device or host allocation failed */
+};
+
+/* Create a solver for A p = b with A the 27-point trilinear-FE discretisation of -div(k grad)
+ * (Eqs. 8, 11-13; readings C1, C2) on `grid`, with `levels` grids
+ * coarsened 2:1 (n_{l+1} = n_l/2, h_{l+1} = 2 h_l, operator rediscretised, reading C5) and the
+ * boundary factors bc[6] = {x-, x+, y-, y+, z-, z+}.  The solver owns its level hierarchy,
+ * scratch, CUDA graph and pinned host words.  Coefficient starts as k = 1 (constant). */
+int mg_create(mg_solver** out, const mg_grid* grid, int levels, const int bc[6], int dtype, void* cuda_stream);
+void mg_destroy(mg_solver* s);
+
+int mg_set_params(mg_solver* s, const mg_params* p); /* defaults: 2, 2, 50, 2, 2/3, 1 */
+int mg_get_params(const mg_solver* s, mg_params* p);
+
+/* Coefficient k (a7).  d_k: nx*ny*nz values of k > 0, or NULL for constant k = 1.  The field is
+ * copied; coarse levels get the arithmetic mean of the 8 children (reading C5). */
+int mg_set_coefficient(mg_solver* s, const void* d_k);
+/* k = 1 / (rho_l alpha + rho_g (1 - alpha)), Eqs. 2 and 19; no clipping (C7). */
+int mg_set_coefficient_from_vof(mg_solver* s, const void* d_alpha, double rho_l, double rho_g);
+
+/* a1: y = A x on the fine level.  d_y must not alias d_x. */
+int mg_apply_operator(mg_solver* s, const void* d_x, void* d_y);
+/* a2: `sweeps` weighted-Jacobi sweeps x <- x + omega (b - A x) / D, in place (two-buffer
+ * inside; every point of a sweep uses the previous sweep's x).  Reading C4. */
+int mg_smooth(mg_solver* s, void* d_x, const void* d_b, int sweeps);
+/* r = b - A x on the fine level. */
+int mg_residual(mg_solver* s, const void* d_x, const void* d_b, void* d_r);
+/* a3..a6: one V(nu_pre, nu_post) cycle in place (Fig. 5; reading C6). */
+int mg_vcycle(mg_solver* s, void* d_x, const void* d_b);
+/* a6: V-cycles until ||b - A x||_2 / ||b||_2 < tol or max_cycles (the paper runs a fixed 20,
+ * P:429).  d_x holds the initial guess on entry and the solution on exit.  cycles_out /
+ * relres_out may be NULL.  Returns MG_OK, MG_NOT_CONVERGED or MG_STAGNATED. */
+int mg_solve(mg_solver* s, void* d_x, const void* d_b, double tol, int max_cycles, int* cycles_out,
+             double* relres_out);
+/* Same with HOST buffers: copies h_b and the guess h_x to the device, solves, copies x back. */
+int mg_solve_host(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out,
+                  double* relres_out);
+/* Relative residual after every cycle of the last mg_solve (up to n entries); returns count. */
+int mg_get_history(const mg_solver* s, double* h_history, int n);
+
+/* Measurement helpers.  mg_level_info: points of level l (returns < 0 if l is out of range).
+ * mg_vcycle_timed: one V-cycle with CUDA events around every level's down leg and up leg;
+ * h_ms_down / h_ms_up receive `levels` floats each (the coarsest level's time is in down). */
+long long mg_level_info(const mg_solver* s, int level, int* nx, int* ny, int* nz);
+int mg_vcycle_timed(mg_solver* s, void* d_x, const void* d_b, float* h_ms_down, float* h_ms_up);
+/* Number of kernel launches the library has enqueued on behalf of this solver so far. */
+long long mg_launch_count(const mg_solver* s);
+/* 0: every level with separate one-sweep kernels (reference path); 1 (default): fused kernels,
+ * single-CTA coarse tail and CUDA-graph replay. */
+int mg_set_fused(mg_solver* s, int fused);
+
+/* ------------------------------------------------------------------------------------------
+ * Explicit stencil residuals feeding the solve (a8-a10).  Stateless; scratch comes from the
+ * stream-ordered pool of `cuda_stream`.  Halos of C, of the velocities and of every derived
+ * field are zero-derivative copies (reading C9-iv).
+ * ------------------------------------------------------------------------------------------ */
+
+/* a8: compressive-advection VoF residual, Eqs. 16, 26/27, 29, 33, 35-42 (P:179-181, 264-288,
+ * 301, 327-401; reading C9 steps 1-12).  d_sC_out (may be NULL) receives the nodal residual
+ * s~_C / m_l; d_Cnew_out (may be NULL) receives C - dt * sC, Eq. 55. */
+int vof_residual(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v,
+                 const void* d_w, double dt, void* d_sC_out, void* d_Cnew_out, void* cuda_stream);
+
+/* a9: momentum advection-diffusion residual and predictor, Eqs. 18, 30-32, 45-46 (P:198-220,
+ * 309-319, 433-441; reading C9 "Momentum").  d_qh[3] = half-level (u, v, w), d_qn[3] = level-n
+ * (u, v, w); d_qt[3] receives q~ = q_n - dt s~/rho, d_qhn[3] (may be NULL) (q_n + q~)/2.
+ * Outputs must not alias inputs. */
+int mom_predictor(const mg_grid* grid, int dtype, const void* d_C, const void* const d_qh[3],
+                  const void* const d_qn[3], double rho_l, double rho_g, double mu_l, double mu_g, double dt,
+                  void* const d_qt[3], void* const d_qhn[3], void* cuda_stream);
+
+/* a10: b = -(1/dt) (f(u; w_x) + f(v; w_y) + f(w; w_z)), nodal FE filters of Eq. 11
+ * (structure of Eq. 53; reading C10). */
+int pressure_rhs(const mg_grid* grid, int dtype, const void* d_u, const void* d_v, const void* d_w, double dt,
+                 void* d_b, void* cuda_stream);
+/* a10: q <- q - dt k f(p; w_x|y|z), Eq. 54 with Eq. 48; halo of p by bc[6]. */
+int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void* d_p, const void* d_k,
+                     double dt, void* d_u, void* d_v, void* d_w, void* cuda_stream);
+
+/* Config-5 time step on device buffers (stages 2-4 of P:403-505 under readings C9, C10):
+ * two momentum predictor iterations, VoF residual + update, k = 1/rho(C^n), pressure RHS,
+ * mg_solve(tol, max_cycles) from a zero guess into d_p, projection.  In place on d_C, d_u,
+ * d_v, d_w.  The solver supplies grid, dtype, bc and stream. */
+int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l,
+                   double rho_g, double mu_l, double mu_g, double dt, double tol, int max_cycles,
+                   int* cycles_out, double* relres_out);
+
+/* Thread-local description of the last error; never freed by the caller. */
+const char* mg_last_error(void);
+/* Library / build identification, e.g. "libmg_b200 sm_100a". */
+const char* mg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG_B200_H */

@@ -1,0 +1,308 @@
+"""Thin ctypes binding of libmg_b200.so (include/mg.h).  Argument marshalling only.
+
+Every function has the name and the arguments of its C-ABI entry point; torch tensors are
+used for device memory and streams and are passed down as raw device pointers.  Tensors are
+contiguous, shape (nz, ny, nx) (x fastest), float32 or float64 matching the solver's dtype.
+There is no CPU fallback: if the library cannot be loaded, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import _build
+
+MG_F32, MG_F64 = 0, 1
+MG_BC_NEUMANN, MG_BC_DIRICHLET, MG_BC_DIRICHLET_HALO = 0, 1, 2
+MG_OK, MG_NOT_CONVERGED, MG_STAGNATED = 0, 1, 2
+MG_EINVAL, MG_ESHAPE, MG_ECUDA, MG_EALLOC = -1, -2, -3, -4
+
+EXPORTS = [
+    "mg_create", "mg_destroy", "mg_set_params", "mg_get_params", "mg_set_coefficient",
+    "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve",
+    "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
+    "vof_residual", "mom_predictor", "pressure_rhs", "project_velocity", "flow_time_step", "mg_last_error",
+    "mg_version",
+]
+
+
+class MgGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("hx", C.c_double), ("hy", C.c_double), ("hz", C.c_double)]
+
+
+class MgParams(C.Structure):
+    _fields_ = [("nu_pre", C.c_int), ("nu_post", C.c_int), ("coarse_sweeps", C.c_int),
+                ("sweeps_per_pass", C.c_int), ("omega", C.c_double), ("mixed_precision", C.c_int)]
+
+
+class MgError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libmg_b200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _load():
+    path = _build.LIB
+    if not os.path.exists(path):
+        path = _build.build()
+    lib = C.CDLL(path)
+    vp, i, d = C.c_void_p, C.c_int, C.c_double
+    pi, pd = C.POINTER(C.c_int), C.POINTER(C.c_double)
+    lib.mg_create.argtypes = [C.POINTER(vp), C.POINTER(MgGrid), i, pi, i, vp]
+    lib.mg_destroy.argtypes = [vp]; lib.mg_destroy.restype = None
+    lib.mg_set_params.argtypes = [vp, C.POINTER(MgParams)]
+    lib.mg_get_params.argtypes = [vp, C.POINTER(MgParams)]
+    lib.mg_set_coefficient.argtypes = [vp, vp]
+    lib.mg_set_coefficient_from_vof.argtypes = [vp, vp, d, d]
+    lib.mg_apply_operator.argtypes = [vp, vp, vp]
+    lib.mg_smooth.argtypes = [vp, vp, vp, i]
+    lib.mg_residual.argtypes = [vp, vp, vp, vp]
+    lib.mg_vcycle.argtypes = [vp, vp, vp]
+    lib.mg_solve.argtypes = [vp, vp, vp, d, i, pi, pd]
+    lib.mg_solve_host.argtypes = [vp, vp, vp, d, i, pi, pd]
+    lib.mg_get_history.argtypes = [vp, pd, i]
+    lib.mg_level_info.argtypes = [vp, i, pi, pi, pi]; lib.mg_level_info.restype = C.c_longlong
+    lib.mg_vcycle_timed.argtypes = [vp, vp, vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    lib.mg_launch_count.argtypes = [vp]; lib.mg_launch_count.restype = C.c_longlong
+    lib.mg_set_fused.argtypes = [vp, i]
+    lib.vof_residual.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, vp, vp, vp]
+    lib.mom_predictor.argtypes = [C.POINTER(MgGrid), i, vp, C.POINTER(vp), C.POINTER(vp), d, d, d, d, d,
+                                  C.POINTER(vp), C.POINTER(vp), vp]
+    lib.pressure_rhs.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, d, vp, vp]
+    lib.project_velocity.argtypes = [C.POINTER(MgGrid), pi, i, vp, vp, d, vp, vp, vp, vp]
+    lib.flow_time_step.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, i, pi, pd]
+    lib.mg_last_error.restype = C.c_char_p
+    lib.mg_version.restype = C.c_char_p
+    return lib
+
+
+_lib = _load()
+
+
+def library_path():
+    return _build.LIB
+
+
+def mg_last_error():
+    return _lib.mg_last_error().decode()
+
+
+def mg_version():
+    return _lib.mg_version().decode()
+
+
+def _check(rc):
+    if rc < 0:
+        raise MgError(rc, mg_last_error())
+    return rc
+
+
+_TORCH_DTYPE = {MG_F32: torch.float32, MG_F64: torch.float64}
+
+
+def _dtype_code(t):
+    return MG_F32 if t.dtype == torch.float32 else MG_F64
+
+
+def _dev(t, shape=None, dtype=None, allow_none=False):
+    """Device pointer of a contiguous CUDA tensor (marshalling checks only)."""
+    if t is None:
+        if allow_none:
+            return None
+        raise ValueError("tensor argument is None")
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError("expected dtype %s, got %s" % (dtype, t.dtype))
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError("expected shape %s, got %s" % (tuple(shape), tuple(t.shape)))
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _grid(nx, ny, nz, hx, hy=None, hz=None):
+    return MgGrid(int(nx), int(ny), int(nz), float(hx), float(hx if hy is None else hy), float(hx if hz is None else hz))
+
+
+class Solver:
+    """Handle returned by mg_create; frees the C object when collected."""
+
+    def __init__(self, handle, grid, levels, bc, dtype, stream):
+        self.handle, self.grid, self.levels, self.bc, self.dtype, self.stream = handle, grid, levels, tuple(bc), dtype, stream
+        self.shape = (grid.nz, grid.ny, grid.nx)
+        self.torch_dtype = _TORCH_DTYPE[dtype]
+
+    def close(self):
+        if self.handle:
+            _lib.mg_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def mg_create(grid, levels, bc, dtype=MG_F32, stream=None):
+    """grid: MgGrid or (nx, ny, nz, hx[, hy, hz]); bc: 6 codes x-,x+,y-,y+,z-,z+."""
+    if not isinstance(grid, MgGrid):
+        grid = _grid(*grid)
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    h = C.c_void_p()
+    bcarr = (C.c_int * 6)(*[int(b) for b in bc])
+    _check(_lib.mg_create(C.byref(h), C.byref(grid), int(levels), bcarr, int(dtype), _stream_ptr(stream)))
+    return Solver(h, grid, levels, bc, dtype, stream)
+
+
+def mg_destroy(s):
+    s.close()
+
+
+def mg_set_params(s, nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=2, omega=2.0 / 3.0, mixed_precision=1):
+    p = MgParams(int(nu_pre), int(nu_post), int(coarse_sweeps), int(sweeps_per_pass), float(omega), int(mixed_precision))
+    return _check(_lib.mg_set_params(s.handle, C.byref(p)))
+
+
+def mg_get_params(s):
+    p = MgParams()
+    _check(_lib.mg_get_params(s.handle, C.byref(p)))
+    return {k: getattr(p, k) for k, _ in MgParams._fields_}
+
+
+def mg_set_fused(s, fused):
+    return _check(_lib.mg_set_fused(s.handle, int(fused)))
+
+
+def mg_set_coefficient(s, k):
+    return _check(_lib.mg_set_coefficient(s.handle, _dev(k, s.shape, s.torch_dtype, allow_none=True)))
+
+
+def mg_set_coefficient_from_vof(s, alpha, rho_l, rho_g):
+    return _check(_lib.mg_set_coefficient_from_vof(s.handle, _dev(alpha, s.shape, s.torch_dtype), float(rho_l), float(rho_g)))
+
+
+def mg_apply_operator(s, x, y):
+    return _check(_lib.mg_apply_operator(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(y, s.shape, s.torch_dtype)))
+
+
+def mg_residual(s, x, b, r):
+    return _check(_lib.mg_residual(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(b, s.shape, s.torch_dtype),
+                                   _dev(r, s.shape, s.torch_dtype)))
+
+
+def mg_smooth(s, x, b, sweeps):
+    return _check(_lib.mg_smooth(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(b, s.shape, s.torch_dtype), int(sweeps)))
+
+
+def mg_vcycle(s, x, b):
+    return _check(_lib.mg_vcycle(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(b, s.shape, s.torch_dtype)))
+
+
+def mg_solve(s, x, b, tol, max_cycles):
+    """Returns (status, cycles, relres)."""
+    cyc, rel = C.c_int(0), C.c_double(0.0)
+    st = _check(_lib.mg_solve(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(b, s.shape, s.torch_dtype), float(tol),
+                              int(max_cycles), C.byref(cyc), C.byref(rel)))
+    return st, cyc.value, rel.value
+
+
+def mg_solve_host(s, x_host, b_host, tol, max_cycles):
+    """x_host, b_host: contiguous CPU tensors (pinned or not).  Returns (status, cycles, relres)."""
+    for t in (x_host, b_host):
+        if t.is_cuda or not t.is_contiguous() or t.dtype != s.torch_dtype or tuple(t.shape) != s.shape:
+            raise ValueError("expected contiguous CPU tensors of the solver's shape and dtype")
+    cyc, rel = C.c_int(0), C.c_double(0.0)
+    st = _check(_lib.mg_solve_host(s.handle, C.c_void_p(x_host.data_ptr()), C.c_void_p(b_host.data_ptr()), float(tol),
+                                   int(max_cycles), C.byref(cyc), C.byref(rel)))
+    return st, cyc.value, rel.value
+
+
+def mg_get_history(s):
+    n = _lib.mg_get_history(s.handle, None, 0)
+    buf = (C.c_double * max(n, 1))()
+    _lib.mg_get_history(s.handle, buf, n)
+    return list(buf[:n])
+
+
+def mg_level_info(s, level):
+    nx, ny, nz = C.c_int(), C.c_int(), C.c_int()
+    n = _lib.mg_level_info(s.handle, int(level), C.byref(nx), C.byref(ny), C.byref(nz))
+    _check(int(n) if n < 0 else 0)
+    return int(n), (nx.value, ny.value, nz.value)
+
+
+def mg_vcycle_timed(s, x, b):
+    """Returns (ms_down[levels], ms_up[levels])."""
+    dn = (C.c_float * s.levels)(); up = (C.c_float * s.levels)()
+    _check(_lib.mg_vcycle_timed(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(b, s.shape, s.torch_dtype), dn, up))
+    return list(dn), list(up)
+
+
+def mg_launch_count(s):
+    return int(_lib.mg_launch_count(s.handle))
+
+
+def _grid_of(t, h):
+    nz, ny, nx = t.shape
+    if isinstance(h, (tuple, list)):
+        return _grid(nx, ny, nz, *h)
+    return _grid(nx, ny, nz, h)
+
+
+def vof_residual(C_, u, v, w, h, dt, sC_out=None, Cnew_out=None, stream=None):
+    g = _grid_of(C_, h)
+    sh, dt_ = tuple(C_.shape), C_.dtype
+    return _check(_lib.vof_residual(C.byref(g), _dtype_code(C_), _dev(C_), _dev(u, sh, dt_), _dev(v, sh, dt_),
+                                    _dev(w, sh, dt_), float(dt), _dev(sC_out, sh, dt_, True), _dev(Cnew_out, sh, dt_, True),
+                                    _stream_ptr(stream)))
+
+
+def _ptr3(ts, sh, dt_, allow_none=False):
+    if ts is None:
+        if allow_none:
+            return None
+        raise ValueError("missing tensor triple")
+    return (C.c_void_p * 3)(*[_dev(t, sh, dt_).value for t in ts])
+
+
+def mom_predictor(C_, qh, qn, h, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn=None, stream=None):
+    g = _grid_of(C_, h)
+    sh, dt_ = tuple(C_.shape), C_.dtype
+    return _check(_lib.mom_predictor(C.byref(g), _dtype_code(C_), _dev(C_), _ptr3(qh, sh, dt_), _ptr3(qn, sh, dt_),
+                                     float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt),
+                                     _ptr3(qt, sh, dt_), _ptr3(qhn, sh, dt_, True), _stream_ptr(stream)))
+
+
+def pressure_rhs(u, v, w, h, dt, b, stream=None):
+    g = _grid_of(u, h)
+    sh, dt_ = tuple(u.shape), u.dtype
+    return _check(_lib.pressure_rhs(C.byref(g), _dtype_code(u), _dev(u), _dev(v, sh, dt_), _dev(w, sh, dt_), float(dt),
+                                    _dev(b, sh, dt_), _stream_ptr(stream)))
+
+
+def project_velocity(p, k, h, bc, dt, u, v, w, stream=None):
+    g = _grid_of(p, h)
+    sh, dt_ = tuple(p.shape), p.dtype
+    bcarr = (C.c_int * 6)(*[int(b) for b in bc])
+    return _check(_lib.project_velocity(C.byref(g), bcarr, _dtype_code(p), _dev(p), _dev(k, sh, dt_), float(dt),
+                                        _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_), _stream_ptr(stream)))
+
+
+def flow_time_step(s, C_, u, v, w, p, rho_l, rho_g, mu_l, mu_g, dt, tol, max_cycles):
+    """Returns (status, cycles, relres)."""
+    cyc, rel = C.c_int(0), C.c_double(0.0)
+    sh, dt_ = s.shape, s.torch_dtype
+    st = _check(_lib.flow_time_step(s.handle, _dev(C_, sh, dt_), _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_),
+                                    _dev(p, sh, dt_), float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt),
+                                    float(tol), int(max_cycles), C.byref(cyc), C.byref(rel)))
+    return st, cyc.value, rel.value

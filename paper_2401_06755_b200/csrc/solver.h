@@ -1,0 +1,54 @@
+// solver.h -- the mg_solver object behind the C ABI of include/mg.h (product code).
+#pragma once
+#include <vector>
+
+#include "../../include/mg.h"
+#include "common.cuh"
+
+namespace mgb {
+
+struct LevelData {
+    int nx = 0, ny = 0, nz = 0;
+    double hx = 0, hy = 0, hz = 0;
+    size_t n = 0;
+    bool uniform = false;
+    // device buffers of the solver's dtype.  Level 0: x and b are the caller's (set per call);
+    // k (NULL while the coefficient is constant) and tmp are the solver's.  Levels >= 1: all owned.
+    void *x = nullptr, *b = nullptr, *k = nullptr, *tmp = nullptr;
+    Level<float> Lf;
+    Level<double> Ld;
+};
+
+}  // namespace mgb
+
+struct mg_solver {
+    mg_grid grid{};
+    int levels = 0;
+    int bc[6] = {0, 0, 0, 0, 0, 0};
+    int dtype = MG_F32;
+    int device = 0;
+    cudaStream_t st = nullptr;
+    mg_params p{2, 2, 50, 2, 2.0 / 3.0, 1};
+    bool var_k = false;
+    int fused = 1;
+    std::vector<mgb::LevelData> lv;
+    // mixed-precision outer loop (MG_F32 only): fp64 iterate and fine coefficient, fp32 residual / correction
+    double* x64 = nullptr;
+    double* k64 = nullptr;
+    float* r32 = nullptr;
+    float* e32 = nullptr;
+    // host-buffer entry points
+    void* hx_dev = nullptr;
+    void* hb_dev = nullptr;
+    // norms
+    double* d_acc = nullptr;
+    double* h_acc = nullptr;  // pinned
+    std::vector<double> history;
+    long long launches = 0;
+    // CUDA-graph replay of the fused V-cycle, keyed by the (x, b) pointers it was captured with
+    cudaGraphExec_t graph_exec = nullptr;
+    const void* graph_x = nullptr;
+    const void* graph_b = nullptr;
+    long long graph_launches = 0;  // kernels inside one replay
+    void* fused_state = nullptr;   // owned by mg_fused.cu
+};

@@ -1,0 +1,123 @@
+"""GPU parity of the explicit stencil residuals (a8-a10) and of the config-5 time step against
+the fp64 CPU oracle, through the C ABI.  Tolerances: relative L2 <= 1e-5 (fp32) / 1e-12 (fp64)
+per kernel pass, as for the sweeps (BASELINE.json)."""
+import numpy as np
+import pytest
+
+from workloads import configs, rng
+from test_gpu_mg import TOL, as_f64, mg, quantise, rel_l2, to_dev  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+N, D, H0 = configs.BC_NEUMANN, configs.BC_DIRICHLET, configs.BC_DIRICHLET_HALO
+
+
+def flow_fields(n, dt, solenoidal=True):
+    """Water-column alpha and a divergence-free velocity, the structure of config 5, at n^3."""
+    w = configs.config5(n, 3)
+    f = w.fields
+    if not solenoidal:
+        f["u"], f["v"], f["w"] = configs.random_velocity((71, 72, 73), w.shape)
+    return w, tuple(quantise(f[q], dt) for q in ("alpha", "u", "v", "w"))
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("shape,h", [((24, 24, 24), 1.0 / 24), ((10, 36, 68), 1.0 / 68), ((40, 40, 40), (0.02, 0.025, 0.03))])
+def test_vof_residual_parity(mg, orc, shape, h, dt):
+    import torch
+    nz, ny, nx = shape
+    hh = h if isinstance(h, tuple) else (h, h, h)
+    g = orc.grid(nx, ny, nz, *hh)
+    # a smeared interface crossing the box obliquely, so every branch (override, w+, w-, clips) is taken
+    x, y, z = configs.centres(nx, ny, nz, 1.0)
+    d = (0.6 * x / nx + 0.5 * y / ny + 0.62 * z / nz) - 0.8
+    Cf = quantise(0.5 * (1 + np.tanh(d * 6.0)) + 0.0 * (x + y + z), dt)
+    n = Cf.size
+    u, v, w = (quantise(0.3 * rng.normal(40 + c, n).reshape(shape) + 0.5, dt) for c in range(3))
+    tstep = 0.1 * min(hh)
+    s_ref, c_ref = orc.vof_residual(g, Cf, u, v, w, tstep)
+    dC, du, dv, dw = (to_dev(a, dt) for a in (Cf, u, v, w))
+    ds, dc = torch.empty_like(dC), torch.empty_like(dC)
+    mg.vof_residual(dC, du, dv, dw, hh, tstep, ds, dc)
+    assert rel_l2(as_f64(ds), s_ref) <= 5 * TOL[dt]     # 3 chained passes (adv -> coefficients -> diffusion)
+    assert rel_l2(as_f64(dc), c_ref) <= TOL[dt]
+    # outputs are optional one at a time
+    dc2 = torch.empty_like(dC)
+    mg.vof_residual(dC, du, dv, dw, hh, tstep, None, dc2)
+    assert torch.equal(dc, dc2)
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_vof_trivial_inputs(mg, dt):
+    import torch
+    tdt = torch.float32 if dt == "f32" else torch.float64
+    C_ = torch.full((16, 16, 16), 0.5, device="cuda", dtype=tdt)
+    q = torch.ones_like(C_)
+    s = torch.empty_like(C_)
+    mg.vof_residual(C_, q, q, q, 1.0 / 16, 0.01, s, None)
+    assert float(s.abs().max()) == 0.0                      # uniform C: residual vanishes
+    Cg = torch.rand(16, 16, 16, device="cuda", dtype=tdt)
+    z = torch.zeros_like(Cg)
+    mg.vof_residual(Cg, z, z, z, 1.0 / 16, 0.01, s, None)
+    assert float(s.abs().max()) == 0.0                      # q = 0: no advection, k_abs = k- = 0
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("n", [24, 40])
+def test_momentum_rhs_projection_parity(mg, orc, n, dt):
+    import torch
+    w, (alpha, u, v, ww) = flow_fields(n, dt)
+    g = orc.grid(n, n, n, w.h)
+    bc = w.bc
+    # momentum predictor, both outputs, half-level velocity different from level n
+    qn = (u, v, ww)
+    qh = tuple(quantise(0.9 * a + 0.05, dt) for a in qn)
+    qt_ref, qhn_ref = orc.mom_predictor(g, alpha, qh, qn, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
+    dC = to_dev(alpha, dt)
+    dqn = [to_dev(a, dt) for a in qn]; dqh = [to_dev(a, dt) for a in qh]
+    dqt = [torch.empty_like(dC) for _ in range(3)]; dqhn = [torch.empty_like(dC) for _ in range(3)]
+    mg.mom_predictor(dC, dqh, dqn, w.h, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, dqt, dqhn)
+    for c in range(3):
+        assert rel_l2(as_f64(dqt[c]), qt_ref[c]) <= TOL[dt]
+        assert rel_l2(as_f64(dqhn[c]), qhn_ref[c]) <= TOL[dt]
+    # pressure RHS
+    b_ref = orc.pressure_rhs(g, u, v, ww, w.dt)
+    db = torch.empty_like(dC)
+    mg.pressure_rhs(dqn[0], dqn[1], dqn[2], w.h, w.dt, db)
+    assert rel_l2(as_f64(db), b_ref) <= TOL[dt] * (50 if dt == "f32" else 1e3)   # divergence of a solenoidal field: cancellation
+    ur, vr, wr = (quantise(rng.normal(90 + c, alpha.size).reshape(alpha.shape), dt) for c in range(3))
+    b_ref = orc.pressure_rhs(g, ur, vr, wr, w.dt)
+    mg.pressure_rhs(to_dev(ur, dt), to_dev(vr, dt), to_dev(wr, dt), w.h, w.dt, db)
+    assert rel_l2(as_f64(db), b_ref) <= TOL[dt]
+    # projection with the solver's BC factors on p
+    p = quantise(rng.normal(95, alpha.size).reshape(alpha.shape), dt)
+    k = quantise(orc.k_from_vof(alpha, w.rho_l, w.rho_g), dt)
+    for bcs in (bc, (D, N, H0, D, N, H0)):
+        u_ref, v_ref, w_ref = orc.project_velocity(g, bcs, p, k, w.dt, u, v, ww)
+        du, dv, dw = to_dev(u, dt), to_dev(v, dt), to_dev(ww, dt)
+        mg.project_velocity(to_dev(p, dt), to_dev(k, dt), w.h, bcs, w.dt, du, dv, dw)
+        for a, r in ((du, u_ref), (dv, v_ref), (dw, w_ref)):
+            assert rel_l2(as_f64(a), r) <= TOL[dt]
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_time_step_parity(mg, orc, dt):
+    """Config 5 at reduced size (32^3, 4 levels): two full time steps against the oracle."""
+    n, levels = 32, 4
+    w = configs.config5(n, levels)
+    g = orc.grid(n, n, n, w.h)
+    Cf, u, v, ww = (quantise(w.fields[q], dt) for q in ("alpha", "u", "v", "w"))
+    s = mg.mg_create((n, n, n, w.h), levels, w.bc, mg.MG_F32 if dt == "f32" else mg.MG_F64)
+    dC, du, dv, dw = (to_dev(a, dt) for a in (Cf, u, v, ww))
+    import torch
+    dp = torch.empty_like(dC)
+    tol = 1e-9    # both sides driven well below config 5's 1e-6 so the comparison is of converged pressures
+    for step in range(2):
+        Cf, u, v, ww, p, cyc_o, rel_o = orc.time_step(g, w.bc, Cf, u, v, ww, levels, w.rho_l, w.rho_g, w.mu_l, w.mu_g,
+                                                      w.dt, tol, 200)
+        status, cyc, rel = mg.flow_time_step(s, dC, du, dv, dw, dp, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, tol, 200)
+        assert status == mg.MG_OK and rel < tol and abs(cyc - cyc_o) <= 2
+        lim = (step + 1) * (2e-5 if dt == "f32" else 1e-7)
+        assert rel_l2(as_f64(dp), p) <= lim * 5
+        for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
+            assert rel_l2(as_f64(a), r) <= lim
+    mg.mg_destroy(s)

@@ -1,0 +1,294 @@
+"""GPU parity: libmg_b200 (through the C ABI) against the fp64 CPU oracle, element by element
+on the same seeded inputs.  Tolerances are BASELINE.json's: per-sweep relative L2 <= 1e-5 (fp32),
+<= 1e-12 (fp64); converged solutions within 1e-6 relative L2 of the oracle's."""
+import numpy as np
+import pytest
+
+from workloads import configs, rng
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f32": 1e-5, "f64": 1e-12}
+N, D, H0 = configs.BC_NEUMANN, configs.BC_DIRICHLET, configs.BC_DIRICHLET_HALO
+BC_MIXES = [(D,) * 6, (N, N, N, N, N, D), (H0,) * 6, (N, D, H0, N, D, H0), (N,) * 6]
+
+
+@pytest.fixture(scope="module")
+def mg():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    import paper_2401_06755_b200 as m
+    return m
+
+
+def rel_l2(a, ref):
+    a = np.asarray(a, dtype=np.float64); ref = np.asarray(ref, dtype=np.float64)
+    return float(np.linalg.norm((a - ref).ravel()) / max(np.linalg.norm(ref.ravel()), 1e-300))
+
+
+def to_dev(a, dt):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).to(torch.float32 if dt == "f32" else torch.float64).cuda()
+
+
+def as_f64(t):
+    return t.detach().cpu().double().numpy()
+
+
+def quantise(a, dt):
+    """Round the fp64 input to the run precision so both sides see the very same numbers."""
+    return np.ascontiguousarray(a, dtype=np.float32).astype(np.float64) if dt == "f32" else np.ascontiguousarray(a)
+
+
+def make_problem(shape, dt, var, seed):
+    n = int(np.prod(shape))
+    x = quantise(rng.normal(seed, n).reshape(shape), dt)
+    b = quantise(rng.uniform(seed + 1, n).reshape(shape), dt)
+    k = None
+    if var:  # strong contrast, like 1/rho with rho in [1, 1000]
+        k = quantise(np.exp(-6.9 * rng.uniform01(seed + 2, n)).reshape(shape), dt)
+    return x, b, k
+
+
+def make_solver(mg, shape, h, levels, bc, dt, k=None, fused=1, **params):
+    nz, ny, nx = shape
+    hh = h if isinstance(h, tuple) else (h, h, h)
+    s = mg.mg_create((nx, ny, nz, *hh), levels, bc, mg.MG_F32 if dt == "f32" else mg.MG_F64)
+    if params:
+        p = dict(nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=2, omega=2.0 / 3.0, mixed_precision=1)
+        p.update(params)
+        mg.mg_set_params(s, **p)
+    mg.mg_set_fused(s, fused)
+    if k is not None:
+        mg.mg_set_coefficient(s, to_dev(k, dt))
+    return s
+
+
+SHAPES = [((32, 32, 32), 1.0 / 32), ((8, 24, 40), 1.0 / 40), ((70, 36, 132), 0.01), ((4, 4, 4), 0.25)]
+
+
+@pytest.mark.parametrize("fused", [0, 1])
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("var", [False, True])
+@pytest.mark.parametrize("bc", BC_MIXES)
+@pytest.mark.parametrize("shape,h", SHAPES)
+def test_operator_residual_and_sweeps(mg, orc, shape, h, bc, var, dt, fused):
+    import torch
+    nz, ny, nx = shape
+    g = orc.grid(nx, ny, nz, h)
+    x, b, k = make_problem(shape, dt, var, 11)
+    s = make_solver(mg, shape, h, 1, bc, dt, k, fused)
+    dx, db = to_dev(x, dt), to_dev(b, dt)
+    dy = torch.empty_like(dx)
+    mg.mg_apply_operator(s, dx, dy)
+    assert rel_l2(as_f64(dy), orc.apply_operator(g, bc, k, x)) <= TOL[dt]
+    mg.mg_residual(s, dx, db, dy)
+    assert rel_l2(as_f64(dy), orc.residual(g, bc, k, x, b)) <= TOL[dt]
+    # per-sweep parity, every sweep restarted from the oracle's iterate
+    xo = x
+    for sweep in range(3):
+        dxs = to_dev(xo, dt)
+        mg.mg_smooth(s, dxs, db, 1)
+        xo_next = orc.jacobi_sweep(g, bc, k, quantise(xo, dt), b, 2.0 / 3.0)
+        assert rel_l2(as_f64(dxs), xo_next) <= TOL[dt], "sweep %d" % sweep
+        xo = xo_next
+    # several sweeps in one call (temporal fusion inside the library must not change the result)
+    for sweeps in (2, 3, 4, 5):
+        dxs = to_dev(x, dt)
+        mg.mg_smooth(s, dxs, db, sweeps)
+        assert rel_l2(as_f64(dxs), orc.smooth(g, bc, k, x, b, 2.0 / 3.0, sweeps)) <= sweeps * TOL[dt]
+    mg.mg_destroy(s)
+
+
+def test_anisotropic_spacing(mg, orc):
+    """hx != hy != hz: all 27 weights differ and some off-diagonals are positive.
+    The coefficient contrast is kept mild so that the Jacobi diagonal stays well away from 0
+    (with positive off-diagonals and a random 1000:1 k it does not, and the sweep is ill-posed)."""
+    import torch
+    shape, bc, hh = (12, 20, 16), (N, D, H0, N, D, N), (0.1, 0.08, 0.125)
+    g = orc.grid(16, 20, 12, *hh)
+    for dt in ("f32", "f64"):
+        x, b, _ = make_problem(shape, dt, False, 21)
+        k = quantise(np.exp(-rng.uniform01(23, x.size)).reshape(shape), dt)
+        diag = orc.diagonal(g, k)
+        assert diag.min() > 0.2 * diag.max()
+        s = make_solver(mg, shape, hh, 2, bc, dt, k)
+        dx, db = to_dev(x, dt), to_dev(b, dt)
+        dy = torch.empty_like(dx)
+        mg.mg_apply_operator(s, dx, dy)
+        assert rel_l2(as_f64(dy), orc.apply_operator(g, bc, k, x)) <= TOL[dt]
+        mg.mg_smooth(s, dx, db, 2)
+        assert rel_l2(as_f64(dx), orc.smooth(g, bc, k, x, b, 2.0 / 3.0, 2)) <= 2 * TOL[dt]
+        dx = to_dev(x, dt)
+        mg.mg_vcycle(s, dx, db)
+        assert rel_l2(as_f64(dx), orc.vcycle(g, bc, k, x, b, 2)) <= 10 * TOL[dt]
+        mg.mg_destroy(s)
+
+
+@pytest.mark.parametrize("fused", [0, 1])
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("var", [False, True])
+@pytest.mark.parametrize("shape,h,levels,bc,nu", [
+    ((32, 32, 32), 1.0 / 32, 4, (D,) * 6, (2, 2)),
+    ((32, 32, 32), 1.0 / 32, 4, (N, N, N, N, N, D), (2, 2)),
+    ((16, 48, 80), 1.0 / 80, 3, (N, D, H0, N, N, D), (1, 3)),
+    ((64, 64, 64), 1.0 / 64, 5, (N, N, N, N, N, D), (2, 2)),
+    ((64, 32, 96), 1.0 / 96, 4, (D, N, N, D, H0, D), (3, 1)),
+    ((32, 32, 32), 1.0 / 32, 3, (D,) * 6, (0, 2)),
+    ((8, 8, 8), 1.0 / 8, 2, (N, N, N, N, N, D), (2, 2)),
+])
+def test_vcycle_parity(mg, orc, shape, h, levels, bc, nu, var, dt, fused):
+    nz, ny, nx = shape
+    g = orc.grid(nx, ny, nz, h)
+    x, b, k = make_problem(shape, dt, var, 31)
+    s = make_solver(mg, shape, h, levels, bc, dt, k, fused, nu_pre=nu[0], nu_post=nu[1], coarse_sweeps=50)
+    dx, db = to_dev(x, dt), to_dev(b, dt)
+    xo = x
+    for cycle in range(2):
+        mg.mg_vcycle(s, dx, db)
+        xo = orc.vcycle(g, bc, k, xo, b, levels, nu[0], nu[1], 50, 2.0 / 3.0)
+        # growth allowance: a cycle is ~ (nu1 + nu2 + transfers) sweeps per level
+        assert rel_l2(as_f64(dx), xo) <= 10 * (cycle + 1) * TOL[dt], "cycle %d" % cycle
+    mg.mg_destroy(s)
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_config1_solve(mg, orc, dt):
+    """BASELINE config 1: 32^3, constant coefficient, zero Dirichlet, 4 levels, V(2,2), tol 1e-8."""
+    w = configs.config1()
+    g = orc.grid(w.nx, w.ny, w.nz, w.h)
+    b = quantise(w.fields["b"], dt)
+    x_ref, n_ref, rel_ref, _ = orc.solve(g, w.bc, None, np.zeros(w.shape), b, w.levels, 1e-12, 100)
+    assert rel_ref < 1e-12
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, dt)
+    dx, db = to_dev(np.zeros(w.shape), dt), to_dev(b, dt)
+    status, cycles, rel = mg.mg_solve(s, dx, db, w.tol, 100)
+    assert status == mg.MG_OK and rel < w.tol
+    hist = mg.mg_get_history(s)
+    assert len(hist) == cycles and all(hist[i + 1] < hist[i] for i in range(len(hist) - 1))
+    # the oracle needs the same number of cycles to reach the same tolerance
+    _, n_tol, _, hist_o = orc.solve(g, w.bc, None, np.zeros(w.shape), b, w.levels, w.tol, 100)
+    assert abs(cycles - n_tol) <= 1
+    assert rel_l2(as_f64(dx), x_ref) <= 1e-6
+    # residual of the GPU solution, evaluated by the oracle
+    r = orc.residual(g, w.bc, None, as_f64(dx), b)
+    assert np.linalg.norm(r) / np.linalg.norm(b) < (2e-7 if dt == "f32" else 1e-8)
+    mg.mg_destroy(s)
+
+
+def test_pure_fp32_solve_stagnates_cleanly(mg, orc):
+    w = configs.config1()
+    b = quantise(w.fields["b"], "f32")
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32", mixed_precision=0)
+    dx, db = to_dev(np.zeros(w.shape), "f32"), to_dev(b, "f32")
+    status, cycles, rel = mg.mg_solve(s, dx, db, 1e-10, 60)
+    assert status in (mg.MG_STAGNATED, mg.MG_NOT_CONVERGED) and rel < 1e-5 and cycles <= 60
+    mg.mg_destroy(s)
+
+
+def test_sawtooth_nu0_reports_instead_of_looping(mg):
+    w = configs.config1()
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32", nu_pre=0, nu_post=1)
+    dx, db = to_dev(np.zeros(w.shape), "f32"), to_dev(w.fields["b"], "f32")
+    status, cycles, rel = mg.mg_solve(s, dx, db, 1e-8, 30)
+    assert status in (mg.MG_OK, mg.MG_STAGNATED, mg.MG_NOT_CONVERGED) and cycles <= 30
+    mg.mg_destroy(s)
+
+
+def _config2_problem(orc, n, levels):
+    w = configs.config2(n, levels)
+    g = orc.grid(w.nx, w.ny, w.nz, w.h)
+    alpha = quantise(w.fields["alpha"], "f32")
+    b = quantise(orc.pressure_rhs(g, w.fields["u"], w.fields["v"], w.fields["w"], 1.0), "f32")
+    return w, g, alpha, b
+
+
+def test_config2_reduced_converged_solution(mg, orc):
+    """Water column at 64^3 (5 levels): converged GPU solution within 1e-6 of the oracle's."""
+    w, g, alpha, b = _config2_problem(orc, 64, 5)
+    k = orc.k_from_vof(alpha, w.rho_l, w.rho_g)
+    x_ref, _, rel_ref, _ = orc.solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, 1e-12, 200)
+    assert rel_ref < 1e-12
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32")
+    mg.mg_set_coefficient_from_vof(s, to_dev(alpha, "f32"), w.rho_l, w.rho_g)
+    dx, db = to_dev(np.zeros(w.shape), "f32"), to_dev(b, "f32")
+    status, cycles, rel = mg.mg_solve(s, dx, db, 1e-9, 200)   # driven below tol: error/residual amplification ~65 (C6-iii)
+    assert status == mg.MG_OK, (status, cycles, rel)
+    assert rel_l2(as_f64(dx), x_ref) <= 1e-6
+    mg.mg_destroy(s)
+
+
+def test_config2_full_size(mg, orc):
+    """BASELINE config 2 at 128^3, 6 levels: solve to 1e-7, cycle count and per-cycle history
+    against the oracle, and the residual of the GPU solution evaluated by the oracle."""
+    w, g, alpha, b = _config2_problem(orc, 128, 6)
+    k = orc.k_from_vof(alpha, w.rho_l, w.rho_g)
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32")
+    mg.mg_set_coefficient_from_vof(s, to_dev(alpha, "f32"), w.rho_l, w.rho_g)
+    dx, db = to_dev(np.zeros(w.shape), "f32"), to_dev(b, "f32")
+    status, cycles, rel = mg.mg_solve(s, dx, db, w.tol, 100)
+    assert status == mg.MG_OK and rel < w.tol
+    x_o, n_o, rel_o, hist_o = orc.solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, w.tol, 100)
+    hist = mg.mg_get_history(s)
+    assert abs(cycles - n_o) <= 1
+    m = min(len(hist), len(hist_o))
+    assert np.allclose(hist[:m], hist_o[:m], rtol=2e-2)
+    r = orc.residual(g, w.bc, k, as_f64(dx), b)
+    assert np.linalg.norm(r) / np.linalg.norm(b) < 2 * w.tol
+    # both stopped at the same residual level: solutions agree to the error/residual amplification
+    assert rel_l2(as_f64(dx), x_o) < 1e-4
+    mg.mg_destroy(s)
+
+
+def test_config3_full_size_cycle_parity(mg, orc):
+    """BASELINE config 3 (256^3 bubble, 7 levels), the launch configuration bench.py times:
+    one fused fp32 V-cycle against the oracle's, element by element."""
+    w = configs.config3()
+    g = orc.grid(w.nx, w.ny, w.nz, w.h)
+    alpha = quantise(w.fields["alpha"], "f32")
+    b = quantise(orc.pressure_rhs(g, w.fields["u"], w.fields["v"], w.fields["w"], 1.0), "f32")
+    k = orc.k_from_vof(alpha, w.rho_l, w.rho_g)
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32")
+    mg.mg_set_coefficient_from_vof(s, to_dev(alpha, "f32"), w.rho_l, w.rho_g)
+    dx, db = to_dev(np.zeros(w.shape), "f32"), to_dev(b, "f32")
+    mg.mg_vcycle(s, dx, db)
+    x_o = orc.vcycle(g, w.bc, k, np.zeros(w.shape), b, w.levels)
+    assert rel_l2(as_f64(dx), x_o) <= 1e-4
+    mg.mg_destroy(s)
+
+
+def test_argument_errors(mg):
+    import torch
+    with pytest.raises(mg.MgError) as e:
+        mg.mg_create((30, 32, 32, 0.1), 3, (N,) * 6)
+    assert e.value.code == mg.MG_ESHAPE
+    with pytest.raises(mg.MgError) as e:
+        mg.mg_create((32, 32, 32, 0.1), 6, (N,) * 6)       # coarsest dimension would be 1
+    assert e.value.code == mg.MG_ESHAPE
+    with pytest.raises(mg.MgError) as e:
+        mg.mg_create((32, 32, 32, 0.1), 2, (N, N, N, N, N, 7))
+    assert e.value.code == mg.MG_EINVAL
+    s = mg.mg_create((32, 32, 32, 0.1), 2, (D,) * 6)
+    x = torch.zeros(32, 32, 32, device="cuda")
+    with pytest.raises(mg.MgError):
+        mg.mg_apply_operator(s, x, x)                        # aliased
+    with pytest.raises(ValueError):
+        mg.mg_apply_operator(s, x, torch.zeros(16, 32, 32, device="cuda"))
+    with pytest.raises(mg.MgError):
+        mg.mg_set_params(s, omega=-1.0)
+    mg.mg_destroy(s)
+
+
+def test_empty_cycles_and_zero_rhs(mg):
+    import torch
+    s = mg.mg_create((16, 16, 16, 1.0 / 16), 3, (D,) * 6)
+    x = torch.zeros(16, 16, 16, device="cuda"); b = torch.zeros_like(x)
+    status, cycles, rel = mg.mg_solve(s, x, b, 1e-8, 10)       # b = 0: converged at once, x stays 0
+    assert status == mg.MG_OK and cycles == 0 and float(x.abs().max()) == 0.0
+    b.fill_(1.0)
+    status, cycles, rel = mg.mg_solve(s, x, b, 1e-8, 0)        # max_cycles = 0
+    assert status == mg.MG_NOT_CONVERGED and cycles == 0
+    mg.mg_smooth(s, x, b, 0)
+    assert float(x.abs().max()) == 0.0
+    mg.mg_destroy(s)
