@@ -8,6 +8,5 @@ bool fused_supported(const mg_solver* s);
 int fused_apply(mg_solver* s, const float* x, float* y);
 int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps);
 int fused_vcycle(mg_solver* s, float* x, const float* b);
-int fused_vcycle_timed(mg_solver* s, float* x, const float* b, float* ms_down, float* ms_up);
 void fused_release(mg_solver* s);
 }  // namespace mgb

@@ -78,10 +78,21 @@ static int smooth_level(mg_solver* s, int l, T* x, const T* b, int sweeps) {
     return 0;
 }
 
+// Optional per-level instrumentation (mg_vcycle_timed): ev[l] at the start of level l's down leg,
+// ev[levels] after the coarsest solve, ev[levels + 1 + (levels - 2 - l)] after level l's up leg.
+static inline void mark(mg_solver* s, int idx) {
+    if (s->timing) cudaEventRecord(s->ev[idx], s->st);
+}
+
 template <typename T>
 static int vcycle_unfused(mg_solver* s, int l, T* x, const T* b) {
     LevelData& L = s->lv[l];
-    if (l == s->levels - 1) return smooth_level<T>(s, l, x, b, s->p.coarse_sweeps);
+    mark(s, l);
+    if (l == s->levels - 1) {
+        int rc0 = smooth_level<T>(s, l, x, b, s->p.coarse_sweeps);
+        mark(s, s->levels);
+        return rc0;
+    }
     LevelData& C = s->lv[l + 1];
     int rc;
     if ((rc = smooth_level<T>(s, l, x, b, s->p.nu_pre))) return rc;
@@ -92,7 +103,9 @@ static int vcycle_unfused(mg_solver* s, int l, T* x, const T* b) {
     if ((rc = vcycle_unfused<T>(s, l + 1, (T*)C.x, (const T*)C.b))) return rc;
     if ((rc = launch_prolong_add<T>(L.nx, L.ny, L.nz, (const T*)C.x, x, s->st))) return rc;
     ++s->launches;
-    return smooth_level<T>(s, l, x, b, s->p.nu_post);
+    rc = smooth_level<T>(s, l, x, b, s->p.nu_post);
+    mark(s, s->levels + 1 + (s->levels - 2 - l));
+    return rc;
 }
 
 template <typename T>
@@ -144,6 +157,7 @@ struct Stop {
     int update(double rel) {
         if (!std::isfinite(rel)) return MG_STAGNATED;
         if (rel < tol) return MG_OK;
+        if (tol == 0.0) return -1;  // fixed cycle count (the paper's mode): no stagnation test
         stag = (rel > 0.95 * prev) ? stag + 1 : 0;
         prev = rel;
         return stag >= 3 ? MG_STAGNATED : -1;
@@ -319,6 +333,7 @@ void mg_destroy(mg_solver* s) {
     cudaStreamSynchronize(s->st);
     invalidate_graph(s);
     fused_release(s);
+    for (auto& e : s->ev) cudaEventDestroy(e);
     for (size_t l = 0; l < s->lv.size(); ++l) {
         LevelData& L = s->lv[l];
         if (l > 0) { cudaFree(L.x); cudaFree(L.b); }
@@ -488,10 +503,24 @@ long long mg_launch_count(const mg_solver* s) { return s ? s->launches : 0; }
 int mg_vcycle_timed(mg_solver* s, void* d_x, const void* d_b, float* h_ms_down, float* h_ms_up) {
     CHECK_SOLVER(s);
     if (!d_x || !d_b || !h_ms_down || !h_ms_up) { set_error("mg_vcycle_timed: NULL argument"); return MG_EINVAL; }
-    if (s->dtype == MG_F32 && s->fused && fused_supported(s))
-        return fused_vcycle_timed(s, (float*)d_x, (const float*)d_b, h_ms_down, h_ms_up);
-    set_error("mg_vcycle_timed: only the fused fp32 path is instrumented");
-    return MG_EINVAL;
+    const int L = s->levels;
+    if (s->ev.empty()) {
+        s->ev.resize(2 * L);
+        for (auto& e : s->ev) MGB_CUDA(cudaEventCreate(&e));
+    }
+    s->timing = true;
+    int rc = (s->dtype == MG_F32) ? vcycle_any<float>(s, (float*)d_x, (const float*)d_b)
+                                  : vcycle_any<double>(s, (double*)d_x, (const double*)d_b);
+    s->timing = false;
+    if (rc) return rc;
+    MGB_CUDA(cudaStreamSynchronize(s->st));
+    for (int l = 0; l < L; ++l) { h_ms_down[l] = 0.f; h_ms_up[l] = 0.f; }
+    for (int l = 0; l < L; ++l) MGB_CUDA(cudaEventElapsedTime(&h_ms_down[l], s->ev[l], s->ev[l + 1]));
+    for (int l = L - 2; l >= 0; --l) {
+        const int e = L + 1 + (L - 2 - l);
+        MGB_CUDA(cudaEventElapsedTime(&h_ms_up[l], s->ev[e - 1], s->ev[e]));
+    }
+    return MG_OK;
 }
 
 }  // extern "C"

@@ -45,6 +45,9 @@ struct mg_solver {
     double* h_acc = nullptr;  // pinned
     std::vector<double> history;
     long long launches = 0;
+    // per-level instrumentation of mg_vcycle_timed
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;
     // CUDA-graph replay of the fused V-cycle, keyed by the (x, b) pointers it was captured with
     cudaGraphExec_t graph_exec = nullptr;
     const void* graph_x = nullptr;

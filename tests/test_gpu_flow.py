@@ -54,7 +54,7 @@ def test_vof_trivial_inputs(mg, dt):
     q = torch.ones_like(C_)
     s = torch.empty_like(C_)
     mg.vof_residual(C_, q, q, q, 1.0 / 16, 0.01, s, None)
-    assert float(s.abs().max()) == 0.0                      # uniform C: residual vanishes
+    assert float(s.abs().max()) <= 1e-5 * 16                # uniform C: residual vanishes (to rounding of |q| C / h)
     Cg = torch.rand(16, 16, 16, device="cuda", dtype=tdt)
     z = torch.zeros_like(Cg)
     mg.vof_residual(Cg, z, z, z, 1.0 / 16, 0.01, s, None)
