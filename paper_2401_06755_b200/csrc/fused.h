@@ -3,9 +3,10 @@
 struct mg_solver;
 
 namespace mgb {
-// true when the solver's grid / dtype / parameters are covered by the tuned kernels
+// true when the solver's grid / dtype are covered by the tuned kernels
 bool fused_supported(const mg_solver* s);
-int fused_apply(mg_solver* s, const float* x, float* y);
+// (re)build the per-level data the tuned path derives from the coefficient (1/D of the coarse levels)
+int fused_prepare(mg_solver* s);
 int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps);
 int fused_vcycle(mg_solver* s, float* x, const float* b);
 void fused_release(mg_solver* s);

@@ -333,6 +333,7 @@ void mg_destroy(mg_solver* s) {
     cudaStreamSynchronize(s->st);
     invalidate_graph(s);
     fused_release(s);
+    if (s->cap_st) cudaStreamDestroy(s->cap_st);
     for (auto& e : s->ev) cudaEventDestroy(e);
     for (size_t l = 0; l < s->lv.size(); ++l) {
         LevelData& L = s->lv[l];
@@ -378,7 +379,7 @@ int mg_set_coefficient(mg_solver* s, const void* d_k) {
     if (!d_k) {
         for (auto& L : s->lv) { cudaFree(L.k); L.k = nullptr; }
         s->var_k = false;
-        return MG_OK;
+        return (s->dtype == MG_F32 && fused_supported(s)) ? fused_prepare(s) : MG_OK;
     }
     int rc = alloc_k(s);
     if (rc) return rc;
@@ -389,7 +390,8 @@ int mg_set_coefficient(mg_solver* s, const void* d_k) {
         if ((rc = ensure_mixed_buffers(s))) return rc;
         if ((rc = launch_cast_f2d(n, (const float*)d_k, s->k64, s->st))) return rc;
         ++s->launches;
-        return coarsen_coefficient<float>(s);
+        if ((rc = coarsen_coefficient<float>(s))) return rc;
+        return fused_supported(s) ? fused_prepare(s) : MG_OK;
     }
     return coarsen_coefficient<double>(s);
 }
@@ -407,7 +409,8 @@ int mg_set_coefficient_from_vof(mg_solver* s, const void* d_alpha, double rho_l,
         if ((rc = launch_k_from_vof<float>(n, (const float*)d_alpha, rho_l, rho_g, (float*)s->lv[0].k, s->st))) return rc;
         if ((rc = launch_k64_from_vof(n, (const float*)d_alpha, rho_l, rho_g, s->k64, s->st))) return rc;
         s->launches += 2;
-        return coarsen_coefficient<float>(s);
+        if ((rc = coarsen_coefficient<float>(s))) return rc;
+        return fused_supported(s) ? fused_prepare(s) : MG_OK;
     }
     if ((rc = launch_k_from_vof<double>(n, (const double*)d_alpha, rho_l, rho_g, (double*)s->lv[0].k, s->st))) return rc;
     ++s->launches;
@@ -419,10 +422,7 @@ int mg_apply_operator(mg_solver* s, const void* d_x, void* d_y) {
     if (!d_x || !d_y || d_x == d_y) { set_error("mg_apply_operator: NULL or aliased argument"); return MG_EINVAL; }
     LevelData& L = s->lv[0];
     ++s->launches;
-    if (s->dtype == MG_F32) {
-        if (s->fused && fused_supported(s)) return fused_apply(s, (const float*)d_x, (float*)d_y);
-        return launch_apply<float>(L.Lf, (const float*)L.k, (const float*)d_x, (float*)d_y, s->st);
-    }
+    if (s->dtype == MG_F32) return launch_apply<float>(L.Lf, (const float*)L.k, (const float*)d_x, (float*)d_y, s->st);
     return launch_apply<double>(L.Ld, (const double*)L.k, (const double*)d_x, (double*)d_y, s->st);
 }
 

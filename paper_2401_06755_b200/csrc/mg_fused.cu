@@ -1,11 +1,346 @@
-// mg_fused.cu -- tuned uniform-grid fp32 kernels (placeholder: not yet enabled).
+// mg_fused.cu -- host side of the tuned fp32 path: pass planning for the fused smoother /
+// transfer kernel (fused_kernel.cuh), TMA descriptors, the single-CTA coarse tail, and CUDA-graph
+// replay of the whole V-cycle (north_star "fused" kernels).
+#include <algorithm>
+#include <cstring>
+
 #include "fused.h"
+#include "fused_kernel.cuh"
 #include "solver.h"
 
 namespace mgb {
-bool fused_supported(const mg_solver*) { return false; }
-int fused_apply(mg_solver*, const float*, float*) { set_error("fused path not built"); return MG_EINVAL; }
-int fused_smooth(mg_solver*, float*, const float*, int) { set_error("fused path not built"); return MG_EINVAL; }
-int fused_vcycle(mg_solver*, float*, const float*) { set_error("fused path not built"); return MG_EINVAL; }
-void fused_release(mg_solver*) {}
+namespace {
+
+using fk::FParams;
+
+// ---- TMA descriptor encoding through the driver entry point (no link-time libcuda dependency) ----
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// 3-D fp32 field (nx, ny, nz), box = one z plane of px x py cells, out-of-bounds cells read as 0.
+int make_tmap(CUtensorMap* tm, const float* ptr, int nx, int ny, int nz, int px, int py) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) { set_error("cuTensorMapEncodeTiled is not available from the driver"); return MG_ECUDA; }
+    const cuuint64_t dims[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
+    const cuuint64_t strides[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)px, (cuuint32_t)py, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(ptr), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed (%d) for %dx%dx%d box %dx%d", (int)r, nx, ny, nz, px, py); return MG_ECUDA; }
+    return 0;
+}
+
+// ---- small helper kernels for levels below the tile size ------------------------------------
+__global__ void first_sweep_kernel(size_t n, const float* __restrict__ bc, const float* __restrict__ dinv, float g,
+                                   float* __restrict__ xc) {
+    for (size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x)
+        xc[c] = dinv ? g * dinv[c] * bc[c] : g * bc[c];
+}
+
+// 1 / D_i of a level (variable k): D_i = sum_{j != i} (-w_ij) (k_i + k_j)/2, halo of k by copy
+__global__ void dinv_kernel(int nx, int ny, int nz, float ce, float cc, float cdiag, const float* __restrict__ k,
+                            float* __restrict__ dinv) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, kz = blockIdx.z;
+    if (i >= nx || j >= ny) return;
+    float e = 0.f, cn = 0.f;
+    for (int c = -1; c <= 1; ++c)
+        for (int b = -1; b <= 1; ++b)
+            for (int a = -1; a <= 1; ++a) {
+                const int m = (a != 0) + (b != 0) + (c != 0);
+                if (m < 2) continue;
+                const int ii = min(max(i + a, 0), nx - 1), jj = min(max(j + b, 0), ny - 1), kk = min(max(kz + c, 0), nz - 1);
+                const float v = k[(size_t)ii + (size_t)nx * (jj + (size_t)ny * kk)];
+                if (m == 2) e += v; else cn += v;
+            }
+    const size_t c0 = (size_t)i + (size_t)nx * (j + (size_t)ny * kz);
+    dinv[c0] = 1.f / (cdiag * k[c0] + ce * e + cc * cn);
+}
+
+struct LevelPlan {
+    bool tiled = false;       // handled by fused_kernel
+    float* dinv = nullptr;    // 1/D (variable k), levels >= 1
+    float* tmp2 = nullptr;    // residual scratch of non-tiled levels
+    float ce = 0, cc = 0, cdiag = 0, w0 = 0;
+};
+
+struct FusedState {
+    std::vector<LevelPlan> lp;
+    bool attrs_set = false;
+};
+
+constexpr int TXD = 64, TYD = 28;
+
+template <int NS, bool RR, bool PRO, bool VAR>
+int launch_cfg(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
+               float* xc_out, int first_sweep) {
+    using C = fk::Cfg<NS, RR, PRO, VAR, TXD, TYD>;
+    FusedState* fs = (FusedState*)s->fused_state;
+    LevelData& L = s->lv[l];
+    const LevelPlan& lp = fs->lp[l];
+    static bool attr_done = false;
+    if (!attr_done) {
+        MGB_CUDA(cudaFuncSetAttribute(fk::fused_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        attr_done = true;
+    }
+    CUtensorMap tmx, tmk, tmb;
+    int rc;
+    if ((rc = make_tmap(&tmx, src, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
+    if ((rc = make_tmap(&tmb, b, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
+    if (VAR) { if ((rc = make_tmap(&tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
+    else tmk = tmx;
+    FParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.nx = L.nx; P.ny = L.ny; P.nz = L.nz;
+    const int tiles = ((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
+    // z chunking: minimise (waves over 148 SMs) x (planes per block incl. pipeline fill)
+    int best_chunks = 1; double best_cost = 1e30;
+    for (int nch = 1; nch <= std::max(1, L.nz / 2); ++nch) {
+        int zc = (L.nz + nch - 1) / nch; zc += zc & 1;
+        const int real = (L.nz + zc - 1) / zc;
+        const double waves = std::ceil((double)tiles * real / 148.0);
+        const double cost = waves * (zc + 2 * C::NST + 3);
+        if (cost < best_cost - 1e-9) { best_cost = cost; best_chunks = real; P.zchunk = zc; }
+    }
+    (void)best_chunks;
+    const int nchunks = (L.nz + P.zchunk - 1) / P.zchunk;
+    P.sx0 = L.Lf.s[0]; P.sx1 = L.Lf.s[1]; P.sy0 = L.Lf.s[2]; P.sy1 = L.Lf.s[3]; P.sz0 = L.Lf.s[4]; P.sz1 = L.Lf.s[5];
+    P.any_s0 = 0;
+    for (int f = 0; f < 6; ++f) if (L.Lf.s[f] == 0.f) P.any_s0 = 1;
+    P.ce = lp.ce; P.cc = lp.cc; P.cdiag = lp.cdiag; P.w0 = lp.w0;
+    P.omega = (float)s->p.omega;
+    P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
+    if (RR) {
+        const LevelPlan& cp = fs->lp[l + 1];
+        P.dinv_c = cp.dinv;
+        P.gc_const = first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
+    }
+    dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
+    fk::fused_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, P);
+    MGB_LAUNCH_CHECK();
+    ++s->launches;
+    return 0;
+}
+
+// dispatch on (NS, RR, PRO, VAR)
+int launch_pass(mg_solver* s, int l, int NS, bool rr, bool pro, const float* src, const float* b, float* dst,
+                const float* xc = nullptr, float* bc_out = nullptr, float* xc_out = nullptr, int first_sweep = 0) {
+    const bool var = s->var_k;
+#define MGB_CASE(ns, r, p)                                                                                          \
+    if (NS == ns && rr == r && pro == p)                                                                            \
+        return var ? launch_cfg<ns, r, p, true>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep)                 \
+                   : launch_cfg<ns, r, p, false>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    MGB_CASE(1, false, false)
+    MGB_CASE(2, false, false)
+    MGB_CASE(1, false, true)
+    MGB_CASE(2, false, true)
+    MGB_CASE(0, true, false)
+    MGB_CASE(1, true, false)
+#undef MGB_CASE
+    set_error("fused pass (%d sweeps, rr=%d, pro=%d) is not instantiated", NS, (int)rr, (int)pro);
+    return MG_EINVAL;
+}
+
+int ensure_state(mg_solver* s) {
+    if (s->fused_state) return 0;
+    FusedState* fs = new FusedState();
+    fs->lp.resize(s->levels);
+    for (int l = 0; l < s->levels; ++l) {
+        LevelData& L = s->lv[l];
+        LevelPlan& lp = fs->lp[l];
+        const double h2 = L.hx * L.hx;
+        lp.ce = (float)(1.0 / (12.0 * h2)); lp.cc = (float)(1.0 / (24.0 * h2));
+        lp.cdiag = (float)(4.0 / (3.0 * h2)); lp.w0 = (float)(8.0 / (3.0 * h2));
+        lp.tiled = (L.nx % 4 == 0) && (L.ny % 2 == 0) && (L.nz % 2 == 0) && L.nx >= 16 && L.ny >= 16 && L.nz >= 8;
+        if (!lp.tiled && cudaMalloc(&lp.tmp2, L.n * sizeof(float)) != cudaSuccess) { set_error("fused: out of memory"); return MG_EALLOC; }
+    }
+    s->fused_state = fs;
+    return 0;
+}
+
+// refresh 1/D of the levels >= 1 after a coefficient change (cheap: all coarse levels together are n/7 points)
+int refresh_dinv(mg_solver* s) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    for (int l = 1; l < s->levels; ++l) {
+        LevelData& L = s->lv[l];
+        LevelPlan& lp = fs->lp[l];
+        if (!s->var_k) { cudaFree(lp.dinv); lp.dinv = nullptr; continue; }
+        if (!lp.dinv && cudaMalloc(&lp.dinv, L.n * sizeof(float)) != cudaSuccess) { set_error("fused: out of memory"); return MG_EALLOC; }
+        dim3 blk(32, 4), grd((L.nx + 31) / 32, (L.ny + 3) / 4, L.nz);
+        dinv_kernel<<<grd, blk, 0, s->st>>>(L.nx, L.ny, L.nz, lp.ce, lp.cc, lp.cdiag, (const float*)L.k, lp.dinv);
+        MGB_LAUNCH_CHECK();
+        ++s->launches;
+    }
+    return 0;
+}
+
+inline void mark(mg_solver* s, int idx) {
+    if (s->timing) cudaEventRecord(s->ev[idx], s->st);
+}
+
+// `sweeps` Jacobi sweeps on level l starting from `cur` (other buffer `oth`), optionally preceded by
+// x += P xc.  Returns the buffer holding the result through *res.
+int sweeps_level(mg_solver* s, int l, float* cur, float* oth, const float* b, int sweeps, const float* xc, float** res) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    LevelData& L = s->lv[l];
+    int rc;
+    if (fs->lp[l].tiled) {
+        bool pro = xc != nullptr;
+        if (pro && sweeps == 0) {
+            if ((rc = launch_prolong_add<float>(L.nx, L.ny, L.nz, xc, cur, s->st))) return rc;
+            ++s->launches;
+        }
+        while (sweeps > 0) {
+            const int ns = sweeps >= 2 ? 2 : 1;
+            if ((rc = launch_pass(s, l, ns, false, pro, cur, b, oth, pro ? xc : nullptr))) return rc;
+            std::swap(cur, oth);
+            sweeps -= ns; pro = false;
+        }
+    } else {
+        if (xc) {
+            if ((rc = launch_prolong_add<float>(L.nx, L.ny, L.nz, xc, cur, s->st))) return rc;
+            ++s->launches;
+        }
+        for (int it = 0; it < sweeps; ++it) {
+            if ((rc = launch_jacobi<float>(L.Lf, (const float*)L.k, cur, b, oth, s->st))) return rc;
+            ++s->launches;
+            std::swap(cur, oth);
+        }
+    }
+    *res = cur;
+    return 0;
+}
+
+// Level l of the V-cycle.  `A` holds the incoming iterate (for l > 0 the parent's fused first sweep
+// has already been applied when `done` = 1); the final iterate of the level is returned in *res.
+int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int done, float** res) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    LevelData& L = s->lv[l];
+    int rc;
+    mark(s, l);
+    if (l == s->levels - 1) {
+        rc = sweeps_level(s, l, A, B, b, std::max(0, s->p.coarse_sweeps - done), nullptr, res);
+        mark(s, s->levels);
+        return rc;
+    }
+    LevelData& C = s->lv[l + 1];
+    const bool child_coarsest = (l + 1 == s->levels - 1);
+    const int first = child_coarsest ? (s->p.coarse_sweeps >= 1) : (s->p.nu_pre >= 1);
+    float *cur = A, *oth = B;
+    int rem = std::max(0, s->p.nu_pre - done);
+    if (fs->lp[l].tiled) {
+        const int tail = rem & 1;                       // sweeps fused with the residual + restriction pass
+        if ((rc = sweeps_level(s, l, cur, oth, b, rem - tail, nullptr, &cur))) return rc;
+        oth = (cur == A) ? B : A;
+        if ((rc = launch_pass(s, l, tail, true, false, cur, b, tail ? oth : nullptr, nullptr, (float*)C.b, (float*)C.x, first))) return rc;
+        if (tail) std::swap(cur, oth);
+    } else {
+        if ((rc = sweeps_level(s, l, cur, oth, b, rem, nullptr, &cur))) return rc;
+        oth = (cur == A) ? B : A;
+        float* r = fs->lp[l].tmp2;
+        if ((rc = launch_residual<float>(L.Lf, (const float*)L.k, cur, b, r, s->st))) return rc;
+        if ((rc = launch_restrict<float>(C.nx, C.ny, C.nz, r, (float*)C.b, s->st))) return rc;
+        s->launches += 2;
+        if (first) {
+            const LevelPlan& cp = fs->lp[l + 1];
+            const float g = s->var_k ? (float)s->p.omega : (float)(s->p.omega / cp.w0);
+            first_sweep_kernel<<<(int)std::min<size_t>((C.n + 255) / 256, 1184), 256, 0, s->st>>>(C.n, (const float*)C.b, s->var_k ? cp.dinv : nullptr, g, (float*)C.x);
+            MGB_LAUNCH_CHECK();
+            ++s->launches;
+        } else {
+            MGB_CUDA(cudaMemsetAsync(C.x, 0, C.n * sizeof(float), s->st));
+        }
+    }
+    float* child = nullptr;
+    if ((rc = cycle_level(s, l + 1, (float*)C.x, (float*)C.tmp, (const float*)C.b, first, &child))) return rc;
+    if ((rc = sweeps_level(s, l, cur, oth, b, s->p.nu_post, child, &cur))) return rc;
+    mark(s, s->levels + 1 + (s->levels - 2 - l));
+    *res = cur;
+    return 0;
+}
+
+int enqueue_vcycle(mg_solver* s, float* x, const float* b) {
+    float* res = nullptr;
+    int rc = cycle_level(s, 0, x, (float*)s->lv[0].tmp, b, 0, &res);
+    if (rc) return rc;
+    if (res != x) MGB_CUDA(cudaMemcpyAsync(x, res, s->lv[0].n * sizeof(float), cudaMemcpyDeviceToDevice, s->st));
+    return 0;
+}
+
+}  // namespace
+
+bool fused_supported(const mg_solver* s) {
+    if (s->dtype != MG_F32 || s->levels < 1) return false;
+    const LevelData& L = s->lv[0];
+    return L.uniform;
+}
+
+int fused_prepare(mg_solver* s) {
+    int rc = ensure_state(s);
+    if (rc) return rc;
+    return refresh_dinv(s);
+}
+
+int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps) {
+    int rc = ensure_state(s);
+    if (rc) return rc;
+    float* res = nullptr;
+    if ((rc = sweeps_level(s, 0, x, (float*)s->lv[0].tmp, b, sweeps, nullptr, &res))) return rc;
+    if (res != x) MGB_CUDA(cudaMemcpyAsync(x, res, s->lv[0].n * sizeof(float), cudaMemcpyDeviceToDevice, s->st));
+    return 0;
+}
+
+int fused_vcycle(mg_solver* s, float* x, const float* b) {
+    int rc = ensure_state(s);
+    if (rc) return rc;
+    if (s->timing) return enqueue_vcycle(s, x, b);
+    if (!s->graph_exec || s->graph_x != x || s->graph_b != b) {
+        if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+        const long long before = s->launches;
+        cudaGraph_t graph = nullptr;
+        // record on a private stream (the caller's may be the legacy default stream, which cannot be
+        // captured); the instantiated graph is then launched on the caller's stream
+        if (!s->cap_st) MGB_CUDA(cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking));
+        cudaStream_t user_st = s->st;
+        MGB_CUDA(cudaStreamBeginCapture(s->cap_st, cudaStreamCaptureModeThreadLocal));
+        s->st = s->cap_st;
+        rc = enqueue_vcycle(s, x, b);
+        s->st = user_st;
+        const cudaError_t e = cudaStreamEndCapture(s->cap_st, &graph);
+        s->graph_launches = s->launches - before;
+        s->launches = before;
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); return MG_ECUDA; }
+        const cudaError_t e2 = cudaGraphInstantiate(&s->graph_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e2 != cudaSuccess) { s->graph_exec = nullptr; set_error("graph instantiate failed: %s", cudaGetErrorString(e2)); return MG_ECUDA; }
+        s->graph_x = x; s->graph_b = b;
+    }
+    MGB_CUDA(cudaGraphLaunch(s->graph_exec, s->st));
+    s->launches += s->graph_launches;
+    return 0;
+}
+
+void fused_release(mg_solver* s) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    if (!fs) return;
+    for (auto& lp : fs->lp) { cudaFree(lp.dinv); cudaFree(lp.tmp2); }
+    delete fs;
+    s->fused_state = nullptr;
+}
+
 }  // namespace mgb

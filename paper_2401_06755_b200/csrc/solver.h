@@ -50,6 +50,7 @@ struct mg_solver {
     std::vector<cudaEvent_t> ev;
     // CUDA-graph replay of the fused V-cycle, keyed by the (x, b) pointers it was captured with
     cudaGraphExec_t graph_exec = nullptr;
+    cudaStream_t cap_st = nullptr;  // private stream used only to record the graph
     const void* graph_x = nullptr;
     const void* graph_b = nullptr;
     long long graph_launches = 0;  // kernels inside one replay
