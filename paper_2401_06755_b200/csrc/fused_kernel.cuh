@@ -68,8 +68,10 @@ struct Cfg {
     static constexpr int DK = NPF + NST + 1;                 // k and b rings (own-point reads lag by up to NST)
     static constexpr int DG = (VAR && NST >= 2) ? NST : 0;   // omega/D (or D) ring for the lagged stages
     static constexpr int NPLANES = DXR + (VAR ? DK : 0) + DK + 2 * NST + (VAR ? NST : 0) + DG;
-    static constexpr size_t SMEM = (size_t)NPLANES * PLANE * sizeof(float) + 128;
+    static constexpr int BAR_FLOATS = 32;                    // mbarriers live in the first 128 bytes
+    static constexpr size_t SMEM = (size_t)NPLANES * PLANE * sizeof(float) + BAR_FLOATS * sizeof(float);
     static_assert(NST >= 1 && NST <= 2, "one or two stencil stages per pass");
+    static_assert(LX == 16 || LX == 32, "a tile row must be a half warp or a warp (x neighbours come by shuffle)");
     static_assert(TX % 4 == 0 && TY % 2 == 0 && PY % RY == 0, "tile shape");
     static_assert((PLANE * 4) % 128 == 0, "TMA destination alignment");
 };
@@ -109,14 +111,15 @@ __device__ __forceinline__ float4 mul4(float4 v, float f) { return make_float4(v
 //   X = f(i-1,j) + f(i+1,j) + f(i,j-1) + f(i,j+1),  Dg = f(i-1,j-1) + f(i+1,j-1) + f(i-1,j+1) + f(i+1,j+1),
 // returned as P = ce X + cc Dg (contribution to the planes below and above) and Q = ce Dg (to the plane itself).
 template <int RY, int PX>
-__device__ __forceinline__ void plane_sums(const float* __restrict__ F, const int (&roff)[RY + 2], int loff, int roffx,
-                                           float ce, float cc, float (&P)[RY][4], float (&Q)[RY][4]) {
+__device__ __forceinline__ void plane_sums(const float* __restrict__ F, const int (&roff)[RY + 2], float ce, float cc,
+                                           float (&P)[RY][4], float (&Q)[RY][4]) {
     float v[RY + 2][4], R[RY + 2][4];
 #pragma unroll
     for (int q = 0; q < RY + 2; ++q) {
-        const float* row = F + roff[q];
-        const float4 c = ld4(row);
-        const float l = row[loff], r = row[roffx];
+        const float4 c = ld4(F + roff[q]);
+        // x neighbours of the patch ends come from the adjacent lanes (same row); the two lanes at
+        // the row ends receive junk, which only reaches the outermost halo column
+        const float l = __shfl_up_sync(0xffffffffu, c.w, 1), r = __shfl_down_sync(0xffffffffu, c.x, 1);
         v[q][0] = c.x; v[q][1] = c.y; v[q][2] = c.z; v[q][3] = c.w;
         R[q][0] = l + c.y; R[q][1] = c.x + c.z; R[q][2] = c.y + c.w; R[q][3] = c.z + r;
     }
@@ -139,15 +142,14 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
     constexpr int NPF = C::NPF, DXR = C::DXR, DK = C::DK, DG = C::DG, HX = C::HX, HY = C::HY;
     constexpr bool RR = C::RR, PRO = C::PRO, VAR = C::VAR;
 
-    extern __shared__ unsigned char smem_raw[];
-    float* sm = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
-    float* XR = sm;                                   // [DXR] raw x planes (TMA)
+    extern __shared__ __align__(1024) float smf[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smf);
+    float* XR = smf + C::BAR_FLOATS;                  // [DXR] raw x planes (TMA)
     float* KR = XR + DXR * PLANE;                     // [DK]  k planes (TMA + ghost fill)       (VAR)
     float* BR = KR + (VAR ? DK : 0) * PLANE;          // [DK]  b planes (TMA + ghost fill)
     float* XS = BR + DK * PLANE;                      // [NST][2] stage inputs x^s
     float* ZS = XS + 2 * NST * PLANE;                 // [NST] k x^s                             (VAR)
     float* GR = ZS + (VAR ? NST : 0) * PLANE;         // [DG]  omega/D (sweep) or D (residual) of lagged planes
-    __shared__ __align__(8) uint64_t bars[NPF];
 
     const int tid = threadIdx.x, lx = tid % C::LX, ly = tid / C::LX;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
@@ -161,7 +163,6 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
     int roff[RY + 2];
 #pragma unroll
     for (int q = 0; q < RY + 2; ++q) roff[q] = min(max(r0 - 1 + q, 0), PY - 1) * PX + c0;
-    const int loff = (lx == 0) ? 0 : -1, roffx = (lx == C::LX - 1) ? 3 : 4;
     int own[RY];
 #pragma unroll
     for (int j = 0; j < RY; ++j) own[j] = (r0 + j) * PX + c0;
@@ -246,6 +247,12 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
 
     const int nxc = nx >> 1, nyc = ny >> 1;
 
+    // ring slots, advanced incrementally (all warp-uniform)
+    int xcur = 0, kcur = 0, bpar = 0;                 // raw-x slot / barrier index, k-b slot, barrier parity
+    int kcs[NST], gcs[NST];                           // k-b slot and g slot of the plane each stage finalises
+#pragma unroll
+    for (int s = 0; s < NST; ++s) { kcs[s] = (8 * DK - s - 1) % DK; gcs[s] = DG > 0 ? (8 * DG - s - 1) % DG : 0; }
+
     for (int p = pbeg; p < pend; ++p) {
         const int it = p - pbeg;
         // ---- prolongation operands (global loads issued before the TMA wait) ------------------
@@ -259,14 +266,14 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
                     pc[j] = *reinterpret_cast<const float2*>(P.xc + ((size_t)ck * nyc + (gjs[j] >> 1)) * nxc + (gis >> 1));
             }
         }
-        mbar_wait(&bars[it % NPF], (it / NPF) & 1);
+        mbar_wait(&bars[xcur], bpar);
 
         // ---- prep: ghost fill of k and b, stage-0 input x^0 (+ prolongation, z factor) and k x^0 ----
         {
             const float fzp = zfac(p);
-            const float* xr = XR + (it % DXR) * PLANE;
-            float* kr = KR + (it % DK) * PLANE;
-            float* br = BR + (it % DK) * PLANE;
+            const float* xr = XR + xcur * PLANE;
+            float* kr = KR + kcur * PLANE;
+            float* br = BR + kcur * PLANE;
             float* x0w = XS + (it & 1) * PLANE;
             float* z0w = ZS;
 #pragma unroll
@@ -304,17 +311,15 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
 #pragma unroll
         for (int s = 0; s < NST; ++s) {
             const int qc = p - s - 1;                          // plane finalised by this stage
-            const int itc = it - s - 1;                        // its step index (may be negative during fill)
             const float* Xin = XS + (2 * s + ((it - s) & 1)) * PLANE;
             const float* Xc = XS + (2 * s + ((it - s - 1) & 1)) * PLANE;
-            const int kslot = ((itc % DK) + DK) % DK;
-            const float* Kc = KR + kslot * PLANE;
-            const float* Bc = BR + kslot * PLANE;
+            const float* Kc = KR + kcs[s] * PLANE;
+            const float* Bc = BR + kcs[s] * PLANE;
             const float fzc = zfac(qc);
             const bool zero_plane = P.any_s0 && ((qc < 0 && P.sz0 == 0.f) || (qc >= nz && P.sz1 == 0.f));
 
             float Px[RY][4], Qx[RY][4];
-            plane_sums<RY, PX>(Xin, roff, loff, roffx, ce, cc, Px, Qx);
+            plane_sums<RY, PX>(Xin, roff, ce, cc, Px, Qx);
             float Sx[RY][4], Sz[RY][4], Dv[RY][4];
 #pragma unroll
             for (int j = 0; j < RY; ++j)
@@ -326,7 +331,7 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
                 }
             if (VAR) {
                 float Pz[RY][4], Qz[RY][4];
-                plane_sums<RY, PX>(ZS + s * PLANE, roff, loff, roffx, ce, cc, Pz, Qz);
+                plane_sums<RY, PX>(ZS + s * PLANE, roff, ce, cc, Pz, Qz);
 #pragma unroll
                 for (int j = 0; j < RY; ++j)
 #pragma unroll
@@ -337,7 +342,7 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
                     }
                 if (s == 0) {   // diagonal of the plane finalised by stage 0: D = cdiag k + S(k)
                     float Pk[RY][4], Qk[RY][4];
-                    plane_sums<RY, PX>(KR + (it % DK) * PLANE, roff, loff, roffx, ce, cc, Pk, Qk);
+                    plane_sums<RY, PX>(KR + kcur * PLANE, roff, ce, cc, Pk, Qk);
 #pragma unroll
                     for (int j = 0; j < RY; ++j)
 #pragma unroll
@@ -368,9 +373,9 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
                             gv[c] = is_rr ? D : __fdividef(omega, D);
                             if (DG > 0) Dv[j][c] = (RR && NS == 1) ? D : gv[c];      // what the lagged stage needs
                         }
-                        if (DG > 0) st4(GR + (((itc % DG) + DG) % DG) * PLANE + own[j], make_float4(Dv[j][0], Dv[j][1], Dv[j][2], Dv[j][3]));
+                        if (DG > 0) st4(GR + gcs[0] * PLANE + own[j], make_float4(Dv[j][0], Dv[j][1], Dv[j][2], Dv[j][3]));
                     } else {
-                        const float4 g4 = ld4(GR + (((itc % DG) + DG) % DG) * PLANE + own[j]);
+                        const float4 g4 = ld4(GR + gcs[s] * PLANE + own[j]);
                         gv[0] = g4.x; gv[1] = g4.y; gv[2] = g4.z; gv[3] = g4.w;
                     }
                 }
@@ -420,6 +425,13 @@ fused_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CU
                 }
             }
             if (s + 1 < NST || NST == 1) __syncthreads();
+        }
+        if (++xcur == NPF) { xcur = 0; bpar ^= 1; }
+        if (++kcur == DK) kcur = 0;
+#pragma unroll
+        for (int s = 0; s < NST; ++s) {
+            if (++kcs[s] == DK) kcs[s] = 0;
+            if (DG > 0 && ++gcs[s] == DG) gcs[s] = 0;
         }
     }
 }

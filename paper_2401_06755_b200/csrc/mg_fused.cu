@@ -7,6 +7,7 @@
 #include "fused.h"
 #include "fused_kernel.cuh"
 #include "solver.h"
+#include "tail_kernel.cuh"
 
 namespace mgb {
 namespace {
@@ -83,7 +84,7 @@ struct FusedState {
     bool attrs_set = false;
 };
 
-constexpr int TXD = 64, TYD = 28;
+constexpr int TXD = 56, TYD = 28;   // + halo = 64 x 32 cells per plane, 16 x 16 threads
 
 template <int NS, bool RR, bool PRO, bool VAR>
 int launch_cfg(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
@@ -225,6 +226,45 @@ int sweeps_level(mg_solver* s, int l, float* cur, float* oth, const float* b, in
     return 0;
 }
 
+// All levels from l down to the coarsest in one thread block (tail_kernel.cuh), if they fit on chip.
+bool tail_fits(const mg_solver* s, int l, size_t* smem_out) {
+    if (l < 1 || s->levels - l > tk::MAXL) return false;
+    const LevelData& L = s->lv[l];
+    if (L.nx > 16 || L.ny > 16 || L.nz > 16) return false;
+    size_t fl = 0;
+    for (int t = l; t < s->levels; ++t) fl += 5 * s->lv[t].n;
+    *smem_out = fl * sizeof(float);
+    return *smem_out <= 200 * 1024;
+}
+
+int launch_tail(mg_solver* s, int l, float* x, const float* b, int done, size_t smem) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    tk::TailParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.nlev = s->levels - l;
+    for (int t = 0; t < P.nlev; ++t) {
+        const LevelData& L = s->lv[l + t];
+        const LevelPlan& lp = fs->lp[l + t];
+        P.nx[t] = L.nx; P.ny[t] = L.ny; P.nz[t] = L.nz;
+        P.k[t] = s->var_k ? (const float*)L.k : nullptr;
+        P.dinv[t] = s->var_k ? lp.dinv : nullptr;
+        P.ce[t] = lp.ce; P.cc[t] = lp.cc; P.dinv_const[t] = 1.f / lp.w0;
+    }
+    for (int f = 0; f < 6; ++f) P.s[f] = s->lv[l].Lf.s[f];
+    P.omega = (float)s->p.omega;
+    P.nu_pre = s->p.nu_pre; P.nu_post = s->p.nu_post; P.coarse_sweeps = s->p.coarse_sweeps;
+    P.first_done = done; P.x = x; P.b = b;
+    static bool attr_done = false;
+    if (!attr_done) {
+        MGB_CUDA(cudaFuncSetAttribute(tk::tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    tk::tail_kernel<<<1, tk::NT, smem, s->st>>>(P);
+    MGB_LAUNCH_CHECK();
+    ++s->launches;
+    return 0;
+}
+
 // Level l of the V-cycle.  `A` holds the incoming iterate (for l > 0 the parent's fused first sweep
 // has already been applied when `done` = 1); the final iterate of the level is returned in *res.
 int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int done, float** res) {
@@ -232,6 +272,14 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     LevelData& L = s->lv[l];
     int rc;
     mark(s, l);
+    size_t tail_smem = 0;
+    if (tail_fits(s, l, &tail_smem)) {
+        rc = launch_tail(s, l, A, b, done, tail_smem);
+        for (int t = l + 1; t <= s->levels; ++t) mark(s, t);                                   // sub-levels are not timed apart
+        for (int t = s->levels - 2; t >= l; --t) mark(s, s->levels + 1 + (s->levels - 2 - t));
+        *res = A;
+        return rc;
+    }
     if (l == s->levels - 1) {
         rc = sweeps_level(s, l, A, B, b, std::max(0, s->p.coarse_sweeps - done), nullptr, res);
         mark(s, s->levels);
