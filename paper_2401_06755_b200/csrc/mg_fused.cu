@@ -7,6 +7,7 @@
 #include "fused.h"
 #include "fused_kernel.cuh"
 #include "solver.h"
+#include "stream_kernel.cuh"
 #include "tail_kernel.cuh"
 
 namespace mgb {
@@ -74,6 +75,7 @@ __global__ void dinv_kernel(int nx, int ny, int nz, float ce, float cc, float cd
 
 struct LevelPlan {
     bool tiled = false;       // handled by fused_kernel
+    bool stream = false;      // handled by stream_kernel
     float* dinv = nullptr;    // 1/D (variable k), levels >= 1
     float* tmp2 = nullptr;    // residual scratch of non-tiled levels
     float ce = 0, cc = 0, cdiag = 0, w0 = 0;
@@ -156,6 +158,83 @@ int launch_pass(mg_solver* s, int l, int NS, bool rr, bool pro, const float* src
     return MG_EINVAL;
 }
 
+// ---- single-stage streaming kernel (stream_kernel.cuh) -----------------------------------------
+template <int LX, int LY, bool VAR, int MODE>
+int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
+                      float* xc_out, int first_sweep) {
+    using C = sk::SCfg<LX, LY, VAR, MODE, (LX * LY >= 256 ? 2 : 4)>;
+    FusedState* fs = (FusedState*)s->fused_state;
+    LevelData& L = s->lv[l];
+    const LevelPlan& lp = fs->lp[l];
+    static int ctas_per_sm = 0;
+    if (!ctas_per_sm) {
+        MGB_CUDA(cudaFuncSetAttribute(sk::stream_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        MGB_CUDA(cudaFuncSetAttribute(sk::stream_kernel<C>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        int nb = 0;
+        MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, sk::stream_kernel<C>, C::NT, C::SMEM));
+        ctas_per_sm = nb > 0 ? nb : 1;
+    }
+    CUtensorMap tmx, tmk, tmb;
+    int rc;
+    if ((rc = make_tmap(&tmx, src, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
+    if ((rc = make_tmap(&tmb, b, L.nx, L.ny, L.nz, C::TX, C::TY))) return rc;
+    if (VAR) { if ((rc = make_tmap(&tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
+    else tmk = tmx;
+    sk::SParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.nx = L.nx; P.ny = L.ny; P.nz = L.nz;
+    const int tiles = ((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
+    // z chunking: minimise (waves over the resident CTA slots) x (planes per block incl. the two halo planes)
+    double best_cost = 1e30;
+    const int slots = 148 * ctas_per_sm;
+    for (int nch = 1; nch <= std::max(1, L.nz / 2); ++nch) {
+        int zc = (L.nz + nch - 1) / nch; zc += zc & 1;
+        const int real = (L.nz + zc - 1) / zc;
+        const double waves = std::ceil((double)tiles * real / (double)slots);
+        const double cost = waves * (zc + 2 + 2);
+        if (cost < best_cost - 1e-9) { best_cost = cost; P.zchunk = zc; }
+    }
+    const int nchunks = (L.nz + P.zchunk - 1) / P.zchunk;
+    P.sx0 = L.Lf.s[0]; P.sx1 = L.Lf.s[1]; P.sy0 = L.Lf.s[2]; P.sy1 = L.Lf.s[3]; P.sz0 = L.Lf.s[4]; P.sz1 = L.Lf.s[5];
+    P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
+    P.omega = (float)s->p.omega;
+    P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
+    if (MODE == sk::MODE_RR) {
+        const LevelPlan& cp = fs->lp[l + 1];
+        P.dinv_c = cp.dinv;
+        P.gc_const = first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
+    }
+    dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
+    sk::stream_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, P);
+    MGB_LAUNCH_CHECK();
+    ++s->launches;
+    return 0;
+}
+
+template <bool VAR, int MODE>
+int launch_stream_lx(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
+                     float* xc_out, int first_sweep) {
+    const int nx = s->lv[l].nx;
+    if (nx >= 96) return launch_stream_cfg<32, 8, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    if (nx >= 48) return launch_stream_cfg<16, 16, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    return launch_stream_cfg<8, 16, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+}
+
+// one streaming pass on level l: mode = sk::MODE_*
+int launch_stream(mg_solver* s, int l, int mode, const float* src, const float* b, float* dst, const float* xc = nullptr,
+                  float* bc_out = nullptr, float* xc_out = nullptr, int first_sweep = 0) {
+#define MGB_SCASE(m)                                                                                             \
+    if (mode == m)                                                                                               \
+        return s->var_k ? launch_stream_lx<true, m>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep)          \
+                        : launch_stream_lx<false, m>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    MGB_SCASE(sk::MODE_SWEEP)
+    MGB_SCASE(sk::MODE_PRO)
+    MGB_SCASE(sk::MODE_RR)
+#undef MGB_SCASE
+    set_error("stream pass mode %d is not instantiated", mode);
+    return MG_EINVAL;
+}
+
 int ensure_state(mg_solver* s) {
     if (s->fused_state) return 0;
     FusedState* fs = new FusedState();
@@ -167,6 +246,7 @@ int ensure_state(mg_solver* s) {
         lp.ce = (float)(1.0 / (12.0 * h2)); lp.cc = (float)(1.0 / (24.0 * h2));
         lp.cdiag = (float)(4.0 / (3.0 * h2)); lp.w0 = (float)(8.0 / (3.0 * h2));
         lp.tiled = (L.nx % 4 == 0) && (L.ny % 2 == 0) && (L.nz % 2 == 0) && L.nx >= 16 && L.ny >= 16 && L.nz >= 8;
+        lp.stream = (L.nx % 4 == 0) && (L.ny % 2 == 0) && (L.nz % 2 == 0) && L.nx >= 8 && L.ny >= 4 && L.nz >= 2;
         if (!lp.tiled && cudaMalloc(&lp.tmp2, L.n * sizeof(float)) != cudaSuccess) { set_error("fused: out of memory"); return MG_EALLOC; }
     }
     s->fused_state = fs;
@@ -199,15 +279,18 @@ int sweeps_level(mg_solver* s, int l, float* cur, float* oth, const float* b, in
     FusedState* fs = (FusedState*)s->fused_state;
     LevelData& L = s->lv[l];
     int rc;
-    if (fs->lp[l].tiled) {
+    const bool stream = fs->lp[l].stream && s->p.sweeps_per_pass == 1;
+    if (stream || fs->lp[l].tiled) {
         bool pro = xc != nullptr;
         if (pro && sweeps == 0) {
             if ((rc = launch_prolong_add<float>(L.nx, L.ny, L.nz, xc, cur, s->st))) return rc;
             ++s->launches;
         }
         while (sweeps > 0) {
-            const int ns = sweeps >= 2 ? 2 : 1;
-            if ((rc = launch_pass(s, l, ns, false, pro, cur, b, oth, pro ? xc : nullptr))) return rc;
+            const int ns = (!stream && sweeps >= 2) ? 2 : 1;
+            if (stream) rc = launch_stream(s, l, pro ? sk::MODE_PRO : sk::MODE_SWEEP, cur, b, oth, pro ? xc : nullptr);
+            else rc = launch_pass(s, l, ns, false, pro, cur, b, oth, pro ? xc : nullptr);
+            if (rc) return rc;
             std::swap(cur, oth);
             sweeps -= ns; pro = false;
         }
@@ -290,7 +373,11 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     const int first = child_coarsest ? (s->p.coarse_sweeps >= 1) : (s->p.nu_pre >= 1);
     float *cur = A, *oth = B;
     int rem = std::max(0, s->p.nu_pre - done);
-    if (fs->lp[l].tiled) {
+    if (fs->lp[l].stream && s->p.sweeps_per_pass == 1) {
+        if ((rc = sweeps_level(s, l, cur, oth, b, rem, nullptr, &cur))) return rc;
+        oth = (cur == A) ? B : A;
+        if ((rc = launch_stream(s, l, sk::MODE_RR, cur, b, nullptr, nullptr, (float*)C.b, (float*)C.x, first))) return rc;
+    } else if (fs->lp[l].tiled) {
         const int tail = rem & 1;                       // sweeps fused with the residual + restriction pass
         if ((rc = sweeps_level(s, l, cur, oth, b, rem - tail, nullptr, &cur))) return rc;
         oth = (cur == A) ? B : A;
