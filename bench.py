@@ -35,6 +35,9 @@ METRIC = "multigrid V-cycles/s at 256^3 fp32 (V(2,2), 7 levels, variable coeffic
 UNIT = "V-cycles/s"
 E2E_CYCLES = 20          # the paper's fixed cycle count per pressure solve
 REF_TIME_BUDGET_S = 150  # wall-clock cap of the oracle arm
+# dram__bytes_read.sum + dram__bytes_write.sum of one fine-level smoother launch, from the ncu --set full
+# capture summarised in profiles/ (bytes per launch); None until a capture of the current kernel exists
+TRAFFIC_NCU = 258.3e6
 
 
 def load_peaks():
@@ -168,7 +171,7 @@ def run_ours(args, rank, local_rank, world):
     mg.pressure_rhs(u, v, ww, w.h, 1.0, b)            # RHS = FE divergence of the seeded velocity (product kernel)
     del u, v, ww
     s = mg.mg_create((w.nx, w.ny, w.nz, w.h), w.levels, w.bc, mg.MG_F32)
-    mg.mg_set_params(s, nu_pre=w.nu_pre, nu_post=w.nu_post, coarse_sweeps=w.coarse_sweeps, sweeps_per_pass=2,
+    mg.mg_set_params(s, nu_pre=w.nu_pre, nu_post=w.nu_post, coarse_sweeps=w.coarse_sweeps, sweeps_per_pass=args.sweeps_per_pass,
                      omega=w.omega, mixed_precision=1)
     mg.mg_set_coefficient_from_vof(s, alpha, w.rho_l, w.rho_g)
     x = torch.zeros_like(b)
@@ -217,13 +220,29 @@ def run_ours(args, rank, local_rank, world):
         per_level = [{"level": l, "points": info[l], "ms_down": float(dn[l]), "ms_up": float(up[l]),
                       "alg_bytes": info[l] * (33.5 if l < w.levels - 1 else 16.0)} for l in range(w.levels)]
         peak, peak_src = load_peaks()
-        # dominant kernel: the fine-level down leg (nu1 sweeps + residual + restriction + coarse first sweep)
-        cand = [("down_leg_level0", 17.0 * info[0], dn[0]), ("up_leg_level0", 16.5 * info[0], up[0])]
-        name, nbytes, t_ms = max(cand, key=lambda c: c[2])
+        # dominant kernel: the fine-level smoother pass (5 of the 6 fine-level passes of a V(2,2) cycle are
+        # this kernel or its PRO / RR variants).  Timed alone, back to back, with CUDA events on the solver's
+        # stream: `nsw` sweeps in one mg_smooth call = nsw / sweeps_per_pass launches, ping-pong between x and
+        # the solver's scratch (nsw even: no copy back).  Algorithmic bytes: x, k, b read + x written = 16 B
+        # per point per pass.
+        nsw = 20 * args.sweeps_per_pass
+        xs = x.clone()
+        mg.mg_smooth(s, xs, b, nsw)
+        torch.cuda.synchronize()
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e2.record()
+        mg.mg_smooth(s, xs, b, nsw)
+        e3.record()
+        torch.cuda.synchronize()
+        launches_sm = nsw // args.sweeps_per_pass
+        t_ms = e2.elapsed_time(e3) / launches_sm
+        nbytes = 16.0 * info[0]
         achieved = nbytes / (t_ms * 1e-3) * 1e-9
-        roofline = {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                    "alg_bytes_per_launch": nbytes, "ms_per_launch": float(t_ms)}
+        roofline = {"bound": "hbm", "kernel": "fine-level smoother pass (%d sweep(s) per launch)" % args.sweeps_per_pass,
+                    "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": TRAFFIC_NCU,
+                    "peak_source": peak_src, "alg_bytes_per_launch": nbytes, "ms_per_launch": float(t_ms),
+                    "launches_timed": launches_sm}
+        del xs
     except mg.MgError as e:   # instrumentation not available on this path: say so instead of inventing a number
         roofline = {"bound": "hbm", "achieved": None, "peak": load_peaks()[0], "unit": "GB/s", "frac": None,
                     "traffic": None, "note": str(e)}
@@ -263,7 +282,7 @@ def run_ours(args, rank, local_rank, world):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": "config3_rising_bubble_256^3 (BASELINE.json configs[2])", "grid": [w.nx, w.ny, w.nz],
                        "levels": w.levels, "cycle": "V(%d,%d)" % (w.nu_pre, w.nu_post), "omega": w.omega,
-                       "coarse_sweeps": w.coarse_sweeps, "bc": "Neumann x5, Dirichlet top",
+                       "coarse_sweeps": w.coarse_sweeps, "bc": "Neumann x5, Dirichlet top", "sweeps_per_pass": args.sweeps_per_pass,
                        "l2_policy": "inputs larger than L2 (x, b, k = 192 MiB > 126 MB)", "parallelism": "replicas x%d" % world},
             "glups": glups, "lups_per_cycle": lups_per_cycle,
             "alg_bytes_per_cycle": algorithmic_bytes_per_cycle(w, info),
@@ -284,6 +303,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweeps-per-pass", type=int, default=1, choices=[1, 2],
+                    help="1: one-stage streaming kernels (default, faster); 2: two-stage temporally fused kernels")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

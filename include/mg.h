@@ -72,7 +72,7 @@ enum {
 int mg_create(mg_solver** out, const mg_grid* grid, int levels, const int bc[6], int dtype, void* cuda_stream);
 void mg_destroy(mg_solver* s);
 
-int mg_set_params(mg_solver* s, const mg_params* p); /* defaults: 2, 2, 50, 2, 2/3, 1 */
+int mg_set_params(mg_solver* s, const mg_params* p); /* defaults: 2, 2, 50, 1, 2/3, 1 */
 int mg_get_params(const mg_solver* s, mg_params* p);
 
 /* Coefficient k (a7).  d_k: nx*ny*nz values of k > 0, or NULL for constant k = 1.  The field is

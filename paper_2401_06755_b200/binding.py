@@ -168,7 +168,7 @@ def mg_destroy(s):
     s.close()
 
 
-def mg_set_params(s, nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=2, omega=2.0 / 3.0, mixed_precision=1):
+def mg_set_params(s, nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=1, omega=2.0 / 3.0, mixed_precision=1):
     p = MgParams(int(nu_pre), int(nu_post), int(coarse_sweeps), int(sweeps_per_pass), float(omega), int(mixed_precision))
     return _check(_lib.mg_set_params(s.handle, C.byref(p)))
 

@@ -28,7 +28,7 @@ struct mg_solver {
     int dtype = MG_F32;
     int device = 0;
     cudaStream_t st = nullptr;
-    mg_params p{2, 2, 50, 2, 2.0 / 3.0, 1};
+    mg_params p{2, 2, 50, 1, 2.0 / 3.0, 1};
     bool var_k = false;
     int fused = 1;
     std::vector<mgb::LevelData> lv;
