@@ -1,0 +1,402 @@
+// lean_kernel.cuh -- the fp32 streaming smoother / transfer kernel for uniform grids (sm_100a).
+//
+// One stencil stage per pass, three variants:
+//   MODE_SWEEP   weighted-Jacobi sweep                                   x            -> x'
+//   MODE_PRO     prolongation + correction + sweep                      x + P x_c    -> x'
+//   MODE_RR      residual, 8-child-mean restriction and the coarse level's first sweep from a
+//                zero guess                                              x            -> b_c, x_c
+//
+// Arithmetic (uniform spacing h; reading C1/C2, Eqs. 8, 12-13 P:109-114, 146-159).  The 6 face
+// weights of the trilinear-FE Laplacian vanish on a uniform grid; the 12 edge neighbours carry
+// -w = 2 cc and the 8 corner neighbours cc, cc = 1/(24 h^2).  With the integer-weight neighbour sum
+//   S(f)_i = 2 E(f)_i + Cn(f)_i            (E = sum over edge neighbours, Cn = over corner neighbours)
+// Eq. 13 with sum_j w_ij = 0 reads
+//   D_i     = cc (32 k_i + S(k)_i)
+//   (A x)_i = D_i x_i - cc (k_i S(x)_i + S(k x)_i)
+//   sweep:  x' = (1 - omega) x + omega / (32 k + S(k)) * (b / cc + k S(x) + S(k x))
+//   resid:  r  = b + cc (k S(x) + S(k x) - (32 k + S(k)) x)
+// Constant coefficient (k = 1): S(k) = 32, S(k x) = S(x).
+//
+// Data flow.  A block owns a TX x TY column of the grid and streams along z.  The z planes of x and
+// k (tile + one halo row / 4 halo columns per side, out-of-bounds cells zero-filled) and the tile of
+// b are staged in shared memory by TMA (cp.async.bulk.tensor.3d) into an NS-deep ring, completion on
+// mbarriers; x' goes from registers to HBM with 128-bit stores.  Each thread owns a 4 (x) by 2 (y)
+// patch of columns.  Per plane it reads its 4 rows as one 128-bit and two 32-bit shared loads per
+// row and field (rows 0 and 2 first, then 1 and 3, to keep few values live) and reduces the plane to
+// the in-plane sums
+//   Dg = 4 diagonal neighbours,   Pp = 2 (4 cross neighbours) + Dg,
+// so that  S[z] = Pp[z-1] + 2 Dg[z] + Pp[z+1]  is accumulated in two registers per point and field
+// and every plane is read from shared memory once.
+//
+// The kernel is bound by instruction issue unless written tightly (profiles/r01_ncu_stream_v1.md:
+// 83 instructions per point), so the arithmetic runs on the packed fp32 pipe (FADD2 / FMUL2 / FFMA2,
+// two columns per instruction: a 128-bit shared load delivers the aligned pairs directly), halo
+// factors are folded into FMAs that are needed anyway, and the plane loop is unrolled by two so that
+// the rolling accumulators and the "own values of the previous plane" are renamed, not moved.
+// Boundary halos (ghost = s * mirror): a ghost row is the mirrored row, its factor s folded
+// into the row combination; a ghost column is the zero-filled halo cell plus s times the patch's own
+// end value (one FMA); a ghost plane is the mirrored plane loaded again, its factor folded into the z
+// accumulation.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <type_traits>
+
+namespace mgb {
+namespace lk {
+
+enum { MODE_SWEEP = 0, MODE_PRO = 1, MODE_RR = 2 };
+
+struct LParams {
+    int nx, ny, nz;
+    int zchunk;                 // output planes per block (even)
+    float sx0, sx1, sy0, sy1, sz0, sz1;
+    float cc, icc;              // 1/(24 h^2) and its inverse
+    float omega;
+    float* out;                 // x' (sweep modes)
+    const float* xc;            // PRO: coarse correction (nx/2 * ny/2 * nz/2)
+    float* bc_out;              // RR: restricted residual
+    float* xc_out;              // RR: coarse first sweep  omega b_c / D_c  (or zeros)
+    const float* dinv_c;        // RR, variable k: 1 / D_c on the coarse level
+    float gc_const;             // RR, constant k: omega / w0_c
+    int first_sweep;            // RR: write x_c = omega b_c / D_c (1) or zeros (0)
+};
+
+template <int LX_, int LY_, bool VAR_, int MODE_, int MINB_>
+struct LCfg {
+    static constexpr int LX = LX_, LY = LY_, MODE = MODE_, MINB = MINB_;
+    static constexpr bool VAR = VAR_;
+    static constexpr int RY = 2;
+    static constexpr int TX = 4 * LX, TY = RY * LY, NT = LX * LY;
+    static constexpr int PX = TX + 8, PY = TY + 2;
+    static constexpr int NS = 4;                                          // ring depth = planes in flight + 1
+    static constexpr int PLANE = ((PX * PY + 31) / 32) * 32;              // floats per staged x / k plane (128-byte multiple)
+    static constexpr int BPLANE = ((TX * TY + 31) / 32) * 32;             // floats per staged b tile
+    static constexpr int SLOT = PLANE * (VAR ? 2 : 1) + BPLANE;           // floats per ring slot: x, (k,) b
+    static constexpr uint32_t BOX_BYTES = (uint32_t)(PX * PY * sizeof(float));
+    static constexpr uint32_t BBOX_BYTES = (uint32_t)(TX * TY * sizeof(float));
+    static constexpr int BAR_FLOATS = 32;
+    static constexpr size_t SMEM = (size_t)(BAR_FLOATS + NS * SLOT) * sizeof(float);
+    static_assert(NT % 32 == 0, "whole warps");
+};
+
+typedef unsigned long long u64;   // two packed floats {lo, hi} = columns {c, c + 1}
+
+__device__ __forceinline__ u64 pk(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float lo(u64 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
+__device__ __forceinline__ float hi(u64 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ u64 bc2(float s) { return pk(s, s); }
+__device__ __forceinline__ float rcpa(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+// shared-memory loads by 32-bit shared-space address (no generic-address arithmetic in the plane loop)
+__device__ __forceinline__ float lds32(uint32_t a) { float r; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(a)); return r; }
+__device__ __forceinline__ void lds128(uint32_t a, u64& p, u64& q) { asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(p), "=l"(q) : "r"(a)); }
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LK_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra LK_DONE_%=;\n"
+        "bra LK_WAIT_%=;\n"
+        "LK_DONE_%=:\n"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_plane(float* dst, const CUtensorMap* tm, uint64_t* bar, int cx, int cy, int cz) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(tm)), "r"(smem_u32(bar)), "r"(cx), "r"(cy), "r"(cz)
+        : "memory");
+}
+
+// One staged row of a thread's patch: columns (c0, c0+1) = p, (c0+2, c0+3) = q and the x neighbours of the patch ends.
+struct Row { u64 p, q; float l, r; };
+// Row-wise x sums of one row:  R(c) = f(c-1) + f(c+1),  T(c) = R(c) + 2 f(c)
+struct RT { u64 rp, rq, tp, tq; };
+
+__device__ __forceinline__ RT row_sums(const Row& w, u64 two) {
+    RT o;
+    o.rp = pk(w.l + hi(w.p), lo(w.p) + lo(w.q));
+    o.rq = pk(hi(w.p) + hi(w.q), lo(w.q) + w.r);
+    o.tp = fma2(w.p, two, o.rp);
+    o.tq = fma2(w.q, two, o.rq);
+    return o;
+}
+
+// row at shared address `a` (its column c0): halo cell (zero outside the domain) + g * own end value
+__device__ __forceinline__ Row load_row(uint32_t a, float gl, float gr) {
+    Row w;
+    lds128(a, w.p, w.q);
+    w.l = lds32(a - 4); w.r = lds32(a + 16);
+    w.l = fmaf(gl, lo(w.p), w.l); w.r = fmaf(gr, hi(w.q), w.r);
+    return w;
+}
+
+// z accumulators of one field for the thread's 2 rows x 2 column pairs
+struct Acc { u64 v[2][2]; };
+
+// In-plane sums of one output row j from its three staged rows (a = row j, m = row j + 1, c = row j + 2; fa / fc
+// are halo factors of a / c, 1 except for a ghost row):
+//   Dg = fa R_a + fc R_c,  Pp = fa T_a + fc T_c + 2 R_m          (FAC: which of a, c can be a ghost row)
+// scattered into the z accumulators with the plane factor fz (1 except for a ghost plane):
+//   S = A + fz Pp (the plane below is complete),  A <- Bin + 2 fz Dg,  Bout <- Pp (the caller scales it by fz).
+template <int FAC>   // 0: no factor, 1: factor on row a, 2: factor on row c
+__device__ __forceinline__ void out_row(const RT& a, const RT& m, const RT& c, u64 f, u64 two, u64 fz2, u64 twofz,
+                                        u64 (&A)[2], const u64 (&Bin)[2], u64 (&Bout)[2], u64 (&S)[2]) {
+    u64 dgp, dgq, ppp, ppq;
+    if (FAC == 1) { dgp = fma2(a.rp, f, c.rp); dgq = fma2(a.rq, f, c.rq); ppp = fma2(a.tp, f, c.tp); ppq = fma2(a.tq, f, c.tq); }
+    else if (FAC == 2) { dgp = fma2(c.rp, f, a.rp); dgq = fma2(c.rq, f, a.rq); ppp = fma2(c.tp, f, a.tp); ppq = fma2(c.tq, f, a.tq); }
+    else { dgp = add2(a.rp, c.rp); dgq = add2(a.rq, c.rq); ppp = add2(a.tp, c.tp); ppq = add2(a.tq, c.tq); }
+    ppp = fma2(m.rp, two, ppp); ppq = fma2(m.rq, two, ppq);
+    if (FAC == 0) {           // the coefficient: ghost = plain copy
+        S[0] = add2(A[0], ppp); S[1] = add2(A[1], ppq);
+        A[0] = fma2(dgp, two, Bin[0]); A[1] = fma2(dgq, two, Bin[1]);
+    } else {
+        S[0] = fma2(ppp, fz2, A[0]); S[1] = fma2(ppq, fz2, A[1]);
+        A[0] = fma2(dgp, twofz, Bin[0]); A[1] = fma2(dgq, twofz, Bin[1]);
+    }
+    Bout[0] = ppp; Bout[1] = ppq;
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::NT, C::MINB)
+lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmk,
+            const __grid_constant__ CUtensorMap tmb, const LParams P) {
+    constexpr int RY = C::RY, PX = C::PX, PY = C::PY, PLANE = C::PLANE, NS = C::NS, LX = C::LX, SLOT = C::SLOT;
+    constexpr bool VAR = C::VAR;
+    constexpr int MODE = C::MODE;
+    constexpr int KOFF = PLANE, BOFF = PLANE * (VAR ? 2 : 1);      // k and b inside a ring slot
+    static_assert(RY == 2, "2 output rows per thread");
+
+    extern __shared__ __align__(1024) float smf[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smf);
+    float* ring = smf + C::BAR_FLOATS;
+
+    const int tid = threadIdx.x, lx = tid % LX, ly = tid / LX;
+    const int nx = P.nx, ny = P.ny, nz = P.nz;
+    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
+    const int zc0 = blockIdx.z * P.zchunk, zc1 = min(zc0 + P.zchunk, nz);
+    const int pbeg = zc0 - 1, niter = zc1 - zc0 + 2;               // even: zchunk and nz are even
+    const int c0 = 4 * lx, gi0 = x0 + c0, gj0 = y0 + RY * ly;
+    const bool active = gi0 < nx && gj0 < ny;
+
+    // ---- z-invariant per-thread set-up ----------------------------------------------------------
+    const uint32_t ring_a = smem_u32(ring);
+    uint32_t raddr[4];                                             // shared address of the 4 staged rows in slot 0
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int gq = gj0 - 1 + q;
+        const int m = gq < 0 ? -1 - gq : (gq >= ny ? 2 * ny - 1 - gq : gq);     // ghost row -> mirrored row
+        raddr[q] = ring_a + 4u * (uint32_t)(min(max(m - (y0 - 1), 0), PY - 1) * PX + 4 + c0);
+    }
+    const uint32_t baddr = ring_a + 4u * (uint32_t)(BOFF + (RY * ly) * C::TX + c0);
+    // only the first and the last staged row of a patch can be ghost rows (factor s of the y faces)
+    const u64 f0 = bc2((gj0 - 1 < 0) ? P.sy0 : 1.f), f3 = bc2((gj0 + RY >= ny) ? P.sy1 : 1.f);
+    // x neighbours of the patch ends: halo cell (zero-filled outside the domain) + s * own end value at a domain face
+    const bool lghost = gi0 == 0, rghost = gi0 + 4 >= nx;
+    const float glx = lghost ? P.sx0 : 0.f, grx = rghost ? P.sx1 : 0.f;
+    const float glk = lghost ? 1.f : 0.f, grk = rghost ? 1.f : 0.f;
+
+    auto zsrc = [&](int p) { return p < 0 ? -1 - p : (p >= nz ? 2 * nz - 1 - p : p); };
+    auto issue = [&](int it) {   // one thread: TMA of the x, k planes of iteration `it` and of the b tile it finalises
+        uint64_t* bar = &bars[it % NS];
+        float* dst = ring + (it % NS) * SLOT;
+        const bool wb = it >= 2;                                   // plane pbeg + it - 1 >= zc0
+        mbar_expect_tx(bar, C::BOX_BYTES * (VAR ? 2u : 1u) + (wb ? C::BBOX_BYTES : 0u));
+        const int z = zsrc(pbeg + it);
+        tma_load_plane(dst, &tmx, bar, x0 - 4, y0 - 1, z);
+        if (VAR) tma_load_plane(dst + KOFF, &tmk, bar, x0 - 4, y0 - 1, z);
+        if (wb) tma_load_plane(dst + BOFF, &tmb, bar, x0, y0, pbeg + it - 1);
+    };
+
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < NS; ++q) mbar_init(&bars[q], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0)
+        for (int q = 0; q < NS && q < niter; ++q) issue(q);
+
+    // ---- per-point state carried along z ---------------------------------------------------------
+    u64 xA[2][2], zA[2][2], kA[2][2];        // S accumulators [row][column pair] of x, k x, k ...
+    u64 xB[2][2][2], zB[2][2][2], kB[2][2][2];   // ... B double-buffered by plane parity [parity][row][pair]
+    u64 xo[2][2][2], ko[2][2][2];            // own values [plane parity][row][column pair]
+    float hold0 = 0.f, hold1 = 0.f;          // restriction: sums of the even plane
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            xA[j][c] = zA[j][c] = kA[j][c] = 0ull;
+            xB[0][j][c] = zB[0][j][c] = kB[0][j][c] = xB[1][j][c] = zB[1][j][c] = kB[1][j][c] = 0ull;
+            xo[0][j][c] = xo[1][j][c] = ko[0][j][c] = ko[1][j][c] = 0ull;
+        }
+    const u64 two = bc2(2.f);
+    const float omega = P.omega;
+    const int nxc = nx >> 1, nyc = ny >> 1;
+
+    // one plane: PAR = parity of the iteration index
+    auto body = [&](auto par_tag, const int it) {
+        constexpr int PAR = decltype(par_tag)::value;
+        const int p = pbeg + it;
+        const int slot = it & (NS - 1);
+        // ---- PRO: coarse correction of the staged rows, issued before the barrier wait ----
+        float2 pc[3]; float pl[3], pr[3];
+        if (MODE == MODE_PRO) {
+            // rows (-1), (0, 1), (2) of the patch lie in 3 coarse rows; the x neighbours in the adjacent coarse cells
+            const size_t cplane = (size_t)(zsrc(p) >> 1) * nyc;
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                pc[q] = make_float2(0.f, 0.f); pl[q] = 0.f; pr[q] = 0.f;
+                const int gq = gj0 - 1 + (q == 0 ? 0 : (q == 1 ? 1 : 3));
+                const int m = gq < 0 ? -1 - gq : (gq >= ny ? 2 * ny - 1 - gq : gq);
+                const float* crow = P.xc + (cplane + (m >> 1)) * nxc;
+                if (active) {
+                    pc[q] = __ldg(reinterpret_cast<const float2*>(crow + (gi0 >> 1)));
+                    if (!lghost) pl[q] = __ldg(crow + ((gi0 - 1) >> 1));
+                    if (!rghost) pr[q] = __ldg(crow + ((gi0 + 4) >> 1));
+                }
+            }
+        }
+        // ---- ring hand-back: everyone has finished iteration it - 1, so its slot can be refilled ----
+        __syncthreads();
+        if (tid == 0 && it >= 1 && it - 1 + NS < niter) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            issue(it - 1 + NS);
+        }
+        mbar_wait(&bars[slot], (uint32_t)((it / NS) & 1));
+
+        const uint32_t so = (uint32_t)(slot * SLOT * 4);
+        const bool zghost = p < 0 || p >= nz;
+        const float fz = zghost ? (p < 0 ? P.sz0 : P.sz1) : 1.f;
+        const u64 fz2 = bc2(fz), twofz = bc2(2.f * fz);
+        u64 Sx[2][2], Sz[2][2], Sk[2][2];
+
+        // staged row q of x (with the PRO correction), of k, and their product; x sums of the three
+        auto stage = [&](int q, RT& sx, RT& sk, RT& sz) {
+            const uint32_t a = raddr[q] + so;
+            Row w;
+            lds128(a, w.p, w.q);
+            w.l = lds32(a - 4); w.r = lds32(a + 16);
+            if (MODE == MODE_PRO) {
+                const int e = q == 0 ? 0 : (q == 3 ? 2 : 1);
+                w.p = add2(w.p, bc2(pc[e].x)); w.q = add2(w.q, bc2(pc[e].y));
+                w.l += pl[e]; w.r += pr[e];
+            }
+            w.l = fmaf(glx, lo(w.p), w.l); w.r = fmaf(grx, hi(w.q), w.r);
+            if (q == 1) { xo[PAR][0][0] = w.p; xo[PAR][0][1] = w.q; }
+            if (q == 2) { xo[PAR][1][0] = w.p; xo[PAR][1][1] = w.q; }
+            sx = row_sums(w, two);
+            if (VAR) {
+                const Row kw = load_row(a + KOFF * 4, glk, grk);
+                if (q == 1) { ko[PAR][0][0] = kw.p; ko[PAR][0][1] = kw.q; }
+                if (q == 2) { ko[PAR][1][0] = kw.p; ko[PAR][1][1] = kw.q; }
+                sk = row_sums(kw, two);
+                Row zw; zw.p = mul2(kw.p, w.p); zw.q = mul2(kw.q, w.q); zw.l = kw.l * w.l; zw.r = kw.r * w.r;
+                sz = row_sums(zw, two);
+            }
+        };
+        {
+            RT sx0, sk0, sz0, sx1, sk1, sz1, sx2, sk2, sz2, sx3, sk3, sz3;
+            stage(0, sx0, sk0, sz0);
+            stage(1, sx1, sk1, sz1);
+            stage(2, sx2, sk2, sz2);
+            out_row<1>(sx0, sx1, sx2, f0, two, fz2, twofz, xA[0], xB[PAR ^ 1][0], xB[PAR][0], Sx[0]);
+            if (VAR) {
+                out_row<1>(sz0, sz1, sz2, f0, two, fz2, twofz, zA[0], zB[PAR ^ 1][0], zB[PAR][0], Sz[0]);
+                out_row<0>(sk0, sk1, sk2, f0, two, fz2, twofz, kA[0], kB[PAR ^ 1][0], kB[PAR][0], Sk[0]);
+            }
+            stage(3, sx3, sk3, sz3);
+            out_row<2>(sx1, sx2, sx3, f3, two, fz2, twofz, xA[1], xB[PAR ^ 1][1], xB[PAR][1], Sx[1]);
+            if (VAR) {
+                out_row<2>(sz1, sz2, sz3, f3, two, fz2, twofz, zA[1], zB[PAR ^ 1][1], zB[PAR][1], Sz[1]);
+                out_row<0>(sk1, sk2, sk3, f3, two, fz2, twofz, kA[1], kB[PAR ^ 1][1], kB[PAR][1], Sk[1]);
+            }
+        }
+
+        if (PAR == 0 && it == 0 && zghost) {   // the ghost plane below the domain: its Pp enters the plane above scaled
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    xB[PAR][j][c] = mul2(xB[PAR][j][c], fz2);
+                    if (VAR) zB[PAR][j][c] = mul2(zB[PAR][j][c], fz2);
+                }
+        }
+
+        // ---- finalise plane p - 1 ----
+        const int qc = p - 1;
+        if (it >= 2) {
+            const u64 icc2 = bc2(P.icc), cc2 = bc2(P.cc), om12 = bc2(1.f - omega);
+            float rs0 = 0.f, rs1 = 0.f;
+#pragma unroll
+            for (int j = 0; j < RY; ++j) {
+                u64 b4[2];
+                lds128(baddr + so + j * (C::TX * 4), b4[0], b4[1]);
+                u64 o[2];
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const u64 bv = b4[c];
+                    const u64 xv = xo[PAR ^ 1][j][c];
+                    if (VAR) {
+                        const u64 kv = ko[PAR ^ 1][j][c];
+                        const u64 Dp = fma2(kv, bc2(32.f), Sk[j][c]);
+                        const u64 t = fma2(kv, Sx[j][c], Sz[j][c]);
+                        if (MODE == MODE_RR) {
+                            o[c] = fma2(mul2(Dp, bc2(-P.cc)), xv, fma2(t, cc2, bv));
+                        } else {
+                            const u64 g = mul2(pk(rcpa(lo(Dp)), rcpa(hi(Dp))), bc2(omega));
+                            o[c] = fma2(g, fma2(bv, icc2, t), mul2(xv, om12));
+                        }
+                    } else {
+                        const u64 s2 = add2(Sx[j][c], Sx[j][c]);
+                        if (MODE == MODE_RR) o[c] = fma2(fma2(xv, bc2(-64.f), s2), cc2, bv);
+                        else o[c] = fma2(bc2(omega * (1.f / 64.f)), fma2(bv, icc2, s2), mul2(xv, om12));
+                    }
+                }
+                if (MODE == MODE_RR) { rs0 += lo(o[0]) + hi(o[0]); rs1 += lo(o[1]) + hi(o[1]); }
+                else if (active)
+                    *reinterpret_cast<ulonglong2*>(P.out + ((size_t)qc * ny + (gj0 + j)) * nx + gi0) = make_ulonglong2(o[0], o[1]);
+            }
+            if (MODE == MODE_RR) {
+                if (PAR == 0) {     // qc = zc0 + it - 2 with zc0 even: PAR 0 <=> qc even
+                    hold0 = rs0; hold1 = rs1;
+                } else if (active) {
+                    const size_t ci = ((size_t)(qc >> 1) * nyc + (gj0 >> 1)) * nxc + (gi0 >> 1);
+                    const float2 bcv = make_float2(0.125f * (hold0 + rs0), 0.125f * (hold1 + rs1));
+                    *reinterpret_cast<float2*>(P.bc_out + ci) = bcv;
+                    float2 xcv = make_float2(0.f, 0.f);
+                    if (P.first_sweep) {
+                        if (VAR) {
+                            const float2 di = __ldg(reinterpret_cast<const float2*>(P.dinv_c + ci));
+                            xcv = make_float2(omega * di.x * bcv.x, omega * di.y * bcv.y);
+                        } else {
+                            xcv = make_float2(P.gc_const * bcv.x, P.gc_const * bcv.y);
+                        }
+                    }
+                    *reinterpret_cast<float2*>(P.xc_out + ci) = xcv;
+                }
+            }
+        }
+    };
+
+    for (int it = 0; it < niter; it += 2) {
+        body(std::integral_constant<int, 0>{}, it);
+        body(std::integral_constant<int, 1>{}, it + 1);
+    }
+}
+
+}  // namespace lk
+}  // namespace mgb

@@ -7,7 +7,7 @@
 #include "fused.h"
 #include "fused_kernel.cuh"
 #include "solver.h"
-#include "stream_kernel.cuh"
+#include "lean_kernel.cuh"
 #include "tail_kernel.cuh"
 
 namespace mgb {
@@ -159,19 +159,19 @@ int launch_pass(mg_solver* s, int l, int NS, bool rr, bool pro, const float* src
 }
 
 // ---- single-stage streaming kernel (stream_kernel.cuh) -----------------------------------------
-template <int LX, int LY, bool VAR, int MODE>
+template <int LX, int LY, int MINB, bool VAR, int MODE>
 int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
                       float* xc_out, int first_sweep) {
-    using C = sk::SCfg<LX, LY, VAR, MODE, (LX * LY >= 256 ? 2 : 4)>;
+    using C = lk::LCfg<LX, LY, VAR, MODE, MINB>;
     FusedState* fs = (FusedState*)s->fused_state;
     LevelData& L = s->lv[l];
     const LevelPlan& lp = fs->lp[l];
     static int ctas_per_sm = 0;
     if (!ctas_per_sm) {
-        MGB_CUDA(cudaFuncSetAttribute(sk::stream_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        MGB_CUDA(cudaFuncSetAttribute(sk::stream_kernel<C>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        MGB_CUDA(cudaFuncSetAttribute(lk::lean_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        MGB_CUDA(cudaFuncSetAttribute(lk::lean_kernel<C>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         int nb = 0;
-        MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, sk::stream_kernel<C>, C::NT, C::SMEM));
+        MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, lk::lean_kernel<C>, C::NT, C::SMEM));
         ctas_per_sm = nb > 0 ? nb : 1;
     }
     CUtensorMap tmx, tmk, tmb;
@@ -180,7 +180,7 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
     if ((rc = make_tmap(&tmb, b, L.nx, L.ny, L.nz, C::TX, C::TY))) return rc;
     if (VAR) { if ((rc = make_tmap(&tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
     else tmk = tmx;
-    sk::SParams P;
+    lk::LParams P;
     std::memset(&P, 0, sizeof(P));
     P.nx = L.nx; P.ny = L.ny; P.nz = L.nz;
     const int tiles = ((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
@@ -199,13 +199,13 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
     P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
     P.omega = (float)s->p.omega;
     P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
-    if (MODE == sk::MODE_RR) {
+    if (MODE == lk::MODE_RR) {
         const LevelPlan& cp = fs->lp[l + 1];
         P.dinv_c = cp.dinv;
         P.gc_const = first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
     }
     dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
-    sk::stream_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, P);
+    lk::lean_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, P);
     MGB_LAUNCH_CHECK();
     ++s->launches;
     return 0;
@@ -215,21 +215,22 @@ template <bool VAR, int MODE>
 int launch_stream_lx(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
                      float* xc_out, int first_sweep) {
     const int nx = s->lv[l].nx;
-    if (nx >= 96) return launch_stream_cfg<32, 8, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
-    if (nx >= 48) return launch_stream_cfg<16, 16, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
-    return launch_stream_cfg<8, 16, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    // 128-thread blocks, 3 per SM: 168 registers per thread keep the per-point state and the staged rows out of local memory
+    if (nx >= 96) return launch_stream_cfg<32, 4, 3, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    if (nx >= 48) return launch_stream_cfg<16, 8, 3, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    return launch_stream_cfg<8, 16, 3, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
 }
 
-// one streaming pass on level l: mode = sk::MODE_*
+// one streaming pass on level l: mode = lk::MODE_*
 int launch_stream(mg_solver* s, int l, int mode, const float* src, const float* b, float* dst, const float* xc = nullptr,
                   float* bc_out = nullptr, float* xc_out = nullptr, int first_sweep = 0) {
 #define MGB_SCASE(m)                                                                                             \
     if (mode == m)                                                                                               \
         return s->var_k ? launch_stream_lx<true, m>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep)          \
                         : launch_stream_lx<false, m>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
-    MGB_SCASE(sk::MODE_SWEEP)
-    MGB_SCASE(sk::MODE_PRO)
-    MGB_SCASE(sk::MODE_RR)
+    MGB_SCASE(lk::MODE_SWEEP)
+    MGB_SCASE(lk::MODE_PRO)
+    MGB_SCASE(lk::MODE_RR)
 #undef MGB_SCASE
     set_error("stream pass mode %d is not instantiated", mode);
     return MG_EINVAL;
@@ -288,7 +289,7 @@ int sweeps_level(mg_solver* s, int l, float* cur, float* oth, const float* b, in
         }
         while (sweeps > 0) {
             const int ns = (!stream && sweeps >= 2) ? 2 : 1;
-            if (stream) rc = launch_stream(s, l, pro ? sk::MODE_PRO : sk::MODE_SWEEP, cur, b, oth, pro ? xc : nullptr);
+            if (stream) rc = launch_stream(s, l, pro ? lk::MODE_PRO : lk::MODE_SWEEP, cur, b, oth, pro ? xc : nullptr);
             else rc = launch_pass(s, l, ns, false, pro, cur, b, oth, pro ? xc : nullptr);
             if (rc) return rc;
             std::swap(cur, oth);
@@ -376,7 +377,7 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     if (fs->lp[l].stream && s->p.sweeps_per_pass == 1) {
         if ((rc = sweeps_level(s, l, cur, oth, b, rem, nullptr, &cur))) return rc;
         oth = (cur == A) ? B : A;
-        if ((rc = launch_stream(s, l, sk::MODE_RR, cur, b, nullptr, nullptr, (float*)C.b, (float*)C.x, first))) return rc;
+        if ((rc = launch_stream(s, l, lk::MODE_RR, cur, b, nullptr, nullptr, (float*)C.b, (float*)C.x, first))) return rc;
     } else if (fs->lp[l].tiled) {
         const int tail = rem & 1;                       // sweeps fused with the residual + restriction pass
         if ((rc = sweeps_level(s, l, cur, oth, b, rem - tail, nullptr, &cur))) return rc;
