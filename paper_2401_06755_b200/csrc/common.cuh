@@ -51,6 +51,11 @@ template <typename T> int launch_residual_norm(const Level<T>& L, const T* k, co
 // mixed precision outer loop: r32 = float(b32 - A64 x64), ||r||^2 into *d_acc
 int launch_residual_mixed(const Level<double>& L, const double* k64, const double* x64, const float* b32, float* r32,
                           double* d_acc, cudaStream_t st);
+// z-marching residual for uniform grids (march_kernel.cuh): r = b - A x (r may be NULL), ||r||^2 added to *acc (may be NULL)
+bool march_supported(int nx, int ny, int nz, double hx, double hy, double hz);
+template <typename TXT, typename TB>
+int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], const TXT* x, const TXT* k, const TB* b, TB* r,
+                          double* acc, cudaStream_t st);
 int launch_axpy_mixed(size_t n, double* x64, const float* e32, cudaStream_t st);  // x64 += e32
 int launch_cast_f2d(size_t n, const float* a, double* b, cudaStream_t st);
 int launch_cast_d2f(size_t n, const double* a, float* b, cudaStream_t st);

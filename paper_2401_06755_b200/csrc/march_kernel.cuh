@@ -1,0 +1,220 @@
+// march_kernel.cuh -- z-marching residual kernel for uniform grids in any precision (sm_100a):
+//   r = b - A x  (optionally stored) and sum r^2 accumulated in fp64,
+// used by the solve loops: TX = double, TB = float is the fp64 defect of the
+// mixed-precision loop (reading C6 "fp32 reading", C8), TX = TB = double / float the plain loops.
+//
+// Same arithmetic as lean_kernel.cuh (reading C1/C2, Eqs. 8, 12-13 P:109-114, 146-159; uniform spacing:
+// the face weights vanish, edge neighbours carry 2 cc, corner neighbours cc, cc = 1/(24 h^2)):
+//   S(f)_i = 2 E(f)_i + Cn(f)_i,   r = b + cc (k S(x) + S(k x) - (32 k + S(k)) x)
+//   constant coefficient: r = b + cc (2 S(x) - 64 x).
+// A block owns a TX x TY column and marches along z.  Each plane of x and k is copied once into a
+// double-buffered shared tile WITH its halo already evaluated (ghost = s * mirror; k ghosts are
+// plain copies), so the arithmetic has no boundary cases.  Each thread owns 4 consecutive x points of one
+// row, reads its 3 rows, forms the row sums R(c) = f(c-1) + f(c+1), T = R + 2 f and the in-plane sums
+//   Dg = R_0 + R_2,  Pp = T_0 + T_2 + 2 R_1,   S[z] = Pp[z-1] + 2 Dg[z] + Pp[z+1]
+// with two rolling accumulators per point and field.  One __syncthreads per plane.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace mgb {
+namespace mk {
+
+struct MParams {
+    int nx, ny, nz;
+    int zchunk;
+    double s[6];     // halo factors x-, x+, y-, y+, z-, z+
+    double cc;       // 1 / (24 h^2)
+};
+
+constexpr int LX = 16, LY = 16, NT = LX * LY;
+constexpr int TX = 4 * LX, TY = LY;
+constexpr int PXS = TX + 8, PYS = TY + 2;     // staged row: [pad.., halo, TX own, halo, pad..]; own columns 16-byte aligned
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { typedef float4 type; };
+template <> struct Vec4<double> { typedef double4 type; };
+
+template <typename T>
+__device__ __forceinline__ void load4(const T* p, T (&v)[4]) {
+    if (sizeof(T) == 4) {
+        const float4 t = *reinterpret_cast<const float4*>(p);
+        v[0] = (T)t.x; v[1] = (T)t.y; v[2] = (T)t.z; v[3] = (T)t.w;
+    } else {
+        const double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2);
+        v[0] = (T)a.x; v[1] = (T)a.y; v[2] = (T)b.x; v[3] = (T)b.y;
+    }
+}
+
+// in-plane sums of one field for the thread's 4 points from its 3 staged rows (each: l, v0..v3, r)
+template <typename T>
+__device__ __forceinline__ void plane_sums(const T (&f)[3][6], T (&Dg)[4], T (&Pp)[4]) {
+    T R[3][4];
+#pragma unroll
+    for (int q = 0; q < 3; ++q)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) R[q][c] = f[q][c] + f[q][c + 2];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        Dg[c] = R[0][c] + R[2][c];
+        Pp[c] = (Dg[c] + T(2) * (f[0][c + 1] + f[2][c + 1])) + T(2) * R[1][c];
+    }
+}
+
+template <typename TXT, typename TB, bool VAR>
+__global__ void __launch_bounds__(NT, (sizeof(TXT) == 8 ? 1 : 2))
+march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __restrict__ kc, const TB* __restrict__ b,
+                      TB* __restrict__ r, double* __restrict__ acc) {
+    typedef TXT T;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    T* sm = reinterpret_cast<T*>(smraw);
+    constexpr int PLANE = PXS * PYS;
+    T* const xs = sm;                  // x planes [2], then k planes [2]
+    T* const ks = sm + 2 * PLANE;
+    __shared__ double red[NT / 32];
+
+    const int tid = threadIdx.x, lx = tid % LX, ly = tid / LX;
+    const int nx = P.nx, ny = P.ny, nz = P.nz;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+    const int zc0 = blockIdx.z * P.zchunk, zc1 = min(zc0 + P.zchunk, nz);
+    const int gi0 = x0 + 4 * lx, gj = y0 + ly;
+    const bool active = gi0 < nx && gj < ny;
+    constexpr int OFF = sizeof(T) == 4 ? 4 : 2;   // staged column of the tile's first own column (16-byte aligned)
+
+    // staging: cell (row rr, column cq) of the tile <- global (y0 - 1 + rr, x0 - 1 + cq), mirrored at the faces.
+    // Each thread stages the same NE cells of every plane: shared offsets, in-plane global offsets and a mask of the
+    // cells that are ghosts are z-invariant.  The copy is asynchronous (cp.async, global -> shared without registers) and
+    // overlaps the arithmetic of the current plane; ghost cells are scaled in place by their owner afterwards.
+    constexpr int NCELL = (TX + 2) * PYS, NE = (NCELL + NT - 1) / NT;
+    int soff[NE], goff[NE];
+    unsigned gmask = 0;                  // bit e: cell e is an x / y ghost (factor may differ from 1)
+    auto xyfac = [&](int e) {            // halo factor of cell e (rare path)
+        const int cell = tid + e * NT, rr = cell / (TX + 2), cq = cell - rr * (TX + 2);
+        const int gy = y0 - 1 + rr, gx = x0 - 1 + cq;
+        T f = T(1);
+        if (gy < 0) f *= (T)P.s[2]; else if (gy >= ny) f *= (T)P.s[3];
+        if (gx < 0) f *= (T)P.s[0]; else if (gx >= nx) f *= (T)P.s[1];
+        return f;
+    };
+#pragma unroll
+    for (int e = 0; e < NE; ++e) {
+        const int cell = min(tid + e * NT, NCELL - 1);          // the surplus threads of the last round repeat the last cell
+        const int rr = cell / (TX + 2), cq = cell - rr * (TX + 2);
+        int gy = y0 - 1 + rr, gx = x0 - 1 + cq;
+        bool gh = false;
+        if (gy < 0) { gy = -1 - gy; gh = true; } else if (gy >= ny) { gy = 2 * ny - 1 - gy; gh = true; }
+        if (gx < 0) { gx = -1 - gx; gh = true; } else if (gx >= nx) { gx = 2 * nx - 1 - gx; gh = true; }
+        gy = min(max(gy, 0), ny - 1); gx = min(max(gx, 0), nx - 1);          // cells beyond a partial tile: any valid address
+        soff[e] = rr * PXS + OFF - 1 + cq;
+        goff[e] = gy * nx + gx;
+        if (gh && tid + e * NT < NCELL) gmask |= 1u << e;
+    }
+    const uint32_t xs_a = (uint32_t)__cvta_generic_to_shared(xs), ks_a = (uint32_t)__cvta_generic_to_shared(ks);
+    auto stage = [&](int p) {            // issue the copies of plane p
+        const int zs = p < 0 ? -1 - p : (p >= nz ? 2 * nz - 1 - p : p);
+        const size_t zoff = (size_t)zs * ny * nx;
+        const uint32_t bo = (uint32_t)((p & 1) * PLANE);
+#pragma unroll
+        for (int e = 0; e < NE; ++e) {
+            const uint32_t so = (bo + (uint32_t)soff[e]) * (uint32_t)sizeof(T);
+            if (sizeof(T) == 4) {
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(xs_a + so), "l"(x + zoff + goff[e]) : "memory");
+                if (VAR) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(ks_a + so), "l"(kc + zoff + goff[e]) : "memory");
+            } else {
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(xs_a + so), "l"(x + zoff + goff[e]) : "memory");
+                if (VAR) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(ks_a + so), "l"(kc + zoff + goff[e]) : "memory");
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    auto stage_finish = [&](int p) {     // wait for this thread's copies of plane p and scale its ghost cells
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        const bool zg = p < 0 || p >= nz;
+        if (gmask || zg) {
+            const T fz = p < 0 ? (T)P.s[4] : (p >= nz ? (T)P.s[5] : T(1));
+            T* xd = xs + (p & 1) * PLANE;
+#pragma unroll
+            for (int e = 0; e < NE; ++e)
+                if (tid + e * NT < NCELL && (zg || ((gmask >> e) & 1u))) xd[soff[e]] *= fz * xyfac(e);
+        }
+    };
+
+    T xA[4], xB[4], zA[4], zB[4], kA[4], kB[4], xo[4], ko[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { xA[c] = xB[c] = zA[c] = zB[c] = kA[c] = kB[c] = xo[c] = T(0); ko[c] = T(1); }
+    double sq = 0.0;
+    const T cc = (T)P.cc;
+
+    stage(zc0 - 1);
+    stage_finish(zc0 - 1);
+    for (int p = zc0 - 1; p <= zc1; ++p) {
+        __syncthreads();                       // plane p is staged; everyone is done reading the other buffer
+        if (p < zc1) stage(p + 1);             // asynchronous copy into the other buffer
+        T bv[4] = {T(0), T(0), T(0), T(0)};
+        const int qc = p - 1;
+        if (qc >= zc0 && active) {
+            TB t4[4];
+            load4<TB>(b + ((size_t)qc * ny + gj) * nx + gi0, t4);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) bv[c] = (T)t4[c];
+        }
+        const T* xr = xs + (p & 1) * PLANE + ly * PXS + OFF - 1 + 4 * lx;      // column c0 - 1 of row ly - 1
+        const T* kr = ks + (p & 1) * PLANE + ly * PXS + OFF - 1 + 4 * lx;
+        T fx[3][6], fk[3][6], fz[3][6];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            fx[q][0] = xr[q * PXS]; fx[q][5] = xr[q * PXS + 5];
+            load4<T>(xr + q * PXS + 1, reinterpret_cast<T(&)[4]>(fx[q][1]));
+            if (VAR) {
+                fk[q][0] = kr[q * PXS]; fk[q][5] = kr[q * PXS + 5];
+                load4<T>(kr + q * PXS + 1, reinterpret_cast<T(&)[4]>(fk[q][1]));
+#pragma unroll
+                for (int c = 0; c < 6; ++c) fz[q][c] = fk[q][c] * fx[q][c];
+            }
+        }
+        T Dg[4], Pp[4], Sx[4], Sz[4], Sk[4];
+        plane_sums<T>(fx, Dg, Pp);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { Sx[c] = xA[c] + Pp[c]; xA[c] = xB[c] + T(2) * Dg[c]; xB[c] = Pp[c]; }
+        if (VAR) {
+            plane_sums<T>(fz, Dg, Pp);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { Sz[c] = zA[c] + Pp[c]; zA[c] = zB[c] + T(2) * Dg[c]; zB[c] = Pp[c]; }
+            plane_sums<T>(fk, Dg, Pp);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { Sk[c] = kA[c] + Pp[c]; kA[c] = kB[c] + T(2) * Dg[c]; kB[c] = Pp[c]; }
+        }
+        if (qc >= zc0 && active) {
+            T rv[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                if (VAR) rv[c] = bv[c] + cc * ((ko[c] * Sx[c] + Sz[c]) - (T(32) * ko[c] + Sk[c]) * xo[c]);
+                else rv[c] = bv[c] + cc * (T(2) * Sx[c] - T(64) * xo[c]);
+                sq += (double)rv[c] * (double)rv[c];
+            }
+            if (r) {
+                TB* dst = r + ((size_t)qc * ny + gj) * nx + gi0;
+                if (sizeof(TB) == 4) *reinterpret_cast<float4*>(dst) = make_float4((float)rv[0], (float)rv[1], (float)rv[2], (float)rv[3]);
+                else { *reinterpret_cast<double2*>(dst) = make_double2((double)rv[0], (double)rv[1]);
+                       *reinterpret_cast<double2*>(dst + 2) = make_double2((double)rv[2], (double)rv[3]); }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { xo[c] = fx[1][c + 1]; if (VAR) ko[c] = fk[1][c + 1]; }
+        if (p < zc1) stage_finish(p + 1);
+    }
+    // block sum of sq -> one atomic per block
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+    if ((tid & 31) == 0) red[tid >> 5] = sq;
+    __syncthreads();
+    if (tid == 0 && acc) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < NT / 32; ++w) t += red[w];
+        atomicAdd(acc, t);
+    }
+}
+
+}  // namespace mk
+}  // namespace mgb

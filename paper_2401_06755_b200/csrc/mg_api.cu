@@ -141,7 +141,10 @@ template <typename T>
 static int residual_norm(mg_solver* s, const T* x, const T* b, double* out) {
     LevelData& L = s->lv[0];
     MGB_CUDA(cudaMemsetAsync(s->d_acc, 0, sizeof(double), s->st));
-    int rc = launch_residual_norm<T>(lvl<T>(L), (const T*)L.k, x, b, (T*)nullptr, s->d_acc, s->st);
+    int rc;
+    if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
+        rc = launch_march_residual<T, T>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, x, (const T*)L.k, b, (T*)nullptr, s->d_acc, s->st);
+    else rc = launch_residual_norm<T>(lvl<T>(L), (const T*)L.k, x, b, (T*)nullptr, s->d_acc, s->st);
     if (rc) return rc;
     ++s->launches;
     double sq;
@@ -198,7 +201,11 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     ++s->launches;
     auto resid = [&](double* rel) -> int {
         MGB_CUDA(cudaMemsetAsync(s->d_acc, 0, sizeof(double), s->st));
-        int r2 = launch_residual_mixed(L.Ld, s->var_k ? s->k64 : nullptr, s->x64, b, s->r32, s->d_acc, s->st);
+        int r2;
+        if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
+            r2 = launch_march_residual<double, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, s->x64, s->var_k ? s->k64 : nullptr, b, s->r32,
+                                                      s->d_acc, s->st);
+        else r2 = launch_residual_mixed(L.Ld, s->var_k ? s->k64 : nullptr, s->x64, b, s->r32, s->d_acc, s->st);
         if (r2) return r2;
         ++s->launches;
         if ((r2 = read_acc(s, &sq))) return r2;

@@ -1,0 +1,41 @@
+// mg_march.cu -- host side of the z-marching residual kernel (march_kernel.cuh).
+#include "march_kernel.cuh"
+#include "solver.h"
+
+namespace mgb {
+
+bool march_supported(int nx, int ny, int nz, double hx, double hy, double hz) {
+    return hx == hy && hy == hz && nx % 4 == 0 && nx >= 4 && ny >= 1 && nz >= 1;
+}
+
+template <typename TXT, typename TB>
+int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], const TXT* x, const TXT* k, const TB* b, TB* r,
+                          double* acc, cudaStream_t st) {
+    mk::MParams P;
+    P.nx = nx; P.ny = ny; P.nz = nz;
+    for (int f = 0; f < 6; ++f) P.s[f] = s[f];
+    P.cc = 1.0 / (24.0 * h * h);
+    const int tx = (nx + mk::TX - 1) / mk::TX, ty = (ny + mk::TY - 1) / mk::TY;
+    // z chunks: one wave of resident blocks; every chunk pays 2 extra planes
+    const size_t smem = (size_t)4 * mk::PXS * mk::PYS * sizeof(TXT);
+    static int per_sm = 0;
+    if (!per_sm) {
+        int nb = 0;
+        MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mk::march_residual_kernel<TXT, TB, true>, mk::NT, smem));
+        per_sm = nb > 0 ? nb : 1;
+    }
+    const int want = (148 * per_sm) / (tx * ty);
+    const int nch = want < 1 ? 1 : (want > nz ? nz : want);
+    P.zchunk = (nz + nch - 1) / nch;
+    const dim3 grid(tx, ty, (nz + P.zchunk - 1) / P.zchunk);
+    if (k) mk::march_residual_kernel<TXT, TB, true><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc);
+    else mk::march_residual_kernel<TXT, TB, false><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc);
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
+
+template int launch_march_residual<double, float>(int, int, int, double, const double*, const double*, const double*, const float*, float*, double*, cudaStream_t);
+template int launch_march_residual<double, double>(int, int, int, double, const double*, const double*, const double*, const double*, double*, double*, cudaStream_t);
+template int launch_march_residual<float, float>(int, int, int, double, const double*, const float*, const float*, const float*, float*, double*, cudaStream_t);
+
+}  // namespace mgb
