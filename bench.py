@@ -37,7 +37,7 @@ E2E_CYCLES = 20          # the paper's fixed cycle count per pressure solve (P:4
 REF_TIME_BUDGET_S = 150  # wall-clock cap of the oracle arm
 # dram__bytes_read.sum + dram__bytes_write.sum of one fine-level smoother launch, from the ncu --set full
 # capture summarised in profiles/ (bytes per launch); None until a capture of the current kernel exists
-TRAFFIC_NCU = 258.3e6
+TRAFFIC_NCU = 250.7e6
 
 
 def load_peaks():
