@@ -2,7 +2,7 @@
 //
 // One stencil stage per pass, three variants:
 //   MODE_SWEEP   weighted-Jacobi sweep                                   x            -> x'
-//   MODE_PRO     prolongation + correction + sweep                      x + P x_c    -> x'
+//   MODE_PRO     prolongation + correction + sweep                      x + P x_c    -> x'   (x_c tile staged by TMA too)
 //   MODE_RR      residual, 8-child-mean restriction and the coarse level's first sweep from a
 //                zero guess                                              x            -> b_c, x_c
 //
@@ -73,7 +73,10 @@ struct LCfg {
     static constexpr int NS = 4;                                          // ring depth = planes in flight + 1
     static constexpr int PLANE = ((PX * PY + 31) / 32) * 32;              // floats per staged x / k plane (128-byte multiple)
     static constexpr int BPLANE = ((TX * TY + 31) / 32) * 32;             // floats per staged b tile
-    static constexpr int SLOT = PLANE * (VAR ? 2 : 1) + BPLANE;           // floats per ring slot: x, (k,) b
+    static constexpr int CPX = TX / 2 + 8, CPY = TY / 2 + 2;              // PRO: staged tile of the coarse correction
+    static constexpr int CPLANE = MODE == 1 ? ((CPX * CPY + 31) / 32) * 32 : 0;
+    static constexpr int SLOT = PLANE * (VAR ? 2 : 1) + BPLANE + CPLANE;  // floats per ring slot: x, (k,) b, (x_c)
+    static constexpr uint32_t CBOX_BYTES = (uint32_t)(CPX * CPY * sizeof(float));
     static constexpr uint32_t BOX_BYTES = (uint32_t)(PX * PY * sizeof(float));
     static constexpr uint32_t BBOX_BYTES = (uint32_t)(TX * TY * sizeof(float));
     static constexpr int BAR_FLOATS = 32;
@@ -93,6 +96,7 @@ __device__ __forceinline__ u64 bc2(float s) { return pk(s, s); }
 __device__ __forceinline__ float rcpa(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 // shared-memory loads by 32-bit shared-space address (no generic-address arithmetic in the plane loop)
 __device__ __forceinline__ float lds32(uint32_t a) { float r; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(a)); return r; }
+__device__ __forceinline__ u64 lds64(uint32_t a) { u64 r; asm volatile("ld.shared.b64 %0, [%1];" : "=l"(r) : "r"(a)); return r; }
 __device__ __forceinline__ void lds128(uint32_t a, u64& p, u64& q) { asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(p), "=l"(q) : "r"(a)); }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -172,11 +176,12 @@ __device__ __forceinline__ void out_row(const RT& a, const RT& m, const RT& c, u
 template <class C>
 __global__ void __launch_bounds__(C::NT, C::MINB)
 lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmk,
-            const __grid_constant__ CUtensorMap tmb, const LParams P) {
+            const __grid_constant__ CUtensorMap tmb, const __grid_constant__ CUtensorMap tmc, const LParams P) {
     constexpr int RY = C::RY, PX = C::PX, PY = C::PY, PLANE = C::PLANE, NS = C::NS, LX = C::LX, SLOT = C::SLOT;
     constexpr bool VAR = C::VAR;
     constexpr int MODE = C::MODE;
     constexpr int KOFF = PLANE, BOFF = PLANE * (VAR ? 2 : 1);      // k and b inside a ring slot
+    constexpr int COFF = BOFF + C::BPLANE;                         // PRO: coarse tile
     static_assert(RY == 2, "2 output rows per thread");
 
     extern __shared__ __align__(1024) float smf[];
@@ -201,6 +206,18 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         raddr[q] = ring_a + 4u * (uint32_t)(min(max(m - (y0 - 1), 0), PY - 1) * PX + 4 + c0);
     }
     const uint32_t baddr = ring_a + 4u * (uint32_t)(BOFF + (RY * ly) * C::TX + c0);
+    // PRO: the staged coarse tile starts at coarse cell (x0/2 - 4, y0/2 - 1): the first coordinate of a TMA box has to be
+    // 16-byte aligned like the x planes' x0 - 4 (a box starting at x0/2 - 1 raised an illegal-instruction fault on B200); rows (-1), (0, 1), (2) of the patch lie in 3
+    // coarse rows, the patch and its x neighbours in the 4 coarse cells gi0/2 - 1 .. gi0/2 + 2 (zero outside the domain)
+    uint32_t caddr[3] = {0u, 0u, 0u};
+    if (MODE == MODE_PRO) {
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            const int gq = gj0 - 1 + (e == 0 ? 0 : (e == 1 ? 1 : 3));
+            const int m = gq < 0 ? -1 - gq : (gq >= ny ? 2 * ny - 1 - gq : gq);
+            caddr[e] = ring_a + 4u * (uint32_t)(COFF + min(max((m >> 1) - ((y0 >> 1) - 1), 0), C::CPY - 1) * C::CPX + 3 + (c0 >> 1));
+        }
+    }
     // only the first and the last staged row of a patch can be ghost rows (factor s of the y faces)
     const u64 f0 = bc2((gj0 - 1 < 0) ? P.sy0 : 1.f), f3 = bc2((gj0 + RY >= ny) ? P.sy1 : 1.f);
     // x neighbours of the patch ends: halo cell (zero-filled outside the domain) + s * own end value at a domain face
@@ -213,11 +230,12 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         uint64_t* bar = &bars[it % NS];
         float* dst = ring + (it % NS) * SLOT;
         const bool wb = it >= 2;                                   // plane pbeg + it - 1 >= zc0
-        mbar_expect_tx(bar, C::BOX_BYTES * (VAR ? 2u : 1u) + (wb ? C::BBOX_BYTES : 0u));
+        mbar_expect_tx(bar, C::BOX_BYTES * (VAR ? 2u : 1u) + (wb ? C::BBOX_BYTES : 0u) + (MODE == MODE_PRO ? C::CBOX_BYTES : 0u));
         const int z = zsrc(pbeg + it);
         tma_load_plane(dst, &tmx, bar, x0 - 4, y0 - 1, z);
         if (VAR) tma_load_plane(dst + KOFF, &tmk, bar, x0 - 4, y0 - 1, z);
         if (wb) tma_load_plane(dst + BOFF, &tmb, bar, x0, y0, pbeg + it - 1);
+        if (MODE == MODE_PRO) tma_load_plane(dst + COFF, &tmc, bar, (x0 >> 1) - 4, (y0 >> 1) - 1, z >> 1);
     };
 
     if (tid == 0) {
@@ -252,24 +270,6 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         constexpr int PAR = decltype(par_tag)::value;
         const int p = pbeg + it;
         const int slot = it & (NS - 1);
-        // ---- PRO: coarse correction of the staged rows, issued before the barrier wait ----
-        float2 pc[3]; float pl[3], pr[3];
-        if (MODE == MODE_PRO) {
-            // rows (-1), (0, 1), (2) of the patch lie in 3 coarse rows; the x neighbours in the adjacent coarse cells
-            const size_t cplane = (size_t)(zsrc(p) >> 1) * nyc;
-#pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                pc[q] = make_float2(0.f, 0.f); pl[q] = 0.f; pr[q] = 0.f;
-                const int gq = gj0 - 1 + (q == 0 ? 0 : (q == 1 ? 1 : 3));
-                const int m = gq < 0 ? -1 - gq : (gq >= ny ? 2 * ny - 1 - gq : gq);
-                const float* crow = P.xc + (cplane + (m >> 1)) * nxc;
-                if (active) {
-                    pc[q] = __ldg(reinterpret_cast<const float2*>(crow + (gi0 >> 1)));
-                    if (!lghost) pl[q] = __ldg(crow + ((gi0 - 1) >> 1));
-                    if (!rghost) pr[q] = __ldg(crow + ((gi0 + 4) >> 1));
-                }
-            }
-        }
         // ---- ring hand-back: everyone has finished iteration it - 1, so its slot can be refilled ----
         __syncthreads();
         if (tid == 0 && it >= 1 && it - 1 + NS < niter) {
@@ -291,9 +291,10 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
             lds128(a, w.p, w.q);
             w.l = lds32(a - 4); w.r = lds32(a + 16);
             if (MODE == MODE_PRO) {
-                const int e = q == 0 ? 0 : (q == 3 ? 2 : 1);
-                w.p = add2(w.p, bc2(pc[e].x)); w.q = add2(w.q, bc2(pc[e].y));
-                w.l += pl[e]; w.r += pr[e];
+                const uint32_t ca = caddr[q == 0 ? 0 : (q == 3 ? 2 : 1)] + so;
+                const u64 c12 = lds64(ca + 4);                       // coarse cells gi0/2, gi0/2 + 1
+                w.p = add2(w.p, bc2(lo(c12))); w.q = add2(w.q, bc2(hi(c12)));
+                w.l += lds32(ca); w.r += lds32(ca + 12);             // gi0/2 - 1, gi0/2 + 2
             }
             w.l = fmaf(glx, lo(w.p), w.l); w.r = fmaf(grx, hi(w.q), w.r);
             if (q == 1) { xo[PAR][0][0] = w.p; xo[PAR][0][1] = w.q; }

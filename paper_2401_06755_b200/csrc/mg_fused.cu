@@ -174,12 +174,14 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
         MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, lk::lean_kernel<C>, C::NT, C::SMEM));
         ctas_per_sm = nb > 0 ? nb : 1;
     }
-    CUtensorMap tmx, tmk, tmb;
+    CUtensorMap tmx, tmk, tmb, tmc;
     int rc;
     if ((rc = make_tmap(&tmx, src, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
     if ((rc = make_tmap(&tmb, b, L.nx, L.ny, L.nz, C::TX, C::TY))) return rc;
     if (VAR) { if ((rc = make_tmap(&tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
     else tmk = tmx;
+    if (MODE == lk::MODE_PRO) { if ((rc = make_tmap(&tmc, xc, L.nx / 2, L.ny / 2, L.nz / 2, C::CPX, C::CPY))) return rc; }
+    else tmc = tmx;
     lk::LParams P;
     std::memset(&P, 0, sizeof(P));
     P.nx = L.nx; P.ny = L.ny; P.nz = L.nz;
@@ -205,7 +207,7 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
         P.gc_const = first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
     }
     dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
-    lk::lean_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, P);
+    lk::lean_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, tmc, P);
     MGB_LAUNCH_CHECK();
     ++s->launches;
     return 0;
@@ -283,9 +285,11 @@ int sweeps_level(mg_solver* s, int l, float* cur, float* oth, const float* b, in
     const bool stream = fs->lp[l].stream && s->p.sweeps_per_pass == 1;
     if (stream || fs->lp[l].tiled) {
         bool pro = xc != nullptr;
-        if (pro && sweeps == 0) {
+        // the PRO pass stages x_c by TMA: its row pitch (nx / 2 floats) must be a multiple of 16 bytes
+        if (pro && (sweeps == 0 || (stream && (L.nx / 2) % 4 != 0))) {
             if ((rc = launch_prolong_add<float>(L.nx, L.ny, L.nz, xc, cur, s->st))) return rc;
             ++s->launches;
+            pro = false;
         }
         while (sweeps > 0) {
             const int ns = (!stream && sweeps >= 2) ? 2 : 1;
