@@ -245,6 +245,10 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
+    // Programmatic dependent launch: everything above touched only kernel parameters; the fields written by the previous
+    // kernel of the cycle are first read below.  The next kernel may begin its own prologue from here on.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0)
         for (int q = 0; q < NS && q < niter; ++q) issue(q);
 

@@ -47,6 +47,19 @@ int make_tmap(CUtensorMap* tm, const float* ptr, int nx, int ny, int nz, int px,
     return 0;
 }
 
+// Launch with programmatic stream serialisation: the kernel may start while its predecessor in the stream is still running
+// and synchronises with it by griddepcontrol.wait before it first touches dependent data.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---- small helper kernels for levels below the tile size ------------------------------------
 __global__ void first_sweep_kernel(size_t n, const float* __restrict__ bc, const float* __restrict__ dinv, float g,
                                    float* __restrict__ xc) {
@@ -207,8 +220,7 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
         P.gc_const = first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
     }
     dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
-    lk::lean_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, tmc, P);
-    MGB_LAUNCH_CHECK();
+    MGB_CUDA(launch_pdl(lk::lean_kernel<C>, grid, dim3(C::NT), C::SMEM, s->st, tmx, tmk, tmb, tmc, P));
     ++s->launches;
     return 0;
 }
@@ -347,8 +359,7 @@ int launch_tail(mg_solver* s, int l, float* x, const float* b, int done, size_t 
         MGB_CUDA(cudaFuncSetAttribute(tk::tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_done = true;
     }
-    tk::tail_kernel<<<1, tk::NT, smem, s->st>>>(P);
-    MGB_LAUNCH_CHECK();
+    MGB_CUDA(launch_pdl(tk::tail_kernel, dim3(1), dim3(tk::NT), smem, s->st, P));
     ++s->launches;
     return 0;
 }

@@ -251,9 +251,13 @@ __global__ void __launch_bounds__(NT, 1) tail_kernel(const TailParams P) {
         for (int idx = threadIdx.x; idx < L.n; idx += NT) {
             L.K[idx] = P.k[t] ? P.k[t][idx] : 1.f;
             L.DI[idx] = P.dinv[t] ? P.dinv[t][idx] : P.dinv_const[t];
-            if (t == 0) { L.X[idx] = P.x[idx]; L.B[idx] = P.b[idx]; }
         }
     }
+    // Programmatic dependent launch: the coefficient data above is static during a cycle; x and b of the tail's finest
+    // level come from the previous kernel.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    for (int idx = threadIdx.x; idx < lv[0].n; idx += NT) { lv[0].X[idx] = P.x[idx]; lv[0].B[idx] = P.b[idx]; }
     __syncthreads();
     const float omega = P.omega;
     const int last = P.nlev - 1;
