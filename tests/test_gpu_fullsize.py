@@ -1,0 +1,91 @@
+"""GPU parity at BASELINE.json's full sizes for configs 4 and 5, in the launch configuration the
+library uses for them (fused fp32 kernels, CUDA graph).  The oracle computes whole-field references
+where one pass is affordable (a V-cycle, a sweep, an explicit stencil stage) and checks properties of
+the GPU result where a full oracle solve would take minutes (the converged pressure of the time step
+is checked through the oracle's residual of it and through the stages that follow, recomputed by
+the oracle from the GPU's pressure)."""
+import numpy as np
+import pytest
+
+from workloads import configs
+from test_gpu_mg import TOL, as_f64, make_solver, mg, quantise, rel_l2, to_dev  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def test_config4_full_size(mg, orc):
+    """BASELINE config 4 (512x512x256, four bubbles, 7 levels): smoothing sweeps and V(nu, nu) cycles."""
+    w = configs.config4()
+    g = orc.grid(w.nx, w.ny, w.nz, w.h)
+    alpha = quantise(w.fields["alpha"], "f32")
+    b = quantise(orc.pressure_rhs(g, w.fields["u"], w.fields["v"], w.fields["w"], 1.0), "f32")
+    k = orc.k_from_vof(alpha, w.rho_l, w.rho_g)
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32")
+    mg.mg_set_coefficient_from_vof(s, to_dev(alpha, "f32"), w.rho_l, w.rho_g)
+    db = to_dev(b, "f32")
+    x0 = quantise(0.01 * b, "f32")
+    dx = to_dev(x0, "f32")
+    mg.mg_smooth(s, dx, db, 3)
+    assert rel_l2(as_f64(dx), orc.smooth(g, w.bc, k, x0, b, w.omega, 3)) <= 3 * TOL["f32"]
+    for nu in (1, 2):
+        mg.mg_set_params(s, nu_pre=nu, nu_post=nu, coarse_sweeps=50, sweeps_per_pass=1, omega=w.omega, mixed_precision=1)
+        dx = to_dev(np.zeros(w.shape), "f32")
+        mg.mg_vcycle(s, dx, db)
+        x_o = orc.vcycle(g, w.bc, k, np.zeros(w.shape), b, w.levels, nu, nu)
+        assert rel_l2(as_f64(dx), x_o) <= 1e-4, "V(%d,%d)" % (nu, nu)
+    mg.mg_destroy(s)
+
+
+def test_config5_full_size(mg, orc):
+    """BASELINE config 5 (256^3 time step): every explicit stage against the oracle on the full grid, then one
+    flow_time_step: the pressure satisfies the oracle's residual test, and velocity / volume fraction equal the
+    oracle's projection and VoF update evaluated with that pressure."""
+    import torch
+    w = configs.config5()
+    g = orc.grid(w.nx, w.ny, w.nz, w.h)
+    Cf, u, v, ww = (quantise(w.fields[q], "f32") for q in ("alpha", "u", "v", "w"))
+    dC, du, dv, dw = (to_dev(a, "f32") for a in (Cf, u, v, ww))
+    # stage 2: two predictor iterations
+    qn = (u, v, ww)
+    qt1, qh1 = orc.mom_predictor(g, Cf, qn, qn, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
+    dqt = [torch.empty_like(dC) for _ in range(3)]; dqh = [torch.empty_like(dC) for _ in range(3)]
+    mg.mom_predictor(dC, (du, dv, dw), (du, dv, dw), w.h, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, dqt, dqh)
+    for c in range(3):
+        assert rel_l2(as_f64(dqt[c]), qt1[c]) <= TOL["f32"] and rel_l2(as_f64(dqh[c]), qh1[c]) <= TOL["f32"]
+    # stage 4 kernel on the initial fields
+    s_ref, c_ref = orc.vof_residual(g, Cf, u, v, ww, w.dt)
+    ds, dcn = torch.empty_like(dC), torch.empty_like(dC)
+    mg.vof_residual(dC, du, dv, dw, w.h, w.dt, ds, dcn)
+    assert rel_l2(as_f64(ds), s_ref) <= 5 * TOL["f32"] and rel_l2(as_f64(dcn), c_ref) <= TOL["f32"]
+    # the right-hand side the step will solve for, through the same public calls flow_time_step makes (deterministic):
+    # the oracle's own b differs from it by the fp32 cancellation error of a divergence (1e-5 relative), which would
+    # mask a 1e-6 residual test
+    dqt2 = [torch.empty_like(dC) for _ in range(3)]
+    mg.mom_predictor(dC, dqh, (du, dv, dw), w.h, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, dqt2, None)
+    db = torch.empty_like(dC)
+    mg.pressure_rhs(dqt2[0], dqt2[1], dqt2[2], w.h, w.dt, db)
+    b_gpu = as_f64(db)
+    qt_gpu = [as_f64(a) for a in dqt2]
+    del ds, dcn, dqt, dqh, dqt2, db, s_ref, c_ref
+    # the whole step on the GPU
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32")
+    dp = torch.empty_like(dC)
+    status, cyc, rel = mg.flow_time_step(s, dC, du, dv, dw, dp, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, w.tol, 100)
+    assert status == mg.MG_OK and rel < w.tol and cyc <= 40
+    # oracle: second predictor iteration and right-hand side (parity of those stages), then the residual of the GPU's pressure
+    qt2, _ = orc.mom_predictor(g, Cf, qh1, qn, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
+    for c in range(3):
+        assert rel_l2(qt_gpu[c], qt2[c]) <= 2 * TOL["f32"]
+    k = orc.k_from_vof(Cf, w.rho_l, w.rho_g)
+    assert rel_l2(b_gpu, orc.pressure_rhs(g, qt2[0], qt2[1], qt2[2], w.dt)) <= 50 * TOL["f32"]
+    p = as_f64(dp)
+    r = orc.residual(g, w.bc, k, p, b_gpu)
+    # the solver converged its fp64 iterate to rel < 1e-6; what it returns is that iterate rounded to fp32, and the
+    # rounding noise (6e-8 relative, all of it high-frequency) is amplified by the operator: floor of a few 1e-6
+    assert np.linalg.norm(r) / np.linalg.norm(b_gpu) < 1e-5
+    un, vn, wn = orc.project_velocity(g, w.bc, p, k, w.dt, qt_gpu[0], qt_gpu[1], qt_gpu[2])
+    for a, ref in ((du, un), (dv, vn), (dw, wn)):
+        assert rel_l2(as_f64(a), ref) <= 2 * TOL["f32"]
+    _, Cn = orc.vof_residual(g, Cf, un, vn, wn, w.dt)
+    assert rel_l2(as_f64(dC), Cn) <= 2 * TOL["f32"]
+    mg.mg_destroy(s)
