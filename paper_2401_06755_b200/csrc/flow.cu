@@ -1,6 +1,7 @@
 // flow.cu -- explicit stencil residuals that feed the pressure solve (rows a8-a10 of the hot
 // path): compressive-advection VoF residual, momentum advection-diffusion predictor, pressure
 // right-hand side and velocity projection, plus the config-5 time step built from them.
+// The kernels are in flow_march.cuh (z-marching, one column per thread).
 //
 // All filters are the NODAL (divided by m_l = dx dy dz, the paper's w_ml^-1) tensor
 // products of the 1-D trilinear-FE factors (Eqs. 9-11):
@@ -42,64 +43,6 @@ Geo<T> make_geo(const mg_grid* g, const int* bc) {
     return G;
 }
 
-constexpr int BX = 64, BY = 4;
-
-template <typename T>
-dim3 grid_for(const Geo<T>& G) { return dim3((G.nx + BX - 1) / BX, (G.ny + BY - 1) / BY, G.nz); }
-
-struct Nb {  // clamped neighbour indices (copy halo)
-    int ix[3], jy[3], kz[3];
-};
-
-template <typename T>
-__device__ __forceinline__ Nb neighbours(const Geo<T>& G, int i, int j, int k) {
-    Nb n;
-    n.ix[0] = i > 0 ? i - 1 : 0; n.ix[1] = i; n.ix[2] = i < G.nx - 1 ? i + 1 : G.nx - 1;
-    n.jy[0] = j > 0 ? j - 1 : 0; n.jy[1] = j; n.jy[2] = j < G.ny - 1 ? j + 1 : G.ny - 1;
-    n.kz[0] = k > 0 ? k - 1 : 0; n.kz[1] = k; n.kz[2] = k < G.nz - 1 ? k + 1 : G.nz - 1;
-    return n;
-}
-
-template <typename T>
-__device__ __forceinline__ size_t at(const Geo<T>& G, const Nb& n, int a, int b, int c) {
-    return (size_t)n.ix[a] + (size_t)G.nx * ((size_t)n.jy[b] + (size_t)G.ny * n.kz[c]);
-}
-
-// gradient of f by the FE first-derivative filters (Eq. 11 / m_l), copy halo
-template <typename T>
-__device__ __forceinline__ void fe_gradient(const Geo<T>& G, const Nb& n, const T* __restrict__ f, T& gx, T& gy, T& gz) {
-    T sx = T(0), sy = T(0), sz = T(0);
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const T v = f[at(G, n, a, b, c)];
-                if (a != 1) sx += (G.D[0][a] * G.M[b] * G.M[c]) * v;
-                if (b != 1) sy += (G.M[a] * G.D[1][b] * G.M[c]) * v;
-                if (c != 1) sz += (G.M[a] * G.M[b] * G.D[2][c]) * v;
-            }
-    gx = sx; gy = sy; gz = sz;
-}
-
-// Eq. 29: a = alpha_a f(adv; w_m/m_l - E), alpha_a = 2
-template <typename T>
-__device__ __forceinline__ T mixed_mass(const Geo<T>& G, const Nb& n, const T* __restrict__ adv) {
-    T s = T(0);
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                T wgt = G.M[a] * G.M[b] * G.M[c];
-                if (a == 1 && b == 1 && c == 1) wgt -= T(1);
-                s += wgt * adv[at(G, n, a, b, c)];
-            }
-    return T(2) * s;
-}
-
 // Eqs. 26/27: alpha_kabs = 1/16 (p = 1), eps_k = 1e-7; Eq. 27 on
 // uniform spacing, Eq. 26 otherwise (reading C9-ii).
 template <typename T>
@@ -114,176 +57,7 @@ __device__ __forceinline__ T k_abs_pg(const Geo<T>& G, T a, T px, T py, T pz) {
 template <typename T> __device__ __forceinline__ T tmin(T a, T b) { return a < b ? a : b; }
 template <typename T> __device__ __forceinline__ T tmax(T a, T b) { return a > b ? a : b; }
 
-#define POINT_PROLOGUE                                                                          \
-    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y, k = blockIdx.z; \
-    if (i >= G.nx || j >= G.ny) return;                                                          \
-    const Nb n = neighbours(G, i, j, k);                                                         \
-    const size_t c0 = (size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k)
-
-// steps 1-2 of reading C9: adv = u psi_x + v psi_y + w psi_z
-template <typename T>
-__global__ void __launch_bounds__(BX* BY) advection_kernel(const Geo<T> G, const T* __restrict__ psi, const T* __restrict__ u,
-                                                          const T* __restrict__ v, const T* __restrict__ w, T* __restrict__ adv) {
-    POINT_PROLOGUE;
-    T px, py, pz;
-    fe_gradient(G, n, psi, px, py, pz);
-    adv[c0] = u[c0] * px + v[c0] * py + w[c0] * pz;
-}
-
-// steps 3-10 of reading C9: directional diffusion coefficients k^x, k^y, k^z of the compressive scheme
-template <typename T>
-__global__ void __launch_bounds__(BX* BY) vof_coeff_kernel(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ u,
-                                                          const T* __restrict__ v, const T* __restrict__ w,
-                                                          const T* __restrict__ adv, T k_min, T k_max, T* __restrict__ kx,
-                                                          T* __restrict__ ky, T* __restrict__ kz) {
-    POINT_PROLOGUE;
-    const T Kp = T(300), Km = T(300);        // K+, K- 
-    const T beta = T(0.1), eps_x = T(1e-4);  // Eq. 36
-    const T Kcal = T(3);                     // Eq. 39
-    T Cx, Cy, Cz;
-    fe_gradient(G, n, C, Cx, Cy, Cz);
-    const T a = mixed_mass(G, n, adv);                                   // step 3, Eq. 29
-    const T kabs = k_abs_pg(G, a, Cx, Cy, Cz);                           // step 4, Eq. 27
-    const T C0 = C[c0];
-    T S[3];                                                              // step 5, Eq. 33
-    S[0] = (C0 - C[at(G, n, 0, 1, 1)]) * (C[at(G, n, 2, 1, 1)] - C0);
-    S[1] = (C0 - C[at(G, n, 1, 0, 1)]) * (C[at(G, n, 1, 2, 1)] - C0);
-    S[2] = (C0 - C[at(G, n, 1, 1, 0)]) * (C[at(G, n, 1, 1, 2)] - C0);
-    if (C0 > T(0.95) || C0 < T(0.05)) S[0] = S[1] = S[2] = T(-1);        // override
-    const T uu = u[c0], vv = v[c0], ww = w[c0];
-    const T g2 = Cx * Cx + Cy * Cy + Cz * Cz;
-    const T gq = (uu * Cx + vv * Cy + ww * Cz) / (eps_x + g2);           // step 7, Eq. 37
-    const T us = gq * Cx, vs = gq * Cy, ws = gq * Cz;
-    const T kneg = -beta * (uu * uu + vv * vv + ww * ww) /               // step 8, Eq. 36
-                   (eps_x + g2 * (fabs(us) + fabs(vs) + fabs(ws)) / T(3));
-    T* const out[3] = {kx, ky, kz};
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        const T wp = -tmax(T(-1), tmin(T(0), Kp * S[d]));                // step 6, Eq. 35
-        const T wm = tmin(T(1), tmax(T(0), Km * S[d]));
-        const T kk = wp * (Kcal * kabs) + wm * (kneg / G.h[d]);          // steps 9, Eqs. 38-40
-        out[d][c0] = tmax(-k_min, tmin(k_max, kk));                      // step 10, Eq. 41
-    }
-}
-
-// steps 11-12: sC = adv + sum_d diff_d, diff_d = sum_{j != i} (-W^dd_ij) 1/2 (k^d_i + k^d_j)(C_i - C_j)
-// (Eq. 12 collapsed); Cnew = C - dt sC (Eq. 55)
-template <typename T>
-__global__ void __launch_bounds__(BX* BY) vof_diffusion_kernel(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ adv,
-                                                              const T* __restrict__ kx, const T* __restrict__ ky,
-                                                              const T* __restrict__ kz, T dt, T* __restrict__ sC,
-                                                              T* __restrict__ Cnew) {
-    POINT_PROLOGUE;
-    const T C0 = C[c0], kx0 = kx[c0], ky0 = ky[c0], kz0 = kz[c0];
-    T dx = T(0), dy = T(0), dz = T(0);
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                if (a == 1 && b == 1 && c == 1) continue;
-                const size_t q = at(G, n, a, b, c);
-                const T dC = T(0.5) * (C0 - C[q]);
-                dx -= (G.K[0][a] * G.M[b] * G.M[c]) * (kx0 + kx[q]) * dC;
-                dy -= (G.M[a] * G.K[1][b] * G.M[c]) * (ky0 + ky[q]) * dC;
-                dz -= (G.M[a] * G.M[b] * G.K[2][c]) * (kz0 + kz[q]) * dC;
-            }
-    const T s = adv[c0] + dx + dy + dz;
-    if (sC) sC[c0] = s;
-    if (Cnew) Cnew[c0] = C0 - dt * s;
-}
-
-// momentum: k_c = rho min{k_max, k_abs(c)} + mu (Eqs. 30-32; k_square of the lost Eq. 28 omitted)
-template <typename T>
-__global__ void __launch_bounds__(BX* BY) mom_coeff_kernel(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ comp,
-                                                          const T* __restrict__ u, const T* __restrict__ v, const T* __restrict__ w,
-                                                          const T* __restrict__ adv, T rho_l, T rho_g, T mu_l, T mu_g,
-                                                          T* __restrict__ kc) {
-    POINT_PROLOGUE;
-    T px, py, pz;
-    fe_gradient(G, n, comp, px, py, pz);
-    const T a = mixed_mass(G, n, adv);
-    const T Cc = C[c0];
-    const T rho = rho_l * Cc + rho_g * (T(1) - Cc);
-    const T mu = mu_l * Cc + mu_g * (T(1) - Cc);
-    const T kmax = G.h[0] * fabs(u[c0]) + G.h[1] * fabs(v[c0]) + G.h[2] * fabs(w[c0]);   // Eq. 30
-    const T kabs = k_abs_pg(G, a, px, py, pz);
-    kc[c0] = rho * tmin(kmax, kabs) + mu;
-}
-
-// s = rho adv + f^lap(c, k_c; w_lap) (Eq. 18 without pressure / source terms), q~ = q_n - dt s / rho (Eq. 45,
-// sigma = 0), q_half' = (q_n + q~)/2 (Eq. 46)
-template <typename T>
-__global__ void __launch_bounds__(BX* BY) mom_update_kernel(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ comp,
-                                                           const T* __restrict__ kc, const T* __restrict__ adv,
-                                                           const T* __restrict__ qn, T rho_l, T rho_g, T dt, T* __restrict__ qt,
-                                                           T* __restrict__ qhn) {
-    POINT_PROLOGUE;
-    const T x0 = comp[c0], k0 = kc[c0];
-    T diff = T(0);
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                if (a == 1 && b == 1 && c == 1) continue;
-                const size_t q = at(G, n, a, b, c);
-                const T wl = G.K[0][a] * G.M[b] * G.M[c] + G.M[a] * G.K[1][b] * G.M[c] + G.M[a] * G.M[b] * G.K[2][c];
-                diff -= wl * T(0.5) * (k0 + kc[q]) * (x0 - comp[q]);
-            }
-    const T Cc = C[c0];
-    const T rho = rho_l * Cc + rho_g * (T(1) - Cc);
-    const T s = rho * adv[c0] + diff;
-    const T t = qn[c0] - dt * s / rho;
-    qt[c0] = t;
-    if (qhn) qhn[c0] = T(0.5) * (qn[c0] + t);
-}
-
-// b = -(1/dt)(f(u; w_x) + f(v; w_y) + f(w; w_z))  (reading C10; Eq. 53 structure)
-template <typename T>
-__global__ void __launch_bounds__(BX* BY) pressure_rhs_kernel(const Geo<T> G, const T* __restrict__ u, const T* __restrict__ v,
-                                                             const T* __restrict__ w, T inv_dt, T* __restrict__ bout) {
-    POINT_PROLOGUE;
-    T sx = T(0), sy = T(0), sz = T(0);
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const size_t q = at(G, n, a, b, c);
-                if (a != 1) sx += (G.D[0][a] * G.M[b] * G.M[c]) * u[q];
-                if (b != 1) sy += (G.M[a] * G.D[1][b] * G.M[c]) * v[q];
-                if (c != 1) sz += (G.M[a] * G.M[b] * G.D[2][c]) * w[q];
-            }
-    bout[c0] = -(sx + sy + sz) * inv_dt;
-}
-
-// q <- q - dt k f(p; w_x|y|z) (Eq. 54); halo of p = s * mirror with the solver's factors
-template <typename T>
-__global__ void __launch_bounds__(BX* BY) project_kernel(const Geo<T> G, const T* __restrict__ p, const T* __restrict__ kc, T dt,
-                                                        T* __restrict__ u, T* __restrict__ v, T* __restrict__ w) {
-    POINT_PROLOGUE;
-    T fx[3] = {i > 0 ? T(1) : G.s[0], T(1), i < G.nx - 1 ? T(1) : G.s[1]};
-    T fy[3] = {j > 0 ? T(1) : G.s[2], T(1), j < G.ny - 1 ? T(1) : G.s[3]};
-    T fz[3] = {k > 0 ? T(1) : G.s[4], T(1), k < G.nz - 1 ? T(1) : G.s[5]};
-    T gx = T(0), gy = T(0), gz = T(0);
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const T val = fx[a] * fy[b] * fz[c] * p[at(G, n, a, b, c)];
-                if (a != 1) gx += (G.D[0][a] * G.M[b] * G.M[c]) * val;
-                if (b != 1) gy += (G.M[a] * G.D[1][b] * G.M[c]) * val;
-                if (c != 1) gz += (G.M[a] * G.M[b] * G.D[2][c]) * val;
-            }
-    const T f = dt * kc[c0];
-    u[c0] -= f * gx; v[c0] -= f * gy; w[c0] -= f * gz;
-}
+#include "flow_march.cuh"
 
 struct Scratch {  // stream-ordered scratch fields
     cudaStream_t st;
@@ -311,10 +85,9 @@ int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T
     T *adv = (T*)ws.p[0], *kx = (T*)ws.p[1], *ky = (T*)ws.p[2], *kz = (T*)ws.p[3];
     const double hmax = fmax(g->hx, fmax(g->hy, g->hz)), hmin = fmin(g->hx, fmin(g->hy, g->hz));
     const double k_min = 1e-4 / dt * hmax * hmax, k_max = 0.05 / dt * hmin * hmin;   // Eq. 42
-    const dim3 grd = grid_for(G), blk(BX, BY);
-    advection_kernel<T><<<grd, blk, 0, st>>>(G, C, u, v, w, adv);
-    vof_coeff_kernel<T><<<grd, blk, 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
-    vof_diffusion_kernel<T><<<grd, blk, 0, st>>>(G, C, adv, kx, ky, kz, (T)dt, sC, Cnew);
+    advection_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv);
+    vof_coeff_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
+    vof_diffusion_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, adv, kx, ky, kz, (T)dt, sC, Cnew);
     MGB_LAUNCH_CHECK();
     return 0;
 }
@@ -328,11 +101,10 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
     int rc = ws.alloc(2, bytes);
     if (rc) return rc;
     T *adv = (T*)ws.p[0], *kc = (T*)ws.p[1];
-    const dim3 grd = grid_for(G), blk(BX, BY);
     for (int c = 0; c < 3; ++c) {
-        advection_kernel<T><<<grd, blk, 0, st>>>(G, qh[c], qh[0], qh[1], qh[2], adv);
-        mom_coeff_kernel<T><<<grd, blk, 0, st>>>(G, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc);
-        mom_update_kernel<T><<<grd, blk, 0, st>>>(G, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c],
+        advection_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, qh[c], qh[0], qh[1], qh[2], adv);
+        mom_coeff_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc);
+        mom_update_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c],
                                                   qhn ? qhn[c] : (T*)nullptr);
     }
     MGB_LAUNCH_CHECK();
@@ -342,7 +114,7 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
 template <typename T>
 int pressure_rhs_t(const mg_grid* g, const T* u, const T* v, const T* w, double dt, T* b, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
-    pressure_rhs_kernel<T><<<grid_for(G), dim3(BX, BY), 0, st>>>(G, u, v, w, (T)(1.0 / dt), b);
+    pressure_rhs_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, u, v, w, (T)(1.0 / dt), b);
     MGB_LAUNCH_CHECK();
     return 0;
 }
@@ -350,7 +122,7 @@ int pressure_rhs_t(const mg_grid* g, const T* u, const T* v, const T* w, double 
 template <typename T>
 int project_t(const mg_grid* g, const int* bc, const T* p, const T* k, double dt, T* u, T* v, T* w, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, bc);
-    project_kernel<T><<<grid_for(G), dim3(BX, BY), 0, st>>>(G, p, k, (T)dt, u, v, w);
+    project_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, p, k, (T)dt, u, v, w);
     MGB_LAUNCH_CHECK();
     return 0;
 }
