@@ -65,6 +65,18 @@ struct Scratch {  // stream-ordered scratch fields
     int n = 0;
     explicit Scratch(cudaStream_t s) : st(s) {}
     int alloc(int count, size_t bytes) {
+        // keep freed scratch in the device's default pool: with the default release threshold (0) every synchronisation
+        // hands the memory back to the driver and the next call pays milliseconds to map it again
+        static bool pool_set[64] = {false};
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && !pool_set[dev]) {
+            cudaMemPool_t pool;
+            if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+                unsigned long long keep = ~0ull;
+                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            }
+            pool_set[dev] = true;
+        }
         for (n = 0; n < count; ++n)
             if (cudaMallocAsync(&p[n], bytes, st) != cudaSuccess) {
                 set_error("flow scratch: cudaMallocAsync failed: %s", cudaGetErrorString(cudaGetLastError()));
