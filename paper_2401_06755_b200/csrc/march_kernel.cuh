@@ -1,5 +1,5 @@
 // march_kernel.cuh -- z-marching residual kernel for uniform grids in any precision (sm_100a):
-//   r = b - A x  (optionally stored) and sum r^2 accumulated in fp64,
+//   r = b - A x  (optionally stored; y = A x when b is NULL) and sum r^2 accumulated in fp64,
 // used by the solve loops: TX = double, TB = float is the fp64 defect of the
 // mixed-precision loop (reading C6 "fp32 reading", C8), TX = TB = double / float the plain loops.
 //
@@ -152,7 +152,7 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
         if (p < zc1) stage(p + 1);             // asynchronous copy into the other buffer
         T bv[4] = {T(0), T(0), T(0), T(0)};
         const int qc = p - 1;
-        if (qc >= zc0 && active) {
+        if (qc >= zc0 && active && b) {
             TB t4[4];
             load4<TB>(b + ((size_t)qc * ny + gj) * nx + gi0, t4);
 #pragma unroll
@@ -190,6 +190,7 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
             for (int c = 0; c < 4; ++c) {
                 if (VAR) rv[c] = bv[c] + cc * ((ko[c] * Sx[c] + Sz[c]) - (T(32) * ko[c] + Sk[c]) * xo[c]);
                 else rv[c] = bv[c] + cc * (T(2) * Sx[c] - T(64) * xo[c]);
+                if (!b) rv[c] = -rv[c];          // no right-hand side: the output is y = A x
                 sq += (double)rv[c] * (double)rv[c];
             }
             if (r) {

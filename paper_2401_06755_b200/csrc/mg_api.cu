@@ -429,6 +429,13 @@ int mg_apply_operator(mg_solver* s, const void* d_x, void* d_y) {
     if (!d_x || !d_y || d_x == d_y) { set_error("mg_apply_operator: NULL or aliased argument"); return MG_EINVAL; }
     LevelData& L = s->lv[0];
     ++s->launches;
+    if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz)) {   // uniform grid: z-marching kernel, b = NULL -> y = A x
+        if (s->dtype == MG_F32)
+            return launch_march_residual<float, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, (const float*)d_x, (const float*)L.k,
+                                                       (const float*)nullptr, (float*)d_y, nullptr, s->st);
+        return launch_march_residual<double, double>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, (const double*)d_x, (const double*)L.k,
+                                                     (const double*)nullptr, (double*)d_y, nullptr, s->st);
+    }
     if (s->dtype == MG_F32) return launch_apply<float>(L.Lf, (const float*)L.k, (const float*)d_x, (float*)d_y, s->st);
     return launch_apply<double>(L.Ld, (const double*)L.k, (const double*)d_x, (double*)d_y, s->st);
 }
@@ -438,6 +445,13 @@ int mg_residual(mg_solver* s, const void* d_x, const void* d_b, void* d_r) {
     if (!d_x || !d_b || !d_r || d_x == d_r) { set_error("mg_residual: NULL or aliased argument"); return MG_EINVAL; }
     LevelData& L = s->lv[0];
     ++s->launches;
+    if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz)) {
+        if (s->dtype == MG_F32)
+            return launch_march_residual<float, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, (const float*)d_x, (const float*)L.k,
+                                                       (const float*)d_b, (float*)d_r, nullptr, s->st);
+        return launch_march_residual<double, double>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, (const double*)d_x, (const double*)L.k,
+                                                     (const double*)d_b, (double*)d_r, nullptr, s->st);
+    }
     if (s->dtype == MG_F32)
         return launch_residual<float>(L.Lf, (const float*)L.k, (const float*)d_x, (const float*)d_b, (float*)d_r, s->st);
     return launch_residual<double>(L.Ld, (const double*)L.k, (const double*)d_x, (const double*)d_b, (double*)d_r, s->st);
