@@ -8,11 +8,12 @@
 //   S(f)_i = 2 E(f)_i + Cn(f)_i,   r = b + cc (k S(x) + S(k x) - (32 k + S(k)) x)
 //   constant coefficient: r = b + cc (2 S(x) - 64 x).
 // A block owns a TX x TY column and marches along z.  Each plane of x and k is copied once into a
-// double-buffered shared tile WITH its halo already evaluated (ghost = s * mirror; k ghosts are
+// 4-deep ring of shared tiles WITH its halo already evaluated (ghost = s * mirror; k ghosts are
 // plain copies), so the arithmetic has no boundary cases.  Each thread owns 4 consecutive x points of one
 // row, reads its 3 rows, forms the row sums R(c) = f(c-1) + f(c+1), T = R + 2 f and the in-plane sums
 //   Dg = R_0 + R_2,  Pp = T_0 + T_2 + 2 R_1,   S[z] = Pp[z-1] + 2 Dg[z] + Pp[z+1]
-// with two rolling accumulators per point and field.  One __syncthreads per plane.
+// with two rolling accumulators per point and field.  One __syncthreads per plane; three planes are in flight (cp.async)
+// while one is consumed.
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -28,8 +29,29 @@ struct MParams {
 };
 
 constexpr int LX = 16, LY = 16, NT = LX * LY;
+constexpr int NSTG = 4;                       // ring of staged planes: 3 planes are in flight while one is consumed
 constexpr int TX = 4 * LX, TY = LY;
-constexpr int PXS = TX + 8, PYS = TY + 2;     // staged row: [pad.., halo, TX own, halo, pad..]; own columns 16-byte aligned
+constexpr int PYS = TY + 2;
+// Layout of one staged row (own columns 0 .. TX - 1, halo columns -1 and TX), chosen so that the 16-byte loads of a warp are
+// bank-conflict free.  fp32: linear, [pad x3, halo, TX own, halo, pad x3]: a thread's 4 floats are one aligned 16-byte word
+// and lanes are contiguous.  fp64: a thread's 4 doubles are two 16-byte pairs 32 bytes apart, a 4-way conflict if stored
+// linearly (measured: 58 % of the shared-memory wavefronts were conflicts); so pairs are numbered pp = (col + 2) / 2 and the
+// odd pairs (a thread's first pair, and its right neighbour) go to the first half of the row, the even pairs (second pair,
+// left neighbour) to the second half -- each load of a warp then touches consecutive 16-byte slots.
+template <typename T> struct Lay;
+template <> struct Lay<float> {
+    static constexpr int ROW = TX + 8;
+    __host__ __device__ static constexpr int off(int col) { return 4 + col; }
+    __host__ __device__ static constexpr int own0(int lx) { return 4 + 4 * lx; }       // columns c0, c0 + 1 (and c0 + 2, c0 + 3: same word)
+    __host__ __device__ static constexpr int own1(int lx) { return 4 + 4 * lx + 2; }
+};
+template <> struct Lay<double> {
+    static constexpr int HB = 2 * (LX + 1);          // start of the second half (even pairs), in elements
+    static constexpr int ROW = HB + 2 * (LX + 2);
+    __host__ __device__ static constexpr int off(int col) { return (((col + 2) >> 1) & 1 ? 0 : HB) + 2 * ((col + 2) >> 2) + ((col + 2) & 1); }
+    __host__ __device__ static constexpr int own0(int lx) { return 2 * lx; }
+    __host__ __device__ static constexpr int own1(int lx) { return HB + 2 * lx + 2; }
+};
 
 template <typename T> struct Vec4;
 template <> struct Vec4<float> { typedef float4 type; };
@@ -42,6 +64,18 @@ __device__ __forceinline__ void load4(const T* p, T (&v)[4]) {
         v[0] = (T)t.x; v[1] = (T)t.y; v[2] = (T)t.z; v[3] = (T)t.w;
     } else {
         const double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2);
+        v[0] = (T)a.x; v[1] = (T)a.y; v[2] = (T)b.x; v[3] = (T)b.y;
+    }
+}
+
+// 4 own values from the staged row: one 16-byte word (fp32; p1 = p0 + 2 is the same word) or two 16-byte pairs (fp64)
+template <typename T>
+__device__ __forceinline__ void load22(const T* p0, const T* p1, T* v) {
+    if (sizeof(T) == 4) {
+        const float4 t = *reinterpret_cast<const float4*>(p0);
+        v[0] = (T)t.x; v[1] = (T)t.y; v[2] = (T)t.z; v[3] = (T)t.w;
+    } else {
+        const double2 a = *reinterpret_cast<const double2*>(p0), b = *reinterpret_cast<const double2*>(p1);
         v[0] = (T)a.x; v[1] = (T)a.y; v[2] = (T)b.x; v[3] = (T)b.y;
     }
 }
@@ -68,9 +102,9 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
     typedef TXT T;
     extern __shared__ __align__(16) unsigned char smraw[];
     T* sm = reinterpret_cast<T*>(smraw);
-    constexpr int PLANE = PXS * PYS;
-    T* const xs = sm;                  // x planes [2], then k planes [2]
-    T* const ks = sm + 2 * PLANE;
+    constexpr int ROW = Lay<T>::ROW, PLANE = ROW * PYS;
+    T* const xs = sm;                  // x planes [NSTG], then k planes [NSTG]
+    T* const ks = sm + NSTG * PLANE;
     __shared__ double red[NT / 32];
 
     const int tid = threadIdx.x, lx = tid % LX, ly = tid / LX;
@@ -79,7 +113,6 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
     const int zc0 = blockIdx.z * P.zchunk, zc1 = min(zc0 + P.zchunk, nz);
     const int gi0 = x0 + 4 * lx, gj = y0 + ly;
     const bool active = gi0 < nx && gj < ny;
-    constexpr int OFF = sizeof(T) == 4 ? 4 : 2;   // staged column of the tile's first own column (16-byte aligned)
 
     // staging: cell (row rr, column cq) of the tile <- global (y0 - 1 + rr, x0 - 1 + cq), mirrored at the faces.
     // Each thread stages the same NE cells of every plane: shared offsets, in-plane global offsets and a mask of the
@@ -105,7 +138,7 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
         if (gy < 0) { gy = -1 - gy; gh = true; } else if (gy >= ny) { gy = 2 * ny - 1 - gy; gh = true; }
         if (gx < 0) { gx = -1 - gx; gh = true; } else if (gx >= nx) { gx = 2 * nx - 1 - gx; gh = true; }
         gy = min(max(gy, 0), ny - 1); gx = min(max(gx, 0), nx - 1);          // cells beyond a partial tile: any valid address
-        soff[e] = rr * PXS + OFF - 1 + cq;
+        soff[e] = rr * ROW + Lay<T>::off(cq - 1);
         goff[e] = gy * nx + gx;
         if (gh && tid + e * NT < NCELL) gmask |= 1u << e;
     }
@@ -113,7 +146,7 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
     auto stage = [&](int p) {            // issue the copies of plane p
         const int zs = p < 0 ? -1 - p : (p >= nz ? 2 * nz - 1 - p : p);
         const size_t zoff = (size_t)zs * ny * nx;
-        const uint32_t bo = (uint32_t)((p & 1) * PLANE);
+        const uint32_t bo = (uint32_t)((p & (NSTG - 1)) * PLANE);
 #pragma unroll
         for (int e = 0; e < NE; ++e) {
             const uint32_t so = (bo + (uint32_t)soff[e]) * (uint32_t)sizeof(T);
@@ -128,11 +161,11 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     auto stage_finish = [&](int p) {     // wait for this thread's copies of plane p and scale its ghost cells
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        asm volatile("cp.async.wait_group %0;" ::"n"(NSTG - 2) : "memory");     // every group but the NSTG - 2 newest has landed
         const bool zg = p < 0 || p >= nz;
         if (gmask || zg) {
             const T fz = p < 0 ? (T)P.s[4] : (p >= nz ? (T)P.s[5] : T(1));
-            T* xd = xs + (p & 1) * PLANE;
+            T* xd = xs + (p & (NSTG - 1)) * PLANE;
 #pragma unroll
             for (int e = 0; e < NE; ++e)
                 if (tid + e * NT < NCELL && (zg || ((gmask >> e) & 1u))) xd[soff[e]] *= fz * xyfac(e);
@@ -145,11 +178,15 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
     double sq = 0.0;
     const T cc = (T)P.cc;
 
-    stage(zc0 - 1);
+    // one commit group per plane, empty past the end of the chunk, so that "all but the NSTG - 2 newest" always means
+    // "up to the plane needed next"
+    auto stage_or_skip = [&](int p) { if (p <= zc1) stage(p); else asm volatile("cp.async.commit_group;" ::: "memory"); };
+#pragma unroll
+    for (int d = 0; d < NSTG - 1; ++d) stage_or_skip(zc0 - 1 + d);
     stage_finish(zc0 - 1);
     for (int p = zc0 - 1; p <= zc1; ++p) {
         __syncthreads();                       // plane p is staged; everyone is done reading the other buffer
-        if (p < zc1) stage(p + 1);             // asynchronous copy into the other buffer
+        stage_or_skip(p + NSTG - 1);           // asynchronous copy into the buffer plane p - 1 has just left
         T bv[4] = {T(0), T(0), T(0), T(0)};
         const int qc = p - 1;
         if (qc >= zc0 && active && b) {
@@ -158,16 +195,17 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
 #pragma unroll
             for (int c = 0; c < 4; ++c) bv[c] = (T)t4[c];
         }
-        const T* xr = xs + (p & 1) * PLANE + ly * PXS + OFF - 1 + 4 * lx;      // column c0 - 1 of row ly - 1
-        const T* kr = ks + (p & 1) * PLANE + ly * PXS + OFF - 1 + 4 * lx;
+        const T* xr = xs + (p & (NSTG - 1)) * PLANE + ly * ROW;      // row ly - 1 of the tile = staged row ly
+        const T* kr = ks + (p & (NSTG - 1)) * PLANE + ly * ROW;
+        const int o0 = Lay<T>::own0(lx), o1 = Lay<T>::own1(lx), ol = Lay<T>::off(4 * lx - 1), orr = Lay<T>::off(4 * lx + 4);
         T fx[3][6], fk[3][6], fz[3][6];
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
-            fx[q][0] = xr[q * PXS]; fx[q][5] = xr[q * PXS + 5];
-            load4<T>(xr + q * PXS + 1, reinterpret_cast<T(&)[4]>(fx[q][1]));
+            fx[q][0] = xr[q * ROW + ol]; fx[q][5] = xr[q * ROW + orr];
+            load22<T>(xr + q * ROW + o0, xr + q * ROW + o1, &fx[q][1]);
             if (VAR) {
-                fk[q][0] = kr[q * PXS]; fk[q][5] = kr[q * PXS + 5];
-                load4<T>(kr + q * PXS + 1, reinterpret_cast<T(&)[4]>(fk[q][1]));
+                fk[q][0] = kr[q * ROW + ol]; fk[q][5] = kr[q * ROW + orr];
+                load22<T>(kr + q * ROW + o0, kr + q * ROW + o1, &fk[q][1]);
 #pragma unroll
                 for (int c = 0; c < 6; ++c) fz[q][c] = fk[q][c] * fx[q][c];
             }

@@ -17,10 +17,12 @@ int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], c
     P.cc = 1.0 / (24.0 * h * h);
     const int tx = (nx + mk::TX - 1) / mk::TX, ty = (ny + mk::TY - 1) / mk::TY;
     // z chunks: one wave of resident blocks; every chunk pays 2 extra planes
-    const size_t smem = (size_t)4 * mk::PXS * mk::PYS * sizeof(TXT);
+    const size_t smem = (size_t)2 * mk::NSTG * mk::Lay<TXT>::ROW * mk::PYS * sizeof(TXT);
     static int per_sm = 0;
     if (!per_sm) {
         int nb = 0;
+        MGB_CUDA(cudaFuncSetAttribute(mk::march_residual_kernel<TXT, TB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MGB_CUDA(cudaFuncSetAttribute(mk::march_residual_kernel<TXT, TB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mk::march_residual_kernel<TXT, TB, true>, mk::NT, smem));
         per_sm = nb > 0 ? nb : 1;
     }
