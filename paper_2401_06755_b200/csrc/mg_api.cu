@@ -118,6 +118,10 @@ int vcycle_any<float>(mg_solver* s, float* x, const float* b) {
     return vcycle_unfused<float>(s, 0, x, b);
 }
 
+// accumulators: slot 0 is read back at once; slots 1.. hold the per-cycle squared residual norms of a fixed-count solve
+// (tol = 0, the paper's mode), which are read back together after the last cycle: no host round trip per cycle
+constexpr int ACC_N = 1 + 4096;
+
 static int read_acc(mg_solver* s, double* out) {
     MGB_CUDA(cudaMemcpyAsync(s->h_acc, s->d_acc, sizeof(double), cudaMemcpyDeviceToHost, s->st));
     MGB_CUDA(cudaStreamSynchronize(s->st));
@@ -199,6 +203,16 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     if ((rc = norm2<float>(s, L.n, b, &nb))) return rc;
     if ((rc = launch_cast_f2d(L.n, x, s->x64, s->st))) return rc;
     ++s->launches;
+    auto resid_into = [&](double* dacc) -> int {      // r32 = float(b - A64 x64), ||r||^2 into *dacc (no read-back)
+        MGB_CUDA(cudaMemsetAsync(dacc, 0, sizeof(double), s->st));
+        int r2;
+        if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
+            r2 = launch_march_residual<double, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, s->x64, s->var_k ? s->k64 : nullptr, b, s->r32,
+                                                      dacc, s->st);
+        else r2 = launch_residual_mixed(L.Ld, s->var_k ? s->k64 : nullptr, s->x64, b, s->r32, dacc, s->st);
+        if (!r2) ++s->launches;
+        return r2;
+    };
     auto resid = [&](double* rel) -> int {
         MGB_CUDA(cudaMemsetAsync(s->d_acc, 0, sizeof(double), s->st));
         int r2;
@@ -216,6 +230,23 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     if ((rc = resid(&rel))) return rc;
     Stop stop{tol, 0, rel};
     int cycles = 0, status = (rel < tol) ? MG_OK : MG_NOT_CONVERGED;
+    if (tol == 0.0 && max_cycles > 0 && max_cycles < ACC_N) {     // fixed cycle count: enqueue everything, read the norms once
+        for (int c = 0; c < max_cycles; ++c) {
+            MGB_CUDA(cudaMemsetAsync(s->e32, 0, L.n * sizeof(float), s->st));
+            if ((rc = vcycle_any<float>(s, s->e32, s->r32))) return rc;
+            if ((rc = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return rc;
+            ++s->launches;
+            if ((rc = resid_into(s->d_acc + 1 + c))) return rc;
+        }
+        MGB_CUDA(cudaMemcpyAsync(s->h_acc + 1, s->d_acc + 1, max_cycles * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+        MGB_CUDA(cudaStreamSynchronize(s->st));
+        for (int c = 0; c < max_cycles; ++c) {
+            rel = nb > 0.0 ? std::sqrt(s->h_acc[1 + c]) / nb : 0.0;
+            s->history.push_back(rel);
+            if (!std::isfinite(rel)) status = MG_STAGNATED;
+        }
+        cycles = max_cycles;
+    }
     while (status == MG_NOT_CONVERGED && cycles < max_cycles) {
         MGB_CUDA(cudaMemsetAsync(s->e32, 0, L.n * sizeof(float), s->st));
         if ((rc = vcycle_any<float>(s, s->e32, s->r32))) return rc;
@@ -323,8 +354,8 @@ int mg_create(mg_solver** out, const mg_grid* grid, int levels, const int bc[6],
         ok = ok && cudaMalloc(&L.tmp, L.n * es) == cudaSuccess;
         if (l > 0) ok = ok && cudaMalloc(&L.x, L.n * es) == cudaSuccess && cudaMalloc(&L.b, L.n * es) == cudaSuccess;
     }
-    ok = ok && cudaMalloc(&s->d_acc, 4 * sizeof(double)) == cudaSuccess;
-    ok = ok && cudaMallocHost(&s->h_acc, 4 * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&s->d_acc, ACC_N * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&s->h_acc, ACC_N * sizeof(double)) == cudaSuccess;
     if (!ok) {
         set_error("mg_create: allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
         mg_destroy(s);
