@@ -2,12 +2,14 @@
 // transfer kernel (fused_kernel.cuh), TMA descriptors, the single-CTA coarse tail, and CUDA-graph
 // replay of the whole V-cycle (north_star "fused" kernels).
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 
 #include "fused.h"
 #include "fused_kernel.cuh"
 #include "solver.h"
 #include "lean_kernel.cuh"
+#include "ctail_kernel.cuh"
 #include "tail_kernel.cuh"
 
 namespace mgb {
@@ -364,6 +366,63 @@ int launch_tail(mg_solver* s, int l, float* x, const float* b, int done, size_t 
     return 0;
 }
 
+// All levels from l down on one 8-block cluster (ctail_kernel.cuh): a prefix of "distributed" levels whose nz is a
+// multiple of 8 (the last of them with nz = 8), then 1-2 "solo" levels in block 0.
+bool ctail_fits(const mg_solver* s, int l, size_t* smem_out, int* nd_out, int* ns_out) {
+    static const bool disabled = getenv("MG_NO_CLUSTER_TAIL") != nullptr;
+    // measured on B200: a 32^3 level is faster as five lean_kernel launches (13 us in the graph) than inside the cluster
+    // (31 us); from 16^3 down the cluster beats the single-block tail (29 us vs 41 us)
+    if (disabled || l < 1 || s->lv[l].n > 8192) return false;
+    int nd = 0;
+    while (l + nd < s->levels && s->lv[l + nd].nz >= ck::NC) ++nd;
+    const int ns = s->levels - l - nd;
+    if (nd < 1 || nd > ck::MAXD || ns < 1 || ns > ck::MAXS) return false;
+    size_t fl = 0;
+    for (int t = 0; t < nd; ++t) {
+        const LevelData& L = s->lv[l + t];
+        if (L.nz % ck::NC || L.nx % 4 || L.ny % 2) return false;
+        const size_t ps = (size_t)L.nx * L.ny, nzl = L.nz / ck::NC;
+        fl += 3 * (nzl + 2) * ps + 2 * nzl * ps;
+    }
+    if (s->lv[l + nd - 1].nz != ck::NC) return false;
+    for (int u = 0; u < ns; ++u) {
+        if (s->lv[l + nd + u].n > 4096) return false;
+        fl += 5 * s->lv[l + nd + u].n;
+    }
+    const LevelData& Ld = s->lv[l + nd - 1];
+    fl += (size_t)ck::NC * (Ld.nx / 2) * (Ld.ny / 2) + s->lv[l + nd].n;
+    *smem_out = fl * sizeof(float);
+    *nd_out = nd; *ns_out = ns;
+    return *smem_out <= 200 * 1024;
+}
+
+int launch_ctail(mg_solver* s, int l, float* x, const float* b, int done, size_t smem, int nd, int ns) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    ck::CParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.nd = nd; P.ns = ns;
+    for (int t = 0; t < nd + ns; ++t) {
+        const LevelData& L = s->lv[l + t];
+        const LevelPlan& lp = fs->lp[l + t];
+        P.nx[t] = L.nx; P.ny[t] = L.ny; P.nz[t] = L.nz;
+        P.k[t] = s->var_k ? (const float*)L.k : nullptr;
+        P.dinv[t] = s->var_k ? lp.dinv : nullptr;
+        P.ce[t] = lp.ce; P.cc[t] = lp.cc; P.dinv_const[t] = 1.f / lp.w0;
+    }
+    for (int f = 0; f < 6; ++f) P.s[f] = s->lv[l].Lf.s[f];
+    P.omega = (float)s->p.omega;
+    P.nu_pre = s->p.nu_pre; P.nu_post = s->p.nu_post; P.coarse_sweeps = s->p.coarse_sweeps;
+    P.first_done = done; P.x = x; P.b = b;
+    static bool attr_done = false;
+    if (!attr_done) {
+        MGB_CUDA(cudaFuncSetAttribute(ck::ctail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    MGB_CUDA(launch_pdl(ck::ctail_kernel, dim3(ck::NC), dim3(ck::NT), smem, s->st, P));
+    ++s->launches;
+    return 0;
+}
+
 // Level l of the V-cycle.  `A` holds the incoming iterate (for l > 0 the parent's fused first sweep
 // has already been applied when `done` = 1); the final iterate of the level is returned in *res.
 int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int done, float** res) {
@@ -372,8 +431,10 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     int rc;
     mark(s, l);
     size_t tail_smem = 0;
-    if (tail_fits(s, l, &tail_smem)) {
-        rc = launch_tail(s, l, A, b, done, tail_smem);
+    int cnd = 0, cns = 0;
+    const bool ctail = ctail_fits(s, l, &tail_smem, &cnd, &cns);
+    if (ctail || tail_fits(s, l, &tail_smem)) {
+        rc = ctail ? launch_ctail(s, l, A, b, done, tail_smem, cnd, cns) : launch_tail(s, l, A, b, done, tail_smem);
         for (int t = l + 1; t <= s->levels; ++t) mark(s, t);                                   // sub-levels are not timed apart
         for (int t = s->levels - 2; t >= l; --t) mark(s, s->levels + 1 + (s->levels - 2 - t));
         *res = A;
