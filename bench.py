@@ -105,6 +105,22 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def max_over_ranks(ms, world, device=None):
+    """Replicas only: the job's time is the slowest rank's, taken on the device timeline."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(units_per_rank, ms, world, device=None):
+    """Whole-job throughput of `world` independent replicas: all ranks' units over the slowest rank's time."""
+    return world * units_per_rank / (max_over_ranks(ms, world, device) * 1e-3)
+
+
 def time_oracle(w, alpha32, b32, cycles, budget_s):
     """The oracle as it stands (fp64, OpenMP over z) on the host cores: `cycles` V-cycles of the workload."""
     import oracle
@@ -199,10 +215,7 @@ def run_ours(args, rank, local_rank, world):
     sampler.stop_flag = True
     launches = mg.mg_launch_count(s) - l0
     ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
     sampler.join(timeout=2.0)
     value = world * args.steps / (ms * 1e-3)
     lups_per_cycle = sum(n * (w.nu_pre + w.nu_post) for n in info[:-1]) + info[-1] * w.coarse_sweeps
@@ -261,10 +274,7 @@ def run_ours(args, rank, local_rank, world):
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms_e2e], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, world, dev)
     e2e = {"value": world * calls * E2E_CYCLES / (ms_e2e * 1e-3), "unit": UNIT,
            "h2d_bytes_per_step": 2 * hb.numel() * 4, "d2h_bytes_per_step": hb.numel() * 4,
            "step": "one mg_solve_host call = %d V-cycles with fp64 residual checks" % E2E_CYCLES, "calls": calls}
