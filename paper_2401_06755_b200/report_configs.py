@@ -1,0 +1,167 @@
+"""Run the five BASELINE.json configurations on cuda:0 and print a markdown report.
+
+    python -m paper_2401_06755_b200.report_configs > gpurun_out/configs.md
+
+Config 1: solve to 1e-8 (fp32 mixed precision and fp64).  Config 2: solve to 1e-7.  Config 3: 20 fixed cycles with
+the residual history, per-level time and algorithmic bytes.  Config 4: V(nu, nu) cycles for nu = 1..4, 10 cycles each.
+Config 5: full time steps.  Inputs are the seeded synthetic workloads of workloads/configs.py; every number is a
+CUDA-event time on the solver's stream after warm-up.  Nothing here touches the oracle.
+"""
+from __future__ import annotations
+
+import os
+import sys
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import paper_2401_06755_b200 as mg          # noqa: E402
+from workloads import configs                # noqa: E402
+
+
+def f32(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def timed(fn, reps):
+    fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        out = fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps, out
+
+
+def rhs_from_velocity(w):
+    b = torch.empty(w.shape, device="cuda")
+    mg.pressure_rhs(f32(w.fields["u"]), f32(w.fields["v"]), f32(w.fields["w"]), w.h, 1.0, b)
+    return b
+
+
+def solver_for(w, dtype=None, **params):
+    s = mg.mg_create((w.nx, w.ny, w.nz, w.h), w.levels, w.bc, dtype if dtype is not None else mg.MG_F32)
+    p = dict(nu_pre=w.nu_pre, nu_post=w.nu_post, coarse_sweeps=w.coarse_sweeps, sweeps_per_pass=1, omega=w.omega, mixed_precision=1)
+    p.update(params)
+    mg.mg_set_params(s, **p)
+    return s
+
+
+def main():
+    torch.cuda.set_device(0)
+    print("# The five BASELINE.json configurations on one B200 (%s)\n" % mg.mg_version())
+    print("Made by `python -m paper_2401_06755_b200.report_configs`; CUDA-event times, fp32 unless noted.\n")
+
+    # ---- config 1 ----
+    w = configs.config1()
+    print("## Config 1: 32^3, constant coefficient, Dirichlet, 4 levels, solve to 1e-8\n")
+    print("| dtype | status | cycles | relative residual | ms per solve |\n|---|---|---|---|---|")
+    for name, dt, tdt in (("fp32 + fp64 defect correction", mg.MG_F32, torch.float32), ("fp64", mg.MG_F64, torch.float64)):
+        s = solver_for(w, dt)
+        b = torch.from_numpy(w.fields["b"]).to(tdt).cuda()
+        x = torch.zeros_like(b)
+
+        def run():
+            x.zero_()
+            return mg.mg_solve(s, x, b, w.tol, 100)
+        ms, (st, cyc, rel) = timed(run, 5)
+        print("| %s | %d | %d | %.2e | %.3f |" % (name, st, cyc, rel, ms))
+        mg.mg_destroy(s)
+
+    # ---- config 2 ----
+    w = configs.config2()
+    print("\n## Config 2: 128^3 water column (rho 1000:1), 6 levels, solve to 1e-7\n")
+    s = solver_for(w)
+    mg.mg_set_coefficient_from_vof(s, f32(w.fields["alpha"]), w.rho_l, w.rho_g)
+    b = rhs_from_velocity(w)
+    x = torch.zeros_like(b)
+
+    def run2():
+        x.zero_()
+        return mg.mg_solve(s, x, b, w.tol, 100)
+    ms, (st, cyc, rel) = timed(run2, 5)
+    print("status %d, %d cycles, relative residual %.2e, %.3f ms per solve (%.3f ms per cycle including the fp64 residual)\n"
+          % (st, cyc, rel, ms, ms / max(cyc, 1)))
+    print("history: " + ", ".join("%.2e" % h for h in mg.mg_get_history(s)))
+    mg.mg_destroy(s)
+
+    # ---- config 3 ----
+    w = configs.config3()
+    print("\n## Config 3: 256^3 rising bubble, 7 levels, 20 fixed V(2,2) cycles (P:429)\n")
+    s = solver_for(w)
+    mg.mg_set_coefficient_from_vof(s, f32(w.fields["alpha"]), w.rho_l, w.rho_g)
+    b = rhs_from_velocity(w)
+    x = torch.zeros_like(b)
+
+    def run3():
+        x.zero_()
+        return mg.mg_solve(s, x, b, 0.0, 20)
+    ms, (st, cyc, rel) = timed(run3, 3)
+    print("20 cycles with fp64 residuals: %.3f ms (%.1f V-cycles/s); final relative residual %.2e\n" % (ms, 20e3 / ms, rel))
+    print("history: " + ", ".join("%.2e" % h for h in mg.mg_get_history(s)) + "\n")
+    msc, _ = timed(lambda: mg.mg_vcycle(s, x, b), 200)
+    print("one V-cycle (CUDA graph): %.1f us = %.0f V-cycles/s\n" % (msc * 1e3, 1e3 / msc))
+    dn = np.zeros(w.levels); up = np.zeros(w.levels)
+    for _ in range(20):
+        a, c = mg.mg_vcycle_timed(s, x, b)
+        dn += a; up += c
+    dn /= 20; up /= 20
+    print("| level | grid | points | down leg us | up leg us | algorithmic MB per cycle (77.5 B/point as launched) |\n|---|---|---|---|---|---|")
+    for l in range(w.levels):
+        n, (nx, ny, nz) = mg.mg_level_info(s, l)
+        print("| %d | %dx%dx%d | %d | %.1f | %.1f | %.1f |" % (l, nx, ny, nz, n, dn[l] * 1e3, up[l] * 1e3, n * 77.5e-6))
+    print("\n(per-level times are taken outside the graph, with events between the launches: their sum exceeds the graph's cycle time;"
+          " the levels from 16^3 down run as one cluster kernel, timed under level 4)")
+    mg.mg_destroy(s)
+
+    # ---- config 4 ----
+    w = configs.config4()
+    print("\n## Config 4: 512x512x256 (3 fields = 0.8 GB), four bubbles, 7 levels, V(nu, nu) for nu = 1..4, 10 cycles each\n")
+    s = solver_for(w)
+    mg.mg_set_coefficient_from_vof(s, f32(w.fields["alpha"]), w.rho_l, w.rho_g)
+    b = rhs_from_velocity(w)
+    x = torch.zeros_like(b)
+    print("| nu | us per cycle | V-cycles/s | GLUPS | residual reduction over 10 cycles |\n|---|---|---|---|---|")
+    npts = [mg.mg_level_info(s, l)[0] for l in range(w.levels)]
+    for nu in (1, 2, 3, 4):
+        mg.mg_set_params(s, nu_pre=nu, nu_post=nu, coarse_sweeps=50, sweeps_per_pass=1, omega=w.omega, mixed_precision=1)
+        x.zero_()
+        st, cyc, rel = mg.mg_solve(s, x, b, 0.0, 10)
+        h = mg.mg_get_history(s)
+        msc, _ = timed(lambda: mg.mg_vcycle(s, x, b), 50)
+        lups = sum(n * 2 * nu for n in npts[:-1]) + npts[-1] * 50
+        print("| %d | %.1f | %.0f | %.1f | %.2e -> %.2e |" % (nu, msc * 1e3, 1e3 / msc, lups / msc * 1e-6, h[0], h[-1]))
+    print("\n(one sweep per pass: the two-stage temporally fused kernel is slower, DESIGN.md 5.7)")
+    mg.mg_destroy(s)
+    del x, b
+
+    # ---- config 5 ----
+    w = configs.config5()
+    print("\n## Config 5: full time step on 256^3 (momentum x2, pressure RHS, solve to 1e-6, projection, VoF)\n")
+    s = solver_for(w)
+    C, u, v, ww = (f32(w.fields[q]) for q in ("alpha", "u", "v", "w"))
+    p = torch.empty_like(C)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    cycs = []
+    for it in range(12):
+        if it == 2:
+            torch.cuda.synchronize(); e0.record()
+        st, cyc, rel = mg.flow_time_step(s, C, u, v, ww, p, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, w.tol, 100)
+        cycs.append(cyc)
+    e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 10
+    print("10 steps after 2 warm-up steps: %.2f ms per step = %.1f time-steps/s; cycles per solve %s; last status %d, relres %.2e"
+          % (ms, 1e3 / ms, cycs[2:], st, rel))
+    print("\nvolume fraction after 12 steps: min %.4f max %.4f; max |q| %.4f" % (float(C.min()), float(C.max()),
+          float(torch.maximum(torch.maximum(u.abs().max(), v.abs().max()), ww.abs().max()))))
+    mg.mg_destroy(s)
+
+
+if __name__ == "__main__":
+    main()
