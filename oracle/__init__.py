@@ -45,6 +45,7 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_norm2.restype = C.c_double
         _lib.orc_solve.restype = C.c_int
+        _lib.orc_pcg_solve.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
     return _lib
 
@@ -162,6 +163,17 @@ def solve(g, bc, k, x, b, levels, tol, max_cycles, nu_pre=2, nu_post=2, coarse_s
     rel = C.c_double(0.0)
     n = lib().orc_solve(C.byref(g), _bc(bc), _p(k), int(levels), int(nu_pre), int(nu_post), int(coarse_sweeps),
                         C.c_double(omega), _p(x), _p(b), C.c_double(tol), int(max_cycles), _p(hist), C.byref(rel))
+    return x, n, rel.value, hist[:n]
+
+
+def pcg_solve(g, bc, k, x, b, levels, tol, max_iter, nu=2, coarse_sweeps=50, omega=2.0 / 3.0):
+    """V-cycle-preconditioned CG.  Returns (x, iterations, relres, history)."""
+    k = _f64(k); b = _f64(b)
+    x = np.array(x, dtype=np.float64, order="C")
+    hist = np.zeros(max(max_iter, 1))
+    rel = C.c_double(0.0)
+    n = lib().orc_pcg_solve(C.byref(g), _bc(bc), _p(k), int(levels), int(nu), int(coarse_sweeps), C.c_double(omega),
+                            _p(x), _p(b), C.c_double(tol), int(max_iter), _p(hist), C.byref(rel))
     return x, n, rel.value, hist[:n]
 
 

@@ -334,6 +334,64 @@ int orc_solve(const orc_grid* g, const int* bc, const double* kcoef, int levels,
     return c;
 }
 
+/* ------------------------------------------------------------------------------------
+ * V-cycle-preconditioned conjugate gradients (SURVEY 8(f) "next 1").
+ * NOT in the paper, which always runs plain cycles; it is the standard remedy for
+ * the slow convergence of those cycles under a 1000:1 coefficient jump (SURVEY hard part 4).
+ * Textbook preconditioned CG for the symmetric positive definite system A x = b, the
+ * preconditioner z = M r being ONE V(nu, nu) cycle on A z = r from z = 0 (symmetric because
+ * nu_pre = nu_post, the Jacobi smoother is symmetric and R = P^T / 8):
+ *   r = b - A x;  z = M r;  p = z;  rz = <r, z>
+ *   repeat:  q = A p;  alpha = rz / <p, q>;  x += alpha p;  r -= alpha q;
+ *            stop if ||r||_2 / ||b||_2 < tol;
+ *            z = M r;  rz' = <r, z>;  beta = rz' / rz;  p = z + beta p;  rz = rz'
+ * history (may be NULL) receives the relative residual after every iteration.  Returns the
+ * number of iterations (= V-cycles after the first).
+ * ------------------------------------------------------------------------------------ */
+static double dot(size_t n, const double* a, const double* b) {
+    double s = 0.0;
+    for (size_t c = 0; c < n; ++c) s += a[c] * b[c];
+    return s;
+}
+
+int orc_pcg_solve(const orc_grid* g, const int* bc, const double* kcoef, int levels, int nu, int coarse_sweeps,
+                  double omega, double* x, const double* b, double tol, int max_iter, double* history,
+                  double* relres_out) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double* r = (double*)malloc(n * sizeof(double));
+    double* z = (double*)malloc(n * sizeof(double));
+    double* p = (double*)malloc(n * sizeof(double));
+    double* q = (double*)malloc(n * sizeof(double));
+    const double nb = orc_norm2(n, b);
+    int it = 0;
+    orc_residual(g, bc, kcoef, x, b, r);
+    double rel = nb > 0.0 ? orc_norm2(n, r) / nb : 0.0;
+    if (!(rel < tol) && max_iter > 0) {
+        memset(z, 0, n * sizeof(double));
+        orc_vcycle(g, bc, kcoef, levels, nu, nu, coarse_sweeps, omega, z, r);
+        memcpy(p, z, n * sizeof(double));
+        double rz = dot(n, r, z);
+        while (it < max_iter) {
+            orc_apply_operator(g, bc, kcoef, p, q);
+            const double alpha = rz / dot(n, p, q);
+            for (size_t c = 0; c < n; ++c) { x[c] += alpha * p[c]; r[c] -= alpha * q[c]; }
+            rel = orc_norm2(n, r) / nb;
+            if (history) history[it] = rel;
+            ++it;
+            if (rel < tol) break;
+            memset(z, 0, n * sizeof(double));
+            orc_vcycle(g, bc, kcoef, levels, nu, nu, coarse_sweeps, omega, z, r);
+            const double rz_new = dot(n, r, z);
+            const double beta = rz_new / rz;
+            for (size_t c = 0; c < n; ++c) p[c] = z[c] + beta * p[c];
+            rz = rz_new;
+        }
+    }
+    if (relres_out) *relres_out = rel;
+    free(r); free(z); free(p); free(q);
+    return it;
+}
+
 /* ====================================================================================
  * Explicit stencil residuals that feed the pressure solve.
  * All derived fields are nodal (divided by m_l); halos of C, of the velocities and of every
