@@ -95,6 +95,13 @@ int mg_vcycle(mg_solver* s, void* d_x, const void* d_b);
  * relres_out may be NULL.  Returns MG_OK, MG_NOT_CONVERGED or MG_STAGNATED. */
 int mg_solve(mg_solver* s, void* d_x, const void* d_b, double tol, int max_cycles, int* cycles_out,
              double* relres_out);
+/* V-cycle-preconditioned conjugate gradients (SURVEY 8(f) "next 1"; NOT in the paper, which runs plain cycles):
+ * textbook PCG for the SPD system A p = b with one V(nu, nu) cycle from a zero guess as preconditioner; it converges in
+ * ~12 iterations where the plain cycle stalls under a 1000:1 coefficient jump.  Needs nu_pre == nu_post >= 1 (symmetric
+ * cycle) and a uniform grid with nx % 4 == 0, else MG_EINVAL.  The CG vectors are fp64 for either dtype.  Same argument
+ * conventions, stopping rule (||b - A x||_2 / ||b||_2 < tol, recursively updated residual) and return values as mg_solve;
+ * iters_out = iterations = V-cycles after the first; mg_get_history gives the residual after every iteration. */
+int mg_pcg_solve(mg_solver* s, void* d_x, const void* d_b, double tol, int max_iter, int* iters_out, double* relres_out);
 /* Same with HOST buffers: copies h_b and the guess h_x to the device, solves, copies x back. */
 int mg_solve_host(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out,
                   double* relres_out);

@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmg_b200.so")
-SOURCES = ["mg_generic.cu", "mg_api.cu", "mg_fused.cu", "mg_march.cu", "flow.cu"]
+SOURCES = ["mg_generic.cu", "mg_api.cu", "mg_fused.cu", "mg_march.cu", "mg_pcg.cu", "flow.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

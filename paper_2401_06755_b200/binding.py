@@ -21,7 +21,7 @@ MG_EINVAL, MG_ESHAPE, MG_ECUDA, MG_EALLOC = -1, -2, -3, -4
 
 EXPORTS = [
     "mg_create", "mg_destroy", "mg_set_params", "mg_get_params", "mg_set_coefficient",
-    "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve",
+    "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
     "vof_residual", "mom_predictor", "pressure_rhs", "project_velocity", "flow_time_step", "mg_last_error",
     "mg_version",
@@ -49,6 +49,10 @@ def _load():
     if not os.path.exists(path):
         path = _build.build()
     lib = C.CDLL(path)
+    if any(not hasattr(lib, name) for name in EXPORTS):     # a stale build from before an entry point was added
+        del lib
+        path = _build.build(force=True)
+        lib = C.CDLL(path)
     vp, i, d = C.c_void_p, C.c_int, C.c_double
     pi, pd = C.POINTER(C.c_int), C.POINTER(C.c_double)
     lib.mg_create.argtypes = [C.POINTER(vp), C.POINTER(MgGrid), i, pi, i, vp]
@@ -63,6 +67,7 @@ def _load():
     lib.mg_vcycle.argtypes = [vp, vp, vp]
     lib.mg_solve.argtypes = [vp, vp, vp, d, i, pi, pd]
     lib.mg_solve_host.argtypes = [vp, vp, vp, d, i, pi, pd]
+    lib.mg_pcg_solve.argtypes = [vp, vp, vp, d, i, pi, pd]
     lib.mg_get_history.argtypes = [vp, pd, i]
     lib.mg_level_info.argtypes = [vp, i, pi, pi, pi]; lib.mg_level_info.restype = C.c_longlong
     lib.mg_vcycle_timed.argtypes = [vp, vp, vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
@@ -214,6 +219,14 @@ def mg_solve(s, x, b, tol, max_cycles):
     st = _check(_lib.mg_solve(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(b, s.shape, s.torch_dtype), float(tol),
                               int(max_cycles), C.byref(cyc), C.byref(rel)))
     return st, cyc.value, rel.value
+
+
+def mg_pcg_solve(s, x, b, tol, max_iter):
+    """V-cycle-preconditioned CG.  Returns (status, iterations, relres)."""
+    it, rel = C.c_int(0), C.c_double(0.0)
+    st = _check(_lib.mg_pcg_solve(s.handle, _dev(x, s.shape, s.torch_dtype), _dev(b, s.shape, s.torch_dtype), float(tol),
+                                  int(max_iter), C.byref(it), C.byref(rel)))
+    return st, it.value, rel.value
 
 
 def mg_solve_host(s, x_host, b_host, tol, max_cycles):

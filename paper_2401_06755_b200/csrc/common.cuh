@@ -55,7 +55,11 @@ int launch_residual_mixed(const Level<double>& L, const double* k64, const doubl
 bool march_supported(int nx, int ny, int nz, double hx, double hy, double hz);
 template <typename TXT, typename TB>
 int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], const TXT* x, const TXT* k, const TB* b, TB* r,
-                          double* acc, cudaStream_t st);
+                          double* acc, cudaStream_t st, int dotx = 0);   // dotx: accumulate sum out * x instead of sum out^2
+}  // namespace mgb
+struct mg_solver;
+namespace mgb {
+int ensure_mixed_buffers(mg_solver* s);   // x64, k64, r32, e32 of the mixed-precision loops (mg_api.cu)
 int launch_axpy_mixed(size_t n, double* x64, const float* e32, cudaStream_t st);  // x64 += e32
 int launch_cast_f2d(size_t n, const float* a, double* b, cudaStream_t st);
 int launch_cast_d2f(size_t n, const double* a, float* b, cudaStream_t st);

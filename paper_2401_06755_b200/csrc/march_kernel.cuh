@@ -26,6 +26,7 @@ struct MParams {
     int zchunk;
     double s[6];     // halo factors x-, x+, y-, y+, z-, z+
     double cc;       // 1 / (24 h^2)
+    int dotx;        // accumulate sum out * x instead of sum out^2 (b = NULL: <x, A x>)
 };
 
 constexpr int LX = 16, LY = 16, NT = LX * LY;
@@ -229,7 +230,7 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
                 if (VAR) rv[c] = bv[c] + cc * ((ko[c] * Sx[c] + Sz[c]) - (T(32) * ko[c] + Sk[c]) * xo[c]);
                 else rv[c] = bv[c] + cc * (T(2) * Sx[c] - T(64) * xo[c]);
                 if (!b) rv[c] = -rv[c];          // no right-hand side: the output is y = A x
-                sq += (double)rv[c] * (double)rv[c];
+                sq += (double)rv[c] * (P.dotx ? (double)xo[c] : (double)rv[c]);
             }
             if (r) {
                 TB* dst = r + ((size_t)qc * ny + gj) * nx + gi0;

@@ -296,7 +296,7 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     return status;
 }
 
-static int ensure_mixed_buffers(mg_solver* s) {
+int ensure_mixed_buffers(mg_solver* s) {
     if (s->x64) return 0;
     const size_t n = s->lv[0].n;
     if (cudaMalloc(&s->x64, n * 8) != cudaSuccess || cudaMalloc(&s->k64, n * 8) != cudaSuccess ||
@@ -409,6 +409,8 @@ void mg_destroy(mg_solver* s) {
         cudaFree(L.k); cudaFree(L.tmp);
     }
     cudaFree(s->x64); cudaFree(s->k64); cudaFree(s->r32); cudaFree(s->e32);
+    for (double* v : s->pcg_v) cudaFree(v);
+    cudaFree(s->pcg_s);
     cudaFree(s->hx_dev); cudaFree(s->hb_dev);
     cudaFree(s->d_acc);
     if (s->h_acc) cudaFreeHost(s->h_acc);

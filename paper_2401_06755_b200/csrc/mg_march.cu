@@ -10,11 +10,12 @@ bool march_supported(int nx, int ny, int nz, double hx, double hy, double hz) {
 
 template <typename TXT, typename TB>
 int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], const TXT* x, const TXT* k, const TB* b, TB* r,
-                          double* acc, cudaStream_t st) {
+                          double* acc, cudaStream_t st, int dotx) {
     mk::MParams P;
     P.nx = nx; P.ny = ny; P.nz = nz;
     for (int f = 0; f < 6; ++f) P.s[f] = s[f];
     P.cc = 1.0 / (24.0 * h * h);
+    P.dotx = dotx;
     const int tx = (nx + mk::TX - 1) / mk::TX, ty = (ny + mk::TY - 1) / mk::TY;
     // z chunks: one wave of resident blocks; every chunk pays 2 extra planes
     const size_t smem = (size_t)2 * mk::NSTG * mk::Lay<TXT>::ROW * mk::PYS * sizeof(TXT);
@@ -36,8 +37,8 @@ int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], c
     return 0;
 }
 
-template int launch_march_residual<double, float>(int, int, int, double, const double*, const double*, const double*, const float*, float*, double*, cudaStream_t);
-template int launch_march_residual<double, double>(int, int, int, double, const double*, const double*, const double*, const double*, double*, double*, cudaStream_t);
-template int launch_march_residual<float, float>(int, int, int, double, const double*, const float*, const float*, const float*, float*, double*, cudaStream_t);
+template int launch_march_residual<double, float>(int, int, int, double, const double*, const double*, const double*, const float*, float*, double*, cudaStream_t, int);
+template int launch_march_residual<double, double>(int, int, int, double, const double*, const double*, const double*, const double*, double*, double*, cudaStream_t, int);
+template int launch_march_residual<float, float>(int, int, int, double, const double*, const float*, const float*, const float*, float*, double*, cudaStream_t, int);
 
 }  // namespace mgb

@@ -37,6 +37,9 @@ struct mg_solver {
     double* k64 = nullptr;
     float* r32 = nullptr;
     float* e32 = nullptr;
+    // mg_pcg_solve (mg_pcg.cu): fp64 CG vectors b, r, p, q (and z for MG_F64), device scalars
+    double* pcg_v[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    double* pcg_s = nullptr;
     // host-buffer entry points
     void* hx_dev = nullptr;
     void* hb_dev = nullptr;

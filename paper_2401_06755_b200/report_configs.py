@@ -105,6 +105,13 @@ def main():
     ms, (st, cyc, rel) = timed(run3, 3)
     print("20 cycles with fp64 residuals: %.3f ms (%.1f V-cycles/s); final relative residual %.2e\n" % (ms, 20e3 / ms, rel))
     print("history: " + ", ".join("%.2e" % h for h in mg.mg_get_history(s)) + "\n")
+    def run3p():
+        x.zero_()
+        return mg.mg_pcg_solve(s, x, b, 1e-7, 100)
+    ms, (st, its, rel) = timed(run3p, 3)
+    print("V-cycle-preconditioned CG (mg_pcg_solve, not in the paper) to 1e-7: status %d, %d iterations, relative residual %.2e, %.2f ms\n"
+          % (st, its, rel, ms))
+    print("history: " + ", ".join("%.2e" % h for h in mg.mg_get_history(s)) + "\n")
     msc, _ = timed(lambda: mg.mg_vcycle(s, x, b), 200)
     print("one V-cycle (CUDA graph): %.1f us = %.0f V-cycles/s\n" % (msc * 1e3, 1e3 / msc))
     dn = np.zeros(w.levels); up = np.zeros(w.levels)
