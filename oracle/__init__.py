@@ -206,6 +206,15 @@ def pressure_rhs(g, u, v, w, dt):
     return b
 
 
+def pressure_rhs_paper(g, Cf, u, v, w, rho_l, rho_g, dt):
+    """Eq. 53's right-hand side (constant-coefficient Laplacian, density on the right)."""
+    Cf = _f64(Cf); u = _f64(u); v = _f64(v); w = _f64(w)
+    b = np.empty(g.shape)
+    lib().orc_pressure_rhs_paper(C.byref(g), _p(Cf), _p(u), _p(v), _p(w), C.c_double(rho_l), C.c_double(rho_g),
+                                 C.c_double(dt), _p(b))
+    return b
+
+
 def project_velocity(g, bc, p, k, dt, u, v, w):
     p = _f64(p); k = _f64(k)
     u, v, w = (np.array(a, dtype=np.float64, order="C") for a in (u, v, w))
@@ -232,3 +241,25 @@ def time_step(g, bc, Cf, u, v, w, levels, rho_l, rho_g, mu_l, mu_g, dt, tol, max
     un, vn, wn = project_velocity(g, bc, p, k, dt, qt[0], qt[1], qt[2])
     _, Cn = vof_residual(g, Cf, un, vn, wn, dt)
     return Cn, un, vn, wn, p, cycles, rel
+
+
+def time_step_paper(g, bc, Cf, u, v, w, levels, rho_l, rho_g, mu_l, mu_g, dt, cycles=20, passes=2,
+                    nu_pre=2, nu_post=2, coarse_sweeps=50, omega=2.0 / 3.0):
+    """One time step with the PAPER'S stage 3: constant-coefficient Laplacian, density on the
+    right (Eqs. 52-53), `cycles` multigrid cycles per solve (fixed 20), velocity correction Eq. 54, the
+    whole stage carried out `passes` times (twice); p_nh accumulates the corrections.  Stages 2 and 4 as
+    time_step().  Returns (C_new, u, v, w, p_nh, relres of the last solve)."""
+    qn = (u, v, w)
+    qt, qh = mom_predictor(g, Cf, qn, qn, rho_l, rho_g, mu_l, mu_g, dt)
+    qt, _ = mom_predictor(g, Cf, qh, qn, rho_l, rho_g, mu_l, mu_g, dt)
+    k = k_from_vof(Cf, rho_l, rho_g)
+    un, vn, wn = qt
+    p = np.zeros(g.shape)
+    rel = 0.0
+    for _ in range(passes):
+        b = pressure_rhs_paper(g, Cf, un, vn, wn, rho_l, rho_g, dt)
+        dp, _, rel, _ = solve(g, bc, None, np.zeros(g.shape), b, levels, 0.0, cycles, nu_pre, nu_post, coarse_sweeps, omega)
+        un, vn, wn = project_velocity(g, bc, dp, k, dt, un, vn, wn)
+        p = p + dp
+    _, Cn = vof_residual(g, Cf, un, vn, wn, dt)
+    return Cn, un, vn, wn, p, rel

@@ -542,6 +542,33 @@ void orc_pressure_rhs(const orc_grid* g, const double* u, const double* v, const
     free(t);
 }
 
+/* The PAPER'S OWN stage-3 right-hand side, Eqs. 52-53 (SURVEY 8(f) "next 2"): the density stays on the right and
+ * the Laplacian is constant-coefficient,
+ *   b = -(1/dt) ( f(rho.u~; w_x) + f(rho.v~; w_y) + f(rho.w~; w_z) )
+ *       +(1/dt) ( u~.f(rho; w_x) + v~.f(rho; w_y) + w~.f(rho; w_z) ),     rho = rho_l C + rho_g (1 - C)  (Eq. 2),
+ * each term written as its own filter application, exactly as Eq. 53 prints them; halos are copies.
+ * With A = f(.; w_lap) positive definite (reading C1-2) the system solved is  A dp = b. */
+void orc_pressure_rhs_paper(const orc_grid* g, const double* C, const double* u, const double* v, const double* w,
+                            double rho_l, double rho_g, double dt, double* b) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wx[27], wy[27], wz[27];
+    orc_filter(g, 1, wx); orc_filter(g, 2, wy); orc_filter(g, 3, wz);
+    double* rho = (double*)malloc(n * sizeof(double));
+    double* m = (double*)malloc(n * sizeof(double));
+    double* t = (double*)malloc(n * sizeof(double));
+    for (size_t c = 0; c < n; ++c) { rho[c] = rho_l * C[c] + rho_g * (1.0 - C[c]); b[c] = 0.0; }
+    const double* vel[3] = {u, v, w};
+    const double* flt[3] = {wx, wy, wz};
+    for (int d = 0; d < 3; ++d) {
+        for (size_t c = 0; c < n; ++c) m[c] = rho[c] * vel[d][c];
+        orc_apply_filter(g, BC_COPY, flt[d], m, t);                       /* f(rho q; w_d) */
+        for (size_t c = 0; c < n; ++c) b[c] -= t[c] / dt;
+        orc_apply_filter(g, BC_COPY, flt[d], rho, t);                     /* q . f(rho; w_d) */
+        for (size_t c = 0; c < n; ++c) b[c] += vel[d][c] * t[c] / dt;
+    }
+    free(rho); free(m); free(t);
+}
+
 /* Velocity projection, Eq. 54 with Eq. 48: q = q~ - dt k . f(p; w_x|y|z),
  * k = 1/rho; halo of p by the solver's BC factors.  In place on u, v, w. */
 void orc_project_velocity(const orc_grid* g, const int* bc, const double* p, const double* kcoef, double dt,

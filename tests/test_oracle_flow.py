@@ -256,3 +256,44 @@ def test_projection_reduces_divergence(orc):
     b2 = orc.pressure_rhs(g, uu, vv, ww, dt)
     sl = (slice(2, -2),) * 3
     assert np.linalg.norm(b2[sl]) < 0.5 * np.linalg.norm(b[sl])
+
+
+# ---------------------------------------------------------------- 8(f) next 2: the paper's own stage-3 right-hand side (Eq. 53)
+def test_rhs_paper_constant_density_is_rho_times_divergence(orc):
+    """rho constant: the rho-gradient terms vanish and Eq. 53's RHS is rho times the FE divergence RHS (already pinned)."""
+    g = orc.grid(10, 12, 8, 0.1, 0.08, 0.125)
+    r = np.random.default_rng(0)
+    u, v, w = (r.standard_normal(g.shape) for _ in range(3))
+    for Cval, rho in ((1.0, 1000.0), (0.0, 1.0), (0.25, 250.75)):
+        b = orc.pressure_rhs_paper(g, np.full(g.shape, Cval), u, v, w, 1000.0, 1.0, 0.02)
+        assert np.allclose(b, rho * orc.pressure_rhs(g, u, v, w, 0.02), rtol=1e-12, atol=1e-9)
+
+
+def test_rhs_paper_linear_fields_closed_form(orc):
+    """u = x, rho = 1 + x (C = x with rho_l = 2, rho_g = 1), v = w = 0: the central difference of the quadratic rho u is
+    exact, so away from the x faces  b = -(1/dt) ((1 + 2x) - x) = -(1 + x)/dt = -rho div(q)/dt."""
+    n, h, dt = 12, 0.05, 0.01
+    g = orc.grid(n, 6, 6, h)
+    x = ((np.arange(n) + 0.5) * h).reshape(1, 1, n) + np.zeros(g.shape)
+    z = np.zeros(g.shape)
+    b = orc.pressure_rhs_paper(g, x, x, z, z, 2.0, 1.0, dt)
+    assert np.allclose(b[:, :, 1:-1], -(1.0 + x[:, :, 1:-1]) / dt, rtol=1e-12)
+    # a sign or a dropped term would show: the two groups of Eq. 53 separately are -(1 + 2x)/dt and +x/dt
+    b_u = orc.pressure_rhs_paper(g, x, x, z, z, 2.0, 1.0, dt) - orc.pressure_rhs_paper(g, z, x, z, z, 2.0, 1.0, dt)
+    assert np.allclose(b_u[:, :, 1:-1], -(x[:, :, 1:-1]) / dt, rtol=1e-11)      # rho_g = 1 part removed: -(x * 1)' - ... = -x/dt
+
+
+def test_time_step_paper_reduces_mass_residual(orc):
+    """Two passes of the paper's stage 3 reduce the right-hand side of Eq. 52 (the mass-conservation defect)."""
+    from workloads import configs
+    w = configs.config5(16, 3)
+    g = orc.grid(16, 16, 16, w.h)
+    Cf, u, v, ww = (w.fields[q] for q in ("alpha", "u", "v", "w"))
+    qn = (u, v, ww)
+    qt, qh = orc.mom_predictor(g, Cf, qn, qn, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
+    qt, _ = orc.mom_predictor(g, Cf, qh, qn, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
+    b0 = orc.pressure_rhs_paper(g, Cf, qt[0], qt[1], qt[2], w.rho_l, w.rho_g, w.dt)
+    Cn, un, vn, wn, p, rel = orc.time_step_paper(g, w.bc, Cf, u, v, ww, 3, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
+    b2 = orc.pressure_rhs_paper(g, Cf, un, vn, wn, w.rho_l, w.rho_g, w.dt)
+    assert np.linalg.norm(b2) < 0.7 * np.linalg.norm(b0)
+    assert np.isfinite(p).all() and 0.0 <= Cn.min() + 1e-3 and Cn.max() <= 1.0 + 1e-3
