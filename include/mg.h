@@ -143,6 +143,10 @@ int mom_predictor(const mg_grid* grid, int dtype, const void* d_C, const void* c
  * (structure of Eq. 53; reading C10). */
 int pressure_rhs(const mg_grid* grid, int dtype, const void* d_u, const void* d_v, const void* d_w, double dt,
                  void* d_b, void* cuda_stream);
+/* SURVEY 8(f) "next 2", the paper's own stage-3 right-hand side, Eqs. 52-53: density on the right, constant-
+ * coefficient Laplacian:  b = -(1/dt) sum_d f(rho q_d; w_d) + (1/dt) sum_d q_d f(rho; w_d),  rho = rho_l C + rho_g (1 - C). */
+int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w,
+                       double rho_l, double rho_g, double dt, void* d_b, void* cuda_stream);
 /* a10: q <- q - dt k f(p; w_x|y|z), Eq. 54 with Eq. 48; halo of p by bc[6]. */
 int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void* d_p, const void* d_k,
                      double dt, void* d_u, void* d_v, void* d_w, void* cuda_stream);
@@ -154,6 +158,13 @@ int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void
 int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l,
                    double rho_g, double mu_l, double mu_g, double dt, double tol, int max_cycles,
                    int* cycles_out, double* relres_out);
+
+/* The same time step with the PAPER'S stage 3 (SURVEY 8(f) "next 2"): constant-coefficient Laplacian with the density on the
+ * right (Eqs. 52-53), `cycles` V-cycles per solve from a zero guess (the paper's fixed 20), velocity correction Eq. 54,
+ * the stage carried out `passes` times (twice).  d_p receives the accumulated p_nh; the solver's coefficient is reset
+ * to constant; relres_out (may be NULL) the relative residual of the last solve. */
+int flow_time_step_paper(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l, double rho_g,
+                         double mu_l, double mu_g, double dt, int cycles, int passes, double* relres_out);
 
 /* Thread-local description of the last error; never freed by the caller. */
 const char* mg_last_error(void);

@@ -23,7 +23,7 @@ EXPORTS = [
     "mg_create", "mg_destroy", "mg_set_params", "mg_get_params", "mg_set_coefficient",
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
-    "vof_residual", "mom_predictor", "pressure_rhs", "project_velocity", "flow_time_step", "mg_last_error",
+    "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "project_velocity", "flow_time_step", "flow_time_step_paper", "mg_last_error",
     "mg_version",
 ]
 
@@ -77,6 +77,8 @@ def _load():
     lib.mom_predictor.argtypes = [C.POINTER(MgGrid), i, vp, C.POINTER(vp), C.POINTER(vp), d, d, d, d, d,
                                   C.POINTER(vp), C.POINTER(vp), vp]
     lib.pressure_rhs.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, d, vp, vp]
+    lib.pressure_rhs_paper.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, d, d, vp, vp]
+    lib.flow_time_step_paper.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, i, i, pd]
     lib.project_velocity.argtypes = [C.POINTER(MgGrid), pi, i, vp, vp, d, vp, vp, vp, vp]
     lib.flow_time_step.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, i, pi, pd]
     lib.mg_last_error.restype = C.c_char_p
@@ -301,6 +303,23 @@ def pressure_rhs(u, v, w, h, dt, b, stream=None):
     sh, dt_ = tuple(u.shape), u.dtype
     return _check(_lib.pressure_rhs(C.byref(g), _dtype_code(u), _dev(u), _dev(v, sh, dt_), _dev(w, sh, dt_), float(dt),
                                     _dev(b, sh, dt_), _stream_ptr(stream)))
+
+
+def pressure_rhs_paper(C_, u, v, w, h, rho_l, rho_g, dt, b, stream=None):
+    g = _grid_of(C_, h)
+    sh, dt_ = tuple(C_.shape), C_.dtype
+    return _check(_lib.pressure_rhs_paper(C.byref(g), _dtype_code(C_), _dev(C_), _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_),
+                                          float(rho_l), float(rho_g), float(dt), _dev(b, sh, dt_), _stream_ptr(stream)))
+
+
+def flow_time_step_paper(s, C_, u, v, w, p, rho_l, rho_g, mu_l, mu_g, dt, cycles=20, passes=2):
+    """Returns the relative residual of the last solve."""
+    rel = C.c_double(0.0)
+    sh, dt_ = s.shape, s.torch_dtype
+    _check(_lib.flow_time_step_paper(s.handle, _dev(C_, sh, dt_), _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_), _dev(p, sh, dt_),
+                                     float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt), int(cycles), int(passes),
+                                     C.byref(rel)))
+    return rel.value
 
 
 def project_velocity(p, k, h, bc, dt, u, v, w, stream=None):

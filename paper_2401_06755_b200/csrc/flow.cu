@@ -9,6 +9,7 @@
 //   w_x = Dx My Mz, ...;  w_xx = Kx My Mz, ...;  w_m/m_l = Mx My Mz;  w_lap = w_xx + w_yy + w_zz.
 // Halos of C, velocities and derived fields are zero-derivative copies (reading C9-iv);
 // the pressure halo in the projection uses the solver's factors (reading C10).
+#include <algorithm>
 #include <cmath>
 
 #include "solver.h"
@@ -58,6 +59,17 @@ template <typename T> __device__ __forceinline__ T tmin(T a, T b) { return a < b
 template <typename T> __device__ __forceinline__ T tmax(T a, T b) { return a > b ? a : b; }
 
 #include "flow_march.cuh"
+
+template <typename T>
+__global__ void __launch_bounds__(256) axpy_kernel(size_t n, T* __restrict__ y, const T* __restrict__ x) {
+    for (size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x) y[c] += x[c];
+}
+template <typename T>
+int launch_axpy(size_t n, T* y, const T* x, cudaStream_t st) {
+    axpy_kernel<T><<<(int)std::min<size_t>((n + 255) / 256, 148 * 16), 256, 0, st>>>(n, y, x);
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
 
 struct Scratch {  // stream-ordered scratch fields
     cudaStream_t st;
@@ -132,6 +144,15 @@ int pressure_rhs_t(const mg_grid* g, const T* u, const T* v, const T* w, double 
 }
 
 template <typename T>
+int pressure_rhs_paper_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double rho_l, double rho_g, double dt, T* b,
+                         cudaStream_t st) {
+    const Geo<T> G = make_geo<T>(g, nullptr);
+    pressure_rhs_paper_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, (T)rho_l, (T)rho_g, (T)(1.0 / dt), b);
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
+
+template <typename T>
 int project_t(const mg_grid* g, const int* bc, const T* p, const T* k, double dt, T* u, T* v, T* w, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, bc);
     project_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, p, k, (T)dt, u, v, w);
@@ -200,6 +221,21 @@ int pressure_rhs(const mg_grid* grid, int dtype, const void* d_u, const void* d_
     return pressure_rhs_t<double>(grid, (const double*)d_u, (const double*)d_v, (const double*)d_w, dt, (double*)d_b, st);
 }
 
+int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double rho_l,
+                       double rho_g, double dt, void* d_b, void* cuda_stream) {
+    if (!grid_ok(grid, dtype)) return MG_EINVAL;
+    if (!d_C || !d_u || !d_v || !d_w || !d_b || !(dt > 0.0) || !(rho_l > 0.0) || !(rho_g > 0.0)) {
+        set_error("pressure_rhs_paper: NULL argument, dt <= 0 or density <= 0");
+        return MG_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (dtype == MG_F32)
+        return pressure_rhs_paper_t<float>(grid, (const float*)d_C, (const float*)d_u, (const float*)d_v, (const float*)d_w, rho_l, rho_g,
+                                           dt, (float*)d_b, st);
+    return pressure_rhs_paper_t<double>(grid, (const double*)d_C, (const double*)d_u, (const double*)d_v, (const double*)d_w, rho_l,
+                                        rho_g, dt, (double*)d_b, st);
+}
+
 int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void* d_p, const void* d_k, double dt, void* d_u,
                      void* d_v, void* d_w, void* cuda_stream) {
     if (!grid_ok(grid, dtype)) return MG_EINVAL;
@@ -253,6 +289,55 @@ int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, voi
             if (cudaGetLastError() != cudaSuccess) { set_error("flow_time_step: copy failed"); rc = MG_ECUDA; }
         }
         if (!rc) rc = status;
+    }
+    if (prev >= 0) cudaSetDevice(prev);
+    return rc;
+}
+
+// Time step with the PAPER'S stage 3 (oracle time_step_paper): constant-coefficient Laplacian, density on the
+// right (Eqs. 52-53), `cycles` multigrid cycles per solve from a zero guess (the paper's fixed 20), correction Eq. 54,
+// the stage repeated `passes` times (twice); d_p receives the accumulated p_nh.  The solver's coefficient is reset to
+// constant.  relres_out: relative residual of the last solve.
+int flow_time_step_paper(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l, double rho_g, double mu_l,
+                         double mu_g, double dt, int cycles, int passes, double* relres_out) {
+    if (!s || !d_C || !d_u || !d_v || !d_w || !d_p || cycles < 1 || passes < 1) { set_error("flow_time_step_paper: invalid argument"); return MG_EINVAL; }
+    int prev = -1;
+    cudaGetDevice(&prev);
+    cudaSetDevice(s->device);
+    const size_t n = s->lv[0].n, es = s->dtype == MG_F64 ? 8 : 4, bytes = n * es;
+    cudaStream_t st = s->st;
+    int rc = 0;
+    {
+        Scratch ws(st), ws2(st);
+        if ((rc = ws.alloc(4, bytes)) || (rc = ws2.alloc(4, bytes))) { if (prev >= 0) cudaSetDevice(prev); return rc; }
+        void* qt[3] = {ws.p[0], ws.p[1], ws.p[2]};
+        void* qh[3] = {ws2.p[0], ws2.p[1], ws2.p[2]};
+        void* bbuf = ws.p[3];
+        void* kbuf = ws2.p[3];
+        void* dp = qh[0];                       // the half-level velocities are dead after stage 2
+        const void* qn[3] = {d_u, d_v, d_w};
+        rc = mom_predictor(&s->grid, s->dtype, d_C, qn, qn, rho_l, rho_g, mu_l, mu_g, dt, qt, qh, st);
+        if (!rc) { const void* qhc[3] = {qh[0], qh[1], qh[2]}; rc = mom_predictor(&s->grid, s->dtype, d_C, qhc, qn, rho_l, rho_g, mu_l, mu_g, dt, qt, nullptr, st); }
+        if (!rc && s->var_k) rc = mg_set_coefficient(s, nullptr);
+        if (!rc) rc = s->dtype == MG_F32 ? launch_k_from_vof<float>(n, (const float*)d_C, rho_l, rho_g, (float*)kbuf, st)
+                                         : launch_k_from_vof<double>(n, (const double*)d_C, rho_l, rho_g, (double*)kbuf, st);
+        if (!rc) rc = cudaMemsetAsync(d_p, 0, bytes, st) == cudaSuccess ? 0 : MG_ECUDA;
+        for (int pass = 0; pass < passes && !rc; ++pass) {
+            rc = pressure_rhs_paper(&s->grid, s->dtype, d_C, qt[0], qt[1], qt[2], rho_l, rho_g, dt, bbuf, st);
+            if (!rc) rc = cudaMemsetAsync(dp, 0, bytes, st) == cudaSuccess ? 0 : MG_ECUDA;
+            if (!rc) { const int status = mg_solve(s, dp, bbuf, 0.0, cycles, nullptr, relres_out); if (status < 0) rc = status; }
+            if (!rc) rc = project_velocity(&s->grid, s->bc, s->dtype, dp, kbuf, dt, qt[0], qt[1], qt[2], st);
+            if (!rc) rc = s->dtype == MG_F32 ? launch_axpy<float>(n, (float*)d_p, (const float*)dp, st)
+                                             : launch_axpy<double>(n, (double*)d_p, (const double*)dp, st);
+        }
+        if (!rc) rc = vof_residual(&s->grid, s->dtype, d_C, qt[0], qt[1], qt[2], dt, nullptr, bbuf, st);
+        if (!rc) {
+            cudaMemcpyAsync(d_C, bbuf, bytes, cudaMemcpyDeviceToDevice, st);
+            cudaMemcpyAsync(d_u, qt[0], bytes, cudaMemcpyDeviceToDevice, st);
+            cudaMemcpyAsync(d_v, qt[1], bytes, cudaMemcpyDeviceToDevice, st);
+            cudaMemcpyAsync(d_w, qt[2], bytes, cudaMemcpyDeviceToDevice, st);
+            if (cudaGetLastError() != cudaSuccess) { set_error("flow_time_step_paper: copy failed"); rc = MG_ECUDA; }
+        }
     }
     if (prev >= 0) cudaSetDevice(prev);
     return rc;

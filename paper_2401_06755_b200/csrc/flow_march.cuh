@@ -324,3 +324,43 @@ __global__ void __launch_bounds__(MBX* MBY) vof_diffusion_march(const Geo<T> G, 
         }
     }
 }
+
+// The paper's own stage-3 right-hand side, Eqs. 52-53: density on the right, constant-coefficient
+// Laplacian:  b = -(1/dt) sum_d f(rho q_d; w_d) + (1/dt) sum_d q_d f(rho; w_d),  rho = rho_l C + rho_g (1 - C)  (Eq. 2).
+template <typename T>
+__global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ u,
+                                                                   const T* __restrict__ v, const T* __restrict__ w, T rho_l, T rho_g,
+                                                                   T inv_dt, T* __restrict__ bout) {
+    const Col<T> c = make_col(G);
+    T suv[3] = {T(0), T(0), T(0)}, aw[3] = {T(0), T(0), T(0)};      // in-plane Dx My (rho u) + Mx Dy (rho v); Mx My (rho w)
+    GradRoll<T> gr; gr.init();                                       // in-plane parts of grad rho
+    T q0[3] = {T(0), T(0), T(0)}, q0n[3] = {T(0), T(0), T(0)};       // u, v, w at the centre of planes q, q + 1
+    for (int z = c.z0 - 1; z <= c.z1; ++z) {
+        T r9[3][3], n9[3][3];
+        load9(G, c, C, z, r9);
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) r9[b][a] = rho_l * r9[b][a] + rho_g * (T(1) - r9[b][a]);
+        gr.add(in_plane<T, true, false>(G, r9));
+        const T* const vel[3] = {u, v, w};
+        T part[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            load9(G, c, vel[d], z, n9);
+            q0[d] = q0n[d]; q0n[d] = n9[1][1];
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) n9[b][a] *= r9[b][a];
+            if (d == 2) part[d] = in_plane<T, false, false>(G, n9).mm;
+            else { const InPlane<T> r = in_plane<T, true, false>(G, n9); part[d] = d == 0 ? r.dm : r.md; }
+        }
+        push(suv, part[0] + part[1]); push(aw, part[2]);
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            T gx, gy, gz; gr.grad(G, gx, gy, gz);
+            bout[c.nxy * q + c.row[1] + c.ix[1]] = (-(zM(G, suv) + zD(G, aw)) + (q0[0] * gx + q0[1] * gy + q0[2] * gz)) * inv_dt;
+        }
+    }
+}

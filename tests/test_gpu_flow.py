@@ -121,3 +121,43 @@ def test_time_step_parity(mg, orc, dt):
         for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
             assert rel_l2(as_f64(a), r) <= lim
     mg.mg_destroy(s)
+
+
+# ---------------------------------------------------------------- the paper's own stage 3
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("shape,h", [((24, 24, 24), 1.0 / 24), ((10, 36, 68), (0.02, 0.025, 0.03))])
+def test_pressure_rhs_paper_parity(mg, orc, shape, h, dt):
+    import torch
+    nz, ny, nx = shape
+    hh = h if isinstance(h, tuple) else (h, h, h)
+    g = orc.grid(nx, ny, nz, *hh)
+    n = nx * ny * nz
+    Cf = quantise(rng.uniform01(71, n).reshape(shape), dt)
+    u, v, w = (quantise(rng.normal(72 + c, n).reshape(shape), dt) for c in range(3))
+    b_ref = orc.pressure_rhs_paper(g, Cf, u, v, w, 1000.0, 1.0, 0.01)
+    db = torch.empty(shape, device="cuda", dtype=torch.float32 if dt == "f32" else torch.float64)
+    mg.pressure_rhs_paper(to_dev(Cf, dt), to_dev(u, dt), to_dev(v, dt), to_dev(w, dt), hh, 1000.0, 1.0, 0.01, db)
+    # rho q - q rho cancels to rho div q: the same cancellation allowance as the divergence right-hand side
+    assert rel_l2(as_f64(db), b_ref) <= TOL[dt] * (50 if dt == "f32" else 1e3)
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_time_step_paper_parity(mg, orc, dt):
+    """Config 5 at 32^3 with the paper's stage 3 (constant-coefficient Laplacian, 2 passes x 20 cycles): two steps."""
+    import torch
+    n, levels = 32, 4
+    w = configs.config5(n, levels)
+    g = orc.grid(n, n, n, w.h)
+    Cf, u, v, ww = (quantise(w.fields[q], dt) for q in ("alpha", "u", "v", "w"))
+    s = mg.mg_create((n, n, n, w.h), levels, w.bc, mg.MG_F32 if dt == "f32" else mg.MG_F64)
+    dC, du, dv, dw = (to_dev(a, dt) for a in (Cf, u, v, ww))
+    dp = torch.empty_like(dC)
+    for step in range(2):
+        Cf, u, v, ww, p, rel_o = orc.time_step_paper(g, w.bc, Cf, u, v, ww, levels, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
+        rel = mg.flow_time_step_paper(s, dC, du, dv, dw, dp, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, 20, 2)
+        lim = (step + 1) * (1e-4 if dt == "f32" else 1e-7)
+        assert abs(rel - rel_o) <= 0.05 * rel_o + 1e-12
+        assert rel_l2(as_f64(dp), p) <= lim * 5
+        for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
+            assert rel_l2(as_f64(a), r) <= lim
+    mg.mg_destroy(s)
