@@ -215,6 +215,16 @@ def pressure_rhs_paper(g, Cf, u, v, w, rho_l, rho_g, dt):
     return b
 
 
+def hydrostatic_rhs(g, Cf, rho_l, rho_g, grav, sigma_t):
+    """Stage 1.  Returns (b_hs, kappa, (s_tu, s_tv, s_tw))."""
+    Cf = _f64(Cf)
+    b = np.empty(g.shape); kap = np.empty(g.shape)
+    st = [np.empty(g.shape) for _ in range(3)]
+    lib().orc_hydrostatic_rhs(C.byref(g), _p(Cf), C.c_double(rho_l), C.c_double(rho_g), C.c_double(grav), C.c_double(sigma_t),
+                              _p(b), _p(kap), _ptr3(st))
+    return b, kap, tuple(st)
+
+
 def project_velocity(g, bc, p, k, dt, u, v, w):
     p = _f64(p); k = _f64(k)
     u, v, w = (np.array(a, dtype=np.float64, order="C") for a in (u, v, w))

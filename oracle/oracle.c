@@ -569,6 +569,72 @@ void orc_pressure_rhs_paper(const orc_grid* g, const double* C, const double* u,
     free(rho); free(m); free(t);
 }
 
+/* ------------------------------------------------------------------------------------
+ * Stage 1, hydrostatic and surface-tension pressure (SURVEY 8(f) "next 3"; Eqs. 4-5, Eqs. 20-23,
+ * P:419-427 Eqs. 43-44, bottom boundary condition P:258).
+ *   C_x, C_y, C_z = nodal FE gradient of C;  l = |grad C|;  n_t = grad C / (eps_t + l),  eps_t = 1e-7 / h     (Eq. 23)
+ *   kappa = f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z)   (nodal: Eq. 22's w_ml^-1)                          (Eq. 22)
+ *   s_t = sigma_t kappa grad C                                                                              (Eq. 21)
+ *   A p_hs = b_hs,  b_hs = f(s_tu; w_x) + f(s_tv; w_y) + f(s_tw + g rho; w_z)                               (Eq. 44)
+ * Readings: Eq. 22 prints n_tu three times and Eq. 23 prints C_x for n_tw -- read as the divergence
+ * of (n_tu, n_tv, n_tw) with n_tw from C_z (Eq. 5).  Eq. 43 and Eq. 44 disagree on the sign of the surface-tension term
+ * relative to gravity.  Eq. 44, the discrete residual the method actually forces to zero, is followed with f(.; w_lap)
+ * positive definite (reading C1-2): it is the form that gives both the hydrostatic balance dp/dz = -rho g and the
+ * Young-Laplace jump (pressure higher inside a drop by 2 sigma / R; with kappa = +div(grad C / |grad C|) as printed in
+ * Eq. 5 the curvature of a drop is negative) -- both pinned in tests/test_oracle_flow.py.
+ * h in eps_t is hx.  Halos of C, n_t, s_t and rho are copies (reading C9-iv).
+ * Bottom boundary condition dp_hs/dz = -rho g: the ghost below the bottom plane is p + hz rho g with the density of
+ * the nearest node, so its contribution sum_j (-w_ij) hz g rho_j over the ghost plane is added to b on the bottom plane;
+ * the solver then treats that face as zero-derivative (copy).
+ * kappa_out, st_out[3] may be NULL.
+ * ------------------------------------------------------------------------------------ */
+void orc_hydrostatic_rhs(const orc_grid* g, const double* C, double rho_l, double rho_g, double grav, double sigma_t,
+                         double* b, double* kappa_out, double* const* st_out) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wx[27], wy[27], wz[27], wl[27];
+    orc_filter(g, 1, wx); orc_filter(g, 2, wy); orc_filter(g, 3, wz); orc_filter(g, 0, wl);
+    double* gc[3]; double* nt[3]; double* st[3];
+    for (int d = 0; d < 3; ++d) { gc[d] = (double*)malloc(n * sizeof(double)); nt[d] = (double*)malloc(n * sizeof(double)); st[d] = (double*)malloc(n * sizeof(double)); }
+    double* kap = (double*)malloc(n * sizeof(double));
+    double* t = (double*)malloc(n * sizeof(double));
+    const double* flt[3] = {wx, wy, wz};
+    const double eps_t = 1e-7 / g->hx;
+    for (int d = 0; d < 3; ++d) orc_apply_filter(g, BC_COPY, flt[d], C, gc[d]);
+    for (size_t c = 0; c < n; ++c) {
+        const double l = sqrt(gc[0][c] * gc[0][c] + gc[1][c] * gc[1][c] + gc[2][c] * gc[2][c]);
+        for (int d = 0; d < 3; ++d) nt[d][c] = gc[d][c] / (eps_t + l);
+        kap[c] = 0.0;
+    }
+    for (int d = 0; d < 3; ++d) {
+        orc_apply_filter(g, BC_COPY, flt[d], nt[d], t);
+        for (size_t c = 0; c < n; ++c) kap[c] += t[c];
+    }
+    for (size_t c = 0; c < n; ++c)
+        for (int d = 0; d < 3; ++d) st[d][c] = sigma_t * kap[c] * gc[d][c];
+    /* b = f(g rho; w_z) + div(s_t)   (Eq. 44) */
+    for (size_t c = 0; c < n; ++c) nt[0][c] = grav * (rho_l * C[c] + rho_g * (1.0 - C[c]));      /* reuse: g rho */
+    orc_apply_filter(g, BC_COPY, wz, nt[0], b);
+    for (int d = 0; d < 3; ++d) {
+        orc_apply_filter(g, BC_COPY, flt[d], st[d], t);
+        for (size_t c = 0; c < n; ++c) b[c] += t[c];
+    }
+    /* bottom boundary: ghost = mirror + hz g rho(mirror) */
+    for (int j = 0; j < g->ny; ++j)
+        for (int i = 0; i < g->nx; ++i) {
+            double add = 0.0;
+            for (int jj = -1; jj <= 1; ++jj)
+                for (int ii = -1; ii <= 1; ++ii)
+                    add += -wl[(ii + 1) + 3 * (jj + 1)] * g->hz * ghost(nt[0], g, BC_COPY, i + ii, j + jj, 0);   /* kk = -1 slice */
+            b[IDX(g, i, j, 0)] += add;
+        }
+    if (kappa_out) memcpy(kappa_out, kap, n * sizeof(double));
+    for (int d = 0; d < 3; ++d) {
+        if (st_out && st_out[d]) memcpy(st_out[d], st[d], n * sizeof(double));
+        free(gc[d]); free(nt[d]); free(st[d]);
+    }
+    free(kap); free(t);
+}
+
 /* Velocity projection, Eq. 54 with Eq. 48: q = q~ - dt k . f(p; w_x|y|z),
  * k = 1/rho; halo of p by the solver's BC factors.  In place on u, v, w. */
 void orc_project_velocity(const orc_grid* g, const int* bc, const double* p, const double* kcoef, double dt,

@@ -297,3 +297,67 @@ def test_time_step_paper_reduces_mass_residual(orc):
     b2 = orc.pressure_rhs_paper(g, Cf, un, vn, wn, w.rho_l, w.rho_g, w.dt)
     assert np.linalg.norm(b2) < 0.7 * np.linalg.norm(b0)
     assert np.isfinite(p).all() and 0.0 <= Cn.min() + 1e-3 and Cn.max() <= 1.0 + 1e-3
+
+
+# ---------------------------------------------------------------- 8(f) next 3: hydrostatic + surface-tension pressure (stage 1)
+BC_PHS = (0, 0, 0, 0, 0, 1)       # p_hs: zero derivative on the sides and (after folding -rho g into b) the bottom, zero value on top
+
+
+def test_hydrostatic_column_is_reproduced_exactly(orc):
+    """One fluid, no surface tension: p = rho g (H - z) is linear, the FE filters are exact for it, and it satisfies
+    dp/dz = -rho g at the bottom and p = 0 on the top face.  So A p = b_hs must hold to rounding, and the multigrid solve of
+    A p = b_hs must return it.  Pins the gravity term, its sign, and the bottom boundary fold."""
+    nx, ny, nz, h = 8, 6, 16, 0.05
+    g = orc.grid(nx, ny, nz, h)
+    rho, grav = 1000.0, 9.81
+    b, kap, st = orc.hydrostatic_rhs(g, np.ones(g.shape), rho, 1.0, grav, 0.0728)
+    assert np.abs(kap).max() < 1e-12 and all(np.abs(a).max() < 1e-12 for a in st)      # no interface: no curvature (rounding only)
+    z = ((np.arange(nz) + 0.5) * h).reshape(nz, 1, 1) + np.zeros(g.shape)
+    p = rho * grav * (nz * h - z)
+    assert np.allclose(orc.apply_operator(g, BC_PHS, None, p), b, rtol=0, atol=1e-8 * rho * grav / h)
+    x, cyc, rel, _ = orc.solve(g, BC_PHS, None, np.zeros(g.shape), b, 2, 1e-12, 200)
+    assert np.allclose(x, p, rtol=1e-9, atol=1e-9 * rho * grav)
+
+
+def test_two_layer_hydrostatic_balance(orc):
+    """Flat interface (water below air), sigma_t = 0: dp/dz = -rho(z) g in both layers away from the smoothed interface."""
+    n, h = 32, 1.0 / 32
+    g = orc.grid(8, 8, n, h)
+    z = ((np.arange(n) + 0.5) * h).reshape(n, 1, 1) + np.zeros(g.shape)
+    Cf = 0.5 * (1 + np.tanh((0.5 - z) / (1.5 * h)))
+    b, kap, _ = orc.hydrostatic_rhs(g, Cf, 1000.0, 1.0, 9.81, 0.0)
+    # flat interface: no curvature where there is an interface (far away, where |grad C| drops below eps_t, the normal of
+    # Eq. 23 decays from 1 to 0 and kappa is not small, but it multiplies grad C ~ 1e-8 there)
+    assert np.abs(kap[np.abs(z - 0.5) < 3 * h]).max() < 1e-3          # vs -8 for the sphere below; the rest is eps_t / |grad C|
+    _, _, st1 = orc.hydrostatic_rhs(g, Cf, 1000.0, 1.0, 9.81, 1.0)
+    assert max(np.abs(a).max() for a in st1) < 1e-3          # vs sigma kappa |grad C| ~ 8 * 20 for the sphere below
+    x, _, rel, _ = orc.solve(g, BC_PHS, None, np.zeros(g.shape), b, 3, 1e-11, 400)
+    dpdz = (x[2:] - x[:-2]) / (2 * h)
+    assert np.allclose(dpdz[2:8, 4, 4], -1000.0 * 9.81, rtol=2e-3)      # in the water
+    assert np.allclose(dpdz[-5:-2, 4, 4], -1.0 * 9.81, rtol=5e-3)       # in the air, clear of the smoothed interface
+
+
+def test_curvature_of_a_sphere(orc):
+    """kappa = div(grad C / |grad C|): for C decreasing outwards from a sphere of radius R the normal is -r_hat and
+    kappa = -2 / r on the interface (second-order filters: a few per cent at 12 cells per radius)."""
+    n = 48
+    h = 1.0 / n
+    g = orc.grid(n, n, n, h)
+    c = (np.arange(n) + 0.5) * h
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    r = np.sqrt((X - 0.5) ** 2 + (Y - 0.5) ** 2 + (Z - 0.5) ** 2)
+    R = 0.25
+    Cf = 0.5 * (1 - np.tanh((r - R) / (2 * h)))         # 1 inside
+    _, kap, st = orc.hydrostatic_rhs(g, Cf, 1000.0, 1.0, 0.0, 1.0)
+    shell = np.abs(r - R) < 0.5 * h
+    assert shell.sum() > 100
+    assert np.allclose(kap[shell] * r[shell], -2.0, rtol=0.05)
+    # sigma kappa grad C as printed (Eqs. 4-5) points along +r_hat here: kappa < 0, grad C along -r_hat
+    sr = (st[0] * (X - 0.5) + st[1] * (Y - 0.5) + st[2] * (Z - 0.5)) / np.maximum(r, 1e-12)
+    assert (sr[shell] > 0).all()
+    # Young-Laplace: the pressure p_hs of Eq. 44 is higher inside the drop by 2 sigma / R
+    b, _, _ = orc.hydrostatic_rhs(g, Cf, 1000.0, 1.0, 0.0, 1.0)
+    x, _, rel, _ = orc.solve(g, (1,) * 6, None, np.zeros(g.shape), b, 4, 1e-10, 300)
+    p_in = x[n // 2, n // 2, n // 2]
+    p_out = x[n // 2, n // 2, 3]
+    assert abs((p_in - p_out) - 2.0 / R) <= 0.1 * 2.0 / R
