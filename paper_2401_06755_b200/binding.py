@@ -23,7 +23,7 @@ EXPORTS = [
     "mg_create", "mg_destroy", "mg_set_params", "mg_get_params", "mg_set_coefficient",
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
-    "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "project_velocity", "flow_time_step", "flow_time_step_paper", "mg_last_error",
+    "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_paper", "mg_last_error",
     "mg_version",
 ]
 
@@ -79,6 +79,7 @@ def _load():
     lib.pressure_rhs.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, d, vp, vp]
     lib.pressure_rhs_paper.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, d, d, vp, vp]
     lib.flow_time_step_paper.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, i, i, pd]
+    lib.hydrostatic_rhs.argtypes = [C.POINTER(MgGrid), i, vp, d, d, d, d, vp, vp, vp]
     lib.project_velocity.argtypes = [C.POINTER(MgGrid), pi, i, vp, vp, d, vp, vp, vp, vp]
     lib.flow_time_step.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, i, pi, pd]
     lib.mg_last_error.restype = C.c_char_p
@@ -320,6 +321,13 @@ def flow_time_step_paper(s, C_, u, v, w, p, rho_l, rho_g, mu_l, mu_g, dt, cycles
                                      float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt), int(cycles), int(passes),
                                      C.byref(rel)))
     return rel.value
+
+
+def hydrostatic_rhs(C_, h, rho_l, rho_g, grav, sigma_t, b, kappa_out=None, stream=None):
+    g = _grid_of(C_, h)
+    sh, dt_ = tuple(C_.shape), C_.dtype
+    return _check(_lib.hydrostatic_rhs(C.byref(g), _dtype_code(C_), _dev(C_), float(rho_l), float(rho_g), float(grav), float(sigma_t),
+                                       _dev(b, sh, dt_), _dev(kappa_out, sh, dt_, True), _stream_ptr(stream)))
 
 
 def project_velocity(p, k, h, bc, dt, u, v, w, stream=None):

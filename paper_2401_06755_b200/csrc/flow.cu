@@ -153,6 +153,23 @@ int pressure_rhs_paper_t(const mg_grid* g, const T* C, const T* u, const T* v, c
 }
 
 template <typename T>
+int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, double grav, double sigma_t, T* b, T* kappa, cudaStream_t st) {
+    const Geo<T> G = make_geo<T>(g, nullptr);
+    const size_t bytes = npts(g->nx, g->ny, g->nz) * sizeof(T);
+    Scratch ws(st), ws2(st);
+    int rc;
+    if ((rc = ws.alloc(3, bytes)) || (rc = ws2.alloc(3, bytes))) return rc;
+    T *n0 = (T*)ws.p[0], *n1 = (T*)ws.p[1], *n2 = (T*)ws.p[2], *f0 = (T*)ws2.p[0], *f1 = (T*)ws2.p[1], *f2 = (T*)ws2.p[2];
+    const dim3 grd = march_grid(G), blk(MBX, MBY);
+    normals_march<T><<<grd, blk, 0, st>>>(G, C, n0, n1, n2);
+    surface_tension_march<T><<<grd, blk, 0, st>>>(G, C, n0, n1, n2, (T)rho_l, (T)rho_g, (T)grav, (T)sigma_t, f0, f1, f2, kappa);
+    pressure_rhs_march<T><<<grd, blk, 0, st>>>(G, f0, f1, f2, T(-1), b);       // b = +(f(fu; w_x) + f(fv; w_y) + f(fw; w_z))
+    bottom_fold_kernel<T><<<dim3((g->nx + 31) / 32, (g->ny + 7) / 8), dim3(32, 8), 0, st>>>(G, C, (T)rho_l, (T)rho_g, (T)grav, b);
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
+
+template <typename T>
 int project_t(const mg_grid* g, const int* bc, const T* p, const T* k, double dt, T* u, T* v, T* w, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, bc);
     project_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, p, k, (T)dt, u, v, w);
@@ -234,6 +251,15 @@ int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const vo
                                            dt, (float*)d_b, st);
     return pressure_rhs_paper_t<double>(grid, (const double*)d_C, (const double*)d_u, (const double*)d_v, (const double*)d_w, rho_l,
                                         rho_g, dt, (double*)d_b, st);
+}
+
+int hydrostatic_rhs(const mg_grid* grid, int dtype, const void* d_C, double rho_l, double rho_g, double grav, double sigma_t, void* d_b,
+                    void* d_kappa_out, void* cuda_stream) {
+    if (!grid_ok(grid, dtype)) return MG_EINVAL;
+    if (!d_C || !d_b || !(rho_l > 0.0) || !(rho_g > 0.0)) { set_error("hydrostatic_rhs: NULL argument or density <= 0"); return MG_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (dtype == MG_F32) return hydrostatic_rhs_t<float>(grid, (const float*)d_C, rho_l, rho_g, grav, sigma_t, (float*)d_b, (float*)d_kappa_out, st);
+    return hydrostatic_rhs_t<double>(grid, (const double*)d_C, rho_l, rho_g, grav, sigma_t, (double*)d_b, (double*)d_kappa_out, st);
 }
 
 int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void* d_p, const void* d_k, double dt, void* d_u,

@@ -364,3 +364,76 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T
         }
     }
 }
+
+// ---- stage 1, hydrostatic and surface-tension pressure (Eqs. 20-23, 44; readings in DESIGN.md) ----
+// n_t = grad C / (eps_t + |grad C|), eps_t = 1e-7 / hx  (Eq. 23)
+template <typename T>
+__global__ void __launch_bounds__(MBX* MBY) normals_march(const Geo<T> G, const T* __restrict__ C, T* __restrict__ nx_, T* __restrict__ ny_,
+                                                        T* __restrict__ nz_) {
+    const Col<T> c = make_col(G);
+    const T eps_t = T(1e-7) / G.h[0];
+    GradRoll<T> g; g.init();
+    for (int z = c.z0 - 1; z <= c.z1; ++z) {
+        T n9[3][3];
+        load9(G, c, C, z, n9);
+        g.add(in_plane<T, true, false>(G, n9));
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            T gx, gy, gz; g.grad(G, gx, gy, gz);
+            const T inv = T(1) / (eps_t + sqrt(gx * gx + gy * gy + gz * gz));
+            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
+            nx_[c0] = gx * inv; ny_[c0] = gy * inv; nz_[c0] = gz * inv;
+        }
+    }
+}
+
+// kappa = f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z) (Eq. 22);  (fu, fv, fw) = sigma_t kappa grad C + (0, 0, g rho) (Eqs. 20-21, 44)
+template <typename T>
+__global__ void __launch_bounds__(MBX* MBY) surface_tension_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ nx_,
+                                                                const T* __restrict__ ny_, const T* __restrict__ nz_, T rho_l, T rho_g,
+                                                                T grav, T sigma_t, T* __restrict__ fu, T* __restrict__ fv,
+                                                                T* __restrict__ fw, T* __restrict__ kappa) {
+    const Col<T> c = make_col(G);
+    GradRoll<T> g; g.init();
+    T sxy[3] = {T(0), T(0), T(0)}, am[3] = {T(0), T(0), T(0)};    // in-plane Dx My n_x + Mx Dy n_y;  Mx My n_z
+    T C0 = T(0), C0n = T(0);
+    for (int z = c.z0 - 1; z <= c.z1; ++z) {
+        T n9[3][3];
+        load9(G, c, C, z, n9);
+        g.add(in_plane<T, true, false>(G, n9));
+        C0 = C0n; C0n = n9[1][1];
+        load9(G, c, nx_, z, n9); const T dx = in_plane<T, true, false>(G, n9).dm;
+        load9(G, c, ny_, z, n9); const T dy = in_plane<T, true, false>(G, n9).md;
+        load9(G, c, nz_, z, n9); const T mz = in_plane<T, false, false>(G, n9).mm;
+        push(sxy, dx + dy); push(am, mz);
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            T gx, gy, gz; g.grad(G, gx, gy, gz);
+            const T kap = zM(G, sxy) + zD(G, am);
+            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
+            const T sk = sigma_t * kap;
+            fu[c0] = sk * gx; fv[c0] = sk * gy;
+            fw[c0] = sk * gz + grav * (rho_l * C0 + rho_g * (T(1) - C0));
+            if (kappa) kappa[c0] = kap;
+        }
+    }
+}
+
+// bottom boundary condition dp_hs/dz = -rho g: ghost below = mirror + hz g rho(mirror); its stencil contribution
+// sum_j (-w_lap_ij) hz g rho_j over the ghost plane is added to b on the bottom plane
+template <typename T>
+__global__ void bottom_fold_kernel(const Geo<T> G, const T* __restrict__ C, T rho_l, T rho_g, T grav, T* __restrict__ b) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= G.nx || j >= G.ny) return;
+    T add = T(0);
+#pragma unroll
+    for (int bb = 0; bb < 3; ++bb)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const int ii = min(max(i + a - 1, 0), G.nx - 1), jj = min(max(j + bb - 1, 0), G.ny - 1);
+            const T Cv = C[(size_t)jj * G.nx + ii];
+            const T wl = (G.K[0][a] * G.M[bb] + G.M[a] * G.K[1][bb]) * G.M[0] + G.M[a] * G.M[bb] * G.K[2][0];
+            add -= wl * G.h[2] * grav * (rho_l * Cv + rho_g * (T(1) - Cv));
+        }
+    b[(size_t)j * G.nx + i] += add;
+}

@@ -161,3 +161,40 @@ def test_time_step_paper_parity(mg, orc, dt):
         for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
             assert rel_l2(as_f64(a), r) <= lim
     mg.mg_destroy(s)
+
+
+# ---------------------------------------------------------------- stage 1, hydrostatic + surface-tension pressure
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_hydrostatic_rhs_and_solve_parity(mg, orc, dt):
+    """A drop (C = 1 inside) above a water layer: curvature, right-hand side of Eq. 44 with the bottom boundary fold, and the
+    p_hs it gives after 20 constant-coefficient V-cycles (the paper's fixed count)."""
+    import torch
+    n, levels = 32, 4
+    h = 1.0 / n
+    g = orc.grid(n, n, n, h)
+    c = (np.arange(n) + 0.5) * h
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    r = np.sqrt((X - 0.5) ** 2 + (Y - 0.45) ** 2 + (Z - 0.65) ** 2)
+    Cf = np.maximum(0.5 * (1 - np.tanh((r - 0.18) / (1.5 * h))), 0.5 * (1 + np.tanh((0.25 - Z) / (1.5 * h))))
+    Cf = quantise(Cf, dt)
+    rho_l, rho_g, grav, sig = 1000.0, 1.0, 9.81, 0.0728
+    b_ref, kap_ref, _ = orc.hydrostatic_rhs(g, Cf, rho_l, rho_g, grav, sig)
+    dC = to_dev(Cf, dt)
+    db, dk = torch.empty_like(dC), torch.empty_like(dC)
+    mg.hydrostatic_rhs(dC, h, rho_l, rho_g, grav, sig, db, dk)
+    # kappa divides by |grad C|, tiny away from the interfaces, where rounding decides it: compare where there is an interface
+    gx = np.gradient(Cf, h)
+    band = np.sqrt(gx[0] ** 2 + gx[1] ** 2 + gx[2] ** 2) > 1.0
+    assert band.sum() > 1000
+    assert rel_l2(as_f64(dk)[band], kap_ref[band]) <= (2e-4 if dt == "f32" else 1e-9)
+    assert rel_l2(as_f64(db), b_ref) <= (5 * TOL[dt] if dt == "f32" else 1e-9)
+    bc = (N, N, N, N, N, D)
+    s = mg.mg_create((n, n, n, h), levels, bc, mg.MG_F32 if dt == "f32" else mg.MG_F64)
+    dp = torch.zeros_like(dC)
+    mg.mg_solve(s, dp, db, 0.0, 20)
+    p_ref, _, _, _ = orc.solve(g, bc, None, np.zeros(g.shape), b_ref, levels, 0.0, 20)
+    assert rel_l2(as_f64(dp), p_ref) <= (1e-4 if dt == "f32" else 1e-8)
+    # physics of the result: hydrostatic at the bottom of the water layer, higher pressure inside the drop
+    p = as_f64(dp)
+    assert abs((p[0, 4, 4] - p[2, 4, 4]) / (2 * h) - rho_l * grav) <= 0.02 * rho_l * grav
+    mg.mg_destroy(s)
