@@ -148,10 +148,10 @@ int pressure_rhs(const mg_grid* grid, int dtype, const void* d_u, const void* d_
 int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w,
                        double rho_l, double rho_g, double dt, void* d_b, void* cuda_stream);
 /* SURVEY 8(f) "next 3", stage 1: right-hand side of the hydrostatic and surface-tension pressure p_hs (Eqs. 20-23, 44;
- * P:226-246, 419-427):  n_t = grad C / (1e-7/hx + |grad C|), kappa = f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z),
- * s_t = sigma_t kappa grad C,  b = f(s_tu; w_x) + f(s_tv; w_y) + f(s_tw + g rho; w_z), plus the contribution of the bottom
+ * P:226-246, 419-427):  n_t = grad C / (1e-7/hx + |grad C|), kappa = -(f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z)),
+ * s_t = sigma_t kappa grad C,  b = f(g rho; w_z) - (f(s_tu; w_x) + f(s_tv; w_y) + f(s_tw; w_z)), plus the contribution of the bottom
  * boundary condition dp_hs/dz = -rho g on the plane z = 0.  Solve A p_hs = b with a constant-coefficient solver and
- * bc = {N, N, N, N, N, D}.  Readings (Eq. 22 / 23 misprints, Eq. 43 vs 44 sign) in DESIGN.md.  d_kappa_out may be NULL. */
+ * bc = {N, N, N, N, N, D}.  Readings (Eq. 22 / 23 misprints; the signs of Eqs. 5, 43, 44) in DESIGN.md N3.  d_kappa_out may be NULL. */
 int hydrostatic_rhs(const mg_grid* grid, int dtype, const void* d_C, double rho_l, double rho_g, double g, double sigma_t,
                     void* d_b, void* d_kappa_out, void* cuda_stream);
 /* a10: q <- q - dt k f(p; w_x|y|z), Eq. 54 with Eq. 48; halo of p by bc[6]. */

@@ -573,15 +573,17 @@ void orc_pressure_rhs_paper(const orc_grid* g, const double* C, const double* u,
  * Stage 1, hydrostatic and surface-tension pressure (SURVEY 8(f) "next 3"; Eqs. 4-5, Eqs. 20-23,
  * P:419-427 Eqs. 43-44, bottom boundary condition P:258).
  *   C_x, C_y, C_z = nodal FE gradient of C;  l = |grad C|;  n_t = grad C / (eps_t + l),  eps_t = 1e-7 / h     (Eq. 23)
- *   kappa = f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z)   (nodal: Eq. 22's w_ml^-1)                          (Eq. 22)
- *   s_t = sigma_t kappa grad C                                                                              (Eq. 21)
- *   A p_hs = b_hs,  b_hs = f(s_tu; w_x) + f(s_tv; w_y) + f(s_tw + g rho; w_z)                               (Eq. 44)
- * Readings: Eq. 22 prints n_tu three times and Eq. 23 prints C_x for n_tw -- read as the divergence
- * of (n_tu, n_tv, n_tw) with n_tw from C_z (Eq. 5).  Eq. 43 and Eq. 44 disagree on the sign of the surface-tension term
- * relative to gravity.  Eq. 44, the discrete residual the method actually forces to zero, is followed with f(.; w_lap)
- * positive definite (reading C1-2): it is the form that gives both the hydrostatic balance dp/dz = -rho g and the
- * Young-Laplace jump (pressure higher inside a drop by 2 sigma / R; with kappa = +div(grad C / |grad C|) as printed in
- * Eq. 5 the curvature of a drop is negative) -- both pinned in tests/test_oracle_flow.py.
+ *   kappa = -( f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z) )   (nodal: Eq. 22's w_ml^-1; sign: see below)    (Eqs. 5, 22)
+ *   s_t = sigma_t kappa grad C                                                                              (Eqs. 4, 21)
+ *   A p_hs = b_hs,  b_hs = f(g rho; w_z) - ( f(s_tu; w_x) + f(s_tv; w_y) + f(s_tw; w_z) )                   (Eq. 43)
+ * Readings (N3): Eq. 22 prints n_tu three times and Eq. 23 prints C_x for n_tw -- read as the divergence of
+ * (n_tu, n_tv, n_tw) with n_tw from C_z (Eq. 5).  The signs of Eq. 5 (kappa = +div n_t), Eq. 43 and Eq. 44 cannot all hold:
+ * with kappa = +div n_t the force sigma kappa grad C points OUT of a drop, Eq. 43 (which is what balances the momentum
+ * equation 17: grad p_hs = s_q + s_t) then puts the lower pressure inside, and Eq. 44 has the opposite sign of Eq. 43 on the
+ * surface-tension term.  The reading taken is the one that satisfies the physics the paper names (continuum surface force
+ * [15], Young-Laplace): kappa = -div n_t, with Eq. 43 and Eq. 17 as printed.  Numerically b_hs is then exactly what Eq. 44
+ * as printed gives with Eq. 5 as printed (the two sign slips cancel).  Pinned: dp/dz = -rho g, kappa = +2/r on a sphere,
+ * force towards the centre, pressure higher inside by 2 sigma / R.
  * h in eps_t is hx.  Halos of C, n_t, s_t and rho are copies (reading C9-iv).
  * Bottom boundary condition dp_hs/dz = -rho g: the ghost below the bottom plane is p + hz rho g with the density of
  * the nearest node, so its contribution sum_j (-w_ij) hz g rho_j over the ghost plane is added to b on the bottom plane;
@@ -607,16 +609,16 @@ void orc_hydrostatic_rhs(const orc_grid* g, const double* C, double rho_l, doubl
     }
     for (int d = 0; d < 3; ++d) {
         orc_apply_filter(g, BC_COPY, flt[d], nt[d], t);
-        for (size_t c = 0; c < n; ++c) kap[c] += t[c];
+        for (size_t c = 0; c < n; ++c) kap[c] -= t[c];
     }
     for (size_t c = 0; c < n; ++c)
         for (int d = 0; d < 3; ++d) st[d][c] = sigma_t * kap[c] * gc[d][c];
-    /* b = f(g rho; w_z) + div(s_t)   (Eq. 44) */
+    /* b = f(g rho; w_z) - div(s_t)   (Eq. 43) */
     for (size_t c = 0; c < n; ++c) nt[0][c] = grav * (rho_l * C[c] + rho_g * (1.0 - C[c]));      /* reuse: g rho */
     orc_apply_filter(g, BC_COPY, wz, nt[0], b);
     for (int d = 0; d < 3; ++d) {
         orc_apply_filter(g, BC_COPY, flt[d], st[d], t);
-        for (size_t c = 0; c < n; ++c) b[c] += t[c];
+        for (size_t c = 0; c < n; ++c) b[c] -= t[c];
     }
     /* bottom boundary: ghost = mirror + hz g rho(mirror) */
     for (int j = 0; j < g->ny; ++j)

@@ -387,7 +387,8 @@ __global__ void __launch_bounds__(MBX* MBY) normals_march(const Geo<T> G, const 
     }
 }
 
-// kappa = f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z) (Eq. 22);  (fu, fv, fw) = sigma_t kappa grad C + (0, 0, g rho) (Eqs. 20-21, 44)
+// kappa = -(f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z)) (Eqs. 5, 22; sign: reading N3);  s_t = sigma_t kappa grad C (Eq. 21);
+// (fu, fv, fw) = -s_t + (0, 0, g rho), whose FE divergence is the right-hand side of Eq. 43
 template <typename T>
 __global__ void __launch_bounds__(MBX* MBY) surface_tension_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ nx_,
                                                                 const T* __restrict__ ny_, const T* __restrict__ nz_, T rho_l, T rho_g,
@@ -409,9 +410,9 @@ __global__ void __launch_bounds__(MBX* MBY) surface_tension_march(const Geo<T> G
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             T gx, gy, gz; g.grad(G, gx, gy, gz);
-            const T kap = zM(G, sxy) + zD(G, am);
+            const T kap = -(zM(G, sxy) + zD(G, am));
             const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            const T sk = sigma_t * kap;
+            const T sk = -sigma_t * kap;                        // -s_t = sk grad C
             fu[c0] = sk * gx; fv[c0] = sk * gy;
             fw[c0] = sk * gz + grav * (rho_l * C0 + rho_g * (T(1) - C0));
             if (kappa) kappa[c0] = kap;

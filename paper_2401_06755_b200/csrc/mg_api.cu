@@ -113,29 +113,7 @@ static int vcycle_unfused(mg_solver* s, int l, T* x, const T* b) {
 template <typename T>
 static int vcycle_unfused_graph(mg_solver* s, T* x, const T* b) {
     if (s->timing) return vcycle_unfused<T>(s, 0, x, b);
-    if (!s->graph_exec || s->graph_x != x || s->graph_b != b) {
-        if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
-        const long long before = s->launches;
-        cudaGraph_t graph = nullptr;
-        if (!s->cap_st) MGB_CUDA(cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking));
-        cudaStream_t user_st = s->st;
-        MGB_CUDA(cudaStreamBeginCapture(s->cap_st, cudaStreamCaptureModeThreadLocal));
-        s->st = s->cap_st;
-        const int rc = vcycle_unfused<T>(s, 0, x, b);
-        s->st = user_st;
-        const cudaError_t e = cudaStreamEndCapture(s->cap_st, &graph);
-        s->graph_launches = s->launches - before;
-        s->launches = before;
-        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
-        if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); return MG_ECUDA; }
-        const cudaError_t e2 = cudaGraphInstantiate(&s->graph_exec, graph, 0);
-        cudaGraphDestroy(graph);
-        if (e2 != cudaSuccess) { s->graph_exec = nullptr; set_error("graph instantiate failed: %s", cudaGetErrorString(e2)); return MG_ECUDA; }
-        s->graph_x = x; s->graph_b = b;
-    }
-    MGB_CUDA(cudaGraphLaunch(s->graph_exec, s->st));
-    s->launches += s->graph_launches;
-    return 0;
+    return replay_graph(s, x, b, [&]() { return vcycle_unfused<T>(s, 0, x, b); });
 }
 
 template <typename T>

@@ -59,3 +59,37 @@ struct mg_solver {
     long long graph_launches = 0;  // kernels inside one replay
     void* fused_state = nullptr;   // owned by mg_fused.cu
 };
+
+namespace mgb {
+
+// Replay `enqueue` (which launches one V-cycle on s->st for the pointer pair (x, b)) from a CUDA graph: recorded once per
+// pointer pair on a private stream (the caller's may be the legacy default stream, which cannot be captured), then launched
+// on the caller's stream.  mg_set_params / mg_set_coefficient / mg_set_fused drop the recorded graph.
+template <class F>
+int replay_graph(mg_solver* s, const void* x, const void* b, F&& enqueue) {
+    if (!s->graph_exec || s->graph_x != x || s->graph_b != b) {
+        if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+        const long long before = s->launches;
+        cudaGraph_t graph = nullptr;
+        if (!s->cap_st) MGB_CUDA(cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking));
+        cudaStream_t user_st = s->st;
+        MGB_CUDA(cudaStreamBeginCapture(s->cap_st, cudaStreamCaptureModeThreadLocal));
+        s->st = s->cap_st;
+        const int rc = enqueue();
+        s->st = user_st;
+        const cudaError_t e = cudaStreamEndCapture(s->cap_st, &graph);
+        s->graph_launches = s->launches - before;
+        s->launches = before;
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); return MG_ECUDA; }
+        const cudaError_t e2 = cudaGraphInstantiate(&s->graph_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e2 != cudaSuccess) { s->graph_exec = nullptr; set_error("graph instantiate failed: %s", cudaGetErrorString(e2)); return MG_ECUDA; }
+        s->graph_x = x; s->graph_b = b;
+    }
+    MGB_CUDA(cudaGraphLaunch(s->graph_exec, s->st));
+    s->launches += s->graph_launches;
+    return 0;
+}
+
+}  // namespace mgb

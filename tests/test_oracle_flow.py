@@ -338,8 +338,9 @@ def test_two_layer_hydrostatic_balance(orc):
 
 
 def test_curvature_of_a_sphere(orc):
-    """kappa = div(grad C / |grad C|): for C decreasing outwards from a sphere of radius R the normal is -r_hat and
-    kappa = -2 / r on the interface (second-order filters: a few per cent at 12 cells per radius)."""
+    """kappa = -div(grad C / |grad C|) (reading N3): for a drop (C = 1 inside a sphere of radius R) the curvature is +2 / r on
+    the interface (second-order filters: a few per cent at 12 cells per radius), the force sigma kappa grad C points to the
+    centre, and p_hs is higher inside by 2 sigma / R (Young-Laplace)."""
     n = 48
     h = 1.0 / n
     g = orc.grid(n, n, n, h)
@@ -351,11 +352,11 @@ def test_curvature_of_a_sphere(orc):
     _, kap, st = orc.hydrostatic_rhs(g, Cf, 1000.0, 1.0, 0.0, 1.0)
     shell = np.abs(r - R) < 0.5 * h
     assert shell.sum() > 100
-    assert np.allclose(kap[shell] * r[shell], -2.0, rtol=0.05)
-    # sigma kappa grad C as printed (Eqs. 4-5) points along +r_hat here: kappa < 0, grad C along -r_hat
+    assert np.allclose(kap[shell] * r[shell], 2.0, rtol=0.05)
+    # sigma kappa grad C points along -r_hat: kappa > 0, grad C along -r_hat
     sr = (st[0] * (X - 0.5) + st[1] * (Y - 0.5) + st[2] * (Z - 0.5)) / np.maximum(r, 1e-12)
-    assert (sr[shell] > 0).all()
-    # Young-Laplace: the pressure p_hs of Eq. 44 is higher inside the drop by 2 sigma / R
+    assert (sr[shell] < 0).all()
+    # Young-Laplace: p_hs is higher inside the drop by 2 sigma / R
     b, _, _ = orc.hydrostatic_rhs(g, Cf, 1000.0, 1.0, 0.0, 1.0)
     x, _, rel, _ = orc.solve(g, (1,) * 6, None, np.zeros(g.shape), b, 4, 1e-10, 300)
     p_in = x[n // 2, n // 2, n // 2]
