@@ -8,6 +8,6 @@ bool fused_supported(const mg_solver* s);
 // (re)build the per-level data the tuned path derives from the coefficient (1/D of the coarse levels)
 int fused_prepare(mg_solver* s);
 int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps);
-int fused_vcycle(mg_solver* s, float* x, const float* b);
+int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess = 0);
 void fused_release(mg_solver* s);
 }  // namespace mgb

@@ -31,6 +31,7 @@ struct MParams {
 
 constexpr int LX = 16, LY = 16, NT = LX * LY;
 constexpr int NSTG = 4;                       // ring of staged planes: 3 planes are in flight while one is consumed
+constexpr int NBS = 8;                        // ring of staged right-hand-side rows (consumed one plane after x: > NSTG slots)
 constexpr int TX = 4 * LX, TY = LY;
 constexpr int PYS = TY + 2;
 // Layout of one staged row (own columns 0 .. TX - 1, halo columns -1 and TX), chosen so that the 16-byte loads of a warp are
@@ -96,7 +97,7 @@ __device__ __forceinline__ void plane_sums(const T (&f)[3][6], T (&Dg)[4], T (&P
     }
 }
 
-template <typename TXT, typename TB, bool VAR>
+template <typename TXT, typename TB, bool VAR, bool HASB>
 __global__ void __launch_bounds__(NT, (sizeof(TXT) == 8 ? 1 : 2))
 march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __restrict__ kc, const TB* __restrict__ b,
                       TB* __restrict__ r, double* __restrict__ acc) {
@@ -106,6 +107,9 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
     constexpr int ROW = Lay<T>::ROW, PLANE = ROW * PYS;
     T* const xs = sm;                  // x planes [NSTG], then k planes [NSTG]
     T* const ks = sm + NSTG * PLANE;
+    // right-hand side: every thread copies the 4 values of its own points (plane p rides in the commit group of x plane p)
+    // and reads them back itself one plane later, so the global-load latency is off the critical path
+    TB* const bs = reinterpret_cast<TB*>(sm + 2 * NSTG * PLANE);
     __shared__ double red[NT / 32];
 
     const int tid = threadIdx.x, lx = tid % LX, ly = tid / LX;
@@ -144,6 +148,8 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
         if (gh && tid + e * NT < NCELL) gmask |= 1u << e;
     }
     const uint32_t xs_a = (uint32_t)__cvta_generic_to_shared(xs), ks_a = (uint32_t)__cvta_generic_to_shared(ks);
+    const uint32_t bs_a = (uint32_t)__cvta_generic_to_shared(bs + 4 * tid);
+    const TB* const bcol = HASB ? b + (size_t)gj * nx + gi0 : nullptr;
     auto stage = [&](int p) {            // issue the copies of plane p
         const int zs = p < 0 ? -1 - p : (p >= nz ? 2 * nz - 1 - p : p);
         const size_t zoff = (size_t)zs * ny * nx;
@@ -158,6 +164,12 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
                 asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(xs_a + so), "l"(x + zoff + goff[e]) : "memory");
                 if (VAR) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(ks_a + so), "l"(kc + zoff + goff[e]) : "memory");
             }
+        }
+        if (HASB && active && p >= zc0 && p < zc1) {
+            const uint32_t so = bs_a + (uint32_t)((p & (NBS - 1)) * NT * 4 * sizeof(TB));
+            const TB* src = bcol + zoff;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(so), "l"(src) : "memory");
+            if (sizeof(TB) == 8) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(so + 16), "l"(src + 2) : "memory");
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -185,14 +197,15 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
 #pragma unroll
     for (int d = 0; d < NSTG - 1; ++d) stage_or_skip(zc0 - 1 + d);
     stage_finish(zc0 - 1);
+#pragma unroll 2
     for (int p = zc0 - 1; p <= zc1; ++p) {
         __syncthreads();                       // plane p is staged; everyone is done reading the other buffer
         stage_or_skip(p + NSTG - 1);           // asynchronous copy into the buffer plane p - 1 has just left
         T bv[4] = {T(0), T(0), T(0), T(0)};
         const int qc = p - 1;
-        if (qc >= zc0 && active && b) {
+        if (HASB && qc >= zc0 && active) {
             TB t4[4];
-            load4<TB>(b + ((size_t)qc * ny + gj) * nx + gi0, t4);
+            load4<TB>(bs + ((qc & (NBS - 1)) * NT + tid) * 4, t4);
 #pragma unroll
             for (int c = 0; c < 4; ++c) bv[c] = (T)t4[c];
         }
@@ -229,8 +242,8 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
             for (int c = 0; c < 4; ++c) {
                 if (VAR) rv[c] = bv[c] + cc * ((ko[c] * Sx[c] + Sz[c]) - (T(32) * ko[c] + Sk[c]) * xo[c]);
                 else rv[c] = bv[c] + cc * (T(2) * Sx[c] - T(64) * xo[c]);
-                if (!b) rv[c] = -rv[c];          // no right-hand side: the output is y = A x
-                sq += (double)rv[c] * (P.dotx ? (double)xo[c] : (double)rv[c]);
+                if (!HASB) rv[c] = -rv[c];       // no right-hand side: the output is y = A x
+                sq += (double)rv[c] * (!HASB && P.dotx ? (double)xo[c] : (double)rv[c]);
             }
             if (r) {
                 TB* dst = r + ((size_t)qc * ny + gj) * nx + gi0;

@@ -126,6 +126,14 @@ int vcycle_any<float>(mg_solver* s, float* x, const float* b) {
     return s->fused ? vcycle_unfused_graph<float>(s, x, b) : vcycle_unfused<float>(s, 0, x, b);
 }
 
+// V-cycle from a zero initial guess: x need not be initialised.  The fused fp32 cycle replaces the first fine sweep by
+// x = omega b / D; the other paths clear x first.
+int vcycle_zero_guess(mg_solver* s, void* x, const void* b) {
+    if (s->dtype == MG_F32 && s->fused && fused_supported(s)) return fused_vcycle(s, (float*)x, (const float*)b, 1);
+    MGB_CUDA(cudaMemsetAsync(x, 0, s->lv[0].n * esize(s), s->st));
+    return s->dtype == MG_F32 ? vcycle_any<float>(s, (float*)x, (const float*)b) : vcycle_any<double>(s, (double*)x, (const double*)b);
+}
+
 // accumulators: slot 0 is read back at once; slots 1.. hold the per-cycle squared residual norms of a fixed-count solve
 // (tol = 0, the paper's mode), which are read back together after the last cycle: no host round trip per cycle
 constexpr int ACC_N = 1 + 4096;
@@ -240,8 +248,7 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     int cycles = 0, status = (rel < tol) ? MG_OK : MG_NOT_CONVERGED;
     if (tol == 0.0 && max_cycles > 0 && max_cycles < ACC_N) {     // fixed cycle count: enqueue everything, read the norms once
         for (int c = 0; c < max_cycles; ++c) {
-            MGB_CUDA(cudaMemsetAsync(s->e32, 0, L.n * sizeof(float), s->st));
-            if ((rc = vcycle_any<float>(s, s->e32, s->r32))) return rc;
+            if ((rc = vcycle_zero_guess(s, s->e32, s->r32))) return rc;
             if ((rc = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return rc;
             ++s->launches;
             if ((rc = resid_into(s->d_acc + 1 + c))) return rc;
@@ -256,8 +263,7 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
         cycles = max_cycles;
     }
     while (status == MG_NOT_CONVERGED && cycles < max_cycles) {
-        MGB_CUDA(cudaMemsetAsync(s->e32, 0, L.n * sizeof(float), s->st));
-        if ((rc = vcycle_any<float>(s, s->e32, s->r32))) return rc;
+        if ((rc = vcycle_zero_guess(s, s->e32, s->r32))) return rc;
         if ((rc = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return rc;
         ++s->launches;
         if ((rc = resid(&rel))) return rc;

@@ -65,8 +65,16 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 // ---- small helper kernels for levels below the tile size ------------------------------------
 __global__ void first_sweep_kernel(size_t n, const float* __restrict__ bc, const float* __restrict__ dinv, float g,
                                    float* __restrict__ xc) {
-    for (size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x)
-        xc[c] = dinv ? g * dinv[c] * bc[c] : g * bc[c];
+    const size_t n4 = n >> 2, stride = (size_t)gridDim.x * blockDim.x, t = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    for (size_t c = t; c < n4; c += stride) {                 // cudaMalloc'ed level arrays: 16-byte aligned
+        float4 v = reinterpret_cast<const float4*>(bc)[c];
+        if (dinv) {
+            const float4 d = reinterpret_cast<const float4*>(dinv)[c];
+            v.x *= d.x; v.y *= d.y; v.z *= d.z; v.w *= d.w;
+        }
+        reinterpret_cast<float4*>(xc)[c] = make_float4(g * v.x, g * v.y, g * v.z, g * v.w);
+    }
+    for (size_t c = 4 * n4 + t; c < n; c += stride) xc[c] = dinv ? g * (dinv[c] * bc[c]) : g * bc[c];
 }
 
 // 1 / D_i of a level (variable k): D_i = sum_{j != i} (-w_ij) (k_i + k_j)/2, halo of k by copy
@@ -91,7 +99,7 @@ __global__ void dinv_kernel(int nx, int ny, int nz, float ce, float cc, float cd
 struct LevelPlan {
     bool tiled = false;       // handled by fused_kernel
     bool stream = false;      // handled by stream_kernel
-    float* dinv = nullptr;    // 1/D (variable k), levels >= 1
+    float* dinv = nullptr;    // 1/D (variable k): levels >= 1, level 0 once a zero-guess cycle has asked for it
     float* tmp2 = nullptr;    // residual scratch of non-tiled levels
     float ce = 0, cc = 0, cdiag = 0, w0 = 0;
 };
@@ -99,6 +107,7 @@ struct LevelPlan {
 struct FusedState {
     std::vector<LevelPlan> lp;
     bool attrs_set = false;
+    bool dinv0 = false;       // keep 1/D of level 0 too (zero-guess cycles)
 };
 
 constexpr int TXD = 56, TYD = 28;   // + halo = 64 x 32 cells per plane, 16 x 16 threads
@@ -270,10 +279,11 @@ int ensure_state(mg_solver* s) {
     return 0;
 }
 
-// refresh 1/D of the levels >= 1 after a coefficient change (cheap: all coarse levels together are n/7 points)
-int refresh_dinv(mg_solver* s) {
+// refresh 1/D of the levels >= 1 after a coefficient change (cheap: all coarse levels together are n/7 points), and of
+// level 0 when zero-guess cycles use it
+int refresh_dinv(mg_solver* s, int from = -1) {
     FusedState* fs = (FusedState*)s->fused_state;
-    for (int l = 1; l < s->levels; ++l) {
+    for (int l = from >= 0 ? from : (fs->dinv0 ? 0 : 1); l < (from >= 0 ? from + 1 : s->levels); ++l) {
         LevelData& L = s->lv[l];
         LevelPlan& lp = fs->lp[l];
         if (!s->var_k) { cudaFree(lp.dinv); lp.dinv = nullptr; continue; }
@@ -485,9 +495,19 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     return 0;
 }
 
-int enqueue_vcycle(mg_solver* s, float* x, const float* b) {
+// zero_guess: x is taken as 0 whatever it holds; the first pre-smoothing sweep is then x = omega b / D (12 bytes per
+// point instead of 16 + the caller's 4 for clearing x)
+int enqueue_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
     float* res = nullptr;
-    int rc = cycle_level(s, 0, x, (float*)s->lv[0].tmp, b, 0, &res);
+    if (zero_guess) {
+        const LevelPlan& lp = ((FusedState*)s->fused_state)->lp[0];
+        const size_t n = s->lv[0].n;
+        const float g = s->var_k ? (float)s->p.omega : (float)(s->p.omega / lp.w0);
+        first_sweep_kernel<<<(int)std::min<size_t>((n + 255) / 256, 148 * 16), 256, 0, s->st>>>(n, b, s->var_k ? lp.dinv : nullptr, g, x);
+        MGB_LAUNCH_CHECK();
+        ++s->launches;
+    }
+    int rc = cycle_level(s, 0, x, (float*)s->lv[0].tmp, b, zero_guess, &res);
     if (rc) return rc;
     if (res != x) MGB_CUDA(cudaMemcpyAsync(x, res, s->lv[0].n * sizeof(float), cudaMemcpyDeviceToDevice, s->st));
     return 0;
@@ -516,11 +536,20 @@ int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps) {
     return 0;
 }
 
-int fused_vcycle(mg_solver* s, float* x, const float* b) {
+int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
     int rc = ensure_state(s);
     if (rc) return rc;
-    if (s->timing) return enqueue_vcycle(s, x, b);
-    return replay_graph(s, x, b, [&]() { return enqueue_vcycle(s, x, b); });
+    if (zero_guess && s->p.nu_pre < 1) {          // no pre-smoothing sweep to replace: clear x and run the general cycle
+        MGB_CUDA(cudaMemsetAsync(x, 0, s->lv[0].n * sizeof(float), s->st));
+        zero_guess = 0;
+    }
+    FusedState* fs = (FusedState*)s->fused_state;
+    if (zero_guess && s->var_k && !fs->lp[0].dinv) {
+        fs->dinv0 = true;
+        if ((rc = refresh_dinv(s, 0))) return rc;
+    }
+    if (s->timing) return enqueue_vcycle(s, x, b, zero_guess);
+    return replay_graph(s, x, b, [&]() { return enqueue_vcycle(s, x, b, zero_guess); }, zero_guess);
 }
 
 void fused_release(mg_solver* s) {

@@ -114,8 +114,7 @@ int pcg_t(mg_solver* s, void* d_x, const void* d_b, double tol, int max_iter, in
         return 0;
     };
     auto precondition = [&]() -> int {            // z = M rin from a zero guess
-        MGB_CUDA(cudaMemsetAsync(z, 0, n * sizeof(TZ), st));
-        return mg_vcycle(s, z, rin);
+        return vcycle_zero_guess(s, z, rin);
     };
     // ||b||, r = b - A x, ||r||
     double bb, rr;

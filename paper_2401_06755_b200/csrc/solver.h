@@ -56,6 +56,7 @@ struct mg_solver {
     cudaStream_t cap_st = nullptr;  // private stream used only to record the graph
     const void* graph_x = nullptr;
     const void* graph_b = nullptr;
+    int graph_flavour = 0;            // 0: general initial guess, 1: zero initial guess (first fine sweep x = omega b / D)
     long long graph_launches = 0;  // kernels inside one replay
     void* fused_state = nullptr;   // owned by mg_fused.cu
 };
@@ -66,8 +67,8 @@ namespace mgb {
 // pointer pair on a private stream (the caller's may be the legacy default stream, which cannot be captured), then launched
 // on the caller's stream.  mg_set_params / mg_set_coefficient / mg_set_fused drop the recorded graph.
 template <class F>
-int replay_graph(mg_solver* s, const void* x, const void* b, F&& enqueue) {
-    if (!s->graph_exec || s->graph_x != x || s->graph_b != b) {
+int replay_graph(mg_solver* s, const void* x, const void* b, F&& enqueue, int flavour = 0) {
+    if (!s->graph_exec || s->graph_x != x || s->graph_b != b || s->graph_flavour != flavour) {
         if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
         const long long before = s->launches;
         cudaGraph_t graph = nullptr;
@@ -85,7 +86,7 @@ int replay_graph(mg_solver* s, const void* x, const void* b, F&& enqueue) {
         const cudaError_t e2 = cudaGraphInstantiate(&s->graph_exec, graph, 0);
         cudaGraphDestroy(graph);
         if (e2 != cudaSuccess) { s->graph_exec = nullptr; set_error("graph instantiate failed: %s", cudaGetErrorString(e2)); return MG_ECUDA; }
-        s->graph_x = x; s->graph_b = b;
+        s->graph_x = x; s->graph_b = b; s->graph_flavour = flavour;
     }
     MGB_CUDA(cudaGraphLaunch(s->graph_exec, s->st));
     s->launches += s->graph_launches;
