@@ -61,6 +61,7 @@ struct LParams {
     const float* dinv_c;        // RR, variable k: 1 / D_c on the coarse level
     float gc_const;             // RR, constant k: omega / w0_c
     int first_sweep;            // RR: write x_c = omega b_c / D_c (1) or zeros (0)
+    int zero_x;                 // SWEEP: the iterate is zero whatever `src` holds: its planes are not read (12 B/point, not 16)
 };
 
 template <int LX_, int LY_, bool VAR_, int MODE_, int MINB_>
@@ -230,9 +231,10 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         uint64_t* bar = &bars[it % NS];
         float* dst = ring + (it % NS) * SLOT;
         const bool wb = it >= 2;                                   // plane pbeg + it - 1 >= zc0
-        mbar_expect_tx(bar, C::BOX_BYTES * (VAR ? 2u : 1u) + (wb ? C::BBOX_BYTES : 0u) + (MODE == MODE_PRO ? C::CBOX_BYTES : 0u));
+        const bool zx = MODE == MODE_SWEEP && P.zero_x;            // x planes stay the zeros written below
+        mbar_expect_tx(bar, C::BOX_BYTES * ((VAR ? 1u : 0u) + (zx ? 0u : 1u)) + (wb ? C::BBOX_BYTES : 0u) + (MODE == MODE_PRO ? C::CBOX_BYTES : 0u));
         const int z = zsrc(pbeg + it);
-        tma_load_plane(dst, &tmx, bar, x0 - 4, y0 - 1, z);
+        if (!zx) tma_load_plane(dst, &tmx, bar, x0 - 4, y0 - 1, z);
         if (VAR) tma_load_plane(dst + KOFF, &tmk, bar, x0 - 4, y0 - 1, z);
         if (wb) tma_load_plane(dst + BOFF, &tmb, bar, x0, y0, pbeg + it - 1);
         if (MODE == MODE_PRO) tma_load_plane(dst + COFF, &tmc, bar, (x0 >> 1) - 4, (y0 >> 1) - 1, z >> 1);
@@ -244,6 +246,8 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
+    if (MODE == MODE_SWEEP && P.zero_x)
+        for (int e = tid; e < NS * PLANE; e += C::NT) ring[(e / PLANE) * SLOT + (e % PLANE)] = 0.f;
     __syncthreads();
     // Programmatic dependent launch: everything above touched only kernel parameters; the fields written by the previous
     // kernel of the cycle are first read below.  The next kernel may begin its own prologue from here on.

@@ -99,7 +99,7 @@ __global__ void dinv_kernel(int nx, int ny, int nz, float ce, float cc, float cd
 struct LevelPlan {
     bool tiled = false;       // handled by fused_kernel
     bool stream = false;      // handled by stream_kernel
-    float* dinv = nullptr;    // 1/D (variable k): levels >= 1, level 0 once a zero-guess cycle has asked for it
+    float* dinv = nullptr;    // 1/D (variable k), levels >= 1
     float* tmp2 = nullptr;    // residual scratch of non-tiled levels
     float ce = 0, cc = 0, cdiag = 0, w0 = 0;
 };
@@ -107,7 +107,7 @@ struct LevelPlan {
 struct FusedState {
     std::vector<LevelPlan> lp;
     bool attrs_set = false;
-    bool dinv0 = false;       // keep 1/D of level 0 too (zero-guess cycles)
+    bool zero_x_once = false; // the next SWEEP launch takes its input iterate as zero (zero-guess cycles)
 };
 
 constexpr int TXD = 56, TYD = 28;   // + halo = 64 x 32 cells per plane, 16 x 16 threads
@@ -225,6 +225,7 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
     P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
     P.omega = (float)s->p.omega;
     P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
+    if (MODE == lk::MODE_SWEEP && fs->zero_x_once) { P.zero_x = 1; fs->zero_x_once = false; }
     if (MODE == lk::MODE_RR) {
         const LevelPlan& cp = fs->lp[l + 1];
         P.dinv_c = cp.dinv;
@@ -279,11 +280,10 @@ int ensure_state(mg_solver* s) {
     return 0;
 }
 
-// refresh 1/D of the levels >= 1 after a coefficient change (cheap: all coarse levels together are n/7 points), and of
-// level 0 when zero-guess cycles use it
-int refresh_dinv(mg_solver* s, int from = -1) {
+// refresh 1/D of the levels >= 1 after a coefficient change (cheap: all coarse levels together are n/7 points)
+int refresh_dinv(mg_solver* s) {
     FusedState* fs = (FusedState*)s->fused_state;
-    for (int l = from >= 0 ? from : (fs->dinv0 ? 0 : 1); l < (from >= 0 ? from + 1 : s->levels); ++l) {
+    for (int l = 1; l < s->levels; ++l) {
         LevelData& L = s->lv[l];
         LevelPlan& lp = fs->lp[l];
         if (!s->var_k) { cudaFree(lp.dinv); lp.dinv = nullptr; continue; }
@@ -495,19 +495,13 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     return 0;
 }
 
-// zero_guess: x is taken as 0 whatever it holds; the first pre-smoothing sweep is then x = omega b / D (12 bytes per
-// point instead of 16 + the caller's 4 for clearing x)
+// zero_guess: x is taken as 0 whatever it holds: the first pre-smoothing pass does not read it (12 bytes per point instead
+// of 16, and the caller need not clear x)
 int enqueue_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
     float* res = nullptr;
-    if (zero_guess) {
-        const LevelPlan& lp = ((FusedState*)s->fused_state)->lp[0];
-        const size_t n = s->lv[0].n;
-        const float g = s->var_k ? (float)s->p.omega : (float)(s->p.omega / lp.w0);
-        first_sweep_kernel<<<(int)std::min<size_t>((n + 255) / 256, 148 * 16), 256, 0, s->st>>>(n, b, s->var_k ? lp.dinv : nullptr, g, x);
-        MGB_LAUNCH_CHECK();
-        ++s->launches;
-    }
-    int rc = cycle_level(s, 0, x, (float*)s->lv[0].tmp, b, zero_guess, &res);
+    ((FusedState*)s->fused_state)->zero_x_once = zero_guess != 0;
+    int rc = cycle_level(s, 0, x, (float*)s->lv[0].tmp, b, 0, &res);
+    ((FusedState*)s->fused_state)->zero_x_once = false;
     if (rc) return rc;
     if (res != x) MGB_CUDA(cudaMemcpyAsync(x, res, s->lv[0].n * sizeof(float), cudaMemcpyDeviceToDevice, s->st));
     return 0;
@@ -539,14 +533,16 @@ int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps) {
 int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
     int rc = ensure_state(s);
     if (rc) return rc;
-    if (zero_guess && s->p.nu_pre < 1) {          // no pre-smoothing sweep to replace: clear x and run the general cycle
-        MGB_CUDA(cudaMemsetAsync(x, 0, s->lv[0].n * sizeof(float), s->st));
-        zero_guess = 0;
-    }
-    FusedState* fs = (FusedState*)s->fused_state;
-    if (zero_guess && s->var_k && !fs->lp[0].dinv) {
-        fs->dinv0 = true;
-        if ((rc = refresh_dinv(s, 0))) return rc;
+    if (zero_guess) {
+        // the first launch of the cycle has to be a lean_kernel sweep of level 0; otherwise clear x and run the general cycle
+        FusedState* fs = (FusedState*)s->fused_state;
+        size_t sm = 0; int a = 0, c = 0;
+        const bool lean0 = fs->lp[0].stream && s->p.sweeps_per_pass == 1 && s->p.nu_pre >= 1 && s->levels > 1 &&
+                           !ctail_fits(s, 0, &sm, &a, &c) && !tail_fits(s, 0, &sm);
+        if (!lean0) {
+            MGB_CUDA(cudaMemsetAsync(x, 0, s->lv[0].n * sizeof(float), s->st));
+            zero_guess = 0;
+        }
     }
     if (s->timing) return enqueue_vcycle(s, x, b, zero_guess);
     return replay_graph(s, x, b, [&]() { return enqueue_vcycle(s, x, b, zero_guess); }, zero_guess);
