@@ -293,3 +293,27 @@ def test_empty_cycles_and_zero_rhs(mg):
     mg.mg_smooth(s, x, b, 0)
     assert float(x.abs().max()) == 0.0
     mg.mg_destroy(s)
+
+
+@pytest.mark.parametrize("var", [False, True])
+@pytest.mark.parametrize("shape,levels,nu", [((64, 48, 96), 4, 2), ((32, 32, 32), 4, 1), ((16, 16, 16), 3, 2), ((40, 24, 48), 3, 0)])
+def test_zero_guess_cycle_equals_cycle_from_cleared_x(mg, shape, levels, nu, var):
+    """The correction cycles of mg_solve / mg_pcg_solve start from x = 0 without reading x (lean_kernel zero_x; cleared x
+    where level 0 is not a lean_kernel level or nu_pre = 0).  One cycle of the mixed-precision solve from x = 0 is
+    x = V(0, float(b)): it must equal the public mg_vcycle from a cleared x up to the fp64 -> fp32 rounding of the result."""
+    dt = "f32"
+    _, b, k = make_problem(shape, dt, var, 77)
+    bc = (N, N, N, N, N, D)
+    s = make_solver(mg, shape, 1.0 / shape[2], levels, bc, dt, k=k if var else None, nu_pre=nu, nu_post=max(nu, 1))
+    db = to_dev(b, dt)
+    x_cycle = to_dev(np.zeros(shape), dt)
+    assert mg.mg_vcycle(s, x_cycle, db) == mg.MG_OK
+    x_solve = to_dev(np.zeros(shape), dt)                  # the solver's correction buffer is uninitialised at this point
+    st, cycles, rel = mg.mg_solve(s, x_solve, db, 0.0, 1)
+    assert cycles == 1
+    assert rel_l2(as_f64(x_solve), as_f64(x_cycle)) <= 2e-7
+    # a second solve reuses the (possibly dirty) correction buffer: same answer
+    x2 = to_dev(np.zeros(shape), dt)
+    mg.mg_solve(s, x2, db, 0.0, 1)
+    assert rel_l2(as_f64(x2), as_f64(x_solve)) == 0.0
+    mg.mg_destroy(s)
