@@ -11,6 +11,8 @@
 // the pressure halo in the projection uses the solver's factors (reading C10).
 #include <algorithm>
 #include <cmath>
+#include <cstdint>
+#include <initializer_list>
 
 #include "solver.h"
 
@@ -59,6 +61,23 @@ template <typename T> __device__ __forceinline__ T tmin(T a, T b) { return a < b
 template <typename T> __device__ __forceinline__ T tmax(T a, T b) { return a > b ? a : b; }
 
 #include "flow_march.cuh"
+
+// W-wide kernels need nx % W == 0 and 16-byte aligned fields (vector loads); otherwise the W = 1 instantiation runs
+template <typename T> constexpr int vec_w() { return sizeof(T) == 4 ? 4 : 2; }
+template <typename T>
+bool can_vec(const mg_grid* g, std::initializer_list<const void*> ptrs) {
+    if (g->nx % vec_w<T>() != 0) return false;
+    for (const void* q : ptrs)
+        if (q && (reinterpret_cast<uintptr_t>(q) & 15u)) return false;
+    return true;
+}
+// WV: the pack width of the vector instantiation (a divisor of vec_w<T>())
+#define MGB_MARCH_W(KERNEL, WV, VEC, G, st, ...)                                                        \
+    do {                                                                                                \
+        if (VEC) KERNEL<T, WV><<<march_grid<T, WV>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__);        \
+        else KERNEL<T, 1><<<march_grid<T, 1>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__);              \
+    } while (0)
+#define MGB_MARCH(KERNEL, VEC, G, st, ...) MGB_MARCH_W(KERNEL, vec_w<T>(), VEC, G, st, __VA_ARGS__)
 
 template <typename T>
 __global__ void __launch_bounds__(256) axpy_kernel(size_t n, T* __restrict__ y, const T* __restrict__ x) {
@@ -109,9 +128,11 @@ int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T
     T *adv = (T*)ws.p[0], *kx = (T*)ws.p[1], *ky = (T*)ws.p[2], *kz = (T*)ws.p[3];
     const double hmax = fmax(g->hx, fmax(g->hy, g->hz)), hmin = fmin(g->hx, fmin(g->hy, g->hz));
     const double k_min = 1e-4 / dt * hmax * hmax, k_max = 0.05 / dt * hmin * hmin;   // Eq. 42
-    advection_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv);
-    vof_coeff_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
-    vof_diffusion_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, adv, kx, ky, kz, (T)dt, sC, Cnew);
+    const bool vec = can_vec<T>(g, {C, u, v, w, sC, Cnew});
+    MGB_MARCH(advection_march, vec, G, st, C, u, v, w, adv);
+    // division-heavy: 4-wide packs cost more in registers than they save in loads (324 vs 395 us at 256^3)
+    MGB_MARCH_W(vof_coeff_march, 2, vec, G, st, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
+    MGB_MARCH(vof_diffusion_march, vec, G, st, C, adv, kx, ky, kz, (T)dt, sC, Cnew);
     MGB_LAUNCH_CHECK();
     return 0;
 }
@@ -125,11 +146,12 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
     int rc = ws.alloc(2, bytes);
     if (rc) return rc;
     T *adv = (T*)ws.p[0], *kc = (T*)ws.p[1];
+    const bool vec = can_vec<T>(g, {C, qh[0], qh[1], qh[2], qn[0], qn[1], qn[2], qt[0], qt[1], qt[2], qhn ? qhn[0] : nullptr,
+                                    qhn ? qhn[1] : nullptr, qhn ? qhn[2] : nullptr});
     for (int c = 0; c < 3; ++c) {
-        advection_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, qh[c], qh[0], qh[1], qh[2], adv);
-        mom_coeff_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc);
-        mom_update_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c],
-                                                  qhn ? qhn[c] : (T*)nullptr);
+        MGB_MARCH(advection_march, vec, G, st, qh[c], qh[0], qh[1], qh[2], adv);
+        MGB_MARCH(mom_coeff_march, vec, G, st, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc);
+        MGB_MARCH(mom_update_march, vec, G, st, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c], qhn ? qhn[c] : (T*)nullptr);
     }
     MGB_LAUNCH_CHECK();
     return 0;
@@ -138,7 +160,7 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
 template <typename T>
 int pressure_rhs_t(const mg_grid* g, const T* u, const T* v, const T* w, double dt, T* b, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
-    pressure_rhs_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, u, v, w, (T)(1.0 / dt), b);
+    MGB_MARCH(pressure_rhs_march, can_vec<T>(g, {u, v, w, b}), G, st, u, v, w, (T)(1.0 / dt), b);
     MGB_LAUNCH_CHECK();
     return 0;
 }
@@ -147,7 +169,7 @@ template <typename T>
 int pressure_rhs_paper_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double rho_l, double rho_g, double dt, T* b,
                          cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
-    pressure_rhs_paper_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, (T)rho_l, (T)rho_g, (T)(1.0 / dt), b);
+    MGB_MARCH(pressure_rhs_paper_march, can_vec<T>(g, {C, u, v, w, b}), G, st, C, u, v, w, (T)rho_l, (T)rho_g, (T)(1.0 / dt), b);
     MGB_LAUNCH_CHECK();
     return 0;
 }
@@ -160,10 +182,10 @@ int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, 
     int rc;
     if ((rc = ws.alloc(3, bytes)) || (rc = ws2.alloc(3, bytes))) return rc;
     T *n0 = (T*)ws.p[0], *n1 = (T*)ws.p[1], *n2 = (T*)ws.p[2], *f0 = (T*)ws2.p[0], *f1 = (T*)ws2.p[1], *f2 = (T*)ws2.p[2];
-    const dim3 grd = march_grid(G), blk(MBX, MBY);
-    normals_march<T><<<grd, blk, 0, st>>>(G, C, n0, n1, n2);
-    surface_tension_march<T><<<grd, blk, 0, st>>>(G, C, n0, n1, n2, (T)rho_l, (T)rho_g, (T)grav, (T)sigma_t, f0, f1, f2, kappa);
-    pressure_rhs_march<T><<<grd, blk, 0, st>>>(G, f0, f1, f2, T(-1), b);       // b = +(f(fu; w_x) + f(fv; w_y) + f(fw; w_z))
+    const bool vec = can_vec<T>(g, {C, b, kappa});
+    MGB_MARCH(normals_march, vec, G, st, C, n0, n1, n2);
+    MGB_MARCH(surface_tension_march, vec, G, st, C, n0, n1, n2, (T)rho_l, (T)rho_g, (T)grav, (T)sigma_t, f0, f1, f2, kappa);
+    MGB_MARCH(pressure_rhs_march, vec, G, st, f0, f1, f2, T(-1), b);       // b = +(f(fu; w_x) + f(fv; w_y) + f(fw; w_z))
     bottom_fold_kernel<T><<<dim3((g->nx + 31) / 32, (g->ny + 7) / 8), dim3(32, 8), 0, st>>>(G, C, (T)rho_l, (T)rho_g, (T)grav, b);
     MGB_LAUNCH_CHECK();
     return 0;
@@ -172,7 +194,7 @@ int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, 
 template <typename T>
 int project_t(const mg_grid* g, const int* bc, const T* p, const T* k, double dt, T* u, T* v, T* w, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, bc);
-    project_march<T><<<march_grid(G), dim3(MBX, MBY), 0, st>>>(G, p, k, (T)dt, u, v, w);
+    MGB_MARCH(project_march, can_vec<T>(g, {p, k, u, v, w}), G, st, p, k, (T)dt, u, v, w);
     MGB_LAUNCH_CHECK();
     return 0;
 }

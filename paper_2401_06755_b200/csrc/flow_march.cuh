@@ -2,166 +2,283 @@
 // namespace, after Geo / k_abs_pg).  Same filters and readings; different evaluation order:
 //
 // Every filter of the path is a tensor product of 1-D factors (Eqs. 9-11): D = [-1,0,1]/(2d),
-// M = [1,4,1]/6, K = [-1,2,-1]/d^2.  A thread owns one (i, j) column of a z chunk and marches along z.  Per plane
-// it loads the 3 x 3 in-plane neighbourhood of each field once (9 loads, served by L1 for the neighbours the
-// other threads of the block also load), applies the x and y factors, and keeps the in-plane results of the last
-// three planes in registers; the z factor is applied when the plane above has arrived.  That is 9 loads per
-// field and point instead of 27.  Halos are zero-derivative copies (clamped indices, reading C9-iv), the
-// pressure halo of the projection carries the solver's factors (reading C10).
+// M = [1,4,1]/6, K = [-1,2,-1]/d^2.  A thread owns W consecutive x points of one (j) row of a z chunk and marches
+// along z (W = 4 in fp32, 2 in fp64; 1 when nx is not a multiple of that or a pointer is not 16-byte aligned).  Per
+// plane and field it loads its 3 rows once -- one 16-byte vector and the two x neighbours per row -- applies the x and
+// y factors, and keeps the in-plane results of the last three planes in registers; the z factor is applied when the
+// plane above has arrived.  That is 9 / W load instructions per field and point instead of 27.  All arithmetic is
+// written once on the W-wide value pack Pk.  Halos are zero-derivative copies (clamped indices, reading
+// C9-iv), the pressure halo of the projection carries the solver's factors (reading C10).
 #pragma once
 
-constexpr int MBX = 32, MBY = 8, MZC = 16;   // block = MBX x MBY columns, MZC output planes per block
+constexpr int MBX = 32, MBY = 4, MZC = 16;   // block = MBX x MBY threads (W MBX x MBY columns), MZC output planes per block
 
-template <typename T>
-struct Col {           // z-invariant addressing of a thread's column
-    int i, j;
-    int ix[3];
-    size_t row[3];     // nx * clamped j
+// ---- W-wide value pack: element-wise arithmetic --------------------------------------------------------------------
+template <typename T, int W>
+struct Pk {
+    T v[W];
+    __device__ __forceinline__ T& operator[](int e) { return v[e]; }
+    __device__ __forceinline__ const T& operator[](int e) const { return v[e]; }
+};
+#define MGB_PK_BIN(OP)                                                                                                  \
+    template <typename T, int W> __device__ __forceinline__ Pk<T, W> operator OP(const Pk<T, W>& a, const Pk<T, W>& b) { \
+        Pk<T, W> r;                                                                                                     \
+        _Pragma("unroll") for (int e = 0; e < W; ++e) r.v[e] = a.v[e] OP b.v[e];                                        \
+        return r;                                                                                                       \
+    }                                                                                                                   \
+    template <typename T, int W> __device__ __forceinline__ Pk<T, W> operator OP(const Pk<T, W>& a, T b) {               \
+        Pk<T, W> r;                                                                                                     \
+        _Pragma("unroll") for (int e = 0; e < W; ++e) r.v[e] = a.v[e] OP b;                                             \
+        return r;                                                                                                       \
+    }                                                                                                                   \
+    template <typename T, int W> __device__ __forceinline__ Pk<T, W> operator OP(T a, const Pk<T, W>& b) {               \
+        Pk<T, W> r;                                                                                                     \
+        _Pragma("unroll") for (int e = 0; e < W; ++e) r.v[e] = a OP b.v[e];                                             \
+        return r;                                                                                                       \
+    }
+MGB_PK_BIN(+)
+MGB_PK_BIN(-)
+MGB_PK_BIN(*)
+MGB_PK_BIN(/)
+#undef MGB_PK_BIN
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> operator-(const Pk<T, W>& a) {
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r.v[e] = -a.v[e];
+    return r;
+}
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> splat(T a) {
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r.v[e] = a;
+    return r;
+}
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pabs(const Pk<T, W>& a) {
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r.v[e] = fabs(a.v[e]);
+    return r;
+}
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> psqrt(const Pk<T, W>& a) {
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r.v[e] = sqrt(a.v[e]);
+    return r;
+}
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pmin(const Pk<T, W>& a, const Pk<T, W>& b) {
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r.v[e] = tmin(a.v[e], b.v[e]);
+    return r;
+}
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pmax(const Pk<T, W>& a, const Pk<T, W>& b) {
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r.v[e] = tmax(a.v[e], b.v[e]);
+    return r;
+}
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pmin(T a, const Pk<T, W>& b) { return pmin(splat<T, W>(a), b); }
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pmax(T a, const Pk<T, W>& b) { return pmax(splat<T, W>(a), b); }
+
+// aligned vector load / store of a pack (W sizeof(T) = 4, 8, 16 or 32 bytes)
+template <typename T, int W>
+__device__ __forceinline__ Pk<T, W> ldv(const T* __restrict__ p) {
+    Pk<T, W> r;
+    if constexpr (W == 1) r.v[0] = *p;
+    else if constexpr (sizeof(T) == 4 && W == 4) { const float4 t = *reinterpret_cast<const float4*>(p); r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; }
+    else if constexpr (sizeof(T) == 8 && W == 2) { const double2 t = *reinterpret_cast<const double2*>(p); r.v[0] = t.x; r.v[1] = t.y; }
+    else {
+#pragma unroll
+        for (int e = 0; e < W; ++e) r.v[e] = p[e];
+    }
+    return r;
+}
+template <typename T, int W>
+__device__ __forceinline__ void stv(T* __restrict__ p, const Pk<T, W>& a) {
+    if constexpr (W == 1) *p = a.v[0];
+    else if constexpr (sizeof(T) == 4 && W == 4) *reinterpret_cast<float4*>(p) = make_float4(a.v[0], a.v[1], a.v[2], a.v[3]);
+    else if constexpr (sizeof(T) == 8 && W == 2) *reinterpret_cast<double2*>(p) = make_double2(a.v[0], a.v[1]);
+    else {
+#pragma unroll
+        for (int e = 0; e < W; ++e) p[e] = a.v[e];
+    }
+}
+
+template <typename T, int W>
+struct Col {           // z-invariant addressing of a thread's W points
+    int i, j;          // first x index (a multiple of W), row
+    int il, ir;        // clamped x neighbours of the pack's ends
+    size_t row[3];     // nx * clamped j - 1, j, j + 1
     size_t nxy;
     int z0, z1;        // output planes [z0, z1)
     bool ok;
 };
 
-template <typename T>
-__device__ __forceinline__ Col<T> make_col(const Geo<T>& G) {
-    Col<T> c;
-    c.i = blockIdx.x * MBX + threadIdx.x; c.j = blockIdx.y * MBY + threadIdx.y;
-    c.ok = c.i < G.nx && c.j < G.ny;
-    const int i = min(c.i, G.nx - 1), j = min(c.j, G.ny - 1);
-    c.ix[0] = max(i - 1, 0); c.ix[1] = i; c.ix[2] = min(i + 1, G.nx - 1);
+template <typename T, int W>
+__device__ __forceinline__ Col<T, W> make_col(const Geo<T>& G) {
+    Col<T, W> c;
+    c.i = W * (blockIdx.x * MBX + threadIdx.x); c.j = blockIdx.y * MBY + threadIdx.y;
+    c.ok = c.i < G.nx && c.j < G.ny;                      // nx is a multiple of W
+    const int j = min(c.j, G.ny - 1);
+    c.i = min(c.i, G.nx - W);
+    c.il = max(c.i - 1, 0); c.ir = min(c.i + W, G.nx - 1);
     c.row[0] = (size_t)G.nx * max(j - 1, 0); c.row[1] = (size_t)G.nx * j; c.row[2] = (size_t)G.nx * min(j + 1, G.ny - 1);
     c.nxy = (size_t)G.nx * G.ny;
     c.z0 = blockIdx.z * MZC; c.z1 = min(c.z0 + MZC, G.nz);
     return c;
 }
 
-template <typename T>
-dim3 march_grid(const Geo<T>& G) { return dim3((G.nx + MBX - 1) / MBX, (G.ny + MBY - 1) / MBY, (G.nz + MZC - 1) / MZC); }
+template <typename T, int W>
+dim3 march_grid(const Geo<T>& G) { return dim3((G.nx + W * MBX - 1) / (W * MBX), (G.ny + MBY - 1) / MBY, (G.nz + MZC - 1) / MZC); }
 
-// the 3 x 3 in-plane neighbourhood v[b][a] (b along y, a along x) of plane z (clamped)
-template <typename T>
-__device__ __forceinline__ void load9(const Geo<T>& G, const Col<T>& c, const T* __restrict__ f, int z, T (&v)[3][3]) {
+// the 3 x 3 in-plane neighbourhood v[b][a] (b along y, a along x) of plane z (clamped) for the thread's W points
+template <typename T, int W>
+__device__ __forceinline__ void load9(const Geo<T>& G, const Col<T, W>& c, const T* __restrict__ f, int z, Pk<T, W> (&v)[3][3]) {
     const T* p = f + c.nxy * (size_t)min(max(z, 0), G.nz - 1);
 #pragma unroll
-    for (int b = 0; b < 3; ++b)
+    for (int b = 0; b < 3; ++b) {
+        const T* r = p + c.row[b];
+        const T l = r[c.il], rr = r[c.ir];
+        v[b][1] = ldv<T, W>(r + c.i);
+        v[b][0][0] = l; v[b][2][W - 1] = rr;
 #pragma unroll
-        for (int a = 0; a < 3; ++a) v[b][a] = p[c.row[b] + c.ix[a]];
+        for (int e = 1; e < W; ++e) { v[b][0][e] = v[b][1][e - 1]; v[b][2][e - 1] = v[b][1][e]; }
+    }
 }
+// index of the thread's first point in plane q
+template <typename T, int W>
+__device__ __forceinline__ size_t at(const Col<T, W>& c, int q) { return c.nxy * q + c.row[1] + c.i; }
 
 // in-plane tensor-product filters of a 3 x 3 neighbourhood
-template <typename T>
+template <typename V>
 struct InPlane {
-    T mm, dm, md, km, mk;    // Mx My, Dx My, Mx Dy, Kx My, Mx Ky
+    V mm, dm, md, km, mk;    // Mx My, Dx My, Mx Dy, Kx My, Mx Ky
 };
-template <typename T, bool NEED_D, bool NEED_K>
-__device__ __forceinline__ InPlane<T> in_plane(const Geo<T>& G, const T (&v)[3][3]) {
+template <typename T, bool NEED_D, bool NEED_K, typename V>
+__device__ __forceinline__ InPlane<V> in_plane(const Geo<T>& G, const V (&v)[3][3]) {
     const T m0 = G.M[0], m1 = G.M[1];
-    T sm[3], sd[3], sk[3];
+    V sm[3], sd[3], sk[3];
 #pragma unroll
     for (int b = 0; b < 3; ++b) {
-        const T e = v[b][0] + v[b][2];
+        const V e = v[b][0] + v[b][2];
         sm[b] = m0 * e + m1 * v[b][1];
         if (NEED_D) sd[b] = G.D[0][2] * (v[b][2] - v[b][0]);
         if (NEED_K) sk[b] = G.K[0][0] * (e - T(2) * v[b][1]);       // K = [-1, 2, -1]/d^2, K[0] = -1/d^2
     }
-    InPlane<T> r;
+    InPlane<V> r;
     r.mm = m0 * (sm[0] + sm[2]) + m1 * sm[1];
-    r.dm = r.md = r.km = r.mk = T(0);
+    r.dm = r.md = r.km = r.mk = V{};
     if (NEED_D) { r.dm = m0 * (sd[0] + sd[2]) + m1 * sd[1]; r.md = G.D[1][2] * (sm[2] - sm[0]); }
     if (NEED_K) { r.km = m0 * (sk[0] + sk[2]) + m1 * sk[1]; r.mk = G.K[1][0] * ((sm[0] + sm[2]) - T(2) * sm[1]); }
     return r;
 }
 
 // z factors over a rolling triple a[0] = plane q - 1, a[1] = plane q, a[2] = plane q + 1
-template <typename T> __device__ __forceinline__ T zM(const Geo<T>& G, const T (&a)[3]) { return G.M[0] * (a[0] + a[2]) + G.M[1] * a[1]; }
-template <typename T> __device__ __forceinline__ T zD(const Geo<T>& G, const T (&a)[3]) { return G.D[2][2] * (a[2] - a[0]); }
-template <typename T> __device__ __forceinline__ T zK(const Geo<T>& G, const T (&a)[3]) { return G.K[2][0] * ((a[0] + a[2]) - T(2) * a[1]); }
-template <typename T> __device__ __forceinline__ void push(T (&a)[3], T v) { a[0] = a[1]; a[1] = a[2]; a[2] = v; }
+template <typename T, typename V> __device__ __forceinline__ V zM(const Geo<T>& G, const V (&a)[3]) { return G.M[0] * (a[0] + a[2]) + G.M[1] * a[1]; }
+template <typename T, typename V> __device__ __forceinline__ V zD(const Geo<T>& G, const V (&a)[3]) { return G.D[2][2] * (a[2] - a[0]); }
+template <typename T, typename V> __device__ __forceinline__ V zK(const Geo<T>& G, const V (&a)[3]) { return G.K[2][0] * ((a[0] + a[2]) - T(2) * a[1]); }
+template <typename V> __device__ __forceinline__ void push(V (&a)[3], const V& v) { a[0] = a[1]; a[1] = a[2]; a[2] = v; }
 
 // b = -(1/dt) (f(u; w_x) + f(v; w_y) + f(w; w_z))  (reading C10; Eq. 53 structure)
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_march(const Geo<T> G, const T* __restrict__ u, const T* __restrict__ v,
                                                              const T* __restrict__ w, T inv_dt, T* __restrict__ bout) {
-    const Col<T> c = make_col(G);
-    T suv[3] = {T(0), T(0), T(0)}, aw[3] = {T(0), T(0), T(0)};
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    V suv[3] = {}, aw[3] = {};
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T n9[3][3];
-        load9(G, c, u, z, n9); const T du = in_plane<T, true, false>(G, n9).dm;
-        load9(G, c, v, z, n9); const T dv = in_plane<T, true, false>(G, n9).md;
-        load9(G, c, w, z, n9); const T mw = in_plane<T, false, false>(G, n9).mm;
+        V n9[3][3];
+        load9(G, c, u, z, n9); const V du = in_plane<T, true, false>(G, n9).dm;
+        load9(G, c, v, z, n9); const V dv = in_plane<T, true, false>(G, n9).md;
+        load9(G, c, w, z, n9); const V mw = in_plane<T, false, false>(G, n9).mm;
         push(suv, du + dv); push(aw, mw);
         const int q = z - 1;
-        if (q >= c.z0 && c.ok) bout[c.nxy * q + c.row[1] + c.ix[1]] = -(zM(G, suv) + zD(G, aw)) * inv_dt;
+        if (q >= c.z0 && c.ok) stv(bout + at(c, q), -(zM(G, suv) + zD(G, aw)) * inv_dt);
     }
 }
 
 // gradient by the FE first-derivative filters from rolling in-plane results
-template <typename T>
+template <typename T, typename V>
 struct GradRoll {
-    T ax[3], ay[3], am[3];
-    __device__ __forceinline__ void init() { for (int e = 0; e < 3; ++e) ax[e] = ay[e] = am[e] = T(0); }
-    __device__ __forceinline__ void add(const InPlane<T>& r) { push(ax, r.dm); push(ay, r.md); push(am, r.mm); }
-    __device__ __forceinline__ void grad(const Geo<T>& G, T& gx, T& gy, T& gz) const { gx = zM(G, ax); gy = zM(G, ay); gz = zD(G, am); }
+    V ax[3], ay[3], am[3];
+    __device__ __forceinline__ void init() { for (int e = 0; e < 3; ++e) ax[e] = ay[e] = am[e] = V{}; }
+    __device__ __forceinline__ void add(const InPlane<V>& r) { push(ax, r.dm); push(ay, r.md); push(am, r.mm); }
+    __device__ __forceinline__ void grad(const Geo<T>& G, V& gx, V& gy, V& gz) const { gx = zM(G, ax); gy = zM(G, ay); gz = zD(G, am); }
 };
 
 // q <- q - dt k f(p; w_x|y|z) (Eq. 54); halo of p = s * mirror with the solver's factors
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) project_march(const Geo<T> G, const T* __restrict__ p, const T* __restrict__ kc, T dt,
                                                         T* __restrict__ u, T* __restrict__ v, T* __restrict__ w) {
-    const Col<T> c = make_col(G);
-    const T fx[3] = {c.i > 0 ? T(1) : G.s[0], T(1), c.i < G.nx - 1 ? T(1) : G.s[1]};
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    // only the outermost lane of a pack's left / right neighbour can be a ghost
+    const T fl = c.i > 0 ? T(1) : G.s[0], fr = c.i + W < G.nx ? T(1) : G.s[1];
     const T fy[3] = {c.j > 0 ? T(1) : G.s[2], T(1), c.j < G.ny - 1 ? T(1) : G.s[3]};
-    GradRoll<T> g; g.init();
+    GradRoll<T, V> g; g.init();
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T n9[3][3];
+        V n9[3][3];
         load9(G, c, p, z, n9);
         const T fz = z < 0 ? G.s[4] : (z >= G.nz ? G.s[5] : T(1));
 #pragma unroll
-        for (int b = 0; b < 3; ++b)
+        for (int b = 0; b < 3; ++b) {
+            n9[b][0][0] *= fl; n9[b][2][W - 1] *= fr;
 #pragma unroll
-            for (int a = 0; a < 3; ++a) n9[b][a] *= fz * fy[b] * fx[a];
+            for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] * (fz * fy[b]);
+        }
         g.add(in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            T gx, gy, gz; g.grad(G, gx, gy, gz);
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            const T f = dt * kc[c0];
-            u[c0] -= f * gx; v[c0] -= f * gy; w[c0] -= f * gz;
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const size_t c0 = at(c, q);
+            const V f = dt * ldv<T, W>(kc + c0);
+            stv(u + c0, ldv<T, W>(u + c0) - f * gx); stv(v + c0, ldv<T, W>(v + c0) - f * gy); stv(w + c0, ldv<T, W>(w + c0) - f * gz);
         }
     }
 }
 
 // steps 1-2 of reading C9: adv = u psi_x + v psi_y + w psi_z
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) advection_march(const Geo<T> G, const T* __restrict__ psi, const T* __restrict__ u,
                                                           const T* __restrict__ v, const T* __restrict__ w, T* __restrict__ adv) {
-    const Col<T> c = make_col(G);
-    GradRoll<T> g; g.init();
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    GradRoll<T, V> g; g.init();
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T n9[3][3];
+        V n9[3][3];
         load9(G, c, psi, z, n9);
         g.add(in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            T gx, gy, gz; g.grad(G, gx, gy, gz);
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            adv[c0] = u[c0] * gx + v[c0] * gy + w[c0] * gz;
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const size_t c0 = at(c, q);
+            stv(adv + c0, ldv<T, W>(u + c0) * gx + ldv<T, W>(v + c0) * gy + ldv<T, W>(w + c0) * gz);
         }
     }
 }
 
+// Eqs. 26/27 on a pack (k_abs_pg of flow.cu lane by lane)
+template <typename T, int W>
+__device__ __forceinline__ Pk<T, W> k_abs_pk(const Geo<T>& G, const Pk<T, W>& a, const Pk<T, W>& px, const Pk<T, W>& py, const Pk<T, W>& pz) {
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r[e] = k_abs_pg(G, a[e], px[e], py[e], pz[e]);
+    return r;
+}
+
 // momentum: k_c = rho min{k_max, k_abs(c)} + mu (Eqs. 30-32; k_square of the lost Eq. 28 omitted);
 // k_abs from the gradient of the component and the mixed-mass residual a = 2 (Mx My Mz - E) adv (Eq. 29)
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) mom_coeff_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ comp,
                                                           const T* __restrict__ u, const T* __restrict__ v, const T* __restrict__ w,
                                                           const T* __restrict__ adv, T rho_l, T rho_g, T mu_l, T mu_g,
                                                           T* __restrict__ kc) {
-    const Col<T> c = make_col(G);
-    GradRoll<T> g; g.init();
-    T am[3] = {T(0), T(0), T(0)}, a0 = T(0), a0n = T(0);     // Mx My adv of three planes; adv at the centre of planes q, q + 1
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    GradRoll<T, V> g; g.init();
+    V am[3] = {}, a0 = {}, a0n = {};     // Mx My adv of three planes; adv at the centre of planes q, q + 1
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T n9[3][3];
+        V n9[3][3];
         load9(G, c, comp, z, n9);
         g.add(in_plane<T, true, false>(G, n9));
         load9(G, c, adv, z, n9);
@@ -169,80 +286,83 @@ __global__ void __launch_bounds__(MBX* MBY) mom_coeff_march(const Geo<T> G, cons
         a0 = a0n; a0n = n9[1][1];
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            T px, py, pz; g.grad(G, px, py, pz);
-            const T a = T(2) * (zM(G, am) - a0);
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            const T Cc = C[c0];
-            const T rho = rho_l * Cc + rho_g * (T(1) - Cc);
-            const T mu = mu_l * Cc + mu_g * (T(1) - Cc);
-            const T kmax = G.h[0] * fabs(u[c0]) + G.h[1] * fabs(v[c0]) + G.h[2] * fabs(w[c0]);   // Eq. 30
-            kc[c0] = rho * tmin(kmax, k_abs_pg(G, a, px, py, pz)) + mu;
+            V px, py, pz; g.grad(G, px, py, pz);
+            const V a = T(2) * (zM(G, am) - a0);
+            const size_t c0 = at(c, q);
+            const V Cc = ldv<T, W>(C + c0);
+            const V rho = rho_l * Cc + rho_g * (T(1) - Cc);
+            const V mu = mu_l * Cc + mu_g * (T(1) - Cc);
+            const V kmax = G.h[0] * pabs(ldv<T, W>(u + c0)) + G.h[1] * pabs(ldv<T, W>(v + c0)) + G.h[2] * pabs(ldv<T, W>(w + c0));   // Eq. 30
+            stv(kc + c0, rho * pmin(kmax, k_abs_pk(G, a, px, py, pz)) + mu);
         }
     }
 }
 
 // rolling in-plane parts of a filter  W = F_xy (x) F_z  applied to three fields (f, k, k f), combined as Eq. 12-13:
 //   sum_j (-W_ij) 1/2 (k_i + k_j)(f_i - f_j) = 1/2 (W(k f) + k W(f) - f W(k))      [sum_j W_ij = 0]
-template <typename T>
+template <typename V>
 struct Diff3 {
-    T f[3], k[3], z[3];
-    __device__ __forceinline__ void init() { for (int e = 0; e < 3; ++e) f[e] = k[e] = z[e] = T(0); }
-    __device__ __forceinline__ void add(T pf, T pk, T pz) { push(f, pf); push(k, pk); push(z, pz); }
+    V f[3], k[3], z[3];
+    __device__ __forceinline__ void init() { for (int e = 0; e < 3; ++e) f[e] = k[e] = z[e] = V{}; }
+    __device__ __forceinline__ void add(const V& pf, const V& pk, const V& pz) { push(f, pf); push(k, pk); push(z, pz); }
 };
 
 // s = rho adv + f^lap(c, k_c; w_lap) (Eq. 18 without pressure / source terms), q~ = q_n - dt s / rho (Eq. 45, sigma = 0),
 // q_half' = (q_n + q~)/2 (Eq. 46).  w_lap = (Kx My + Mx Ky) Mz + Mx My Kz.
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) mom_update_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ comp,
                                                            const T* __restrict__ kc, const T* __restrict__ adv,
                                                            const T* __restrict__ qn, T rho_l, T rho_g, T dt, T* __restrict__ qt,
                                                            T* __restrict__ qhn) {
-    const Col<T> c = make_col(G);
-    Diff3<T> p1, p2; p1.init(); p2.init();       // in-plane (Kx My + Mx Ky) and Mx My of x, k, k x
-    T x0 = T(0), x0n = T(0), k0 = T(0), k0n = T(0);
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    Diff3<V> p1, p2; p1.init(); p2.init();       // in-plane (Kx My + Mx Ky) and Mx My of x, k, k x
+    V x0 = {}, x0n = {}, k0 = {}, k0n = {};
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T nx9[3][3], nk9[3][3], nz9[3][3];
+        V nx9[3][3], nk9[3][3], nz9[3][3];
         load9(G, c, comp, z, nx9);
         load9(G, c, kc, z, nk9);
 #pragma unroll
         for (int b = 0; b < 3; ++b)
 #pragma unroll
             for (int a = 0; a < 3; ++a) nz9[b][a] = nk9[b][a] * nx9[b][a];
-        const InPlane<T> rx = in_plane<T, false, true>(G, nx9), rk = in_plane<T, false, true>(G, nk9), rz = in_plane<T, false, true>(G, nz9);
+        const InPlane<V> rx = in_plane<T, false, true>(G, nx9), rk = in_plane<T, false, true>(G, nk9), rz = in_plane<T, false, true>(G, nz9);
         p1.add(rx.km + rx.mk, rk.km + rk.mk, rz.km + rz.mk);
         p2.add(rx.mm, rk.mm, rz.mm);
         x0 = x0n; x0n = nx9[1][1]; k0 = k0n; k0n = nk9[1][1];
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            const T Lx = zM(G, p1.f) + zK(G, p2.f), Lk = zM(G, p1.k) + zK(G, p2.k), Lz = zM(G, p1.z) + zK(G, p2.z);
-            const T diff = T(0.5) * (Lz + k0 * Lx - x0 * Lk);
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            const T Cc = C[c0];
-            const T rho = rho_l * Cc + rho_g * (T(1) - Cc);
-            const T s = rho * adv[c0] + diff;
-            const T t = qn[c0] - dt * s / rho;
-            qt[c0] = t;
-            if (qhn) qhn[c0] = T(0.5) * (qn[c0] + t);
+            const V Lx = zM(G, p1.f) + zK(G, p2.f), Lk = zM(G, p1.k) + zK(G, p2.k), Lz = zM(G, p1.z) + zK(G, p2.z);
+            const V diff = T(0.5) * (Lz + k0 * Lx - x0 * Lk);
+            const size_t c0 = at(c, q);
+            const V Cc = ldv<T, W>(C + c0);
+            const V rho = rho_l * Cc + rho_g * (T(1) - Cc);
+            const V s = rho * ldv<T, W>(adv + c0) + diff;
+            const V qv = ldv<T, W>(qn + c0);
+            const V t = qv - dt * s / rho;
+            stv(qt + c0, t);
+            if (qhn) stv(qhn + c0, T(0.5) * (qv + t));
         }
     }
 }
 
 // steps 3-10 of reading C9: directional diffusion coefficients k^x, k^y, k^z of the compressive scheme
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ u,
                                                           const T* __restrict__ v, const T* __restrict__ w,
                                                           const T* __restrict__ adv, T k_min, T k_max, T* __restrict__ kx,
                                                           T* __restrict__ ky, T* __restrict__ kz) {
-    const Col<T> c = make_col(G);
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
     const T Kp = T(300), Km = T(300);        // K+, K- 
     const T beta = T(0.1), eps_x = T(1e-4);  // Eq. 36
     const T Kcal = T(3);                     // Eq. 39
-    GradRoll<T> g; g.init();
-    T am[3] = {T(0), T(0), T(0)}, a0 = T(0), a0n = T(0);          // Mx My adv; adv at the centre of planes q, q + 1
-    T Cc[3] = {T(0), T(0), T(0)};                                 // C at the centre of planes q - 1, q, q + 1
-    T Sx = T(0), Sxn = T(0), Sy = T(0), Syn = T(0);               // Eq. 33 in-plane products of planes q, q + 1
+    GradRoll<T, V> g; g.init();
+    V am[3] = {}, a0 = {}, a0n = {};                              // Mx My adv; adv at the centre of planes q, q + 1
+    V Cc[3] = {};                                                 // C at the centre of planes q - 1, q, q + 1
+    V Sx = {}, Sxn = {}, Sy = {}, Syn = {};                       // Eq. 33 in-plane products of planes q, q + 1
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T n9[3][3];
+        V n9[3][3];
         load9(G, c, C, z, n9);
         g.add(in_plane<T, true, false>(G, n9));
         push(Cc, n9[1][1]);
@@ -253,26 +373,28 @@ __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, cons
         a0 = a0n; a0n = n9[1][1];
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            T Cx, Cy, Cz; g.grad(G, Cx, Cy, Cz);
-            const T a = T(2) * (zM(G, am) - a0);                                 // step 3, Eq. 29
-            const T kabs = k_abs_pg(G, a, Cx, Cy, Cz);                           // step 4, Eq. 27
-            const T C0 = Cc[1];
-            T S[3] = {Sx, Sy, (C0 - Cc[0]) * (Cc[2] - C0)};                      // step 5, Eq. 33
-            if (C0 > T(0.95) || C0 < T(0.05)) S[0] = S[1] = S[2] = T(-1);        // override
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            const T uu = u[c0], vv = v[c0], ww = w[c0];
-            const T g2 = Cx * Cx + Cy * Cy + Cz * Cz;
-            const T gq = (uu * Cx + vv * Cy + ww * Cz) / (eps_x + g2);           // step 7, Eq. 37
-            const T us = gq * Cx, vs = gq * Cy, ws = gq * Cz;
-            const T kneg = -beta * (uu * uu + vv * vv + ww * ww) /               // step 8, Eq. 36
-                           (eps_x + g2 * (fabs(us) + fabs(vs) + fabs(ws)) / T(3));
+            V Cx, Cy, Cz; g.grad(G, Cx, Cy, Cz);
+            const V a = T(2) * (zM(G, am) - a0);                                 // step 3, Eq. 29
+            const V kabs = k_abs_pk(G, a, Cx, Cy, Cz);                           // step 4, Eq. 27
+            const V C0 = Cc[1];
+            V S[3] = {Sx, Sy, (C0 - Cc[0]) * (Cc[2] - C0)};                      // step 5, Eq. 33
+#pragma unroll
+            for (int e = 0; e < W; ++e)
+                if (C0[e] > T(0.95) || C0[e] < T(0.05)) S[0][e] = S[1][e] = S[2][e] = T(-1);   // override
+            const size_t c0 = at(c, q);
+            const V uu = ldv<T, W>(u + c0), vv = ldv<T, W>(v + c0), ww = ldv<T, W>(w + c0);
+            const V g2 = Cx * Cx + Cy * Cy + Cz * Cz;
+            const V gq = (uu * Cx + vv * Cy + ww * Cz) / (eps_x + g2);           // step 7, Eq. 37
+            const V us = gq * Cx, vs = gq * Cy, ws = gq * Cz;
+            const V kneg = -beta * (uu * uu + vv * vv + ww * ww) /               // step 8, Eq. 36
+                           (eps_x + g2 * (pabs(us) + pabs(vs) + pabs(ws)) / T(3));
             T* const out[3] = {kx, ky, kz};
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                const T wp = -tmax(T(-1), tmin(T(0), Kp * S[d]));                // step 6, Eq. 35
-                const T wm = tmin(T(1), tmax(T(0), Km * S[d]));
-                const T kk = wp * (Kcal * kabs) + wm * (kneg / G.h[d]);          // steps 9, Eqs. 38-40
-                out[d][c0] = tmax(-k_min, tmin(k_max, kk));                      // step 10, Eq. 41
+                const V wp = -pmax(T(-1), pmin(T(0), Kp * S[d]));                // step 6, Eq. 35
+                const V wm = pmin(T(1), pmax(T(0), Km * S[d]));
+                const V kk = wp * (Kcal * kabs) + wm * (kneg / G.h[d]);          // steps 9, Eqs. 38-40
+                stv(out[d] + c0, pmax(-k_min, pmin(k_max, kk)));                 // step 10, Eq. 41
             }
         }
     }
@@ -281,21 +403,22 @@ __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, cons
 // steps 11-12: sC = adv + sum_d diff_d, diff_d = sum_{j != i} (-W^dd_ij) 1/2 (k^d_i + k^d_j)(C_i - C_j) (Eq. 12 collapsed,
 // P:146-151) evaluated as 1/2 (W^dd(k^d C) + k^d W^dd(C) - C W^dd(k^d)), W^xx = Kx My Mz, W^yy = Mx Ky Mz, W^zz = Mx My Kz;
 // Cnew = C - dt sC (Eq. 55)
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) vof_diffusion_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ adv,
                                                               const T* __restrict__ kx, const T* __restrict__ ky,
                                                               const T* __restrict__ kz, T dt, T* __restrict__ sC,
                                                               T* __restrict__ Cnew) {
-    const Col<T> c = make_col(G);
-    Diff3<T> dx, dy, dz; dx.init(); dy.init(); dz.init();     // in-plane Kx My / Mx Ky / Mx My of (C, k^d, k^d C)
-    T C0 = T(0), C0n = T(0), k0[3] = {T(0), T(0), T(0)}, k0n[3] = {T(0), T(0), T(0)};
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    Diff3<V> dx, dy, dz; dx.init(); dy.init(); dz.init();     // in-plane Kx My / Mx Ky / Mx My of (C, k^d, k^d C)
+    V C0 = {}, C0n = {}, k0[3] = {}, k0n[3] = {};
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T nc[3][3], nk[3][3], nz9[3][3];
+        V nc[3][3], nk[3][3], nz9[3][3];
         load9(G, c, C, z, nc);
-        const InPlane<T> rc = in_plane<T, false, true>(G, nc);
+        const InPlane<V> rc = in_plane<T, false, true>(G, nc);
         C0 = C0n; C0n = nc[1][1];
         const T* const kd[3] = {kx, ky, kz};
-        T pk[3], pz[3];
+        V pk[3], pz[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             load9(G, c, kd[d], z, nk);
@@ -307,36 +430,37 @@ __global__ void __launch_bounds__(MBX* MBY) vof_diffusion_march(const Geo<T> G, 
             if (d == 2) {
                 pk[d] = in_plane<T, false, false>(G, nk).mm; pz[d] = in_plane<T, false, false>(G, nz9).mm;
             } else {
-                const InPlane<T> rk = in_plane<T, false, true>(G, nk), rz = in_plane<T, false, true>(G, nz9);
+                const InPlane<V> rk = in_plane<T, false, true>(G, nk), rz = in_plane<T, false, true>(G, nz9);
                 pk[d] = d == 0 ? rk.km : rk.mk; pz[d] = d == 0 ? rz.km : rz.mk;
             }
         }
         dx.add(rc.km, pk[0], pz[0]); dy.add(rc.mk, pk[1], pz[1]); dz.add(rc.mm, pk[2], pz[2]);
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            const T ddx = T(0.5) * (zM(G, dx.z) + k0[0] * zM(G, dx.f) - C0 * zM(G, dx.k));
-            const T ddy = T(0.5) * (zM(G, dy.z) + k0[1] * zM(G, dy.f) - C0 * zM(G, dy.k));
-            const T ddz = T(0.5) * (zK(G, dz.z) + k0[2] * zK(G, dz.f) - C0 * zK(G, dz.k));
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            const T s = adv[c0] + ddx + ddy + ddz;
-            if (sC) sC[c0] = s;
-            if (Cnew) Cnew[c0] = C0 - dt * s;
+            const V ddx = T(0.5) * (zM(G, dx.z) + k0[0] * zM(G, dx.f) - C0 * zM(G, dx.k));
+            const V ddy = T(0.5) * (zM(G, dy.z) + k0[1] * zM(G, dy.f) - C0 * zM(G, dy.k));
+            const V ddz = T(0.5) * (zK(G, dz.z) + k0[2] * zK(G, dz.f) - C0 * zK(G, dz.k));
+            const size_t c0 = at(c, q);
+            const V s = ldv<T, W>(adv + c0) + ddx + ddy + ddz;
+            if (sC) stv(sC + c0, s);
+            if (Cnew) stv(Cnew + c0, C0 - dt * s);
         }
     }
 }
 
 // The paper's own stage-3 right-hand side, Eqs. 52-53: density on the right, constant-coefficient
 // Laplacian:  b = -(1/dt) sum_d f(rho q_d; w_d) + (1/dt) sum_d q_d f(rho; w_d),  rho = rho_l C + rho_g (1 - C)  (Eq. 2).
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ u,
                                                                    const T* __restrict__ v, const T* __restrict__ w, T rho_l, T rho_g,
                                                                    T inv_dt, T* __restrict__ bout) {
-    const Col<T> c = make_col(G);
-    T suv[3] = {T(0), T(0), T(0)}, aw[3] = {T(0), T(0), T(0)};      // in-plane Dx My (rho u) + Mx Dy (rho v); Mx My (rho w)
-    GradRoll<T> gr; gr.init();                                       // in-plane parts of grad rho
-    T q0[3] = {T(0), T(0), T(0)}, q0n[3] = {T(0), T(0), T(0)};       // u, v, w at the centre of planes q, q + 1
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    V suv[3] = {}, aw[3] = {};                                       // in-plane Dx My (rho u) + Mx Dy (rho v); Mx My (rho w)
+    GradRoll<T, V> gr; gr.init();                                    // in-plane parts of grad rho
+    V q0[3] = {}, q0n[3] = {};                                       // u, v, w at the centre of planes q, q + 1
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T r9[3][3], n9[3][3];
+        V r9[3][3], n9[3][3];
         load9(G, c, C, z, r9);
 #pragma unroll
         for (int b = 0; b < 3; ++b)
@@ -344,7 +468,7 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T
             for (int a = 0; a < 3; ++a) r9[b][a] = rho_l * r9[b][a] + rho_g * (T(1) - r9[b][a]);
         gr.add(in_plane<T, true, false>(G, r9));
         const T* const vel[3] = {u, v, w};
-        T part[3];
+        V part[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             load9(G, c, vel[d], z, n9);
@@ -352,70 +476,72 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T
 #pragma unroll
             for (int b = 0; b < 3; ++b)
 #pragma unroll
-                for (int a = 0; a < 3; ++a) n9[b][a] *= r9[b][a];
+                for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] * r9[b][a];
             if (d == 2) part[d] = in_plane<T, false, false>(G, n9).mm;
-            else { const InPlane<T> r = in_plane<T, true, false>(G, n9); part[d] = d == 0 ? r.dm : r.md; }
+            else { const InPlane<V> r = in_plane<T, true, false>(G, n9); part[d] = d == 0 ? r.dm : r.md; }
         }
         push(suv, part[0] + part[1]); push(aw, part[2]);
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            T gx, gy, gz; gr.grad(G, gx, gy, gz);
-            bout[c.nxy * q + c.row[1] + c.ix[1]] = (-(zM(G, suv) + zD(G, aw)) + (q0[0] * gx + q0[1] * gy + q0[2] * gz)) * inv_dt;
+            V gx, gy, gz; gr.grad(G, gx, gy, gz);
+            stv(bout + at(c, q), (-(zM(G, suv) + zD(G, aw)) + (q0[0] * gx + q0[1] * gy + q0[2] * gz)) * inv_dt);
         }
     }
 }
 
 // ---- stage 1, hydrostatic and surface-tension pressure (Eqs. 20-23, 44; readings in DESIGN.md) ----
 // n_t = grad C / (eps_t + |grad C|), eps_t = 1e-7 / hx  (Eq. 23)
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) normals_march(const Geo<T> G, const T* __restrict__ C, T* __restrict__ nx_, T* __restrict__ ny_,
                                                         T* __restrict__ nz_) {
-    const Col<T> c = make_col(G);
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
     const T eps_t = T(1e-7) / G.h[0];
-    GradRoll<T> g; g.init();
+    GradRoll<T, V> g; g.init();
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T n9[3][3];
+        V n9[3][3];
         load9(G, c, C, z, n9);
         g.add(in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            T gx, gy, gz; g.grad(G, gx, gy, gz);
-            const T inv = T(1) / (eps_t + sqrt(gx * gx + gy * gy + gz * gz));
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            nx_[c0] = gx * inv; ny_[c0] = gy * inv; nz_[c0] = gz * inv;
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const V inv = T(1) / (eps_t + psqrt(gx * gx + gy * gy + gz * gz));
+            const size_t c0 = at(c, q);
+            stv(nx_ + c0, gx * inv); stv(ny_ + c0, gy * inv); stv(nz_ + c0, gz * inv);
         }
     }
 }
 
 // kappa = -(f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z)) (Eqs. 5, 22; sign: reading N3);  s_t = sigma_t kappa grad C (Eq. 21);
 // (fu, fv, fw) = -s_t + (0, 0, g rho), whose FE divergence is the right-hand side of Eq. 43
-template <typename T>
+template <typename T, int W>
 __global__ void __launch_bounds__(MBX* MBY) surface_tension_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ nx_,
                                                                 const T* __restrict__ ny_, const T* __restrict__ nz_, T rho_l, T rho_g,
                                                                 T grav, T sigma_t, T* __restrict__ fu, T* __restrict__ fv,
                                                                 T* __restrict__ fw, T* __restrict__ kappa) {
-    const Col<T> c = make_col(G);
-    GradRoll<T> g; g.init();
-    T sxy[3] = {T(0), T(0), T(0)}, am[3] = {T(0), T(0), T(0)};    // in-plane Dx My n_x + Mx Dy n_y;  Mx My n_z
-    T C0 = T(0), C0n = T(0);
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    GradRoll<T, V> g; g.init();
+    V sxy[3] = {}, am[3] = {};                                    // in-plane Dx My n_x + Mx Dy n_y;  Mx My n_z
+    V C0 = {}, C0n = {};
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
-        T n9[3][3];
+        V n9[3][3];
         load9(G, c, C, z, n9);
         g.add(in_plane<T, true, false>(G, n9));
         C0 = C0n; C0n = n9[1][1];
-        load9(G, c, nx_, z, n9); const T dx = in_plane<T, true, false>(G, n9).dm;
-        load9(G, c, ny_, z, n9); const T dy = in_plane<T, true, false>(G, n9).md;
-        load9(G, c, nz_, z, n9); const T mz = in_plane<T, false, false>(G, n9).mm;
+        load9(G, c, nx_, z, n9); const V dx = in_plane<T, true, false>(G, n9).dm;
+        load9(G, c, ny_, z, n9); const V dy = in_plane<T, true, false>(G, n9).md;
+        load9(G, c, nz_, z, n9); const V mz = in_plane<T, false, false>(G, n9).mm;
         push(sxy, dx + dy); push(am, mz);
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            T gx, gy, gz; g.grad(G, gx, gy, gz);
-            const T kap = -(zM(G, sxy) + zD(G, am));
-            const size_t c0 = c.nxy * q + c.row[1] + c.ix[1];
-            const T sk = -sigma_t * kap;                        // -s_t = sk grad C
-            fu[c0] = sk * gx; fv[c0] = sk * gy;
-            fw[c0] = sk * gz + grav * (rho_l * C0 + rho_g * (T(1) - C0));
-            if (kappa) kappa[c0] = kap;
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const V kap = -(zM(G, sxy) + zD(G, am));
+            const size_t c0 = at(c, q);
+            const V sk = -sigma_t * kap;                        // -s_t = sk grad C
+            stv(fu + c0, sk * gx); stv(fv + c0, sk * gy);
+            stv(fw + c0, sk * gz + grav * (rho_l * C0 + rho_g * (T(1) - C0)));
+            if (kappa) stv(kappa + c0, kap);
         }
     }
 }
