@@ -173,10 +173,18 @@ __device__ __forceinline__ InPlane<V> in_plane(const Geo<T>& G, const V (&v)[3][
     return r;
 }
 
-// z factors over a rolling triple a[0] = plane q - 1, a[1] = plane q, a[2] = plane q + 1
-template <typename T, typename V> __device__ __forceinline__ V zM(const Geo<T>& G, const V (&a)[3]) { return G.M[0] * (a[0] + a[2]) + G.M[1] * a[1]; }
-template <typename T, typename V> __device__ __forceinline__ V zD(const Geo<T>& G, const V (&a)[3]) { return G.D[2][2] * (a[2] - a[0]); }
-template <typename T, typename V> __device__ __forceinline__ V zK(const Geo<T>& G, const V (&a)[3]) { return G.K[2][0] * ((a[0] + a[2]) - T(2) * a[1]); }
+// z factor applied on arrival: plane z of an in-plane result contributes `up` to the output of plane z - 1, `mid` to plane z
+// and `dn` to plane z + 1; step() takes the three and returns the finished output of plane z - 1.  Two running sums per
+// filtered quantity instead of three stored planes (and no register shuffling per plane).
+template <typename V>
+struct ZAcc {
+    V A, B;       // partial outputs of planes z - 1 and z before plane z has arrived
+    __device__ __forceinline__ void init() { A = V{}; B = V{}; }
+    __device__ __forceinline__ V step(const V& up, const V& mid, const V& dn) { const V done = A + up; A = B + mid; B = dn; return done; }
+    template <typename T> __device__ __forceinline__ V stepM(const Geo<T>& G, const V& v) { const V t = G.M[0] * v; return step(t, G.M[1] * v, t); }   // Mz
+    template <typename T> __device__ __forceinline__ V stepK(const Geo<T>& G, const V& v) { const V t = G.K[2][0] * v; return step(t, G.K[2][1] * v, t); }   // Kz
+    template <typename T> __device__ __forceinline__ V stepD(const Geo<T>& G, const V& v) { const V t = G.D[2][2] * v; const V done = A + t; A = B; B = -t; return done; }   // Dz
+};
 template <typename V> __device__ __forceinline__ void push(V (&a)[3], const V& v) { a[0] = a[1]; a[1] = a[2]; a[2] = v; }
 
 // b = -(1/dt) (f(u; w_x) + f(v; w_y) + f(w; w_z))  (reading C10; Eq. 53 structure)
@@ -185,25 +193,27 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_march(const Geo<T> G, c
                                                              const T* __restrict__ w, T inv_dt, T* __restrict__ bout) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
-    V suv[3] = {}, aw[3] = {};
+    ZAcc<V> acc; acc.init();       // Mz (Dx My u + Mx Dy v) + Dz (Mx My w)
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, u, z, n9); const V du = in_plane<T, true, false>(G, n9).dm;
         load9(G, c, v, z, n9); const V dv = in_plane<T, true, false>(G, n9).md;
         load9(G, c, w, z, n9); const V mw = in_plane<T, false, false>(G, n9).mm;
-        push(suv, du + dv); push(aw, mw);
+        const V ms = G.M[0] * (du + dv), dw = G.D[2][2] * mw;
+        const V div = acc.step(ms + dw, G.M[1] * (du + dv), ms - dw);
         const int q = z - 1;
-        if (q >= c.z0 && c.ok) stv(bout + at(c, q), -(zM(G, suv) + zD(G, aw)) * inv_dt);
+        if (q >= c.z0 && c.ok) stv(bout + at(c, q), -div * inv_dt);
     }
 }
 
 // gradient by the FE first-derivative filters from rolling in-plane results
 template <typename T, typename V>
 struct GradRoll {
-    V ax[3], ay[3], am[3];
-    __device__ __forceinline__ void init() { for (int e = 0; e < 3; ++e) ax[e] = ay[e] = am[e] = V{}; }
-    __device__ __forceinline__ void add(const InPlane<V>& r) { push(ax, r.dm); push(ay, r.md); push(am, r.mm); }
-    __device__ __forceinline__ void grad(const Geo<T>& G, V& gx, V& gy, V& gz) const { gx = zM(G, ax); gy = zM(G, ay); gz = zD(G, am); }
+    ZAcc<V> ax, ay, az;
+    V gx, gy, gz;       // gradient at plane z - 1 after add() of plane z
+    __device__ __forceinline__ void init() { ax.init(); ay.init(); az.init(); }
+    __device__ __forceinline__ void add(const Geo<T>& G, const InPlane<V>& r) { gx = ax.stepM(G, r.dm); gy = ay.stepM(G, r.md); gz = az.stepD(G, r.mm); }
+    __device__ __forceinline__ void grad(const Geo<T>&, V& ox, V& oy, V& oz) const { ox = gx; oy = gy; oz = gz; }
 };
 
 // q <- q - dt k f(p; w_x|y|z) (Eq. 54); halo of p = s * mirror with the solver's factors
@@ -226,7 +236,7 @@ __global__ void __launch_bounds__(MBX* MBY) project_march(const Geo<T> G, const 
 #pragma unroll
             for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] * (fz * fy[b]);
         }
-        g.add(in_plane<T, true, false>(G, n9));
+        g.add(G, in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             V gx, gy, gz; g.grad(G, gx, gy, gz);
@@ -247,7 +257,7 @@ __global__ void __launch_bounds__(MBX* MBY) advection_march(const Geo<T> G, cons
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, psi, z, n9);
-        g.add(in_plane<T, true, false>(G, n9));
+        g.add(G, in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             V gx, gy, gz; g.grad(G, gx, gy, gz);
@@ -276,18 +286,19 @@ __global__ void __launch_bounds__(MBX* MBY) mom_coeff_march(const Geo<T> G, cons
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
     GradRoll<T, V> g; g.init();
-    V am[3] = {}, a0 = {}, a0n = {};     // Mx My adv of three planes; adv at the centre of planes q, q + 1
+    ZAcc<V> am; am.init();               // Mz of Mx My adv
+    V a0 = {}, a0n = {};                 // adv at the centre of planes q, q + 1
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, comp, z, n9);
-        g.add(in_plane<T, true, false>(G, n9));
+        g.add(G, in_plane<T, true, false>(G, n9));
         load9(G, c, adv, z, n9);
-        push(am, in_plane<T, false, false>(G, n9).mm);
+        const V madv = am.stepM(G, in_plane<T, false, false>(G, n9).mm);
         a0 = a0n; a0n = n9[1][1];
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             V px, py, pz; g.grad(G, px, py, pz);
-            const V a = T(2) * (zM(G, am) - a0);
+            const V a = T(2) * (madv - a0);
             const size_t c0 = at(c, q);
             const V Cc = ldv<T, W>(C + c0);
             const V rho = rho_l * Cc + rho_g * (T(1) - Cc);
@@ -302,9 +313,8 @@ __global__ void __launch_bounds__(MBX* MBY) mom_coeff_march(const Geo<T> G, cons
 //   sum_j (-W_ij) 1/2 (k_i + k_j)(f_i - f_j) = 1/2 (W(k f) + k W(f) - f W(k))      [sum_j W_ij = 0]
 template <typename V>
 struct Diff3 {
-    V f[3], k[3], z[3];
-    __device__ __forceinline__ void init() { for (int e = 0; e < 3; ++e) f[e] = k[e] = z[e] = V{}; }
-    __device__ __forceinline__ void add(const V& pf, const V& pk, const V& pz) { push(f, pf); push(k, pk); push(z, pz); }
+    ZAcc<V> f, k, z;
+    __device__ __forceinline__ void init() { f.init(); k.init(); z.init(); }
 };
 
 // s = rho adv + f^lap(c, k_c; w_lap) (Eq. 18 without pressure / source terms), q~ = q_n - dt s / rho (Eq. 45, sigma = 0),
@@ -316,7 +326,7 @@ __global__ void __launch_bounds__(MBX* MBY) mom_update_march(const Geo<T> G, con
                                                            T* __restrict__ qhn) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
-    Diff3<V> p1, p2; p1.init(); p2.init();       // in-plane (Kx My + Mx Ky) and Mx My of x, k, k x
+    Diff3<V> L; L.init();                        // w_lap of x, k, k x: Mz of the in-plane (Kx My + Mx Ky) + Kz of the in-plane Mx My
     V x0 = {}, x0n = {}, k0 = {}, k0n = {};
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V nx9[3][3], nk9[3][3], nz9[3][3];
@@ -327,12 +337,14 @@ __global__ void __launch_bounds__(MBX* MBY) mom_update_march(const Geo<T> G, con
 #pragma unroll
             for (int a = 0; a < 3; ++a) nz9[b][a] = nk9[b][a] * nx9[b][a];
         const InPlane<V> rx = in_plane<T, false, true>(G, nx9), rk = in_plane<T, false, true>(G, nk9), rz = in_plane<T, false, true>(G, nz9);
-        p1.add(rx.km + rx.mk, rk.km + rk.mk, rz.km + rz.mk);
-        p2.add(rx.mm, rk.mm, rz.mm);
+        auto lap = [&](ZAcc<V>& a, const InPlane<V>& r) {
+            const V p1 = r.km + r.mk, t = G.M[0] * p1 + G.K[2][0] * r.mm;
+            return a.step(t, G.M[1] * p1 + G.K[2][1] * r.mm, t);
+        };
+        const V Lx = lap(L.f, rx), Lk = lap(L.k, rk), Lz = lap(L.z, rz);
         x0 = x0n; x0n = nx9[1][1]; k0 = k0n; k0n = nk9[1][1];
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            const V Lx = zM(G, p1.f) + zK(G, p2.f), Lk = zM(G, p1.k) + zK(G, p2.k), Lz = zM(G, p1.z) + zK(G, p2.z);
             const V diff = T(0.5) * (Lz + k0 * Lx - x0 * Lk);
             const size_t c0 = at(c, q);
             const V Cc = ldv<T, W>(C + c0);
@@ -357,24 +369,26 @@ __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, cons
     const T Kp = T(300), Km = T(300);        // K+, K- 
     const T beta = T(0.1), eps_x = T(1e-4);  // Eq. 36
     const T Kcal = T(3);                     // Eq. 39
+    const T ih[3] = {T(1) / G.h[0], T(1) / G.h[1], T(1) / G.h[2]};
     GradRoll<T, V> g; g.init();
-    V am[3] = {}, a0 = {}, a0n = {};                              // Mx My adv; adv at the centre of planes q, q + 1
+    ZAcc<V> am; am.init();                                        // Mz of Mx My adv
+    V a0 = {}, a0n = {};                                          // adv at the centre of planes q, q + 1
     V Cc[3] = {};                                                 // C at the centre of planes q - 1, q, q + 1
     V Sx = {}, Sxn = {}, Sy = {}, Syn = {};                       // Eq. 33 in-plane products of planes q, q + 1
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, C, z, n9);
-        g.add(in_plane<T, true, false>(G, n9));
+        g.add(G, in_plane<T, true, false>(G, n9));
         push(Cc, n9[1][1]);
         Sx = Sxn; Sxn = (n9[1][1] - n9[1][0]) * (n9[1][2] - n9[1][1]);
         Sy = Syn; Syn = (n9[1][1] - n9[0][1]) * (n9[2][1] - n9[1][1]);
         load9(G, c, adv, z, n9);
-        push(am, in_plane<T, false, false>(G, n9).mm);
+        const V madv = am.stepM(G, in_plane<T, false, false>(G, n9).mm);
         a0 = a0n; a0n = n9[1][1];
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             V Cx, Cy, Cz; g.grad(G, Cx, Cy, Cz);
-            const V a = T(2) * (zM(G, am) - a0);                                 // step 3, Eq. 29
+            const V a = T(2) * (madv - a0);                                      // step 3, Eq. 29
             const V kabs = k_abs_pk(G, a, Cx, Cy, Cz);                           // step 4, Eq. 27
             const V C0 = Cc[1];
             V S[3] = {Sx, Sy, (C0 - Cc[0]) * (Cc[2] - C0)};                      // step 5, Eq. 33
@@ -387,13 +401,13 @@ __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, cons
             const V gq = (uu * Cx + vv * Cy + ww * Cz) / (eps_x + g2);           // step 7, Eq. 37
             const V us = gq * Cx, vs = gq * Cy, ws = gq * Cz;
             const V kneg = -beta * (uu * uu + vv * vv + ww * ww) /               // step 8, Eq. 36
-                           (eps_x + g2 * (pabs(us) + pabs(vs) + pabs(ws)) / T(3));
+                           (eps_x + g2 * (pabs(us) + pabs(vs) + pabs(ws)) * T(1.0 / 3.0));
             T* const out[3] = {kx, ky, kz};
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const V wp = -pmax(T(-1), pmin(T(0), Kp * S[d]));                // step 6, Eq. 35
                 const V wm = pmin(T(1), pmax(T(0), Km * S[d]));
-                const V kk = wp * (Kcal * kabs) + wm * (kneg / G.h[d]);          // steps 9, Eqs. 38-40
+                const V kk = wp * (Kcal * kabs) + wm * (kneg * ih[d]);           // steps 9, Eqs. 38-40
                 stv(out[d] + c0, pmax(-k_min, pmin(k_max, kk)));                 // step 10, Eq. 41
             }
         }
@@ -434,12 +448,14 @@ __global__ void __launch_bounds__(MBX* MBY) vof_diffusion_march(const Geo<T> G, 
                 pk[d] = d == 0 ? rk.km : rk.mk; pz[d] = d == 0 ? rz.km : rz.mk;
             }
         }
-        dx.add(rc.km, pk[0], pz[0]); dy.add(rc.mk, pk[1], pz[1]); dz.add(rc.mm, pk[2], pz[2]);
+        const V xf = dx.f.stepM(G, rc.km), xk = dx.k.stepM(G, pk[0]), xz = dx.z.stepM(G, pz[0]);
+        const V yf = dy.f.stepM(G, rc.mk), yk = dy.k.stepM(G, pk[1]), yz = dy.z.stepM(G, pz[1]);
+        const V zf = dz.f.stepK(G, rc.mm), zk = dz.k.stepK(G, pk[2]), zz = dz.z.stepK(G, pz[2]);
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
-            const V ddx = T(0.5) * (zM(G, dx.z) + k0[0] * zM(G, dx.f) - C0 * zM(G, dx.k));
-            const V ddy = T(0.5) * (zM(G, dy.z) + k0[1] * zM(G, dy.f) - C0 * zM(G, dy.k));
-            const V ddz = T(0.5) * (zK(G, dz.z) + k0[2] * zK(G, dz.f) - C0 * zK(G, dz.k));
+            const V ddx = T(0.5) * (xz + k0[0] * xf - C0 * xk);
+            const V ddy = T(0.5) * (yz + k0[1] * yf - C0 * yk);
+            const V ddz = T(0.5) * (zz + k0[2] * zf - C0 * zk);
             const size_t c0 = at(c, q);
             const V s = ldv<T, W>(adv + c0) + ddx + ddy + ddz;
             if (sC) stv(sC + c0, s);
@@ -456,7 +472,7 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T
                                                                    T inv_dt, T* __restrict__ bout) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
-    V suv[3] = {}, aw[3] = {};                                       // in-plane Dx My (rho u) + Mx Dy (rho v); Mx My (rho w)
+    ZAcc<V> acc; acc.init();                                         // Mz (Dx My (rho u) + Mx Dy (rho v)) + Dz (Mx My (rho w))
     GradRoll<T, V> gr; gr.init();                                    // in-plane parts of grad rho
     V q0[3] = {}, q0n[3] = {};                                       // u, v, w at the centre of planes q, q + 1
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
@@ -466,7 +482,7 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T
         for (int b = 0; b < 3; ++b)
 #pragma unroll
             for (int a = 0; a < 3; ++a) r9[b][a] = rho_l * r9[b][a] + rho_g * (T(1) - r9[b][a]);
-        gr.add(in_plane<T, true, false>(G, r9));
+        gr.add(G, in_plane<T, true, false>(G, r9));
         const T* const vel[3] = {u, v, w};
         V part[3];
 #pragma unroll
@@ -480,11 +496,12 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T
             if (d == 2) part[d] = in_plane<T, false, false>(G, n9).mm;
             else { const InPlane<V> r = in_plane<T, true, false>(G, n9); part[d] = d == 0 ? r.dm : r.md; }
         }
-        push(suv, part[0] + part[1]); push(aw, part[2]);
+        const V ms = G.M[0] * (part[0] + part[1]), dw = G.D[2][2] * part[2];
+        const V div = acc.step(ms + dw, G.M[1] * (part[0] + part[1]), ms - dw);
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             V gx, gy, gz; gr.grad(G, gx, gy, gz);
-            stv(bout + at(c, q), (-(zM(G, suv) + zD(G, aw)) + (q0[0] * gx + q0[1] * gy + q0[2] * gz)) * inv_dt);
+            stv(bout + at(c, q), (-div + (q0[0] * gx + q0[1] * gy + q0[2] * gz)) * inv_dt);
         }
     }
 }
@@ -501,7 +518,7 @@ __global__ void __launch_bounds__(MBX* MBY) normals_march(const Geo<T> G, const 
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, C, z, n9);
-        g.add(in_plane<T, true, false>(G, n9));
+        g.add(G, in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             V gx, gy, gz; g.grad(G, gx, gy, gz);
@@ -522,21 +539,22 @@ __global__ void __launch_bounds__(MBX* MBY) surface_tension_march(const Geo<T> G
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
     GradRoll<T, V> g; g.init();
-    V sxy[3] = {}, am[3] = {};                                    // in-plane Dx My n_x + Mx Dy n_y;  Mx My n_z
+    ZAcc<V> acc; acc.init();                                      // Mz (Dx My n_x + Mx Dy n_y) + Dz (Mx My n_z)
     V C0 = {}, C0n = {};
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, C, z, n9);
-        g.add(in_plane<T, true, false>(G, n9));
+        g.add(G, in_plane<T, true, false>(G, n9));
         C0 = C0n; C0n = n9[1][1];
         load9(G, c, nx_, z, n9); const V dx = in_plane<T, true, false>(G, n9).dm;
         load9(G, c, ny_, z, n9); const V dy = in_plane<T, true, false>(G, n9).md;
         load9(G, c, nz_, z, n9); const V mz = in_plane<T, false, false>(G, n9).mm;
-        push(sxy, dx + dy); push(am, mz);
+        const V ms = G.M[0] * (dx + dy), dn = G.D[2][2] * mz;
+        const V divn = acc.step(ms + dn, G.M[1] * (dx + dy), ms - dn);
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
             V gx, gy, gz; g.grad(G, gx, gy, gz);
-            const V kap = -(zM(G, sxy) + zD(G, am));
+            const V kap = -divn;
             const size_t c0 = at(c, q);
             const V sk = -sigma_t * kap;                        // -s_t = sk grad C
             stv(fu + c0, sk * gx); stv(fv + c0, sk * gy);
