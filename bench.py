@@ -36,8 +36,8 @@ UNIT = "V-cycles/s"
 E2E_CYCLES = 20          # the paper's fixed cycle count per pressure solve
 REF_TIME_BUDGET_S = 150  # wall-clock cap of the oracle arm
 # dram__bytes_read.sum + dram__bytes_write.sum of one fine-level smoother launch, from the ncu --set full
-# capture summarised in profiles/ (bytes per launch); None until a capture of the current kernel exists
-TRAFFIC_NCU = 250.7e6
+# capture summarised in profiles/r01_ncu_lean.md (bytes per launch); None until a capture of the current kernel exists
+TRAFFIC_NCU = 252.9e6
 
 
 def load_peaks():
