@@ -166,6 +166,13 @@ int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, voi
                    double rho_g, double mu_l, double mu_g, double dt, double tol, int max_cycles,
                    int* cycles_out, double* relres_out);
 
+/* The same time step with the pressure equation solved by mg_pcg_solve(tol, max_iter) from a zero guess (SURVEY 8(f) "next 1":
+ * V-cycle-preconditioned CG, not in the paper, whose plain cycles converge at 0.95 per cycle under the 1000:1 density jump);
+ * needs nu_pre == nu_post >= 1 and a uniform grid with nx % 4 == 0 like mg_pcg_solve.  Everything else as flow_time_step. */
+int flow_time_step_pcg(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l,
+                       double rho_g, double mu_l, double mu_g, double dt, double tol, int max_iter,
+                       int* iters_out, double* relres_out);
+
 /* The same time step with the PAPER'S stage 3 (SURVEY 8(f) "next 2"): constant-coefficient Laplacian with the density on the
  * right (Eqs. 52-53), `cycles` V-cycles per solve from a zero guess (the paper's fixed 20), velocity correction Eq. 54,
  * the stage carried out `passes` times (twice).  d_p receives the accumulated p_nh; the solver's coefficient is reset

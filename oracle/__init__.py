@@ -233,21 +233,25 @@ def project_velocity(g, bc, p, k, dt, u, v, w):
 
 
 def time_step(g, bc, Cf, u, v, w, levels, rho_l, rho_g, mu_l, mu_g, dt, tol, max_cycles,
-              nu_pre=2, nu_post=2, coarse_sweeps=50, omega=2.0 / 3.0):
+              nu_pre=2, nu_post=2, coarse_sweeps=50, omega=2.0 / 3.0, solver="mg"):
     """One time step of BASELINE config 5, stages 2-4 of PAPER.md:403-505 under the readings
     C9/C10 of DESIGN.md, composed from the oracle's own steps:
       stage 2: q_half = q_n; two predictor iterations (Eqs. 45-46)
       stage 3: k = 1/rho(C_n); b = -(1/dt) D.q~; solve A(k) p = b from p = 0; q = q~ - dt k G p
                (Eqs. 48, 52-54, PAPER.md:455-492)
       stage 4: C_new = C_n - dt s~_C(C_n, q) (Eqs. 16, 55)
+    solver = "mg": plain V-cycles (the paper); "pcg": pcg_solve (nu_pre == nu_post).
     Returns (C_new, u, v, w, p, cycles, relres)."""
     qn = (u, v, w)
     qt, qh = mom_predictor(g, Cf, qn, qn, rho_l, rho_g, mu_l, mu_g, dt)
     qt, _ = mom_predictor(g, Cf, qh, qn, rho_l, rho_g, mu_l, mu_g, dt)
     k = k_from_vof(Cf, rho_l, rho_g)
     b = pressure_rhs(g, qt[0], qt[1], qt[2], dt)
-    p, cycles, rel, _ = solve(g, bc, k, np.zeros(g.shape), b, levels, tol, max_cycles, nu_pre, nu_post,
-                              coarse_sweeps, omega)
+    if solver == "pcg":
+        p, cycles, rel, _ = pcg_solve(g, bc, k, np.zeros(g.shape), b, levels, tol, max_cycles, nu_pre, coarse_sweeps, omega)
+    else:
+        p, cycles, rel, _ = solve(g, bc, k, np.zeros(g.shape), b, levels, tol, max_cycles, nu_pre, nu_post,
+                                  coarse_sweeps, omega)
     un, vn, wn = project_velocity(g, bc, p, k, dt, qt[0], qt[1], qt[2])
     _, Cn = vof_residual(g, Cf, un, vn, wn, dt)
     return Cn, un, vn, wn, p, cycles, rel

@@ -23,7 +23,7 @@ EXPORTS = [
     "mg_create", "mg_destroy", "mg_set_params", "mg_get_params", "mg_set_coefficient",
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
-    "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_paper", "mg_last_error",
+    "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_pcg", "flow_time_step_paper", "mg_last_error",
     "mg_version",
 ]
 
@@ -82,6 +82,7 @@ def _load():
     lib.hydrostatic_rhs.argtypes = [C.POINTER(MgGrid), i, vp, d, d, d, d, vp, vp, vp]
     lib.project_velocity.argtypes = [C.POINTER(MgGrid), pi, i, vp, vp, d, vp, vp, vp, vp]
     lib.flow_time_step.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, i, pi, pd]
+    lib.flow_time_step_pcg.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, i, pi, pd]
     lib.mg_last_error.restype = C.c_char_p
     lib.mg_version.restype = C.c_char_p
     return lib
@@ -336,6 +337,16 @@ def project_velocity(p, k, h, bc, dt, u, v, w, stream=None):
     bcarr = (C.c_int * 6)(*[int(b) for b in bc])
     return _check(_lib.project_velocity(C.byref(g), bcarr, _dtype_code(p), _dev(p), _dev(k, sh, dt_), float(dt),
                                         _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_), _stream_ptr(stream)))
+
+
+def flow_time_step_pcg(s, C_, u, v, w, p, rho_l, rho_g, mu_l, mu_g, dt, tol, max_iter):
+    """Returns (status, iterations, relres)."""
+    its, rel = C.c_int(0), C.c_double(0.0)
+    sh, dt_ = s.shape, s.torch_dtype
+    st = _check(_lib.flow_time_step_pcg(s.handle, _dev(C_, sh, dt_), _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_),
+                                        _dev(p, sh, dt_), float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt),
+                                        float(tol), int(max_iter), C.byref(its), C.byref(rel)))
+    return st, its.value, rel.value
 
 
 def flow_time_step(s, C_, u, v, w, p, rho_l, rho_g, mu_l, mu_g, dt, tol, max_cycles):

@@ -301,8 +301,8 @@ int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void
 //   stage 2: q_half = q_n; twice: (q~, q_half) = predictor(C_n; q_half, q_n)        (Eqs. 45-46, two iterations P:443)
 //   stage 3: k = 1/rho(C_n); b = -(1/dt) D.q~; solve A(k) p = b from p = 0; q = q~ - dt k G p   (Eqs. 48, 52-54)
 //   stage 4: C <- C - dt s~_C(C_n, q)                                              (Eqs. 16, 55)
-int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l, double rho_g, double mu_l,
-                   double mu_g, double dt, double tol, int max_cycles, int* cycles_out, double* relres_out) {
+static int time_step_impl(mg_solver* s, bool pcg, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l, double rho_g,
+                          double mu_l, double mu_g, double dt, double tol, int max_cycles, int* cycles_out, double* relres_out) {
     if (!s || !d_C || !d_u || !d_v || !d_w || !d_p) { set_error("flow_time_step: NULL argument"); return MG_EINVAL; }
     int prev = -1;
     cudaGetDevice(&prev);
@@ -324,7 +324,8 @@ int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, voi
         int status = 0;
         if (!rc) {
             rc = cudaMemsetAsync(d_p, 0, bytes, st) == cudaSuccess ? 0 : MG_ECUDA;
-            if (!rc) status = mg_solve(s, d_p, bbuf, tol, max_cycles, cycles_out, relres_out);
+            if (!rc) status = pcg ? mg_pcg_solve(s, d_p, bbuf, tol, max_cycles, cycles_out, relres_out)
+                                  : mg_solve(s, d_p, bbuf, tol, max_cycles, cycles_out, relres_out);
             if (status < 0) rc = status;
         }
         if (!rc) rc = project_velocity(&s->grid, s->bc, s->dtype, d_p, s->lv[0].k, dt, qt[0], qt[1], qt[2], st);
@@ -341,6 +342,17 @@ int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, voi
     }
     if (prev >= 0) cudaSetDevice(prev);
     return rc;
+}
+
+int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l, double rho_g, double mu_l,
+                   double mu_g, double dt, double tol, int max_cycles, int* cycles_out, double* relres_out) {
+    return time_step_impl(s, false, d_C, d_u, d_v, d_w, d_p, rho_l, rho_g, mu_l, mu_g, dt, tol, max_cycles, cycles_out, relres_out);
+}
+
+// The same step with the pressure solved by V-cycle-preconditioned CG (oracle time_step(solver="pcg"))
+int flow_time_step_pcg(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l, double rho_g, double mu_l,
+                       double mu_g, double dt, double tol, int max_iter, int* iters_out, double* relres_out) {
+    return time_step_impl(s, true, d_C, d_u, d_v, d_w, d_p, rho_l, rho_g, mu_l, mu_g, dt, tol, max_iter, iters_out, relres_out);
 }
 
 // Time step with the PAPER'S stage 3 (oracle time_step_paper): constant-coefficient Laplacian, density on the

@@ -123,6 +123,30 @@ def test_time_step_parity(mg, orc, dt):
     mg.mg_destroy(s)
 
 
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_time_step_pcg_parity(mg, orc, dt):
+    """Config 5 at 32^3 with the pressure solved by V-cycle-preconditioned CG (flow_time_step_pcg): two steps."""
+    import torch
+    n, levels = 32, 4
+    w = configs.config5(n, levels)
+    g = orc.grid(n, n, n, w.h)
+    Cf, u, v, ww = (quantise(w.fields[q], dt) for q in ("alpha", "u", "v", "w"))
+    s = mg.mg_create((n, n, n, w.h), levels, w.bc, mg.MG_F32 if dt == "f32" else mg.MG_F64)
+    dC, du, dv, dw = (to_dev(a, dt) for a in (Cf, u, v, ww))
+    dp = torch.empty_like(dC)
+    tol = 1e-9
+    for step in range(2):
+        Cf, u, v, ww, p, it_o, rel_o = orc.time_step(g, w.bc, Cf, u, v, ww, levels, w.rho_l, w.rho_g, w.mu_l, w.mu_g,
+                                                     w.dt, tol, 200, solver="pcg")
+        status, its, rel = mg.flow_time_step_pcg(s, dC, du, dv, dw, dp, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, tol, 200)
+        assert status == mg.MG_OK and rel < tol and abs(its - it_o) <= 2
+        lim = (step + 1) * (2e-5 if dt == "f32" else 1e-7)
+        assert rel_l2(as_f64(dp), p) <= lim * 5
+        for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
+            assert rel_l2(as_f64(a), r) <= lim
+    mg.mg_destroy(s)
+
+
 # ---------------------------------------------------------------- SURVEY 8(f) next 2: the paper's own stage 3
 @pytest.mark.parametrize("dt", ["f32", "f64"])
 @pytest.mark.parametrize("shape,h", [((24, 24, 24), 1.0 / 24), ((10, 36, 68), (0.02, 0.025, 0.03))])
