@@ -206,6 +206,32 @@ def main():
     x = torch.zeros_like(C); b = torch.randn_like(C)
     msc, _ = timed(lambda: mg.mg_vcycle(s, x, b), 200)
     print("\none constant-coefficient V-cycle (12 B per point update): %.1f us = %.0f V-cycles/s" % (msc * 1e3, 1e3 / msc))
+
+    # Eq. 56: wall time per step and node = M_s + N_I N_nh H_s (no hydrostatic solve in this step: N_h = 0)
+    print("\n### The paper's cost model, Eq. 56, fitted on this GPU (strategies i-j of Fig. 18, P:668: i corrections x j multigrid "
+          "iterations)\n")
+    print("| multigrid iteration | 1-10 ms | 2-10 ms | 1-20 ms | 2-20 ms | M_s s/node/step | H_s s/node/iteration | worst fit error |\n|---|---|---|---|---|---|---|---|")
+    nn = float(C.numel())
+    for label, nu, mp in (("V(2,2) + fp64 defect per iteration (the default here)", 2, 1), ("V(1,1), fp32 residual norm per iteration", 1, 0)):
+        mg.mg_set_params(s, nu_pre=nu, nu_post=nu, coarse_sweeps=50, sweeps_per_pass=1, omega=w.omega, mixed_precision=mp)
+        pts = []
+        for i, j in ((1, 10), (2, 10), (1, 20), (2, 20)):
+            tot = 0.0
+            for it in range(4):
+                for dst, src in zip((C, u, v, ww), init):
+                    dst.copy_(src)
+                e0.record()
+                mg.flow_time_step_paper(s, C, u, v, ww, p, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, j, i)
+                e1.record(); torch.cuda.synchronize()
+                if it >= 1:
+                    tot += e0.elapsed_time(e1)
+            pts.append((i * j, tot / 3))
+        A = np.array([[1.0, q] for q, _ in pts]); y = np.array([t for _, t in pts])
+        (a0, a1), *_ = np.linalg.lstsq(A, y, rcond=None)
+        err = float(np.max(np.abs(A @ np.array([a0, a1]) - y) / y))
+        print("| %s | %s | %.2e | %.2e | %.1f %% |" % (label, " | ".join("%.2f" % t for _, t in pts), a0 * 1e-3 / nn, a1 * 1e-3 / nn, 100 * err))
+    print("\nThe paper's fit on an NVIDIA A10 (P:515): M_s = 1.2e-8, H_s = 1.1e-10 s per node; its multigrid iteration is a saw-tooth cycle "
+          "whose sweep counts are not given (BASELINE.md), so H_s compares only in order of magnitude.")
     mg.mg_destroy(s)
 
 
