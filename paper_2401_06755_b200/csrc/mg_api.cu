@@ -429,7 +429,9 @@ int mg_set_fused(mg_solver* s, int fused) {
 
 int mg_set_coefficient(mg_solver* s, const void* d_k) {
     CHECK_SOLVER(s);
-    invalidate_graph(s);
+    // the recorded cycle holds pointers and sizes, not coefficient values: it stays valid while the solver goes from one
+    // variable coefficient to the next (same buffers), and is dropped when it changes between constant and variable
+    if (!d_k || !s->var_k) invalidate_graph(s);
     if (!d_k) {
         for (auto& L : s->lv) { cudaFree(L.k); L.k = nullptr; }
         s->var_k = false;
@@ -453,7 +455,7 @@ int mg_set_coefficient(mg_solver* s, const void* d_k) {
 int mg_set_coefficient_from_vof(mg_solver* s, const void* d_alpha, double rho_l, double rho_g) {
     CHECK_SOLVER(s);
     if (!d_alpha || !(rho_l > 0.0) || !(rho_g > 0.0)) { set_error("mg_set_coefficient_from_vof: invalid argument"); return MG_EINVAL; }
-    invalidate_graph(s);
+    if (!s->var_k) invalidate_graph(s);
     int rc = alloc_k(s);
     if (rc) return rc;
     const size_t n = s->lv[0].n;

@@ -317,3 +317,27 @@ def test_zero_guess_cycle_equals_cycle_from_cleared_x(mg, shape, levels, nu, var
     mg.mg_solve(s, x2, db, 0.0, 1)
     assert rel_l2(as_f64(x2), as_f64(x_solve)) == 0.0
     mg.mg_destroy(s)
+
+
+def test_recorded_cycle_survives_a_coefficient_change(mg, orc):
+    """mg_vcycle replays a recorded CUDA graph; a new variable coefficient reuses the solver's buffers, so the recording is
+    kept -- and must then use the NEW coefficient: cycle parity against the oracle before and after the change, and after
+    going to a constant coefficient and back."""
+    shape, levels, dt = (32, 32, 32), 4, "f32"
+    bc = (N, N, N, N, N, D)
+    g = orc.grid(32, 32, 32, 1.0 / 32)
+    x0, b, k1 = make_problem(shape, dt, True, 5)
+    _, _, k2 = make_problem(shape, dt, True, 9)
+    s = make_solver(mg, shape, 1.0 / 32, levels, bc, dt, k=k1)
+    db = to_dev(b, dt)
+    for k in (k1, k2, k1, None, k2):
+        if k is None:
+            mg.mg_set_coefficient(s, None)
+        else:
+            mg.mg_set_coefficient(s, to_dev(k, dt))
+        for rep in range(2):                                   # first call records (or reuses), second replays
+            dx = to_dev(x0, dt)
+            assert mg.mg_vcycle(s, dx, db) == mg.MG_OK
+            ref = orc.vcycle(g, bc, k, x0, b, levels, 2, 2, 50, 2.0 / 3.0)
+            assert rel_l2(as_f64(dx), ref) <= 20 * TOL[dt]
+    mg.mg_destroy(s)
