@@ -1,7 +1,7 @@
 // flow.cu -- explicit stencil residuals that feed the pressure solve (rows a8-a10 of the hot
 // path): compressive-advection VoF residual, momentum advection-diffusion predictor, pressure
 // right-hand side and velocity projection, plus the config-5 time step built from them.
-// The kernels are in flow_march.cuh (z-marching, one column per thread).
+// The kernels are in flow_march.cuh (z-marching, W consecutive x points per thread).
 //
 // All filters are the NODAL (divided by m_l = dx dy dz, the paper's w_ml^-1) tensor
 // products of the 1-D trilinear-FE factors (Eqs. 9-11):
