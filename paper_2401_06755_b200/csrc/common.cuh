@@ -55,7 +55,8 @@ int launch_residual_mixed(const Level<double>& L, const double* k64, const doubl
 bool march_supported(int nx, int ny, int nz, double hx, double hy, double hz);
 template <typename TXT, typename TB>
 int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], const TXT* x, const TXT* k, const TB* b, TB* r,
-                          double* acc, cudaStream_t st, int dotx = 0);   // dotx: accumulate sum out * x instead of sum out^2
+                          double* acc, cudaStream_t st, int dotx = 0,    // dotx: accumulate sum out * x instead of sum out^2
+                          float* yout = nullptr);   // yout: also store out / D (fp32), the Jacobi seed of a correction cycle
 }  // namespace mgb
 struct mg_solver;
 namespace mgb {

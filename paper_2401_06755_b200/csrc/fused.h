@@ -8,6 +8,7 @@ bool fused_supported(const mg_solver* s);
 // (re)build the per-level data the tuned path derives from the coefficient (1/D of the coarse levels)
 int fused_prepare(mg_solver* s);
 int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps);
-int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess = 0);
+int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess = 0);   // 1: x = 0 implied; 2: x holds b / D (mg_fused.cu)
+bool fused_seed_supported(mg_solver* s);
 void fused_release(mg_solver* s);
 }  // namespace mgb

@@ -100,7 +100,7 @@ __device__ __forceinline__ void plane_sums(const T (&f)[3][6], T (&Dg)[4], T (&P
 template <typename TXT, typename TB, bool VAR, bool HASB>
 __global__ void __launch_bounds__(NT, (sizeof(TXT) == 8 ? 1 : 2))
 march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __restrict__ kc, const TB* __restrict__ b,
-                      TB* __restrict__ r, double* __restrict__ acc) {
+                      TB* __restrict__ r, double* __restrict__ acc, float* __restrict__ yout = nullptr) {
     typedef TXT T;
     extern __shared__ __align__(16) unsigned char smraw[];
     T* sm = reinterpret_cast<T*>(smraw);
@@ -244,6 +244,16 @@ march_residual_kernel(const MParams P, const TXT* __restrict__ x, const TXT* __r
                 else rv[c] = bv[c] + cc * (T(2) * Sx[c] - T(64) * xo[c]);
                 if (!HASB) rv[c] = -rv[c];       // no right-hand side: the output is y = A x
                 sq += (double)rv[c] * (!HASB && P.dotx ? (double)xo[c] : (double)rv[c]);
+            }
+            if (yout) {                // r / D, D = cc (32 k + S(k)): the Jacobi seed of the next correction cycle
+                float yv[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double rd;    // approximate reciprocal (as lean_kernel's own 1 / D): the seed feeds a smoother, not the iterate
+                    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rd) : "d"((double)(cc * (VAR ? T(32) * ko[c] + Sk[c] : T(64)))));
+                    yv[c] = (float)((double)rv[c] * rd);
+                }
+                *reinterpret_cast<float4*>(yout + ((size_t)qc * ny + gj) * nx + gi0) = make_float4(yv[0], yv[1], yv[2], yv[3]);
             }
             if (r) {
                 TB* dst = r + ((size_t)qc * ny + gj) * nx + gi0;

@@ -219,12 +219,16 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     if ((rc = norm2<float>(s, L.n, b, &nb))) return rc;
     if ((rc = launch_cast_f2d(L.n, x, s->x64, s->st))) return rc;
     ++s->launches;
+    // Seeded correction cycles: the defect kernel also writes y = r32 / D into e32, and the cycle's first pass turns y into the
+    // iterate after two sweeps from a zero guess (mg_fused.cu) -- one 12-byte pass instead of a 12-byte and a 16-byte one.
+    const bool seeded = s->fused && fused_supported(s) && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz) && fused_seed_supported(s);
+    auto correction_cycle = [&]() -> int { return seeded ? fused_vcycle(s, s->e32, s->r32, 2) : vcycle_zero_guess(s, s->e32, s->r32); };
     auto resid_into = [&](double* dacc) -> int {      // r32 = float(b - A64 x64), ||r||^2 into *dacc (no read-back)
         MGB_CUDA(cudaMemsetAsync(dacc, 0, sizeof(double), s->st));
         int r2;
         if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
             r2 = launch_march_residual<double, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, s->x64, s->var_k ? s->k64 : nullptr, b, s->r32,
-                                                      dacc, s->st);
+                                                      dacc, s->st, 0, seeded ? s->e32 : nullptr);
         else r2 = launch_residual_mixed(L.Ld, s->var_k ? s->k64 : nullptr, s->x64, b, s->r32, dacc, s->st);
         if (!r2) ++s->launches;
         return r2;
@@ -234,7 +238,7 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
         int r2;
         if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
             r2 = launch_march_residual<double, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, s->x64, s->var_k ? s->k64 : nullptr, b, s->r32,
-                                                      s->d_acc, s->st);
+                                                      s->d_acc, s->st, 0, seeded ? s->e32 : nullptr);
         else r2 = launch_residual_mixed(L.Ld, s->var_k ? s->k64 : nullptr, s->x64, b, s->r32, s->d_acc, s->st);
         if (r2) return r2;
         ++s->launches;
@@ -248,7 +252,7 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     int cycles = 0, status = (rel < tol) ? MG_OK : MG_NOT_CONVERGED;
     if (tol == 0.0 && max_cycles > 0 && max_cycles < ACC_N) {     // fixed cycle count: enqueue everything, read the norms once
         for (int c = 0; c < max_cycles; ++c) {
-            if ((rc = vcycle_zero_guess(s, s->e32, s->r32))) return rc;
+            if ((rc = correction_cycle())) return rc;
             if ((rc = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return rc;
             ++s->launches;
             if ((rc = resid_into(s->d_acc + 1 + c))) return rc;
@@ -263,7 +267,7 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
         cycles = max_cycles;
     }
     while (status == MG_NOT_CONVERGED && cycles < max_cycles) {
-        if ((rc = vcycle_zero_guess(s, s->e32, s->r32))) return rc;
+        if ((rc = correction_cycle())) return rc;
         if ((rc = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return rc;
         ++s->launches;
         if ((rc = resid(&rel))) return rc;

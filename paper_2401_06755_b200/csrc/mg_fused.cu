@@ -108,6 +108,7 @@ struct FusedState {
     std::vector<LevelPlan> lp;
     bool attrs_set = false;
     bool zero_x_once = false; // the next SWEEP launch takes its input iterate as zero (zero-guess cycles)
+    bool seed_once = false;   // the next SWEEP launch is the two-sweeps-in-one pass over the Jacobi seed y = b / D
 };
 
 constexpr int TXD = 56, TYD = 28;   // + halo = 64 x 32 cells per plane, 16 x 16 threads
@@ -225,7 +226,12 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
     P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
     P.omega = (float)s->p.omega;
     P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
+    P.om_g = P.omega; P.om_x = 1.f - P.omega;
     if (MODE == lk::MODE_SWEEP && fs->zero_x_once) { P.zero_x = 1; fs->zero_x_once = false; }
+    if (MODE == lk::MODE_SWEEP && fs->seed_once) {
+        P.om_g = P.omega * P.omega; P.om_x = P.omega * (2.f - P.omega); P.icc = 0.f; P.zero_b = 1;
+        fs->seed_once = false;
+    }
     if (MODE == lk::MODE_RR) {
         const LevelPlan& cp = fs->lp[l + 1];
         P.dinv_c = cp.dinv;
@@ -495,13 +501,26 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     return 0;
 }
 
-// zero_guess: x is taken as 0 whatever it holds: the first pre-smoothing pass does not read it (12 bytes per point instead
-// of 16, and the caller need not clear x)
+// zero_guess 1: x is taken as 0 whatever it holds: the first pre-smoothing pass does not read it (12 bytes per point instead
+// of 16, and the caller need not clear x).  zero_guess 2: x holds the Jacobi seed y = b / D of a cycle from a zero guess
+// (written by the defect kernel); the first pass turns it into the iterate after TWO sweeps,
+// x_2 = omega (2 - omega) y - omega^2 D^-1 (A - D) y, without reading b: one 12-byte pass instead of two sweeps.
 int enqueue_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
+    FusedState* fs = (FusedState*)s->fused_state;
     float* res = nullptr;
-    ((FusedState*)s->fused_state)->zero_x_once = zero_guess != 0;
-    int rc = cycle_level(s, 0, x, (float*)s->lv[0].tmp, b, 0, &res);
-    ((FusedState*)s->fused_state)->zero_x_once = false;
+    float *A = x, *B = (float*)s->lv[0].tmp;
+    int done = 0, rc;
+    if (zero_guess == 2) {
+        fs->seed_once = true;
+        rc = launch_stream(s, 0, lk::MODE_SWEEP, x, b, B);
+        fs->seed_once = false;
+        if (rc) return rc;
+        std::swap(A, B);
+        done = 2;
+    }
+    fs->zero_x_once = zero_guess == 1;
+    rc = cycle_level(s, 0, A, B, b, done, &res);
+    fs->zero_x_once = false;
     if (rc) return rc;
     if (res != x) MGB_CUDA(cudaMemcpyAsync(x, res, s->lv[0].n * sizeof(float), cudaMemcpyDeviceToDevice, s->st));
     return 0;
@@ -539,6 +558,7 @@ int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
         size_t sm = 0; int a = 0, c = 0;
         const bool lean0 = fs->lp[0].stream && s->p.sweeps_per_pass == 1 && s->p.nu_pre >= 1 && s->levels > 1 &&
                            !ctail_fits(s, 0, &sm, &a, &c) && !tail_fits(s, 0, &sm);
+        if (zero_guess == 2 && !(lean0 && s->p.nu_pre >= 2)) { set_error("fused_vcycle: the seeded cycle is not available"); return MG_EINVAL; }
         if (!lean0) {
             MGB_CUDA(cudaMemsetAsync(x, 0, s->lv[0].n * sizeof(float), s->st));
             zero_guess = 0;
@@ -546,6 +566,15 @@ int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
     }
     if (s->timing) return enqueue_vcycle(s, x, b, zero_guess);
     return replay_graph(s, x, b, [&]() { return enqueue_vcycle(s, x, b, zero_guess); }, zero_guess);
+}
+
+// the seeded cycle (zero_guess 2) needs a lean_kernel sweep as the first launch of level 0 and two pre-smoothing sweeps
+bool fused_seed_supported(mg_solver* s) {
+    if (ensure_state(s)) return false;
+    FusedState* fs = (FusedState*)s->fused_state;
+    size_t sm = 0; int a = 0, c = 0;
+    return fs->lp[0].stream && s->p.sweeps_per_pass == 1 && s->p.nu_pre >= 2 && s->levels > 1 && !ctail_fits(s, 0, &sm, &a, &c) &&
+           !tail_fits(s, 0, &sm);
 }
 
 void fused_release(mg_solver* s) {

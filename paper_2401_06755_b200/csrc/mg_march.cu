@@ -10,7 +10,7 @@ bool march_supported(int nx, int ny, int nz, double hx, double hy, double hz) {
 
 template <typename TXT, typename TB>
 int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], const TXT* x, const TXT* k, const TB* b, TB* r,
-                          double* acc, cudaStream_t st, int dotx) {
+                          double* acc, cudaStream_t st, int dotx, float* yout) {
     mk::MParams P;
     P.nx = nx; P.ny = ny; P.nz = nz;
     for (int f = 0; f < 6; ++f) P.s[f] = s[f];
@@ -34,16 +34,16 @@ int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], c
     P.zchunk = (nz + nch - 1) / nch;
     const dim3 grid(tx, ty, (nz + P.zchunk - 1) / P.zchunk);
     if (b && dotx) { set_error("march residual: dotx needs b == NULL"); return MG_EINVAL; }
-    if (k && b) mk::march_residual_kernel<TXT, TB, true, true><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc);
-    else if (k) mk::march_residual_kernel<TXT, TB, true, false><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc);
-    else if (b) mk::march_residual_kernel<TXT, TB, false, true><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc);
-    else mk::march_residual_kernel<TXT, TB, false, false><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc);
+    if (k && b) mk::march_residual_kernel<TXT, TB, true, true><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc, yout);
+    else if (k) mk::march_residual_kernel<TXT, TB, true, false><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc, yout);
+    else if (b) mk::march_residual_kernel<TXT, TB, false, true><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc, yout);
+    else mk::march_residual_kernel<TXT, TB, false, false><<<grid, mk::NT, smem, st>>>(P, x, k, b, r, acc, yout);
     MGB_LAUNCH_CHECK();
     return 0;
 }
 
-template int launch_march_residual<double, float>(int, int, int, double, const double*, const double*, const double*, const float*, float*, double*, cudaStream_t, int);
-template int launch_march_residual<double, double>(int, int, int, double, const double*, const double*, const double*, const double*, double*, double*, cudaStream_t, int);
-template int launch_march_residual<float, float>(int, int, int, double, const double*, const float*, const float*, const float*, float*, double*, cudaStream_t, int);
+template int launch_march_residual<double, float>(int, int, int, double, const double*, const double*, const double*, const float*, float*, double*, cudaStream_t, int, float*);
+template int launch_march_residual<double, double>(int, int, int, double, const double*, const double*, const double*, const double*, double*, double*, cudaStream_t, int, float*);
+template int launch_march_residual<float, float>(int, int, int, double, const double*, const float*, const float*, const float*, float*, double*, cudaStream_t, int, float*);
 
 }  // namespace mgb
