@@ -296,10 +296,12 @@ def test_empty_cycles_and_zero_rhs(mg):
 
 
 @pytest.mark.parametrize("var", [False, True])
-@pytest.mark.parametrize("shape,levels,nu", [((64, 48, 96), 4, 2), ((32, 32, 32), 4, 1), ((16, 16, 16), 3, 2), ((40, 24, 48), 3, 0)])
+@pytest.mark.parametrize("shape,levels,nu", [((64, 48, 96), 4, 2), ((32, 32, 32), 4, 1), ((16, 16, 16), 3, 2), ((40, 24, 48), 3, 0),
+                                             ((32, 48, 64), 3, 3)])
 def test_zero_guess_cycle_equals_cycle_from_cleared_x(mg, shape, levels, nu, var):
     """The correction cycles of mg_solve / mg_pcg_solve start from x = 0 without reading x (lean_kernel zero_x; cleared x
-    where level 0 is not a lean_kernel level or nu_pre = 0).  One cycle of the mixed-precision solve from x = 0 is
+    where level 0 is not a lean_kernel level or nu_pre = 0); with nu_pre >= 2 mg_solve's cycles start from the seed y = r / D
+    written by the defect kernel and do the first two sweeps in one pass.  One cycle of the mixed-precision solve from x = 0 is
     x = V(0, float(b)): it must equal the public mg_vcycle from a cleared x up to the fp64 -> fp32 rounding of the result."""
     dt = "f32"
     _, b, k = make_problem(shape, dt, var, 77)
