@@ -46,7 +46,7 @@
 namespace mgb {
 namespace lk {
 
-enum { MODE_SWEEP = 0, MODE_PRO = 1, MODE_RR = 2 };
+enum { MODE_SWEEP = 0, MODE_PRO = 1, MODE_RR = 2, MODE_SEED = 3 };
 
 struct LParams {
     int nx, ny, nz;
@@ -62,12 +62,11 @@ struct LParams {
     float gc_const;             // RR, constant k: omega / w0_c
     int first_sweep;            // RR: write x_c = omega b_c / D_c (1) or zeros (0)
     int zero_x;                 // SWEEP: the iterate is zero whatever `src` holds: its planes are not read (12 B/point, not 16)
-    // sweep weights: x' = om_x x + (om_g / D)(b + cc (k S(x) + S(k x))).  Normally om_g = omega, om_x = 1 - omega.  The
-    // first TWO sweeps of a cycle from a zero guess collapse into one pass over y = b / D (written by the defect kernel):
-    // x_2 = omega (2 - omega) y + (omega^2 / D) cc (k S(y) + S(k y)), i.e. om_g = omega^2, om_x = omega (2 - omega) and no
-    // b term (zero_b: the b tiles are not fetched, their ring slots are cleared; 12 B/point)
+    // MODE_SEED: the first TWO sweeps of a cycle from a zero guess in one pass over y = b / D (written by the defect kernel):
+    // x_2 = omega (2 - omega) y + (omega^2 / D) cc (k S(y) + S(k y)) -- the sweep formula x' = om_x x + (om_g / D)(b + cc (..))
+    // with om_g = omega^2, om_x = omega (2 - omega) and no b term (the b tiles are not fetched, their ring slots are cleared;
+    // 12 B/point).  A mode of its own so that the code of the other modes is untouched.
     float om_g, om_x;
-    int zero_b;
 };
 
 template <int LX_, int LY_, bool VAR_, int MODE_, int MINB_>
@@ -236,7 +235,7 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
     auto issue = [&](int it) {   // one thread: TMA of the x, k planes of iteration `it` and of the b tile it finalises
         uint64_t* bar = &bars[it % NS];
         float* dst = ring + (it % NS) * SLOT;
-        const bool wb = it >= 2 && !(MODE == MODE_SWEEP && P.zero_b);   // plane pbeg + it - 1 >= zc0
+        const bool wb = it >= 2 && MODE != MODE_SEED;              // plane pbeg + it - 1 >= zc0
         const bool zx = MODE == MODE_SWEEP && P.zero_x;            // x planes stay the zeros written below
         mbar_expect_tx(bar, C::BOX_BYTES * ((VAR ? 1u : 0u) + (zx ? 0u : 1u)) + (wb ? C::BBOX_BYTES : 0u) + (MODE == MODE_PRO ? C::CBOX_BYTES : 0u));
         const int z = zsrc(pbeg + it);
@@ -254,7 +253,7 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
     }
     if (MODE == MODE_SWEEP && P.zero_x)
         for (int e = tid; e < NS * PLANE; e += C::NT) ring[(e / PLANE) * SLOT + (e % PLANE)] = 0.f;
-    if (MODE == MODE_SWEEP && P.zero_b)
+    if (MODE == MODE_SEED)
         for (int e = tid; e < NS * C::BPLANE; e += C::NT) ring[(e / C::BPLANE) * SLOT + BOFF + (e % C::BPLANE)] = 0.f;
     __syncthreads();
     // Programmatic dependent launch: everything above touched only kernel parameters; the fields written by the previous
@@ -356,7 +355,8 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         // ---- finalise plane p - 1 ----
         const int qc = p - 1;
         if (it >= 2) {
-            const u64 icc2 = bc2(P.icc), cc2 = bc2(P.cc), om12 = bc2(P.om_x);
+            const u64 icc2 = bc2(P.icc), cc2 = bc2(P.cc), om12 = bc2(MODE == MODE_SEED ? P.om_x : 1.f - omega);
+            const float om_g = MODE == MODE_SEED ? P.om_g : omega;
             float rs0 = 0.f, rs1 = 0.f;
 #pragma unroll
             for (int j = 0; j < RY; ++j) {
@@ -374,13 +374,13 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
                         if (MODE == MODE_RR) {
                             o[c] = fma2(mul2(Dp, bc2(-P.cc)), xv, fma2(t, cc2, bv));
                         } else {
-                            const u64 g = mul2(pk(rcpa(lo(Dp)), rcpa(hi(Dp))), bc2(P.om_g));
+                            const u64 g = mul2(pk(rcpa(lo(Dp)), rcpa(hi(Dp))), bc2(om_g));
                             o[c] = fma2(g, fma2(bv, icc2, t), mul2(xv, om12));
                         }
                     } else {
                         const u64 s2 = add2(Sx[j][c], Sx[j][c]);
                         if (MODE == MODE_RR) o[c] = fma2(fma2(xv, bc2(-64.f), s2), cc2, bv);
-                        else o[c] = fma2(bc2(P.om_g * (1.f / 64.f)), fma2(bv, icc2, s2), mul2(xv, om12));
+                        else o[c] = fma2(bc2(om_g * (1.f / 64.f)), fma2(bv, icc2, s2), mul2(xv, om12));
                     }
                 }
                 if (MODE == MODE_RR) { rs0 += lo(o[0]) + hi(o[0]); rs1 += lo(o[1]) + hi(o[1]); }

@@ -108,7 +108,6 @@ struct FusedState {
     std::vector<LevelPlan> lp;
     bool attrs_set = false;
     bool zero_x_once = false; // the next SWEEP launch takes its input iterate as zero (zero-guess cycles)
-    bool seed_once = false;   // the next SWEEP launch is the two-sweeps-in-one pass over the Jacobi seed y = b / D
 };
 
 constexpr int TXD = 56, TYD = 28;   // + halo = 64 x 32 cells per plane, 16 x 16 threads
@@ -226,12 +225,8 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
     P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
     P.omega = (float)s->p.omega;
     P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
-    P.om_g = P.omega; P.om_x = 1.f - P.omega;
     if (MODE == lk::MODE_SWEEP && fs->zero_x_once) { P.zero_x = 1; fs->zero_x_once = false; }
-    if (MODE == lk::MODE_SWEEP && fs->seed_once) {
-        P.om_g = P.omega * P.omega; P.om_x = P.omega * (2.f - P.omega); P.icc = 0.f; P.zero_b = 1;
-        fs->seed_once = false;
-    }
+    if (MODE == lk::MODE_SEED) { P.om_g = P.omega * P.omega; P.om_x = P.omega * (2.f - P.omega); P.icc = 0.f; }
     if (MODE == lk::MODE_RR) {
         const LevelPlan& cp = fs->lp[l + 1];
         P.dinv_c = cp.dinv;
@@ -263,6 +258,7 @@ int launch_stream(mg_solver* s, int l, int mode, const float* src, const float* 
     MGB_SCASE(lk::MODE_SWEEP)
     MGB_SCASE(lk::MODE_PRO)
     MGB_SCASE(lk::MODE_RR)
+    MGB_SCASE(lk::MODE_SEED)
 #undef MGB_SCASE
     set_error("stream pass mode %d is not instantiated", mode);
     return MG_EINVAL;
@@ -511,10 +507,7 @@ int enqueue_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
     float *A = x, *B = (float*)s->lv[0].tmp;
     int done = 0, rc;
     if (zero_guess == 2) {
-        fs->seed_once = true;
-        rc = launch_stream(s, 0, lk::MODE_SWEEP, x, b, B);
-        fs->seed_once = false;
-        if (rc) return rc;
+        if ((rc = launch_stream(s, 0, lk::MODE_SEED, x, b, B))) return rc;
         std::swap(A, B);
         done = 2;
     }
