@@ -207,3 +207,26 @@ def test_vcycle_zero_guess_first_sweep_is_pointwise(orc):
     k = np.exp(_rand(g.shape, 5)); b = _rand(g.shape, 6)
     y = orc.jacobi_sweep(g, (N,) * 5 + (D,), k, np.zeros(g.shape), b, 2 / 3)
     assert np.abs(y - (2 / 3) * b / orc.diagonal(g, k)).max() < 1e-15 * np.abs(y).max()
+
+
+@pytest.mark.parametrize("var", [False, True])
+def test_two_sweeps_from_zero_are_one_pass_over_the_jacobi_seed(orc, var):
+    """The identity behind the CUDA path's seeded correction cycles: with y = b / D, two weighted-Jacobi sweeps
+    from x = 0 give x_2 = omega (2 - omega) y - omega^2 D^-1 (A - D) y.  Checked with the oracle's own sweeps, operator and
+    diagonal on a mixed-BC, variable-coefficient problem; a wrong weight or sign in either form shows at O(1)."""
+    from workloads import rng
+    nx, ny, nz, h = 12, 10, 8, 0.05
+    g = orc.grid(nx, ny, nz, h)
+    bc = (0, 1, 2, 0, 1, 0)
+    n = nx * ny * nz
+    b = rng.normal(301, n).reshape(nz, ny, nx)
+    k = np.exp(-3.0 * rng.uniform01(302, n)).reshape(nz, ny, nx) if var else None
+    omega = 2.0 / 3.0
+    x2 = orc.smooth(g, bc, k, np.zeros_like(b), b, omega, 2)
+    D = orc.diagonal(g, k)
+    y = b / D
+    Ay = orc.apply_operator(g, bc, k, y)
+    seeded = omega * (2.0 - omega) * y - omega ** 2 * (Ay - D * y) / D
+    assert np.linalg.norm(seeded - x2) <= 1e-13 * np.linalg.norm(x2)
+    x1 = orc.smooth(g, bc, k, np.zeros_like(b), b, omega, 1)
+    assert np.linalg.norm(x1 - omega * y) <= 1e-14 * np.linalg.norm(x1)
