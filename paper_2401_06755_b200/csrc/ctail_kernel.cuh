@@ -44,6 +44,10 @@ struct CParams {
     int first_done;                           // the parent already applied the first sweep to x (level 0 of the tail)
     float* x;                                 // level-0 iterate of the tail (in / out)
     const float* b;                           // level-0 right-hand side
+    // The coarsest solve (coarse_sweeps Jacobi sweeps from a zero guess) is a fixed linear map x = M b of the n_c coarsest
+    // points; when the host has tabulated it (n_c <= 64; cmat[j * n_c + i] = M_ij, rebuilt when the coefficient or the
+    // parameters change) one n_c x n_c product replaces the serial chain of sweeps.  NULL: run the sweeps.
+    const float* cmat;
 };
 
 // one block's slab of a distributed level
@@ -284,7 +288,22 @@ __global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(NT, 1) ctail_kernel
             }
             __syncthreads();
         }
-        tk::sweeps(lv[last], s, omega, max(0, P.coarse_sweeps - ((P.coarse_sweeps >= 1) ? 1 : 0)));   // coarsest
+        if (P.cmat) {                                               // coarsest: x = M b
+            tk::Lv& L = lv[last];
+            if (tid < L.n) {
+                const float* __restrict__ m = P.cmat + tid;
+                float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll 4
+                for (int j = 0; j < L.n; j += 4) {
+                    a0 = fmaf(m[(j + 0) * L.n], L.B[j + 0], a0); a1 = fmaf(m[(j + 1) * L.n], L.B[j + 1], a1);
+                    a2 = fmaf(m[(j + 2) * L.n], L.B[j + 2], a2); a3 = fmaf(m[(j + 3) * L.n], L.B[j + 3], a3);
+                }
+                L.X[tid] = (a0 + a1) + (a2 + a3);
+            }
+            __syncthreads();
+        } else {
+            tk::sweeps(lv[last], s, omega, max(0, P.coarse_sweeps - ((P.coarse_sweeps >= 1) ? 1 : 0)));   // coarsest
+        }
         for (int u = last - 1; u >= 0; --u) {                       // up leg
             tk::Lv& L = lv[u];
             tk::Lv& C = lv[u + 1];

@@ -108,6 +108,8 @@ struct FusedState {
     std::vector<LevelPlan> lp;
     bool attrs_set = false;
     bool zero_x_once = false; // the next SWEEP launch takes its input iterate as zero (zero-guess cycles)
+    float* cmat = nullptr;    // the coarsest solve tabulated as a matrix (ctail_kernel.cuh), n_c <= 64
+    bool cmat_valid = false;
 };
 
 constexpr int TXD = 56, TYD = 28;   // + halo = 64 x 32 cells per plane, 16 x 16 threads
@@ -408,6 +410,51 @@ bool ctail_fits(const mg_solver* s, int l, size_t* smem_out, int* nd_out, int* n
     return *smem_out <= 200 * 1024;
 }
 
+struct Fac6 { float v[6]; };
+// column `blockIdx.x` of the coarsest-solve matrix: `sweeps` Jacobi sweeps from a zero guess on the unit vector
+__global__ void __launch_bounds__(tk::NT, 1) coarse_matrix_kernel(int nx, int ny, int nz, const float* __restrict__ k, const float* __restrict__ dinv,
+                                                                 float dinv_const, float ce, float cc, Fac6 fac, float omega, int sweeps,
+                                                                 float* __restrict__ cmat) {
+    extern __shared__ __align__(16) float sm[];
+    __shared__ float sf[6];
+    tk::Lv L;
+    L.nx = nx; L.ny = ny; L.nz = nz; L.n = nx * ny * nz; L.ce = ce; L.cc = cc;
+    L.X = sm; L.Y = sm + L.n; L.B = sm + 2 * L.n; L.K = sm + 3 * L.n; L.DI = sm + 4 * L.n;
+    if (threadIdx.x < 6) sf[threadIdx.x] = fac.v[threadIdx.x];
+    const int col = blockIdx.x;
+    for (int idx = threadIdx.x; idx < L.n; idx += tk::NT) {
+        L.K[idx] = k ? k[idx] : 1.f;
+        L.DI[idx] = dinv ? dinv[idx] : dinv_const;
+        const float bi = idx == col ? 1.f : 0.f;
+        L.B[idx] = bi;
+        L.X[idx] = sweeps >= 1 ? omega * L.DI[idx] * bi : 0.f;
+        L.Y[idx] = 0.f;
+    }
+    __syncthreads();
+    tk::sweeps(L, sf, omega, max(0, sweeps - 1));
+    for (int idx = threadIdx.x; idx < L.n; idx += tk::NT) cmat[(size_t)col * L.n + idx] = L.X[idx];
+}
+
+// (re)tabulate the coarsest solve; stream-ordered after the coefficient set-up, before the cycle that uses it
+int refresh_cmat(mg_solver* s) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    const int lc = s->levels - 1;
+    const LevelData& L = s->lv[lc];
+    static const bool disabled = getenv("MG_NO_COARSE_MATRIX") != nullptr;
+    if (disabled || s->levels < 2 || L.n > 64 || L.n % 4 || s->p.coarse_sweeps < 1) { fs->cmat_valid = false; return 0; }
+    if (!fs->cmat && cudaMalloc(&fs->cmat, 64 * 64 * sizeof(float)) != cudaSuccess) { set_error("fused: out of memory"); return MG_EALLOC; }
+    const LevelPlan& lp = fs->lp[lc];
+    Fac6 fac;
+    for (int f = 0; f < 6; ++f) fac.v[f] = L.Lf.s[f];
+    coarse_matrix_kernel<<<(int)L.n, tk::NT, 5 * L.n * sizeof(float), s->st>>>(L.nx, L.ny, L.nz, s->var_k ? (const float*)L.k : nullptr,
+                                                                             s->var_k ? lp.dinv : nullptr, 1.f / lp.w0, lp.ce, lp.cc, fac,
+                                                                             (float)s->p.omega, s->p.coarse_sweeps, fs->cmat);
+    MGB_LAUNCH_CHECK();
+    ++s->launches;
+    fs->cmat_valid = true;
+    return 0;
+}
+
 int launch_ctail(mg_solver* s, int l, float* x, const float* b, int done, size_t smem, int nd, int ns) {
     FusedState* fs = (FusedState*)s->fused_state;
     ck::CParams P;
@@ -425,6 +472,7 @@ int launch_ctail(mg_solver* s, int l, float* x, const float* b, int done, size_t
     P.omega = (float)s->p.omega;
     P.nu_pre = s->p.nu_pre; P.nu_post = s->p.nu_post; P.coarse_sweeps = s->p.coarse_sweeps;
     P.first_done = done; P.x = x; P.b = b;
+    P.cmat = fs->cmat_valid ? fs->cmat : nullptr;
     static bool attr_done = false;
     if (!attr_done) {
         MGB_CUDA(cudaFuncSetAttribute(ck::ctail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
@@ -530,6 +578,7 @@ bool fused_supported(const mg_solver* s) {
 int fused_prepare(mg_solver* s) {
     int rc = ensure_state(s);
     if (rc) return rc;
+    ((FusedState*)s->fused_state)->cmat_valid = false;       // rebuilt before the next cycle (fused_vcycle)
     return refresh_dinv(s);
 }
 
@@ -545,6 +594,9 @@ int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps) {
 int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
     int rc = ensure_state(s);
     if (rc) return rc;
+    // the tabulated coarsest solve follows the coefficient (fused_prepare clears the flag) and the parameters (a parameter
+    // change drops the recorded graph)
+    if ((!((FusedState*)s->fused_state)->cmat_valid || !s->graph_exec) && (rc = refresh_cmat(s))) return rc;
     if (zero_guess) {
         // the first launch of the cycle has to be a lean_kernel sweep of level 0; otherwise clear x and run the general cycle
         FusedState* fs = (FusedState*)s->fused_state;
@@ -574,6 +626,7 @@ void fused_release(mg_solver* s) {
     FusedState* fs = (FusedState*)s->fused_state;
     if (!fs) return;
     for (auto& lp : fs->lp) { cudaFree(lp.dinv); cudaFree(lp.tmp2); }
+    cudaFree(fs->cmat);
     delete fs;
     s->fused_state = nullptr;
 }

@@ -343,3 +343,27 @@ def test_recorded_cycle_survives_a_coefficient_change(mg, orc):
             ref = orc.vcycle(g, bc, k, x0, b, levels, 2, 2, 50, 2.0 / 3.0)
             assert rel_l2(as_f64(dx), ref) <= 20 * TOL[dt]
     mg.mg_destroy(s)
+
+
+@pytest.mark.parametrize("var", [False, True])
+def test_tabulated_coarsest_solve_follows_parameters_and_coefficient(mg, orc, var):
+    """On a 4^3 coarsest level the cluster tail applies the coarse_sweeps Jacobi sweeps as one tabulated matrix
+    (ctail_kernel.cuh `cmat`).  The table must follow coarse_sweeps, omega and the coefficient: cycle parity against the
+    oracle after each change, and with the table switched off by a coarsest level that is not 4^3."""
+    dt, bc = "f32", (N, N, N, N, N, D)
+    shape = (64, 64, 64)
+    g = orc.grid(64, 64, 64, 1.0 / 64)
+    x0, b, k1 = make_problem(shape, dt, var, 41)
+    _, _, k2 = make_problem(shape, dt, var, 43)
+    for levels in (5, 4):                                   # coarsest 4^3 (tabulated) and 8^3 (sweeps)
+        s = make_solver(mg, shape, 1.0 / 64, levels, bc, dt, k=k1)
+        db = to_dev(b, dt)
+        for cs, omega, k in ((50, 2.0 / 3.0, k1), (7, 2.0 / 3.0, k1), (7, 0.8, k1), (7, 0.8, k2), (1, 0.8, k2), (50, 2.0 / 3.0, k2)):
+            mg.mg_set_params(s, nu_pre=2, nu_post=2, coarse_sweeps=cs, sweeps_per_pass=1, omega=omega, mixed_precision=1)
+            if var:
+                mg.mg_set_coefficient(s, to_dev(k, dt))
+            dx = to_dev(x0, dt)
+            assert mg.mg_vcycle(s, dx, db) == mg.MG_OK
+            ref = orc.vcycle(g, bc, k if var else None, x0, b, levels, 2, 2, cs, omega)
+            assert rel_l2(as_f64(dx), ref) <= 20 * TOL[dt], (levels, cs, omega)
+        mg.mg_destroy(s)
