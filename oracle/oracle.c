@@ -15,7 +15,10 @@
  * Parity pins (tests/test_oracle_*.py, -m "not gpu"): Eq. 11's printed weights, the closed
  * form discrete eigenpair, 2nd-order manufactured solution, symmetry, constant null space,
  * literal Eq. 13 == collapsed difference form, dense direct solves on <= 8^3, Fourier-mode
- * Jacobi factors, transfer adjointness, hand-computed VoF cases.
+ * Jacobi factors, transfer adjointness, hand-computed VoF cases, the hand-reduced 1-D momentum scheme
+ * (both branches of min{k_max, k_abs} of Eqs. 30-32 under varying rho and mu), and -- for the step composition in
+ * oracle/__init__.py -- the stages chained by hand, the potential-flow property of stage 4 (Eq. 16 advects with
+ * u^{n+1}) and the second-order accuracy of the two predictor iterations (tests/test_oracle_step.py).
  * PARITY UNPINNED against the paper (no worked example exists in its text): the transfer
  * operators / coarse operator (Fig. 5 is an image), the momentum residual without the
  * missing Eq. 28, and vof_residual beyond its hand-computable special cases.

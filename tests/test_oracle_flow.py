@@ -205,6 +205,73 @@ def test_momentum_viscous_limit_is_eigenmode_decay(orc):
     assert np.abs(qt[0] - (1 - dt * mu / rho * lam) * u).max() < 1e-5 * eps * dt * mu / rho * lam
 
 
+def _mom_1d(c, adv_vel, speed_sum, C, cn, h, dt, rho_l, rho_g, mu_l, mu_g):
+    """Eqs. 18 (advection + diffusion part), 27, 29, 30-32, 45-46 reduced BY HAND to fields that vary along ONE axis
+    (P:198-220, 284-305, 309-319, 433-441): every 3x3x3 filter collapses to its 1-D factor (the mass factors sum to one);
+    `adv_vel` is the velocity component along that axis, `speed_sum` = |u| + |v| + |w| (uniform spacing, Eq. 30).
+    Returns (c~, c_half', k_max, k_abs, k_c)."""
+    cp = np.pad(c, 1, mode="edge")
+    cx = (cp[2:] - cp[:-2]) / (2 * h)
+    adv = adv_vel * cx
+    ap = np.pad(adv, 1, mode="edge")
+    a = 2.0 * (ap[:-2] - 2 * adv + ap[2:]) / 6.0                       # Eq. 29, alpha_a = 2
+    kabs = (1.0 / 16.0) * h * np.abs(a) / (1e-7 + np.abs(cx) / 3.0)    # Eq. 27, alpha_kabs = 1/16 (P:294), eps_k (P:278)
+    kmax = h * speed_sum                                               # Eq. 30 (P:309-311)
+    rho = rho_l * C + rho_g * (1 - C)                                  # Eq. 2 (P:67)
+    mu = mu_l * C + mu_g * (1 - C)
+    kc = rho * np.minimum(kmax, kabs) + mu                             # Eqs. 31-32 (P:313-319), k_square (lost Eq. 28) omitted
+    kp = np.pad(kc, 1, mode="edge")
+    diff = (0.5 * (kc + kp[:-2]) * (c - cp[:-2]) + 0.5 * (kc + kp[2:]) * (c - cp[2:])) / (h * h)   # Eq. 13 collapsed, 1-D
+    s = rho * adv + diff
+    ct = cn - dt * s / rho                                             # Eq. 45, sigma = 0
+    return ct, 0.5 * (cn + ct), kmax, kabs, kc
+
+
+@pytest.mark.parametrize("axis", [2, 1, 0])
+def test_momentum_one_dimensional_profile_pins_the_petrov_galerkin_coefficient(orc, axis):
+    """Velocity components and C varying along one axis, against the hand-reduced 1-D scheme.  The profiles are built so
+    that min{k_max, k_abs} takes BOTH branches at many cells with rho and mu varying by orders of magnitude across them:
+    dropping rho, dropping the min, a wrong k_max or dropping mu each change c~ far beyond the tolerance (asserted
+    below on the hand side, so the case stays discriminating if the profiles are edited)."""
+    n, h, dt = 32, 0.05, 0.004
+    rho_l, rho_g, mu_l, mu_g = 1000.0, 1.0, 0.5, 0.02
+    i = np.arange(n)
+    along_of = {2: 0, 1: 1, 0: 2}                                            # component index of the velocity along `axis`
+    C = 0.5 * (1 + np.tanh((i - 15.2) / 2.5))                                # rho from 1 to 1000 across the profile
+    # cos(2 pi (i - i0) / P) with integer i0 and even P is symmetric about the cells i0 + m P / 2: the central gradient
+    # vanishes there while the mixed-mass residual a of Eq. 29 does not (the advecting velocity is not symmetric about
+    # them), so k_abs >> k_max at those cells (Eq. 27's eps_k in the denominator) and k_abs << k_max elsewhere
+    prof = [0.25 * np.cos(2 * np.pi * i / 8) + 0.05, 0.2 * np.cos(2 * np.pi * (i - 1) / 6) - 0.03,
+            0.15 * np.cos(2 * np.pi * (i - 2) / 10) + 0.1]
+    prof[along_of[axis]] = 0.22 * np.sin(0.47 * i + 0.3) + 0.06              # the advecting component: no symmetric cells
+    prof_n = [p + 0.01 * np.cos(1.3 * i + m) for m, p in enumerate(prof)]    # q_n differs from q_half
+    along = along_of[axis]
+    speed = sum(np.abs(p) for p in prof)
+    shape = [4, 4, 4]; shape[axis] = n
+    bshape = [1, 1, 1]; bshape[axis] = n
+    g = orc.grid(shape[2], shape[1], shape[0], h)
+    b3 = lambda a: np.broadcast_to(a.reshape(bshape), shape).copy()
+    qh = tuple(b3(p) for p in prof); qn = tuple(b3(p) for p in prof_n)
+    qt, qhn = orc.mom_predictor(g, b3(C), qh, qn, rho_l, rho_g, mu_l, mu_g, dt)
+    for comp in range(3):
+        ct, chalf, kmax, kabs, kc = _mom_1d(prof[comp], prof[along], speed, C, prof_n[comp], h, dt, rho_l, rho_g, mu_l, mu_g)
+        lo, hi = (kabs < kmax) & (kabs > 1e-3 * kmax), kabs > kmax
+        # both branches of the min{} are taken (the self-advected component has no cell with k_abs > k_max)
+        assert lo.sum() >= 4 and (hi.sum() >= 3 or comp == along), (comp, lo.sum(), hi.sum())
+        scale = np.abs(ct - prof_n[comp]).max()
+        assert np.abs(qt[comp] - ct.reshape(bshape)).max() < 1e-11 * scale
+        assert np.abs(qhn[comp] - chalf.reshape(bshape)).max() < 1e-11 * np.abs(chalf).max()
+        # the case discriminates: each plausible slip in Eqs. 30-32 moves c~ by much more than the tolerance
+        rho = rho_l * C + rho_g * (1 - C); mu = mu_l * C + mu_g * (1 - C)
+        for bad in (np.minimum(kmax, kabs) + mu, rho * kabs + mu, rho * np.minimum(2 * kmax, kabs) + mu,
+                    rho * np.minimum(kmax, kabs), rho * np.minimum(kmax, kabs) + mu_l):
+            kp = np.pad(bad, 1, mode="edge"); cp = np.pad(prof[comp], 1, mode="edge")
+            diff = (0.5 * (bad + kp[:-2]) * (prof[comp] - cp[:-2]) + 0.5 * (bad + kp[2:]) * (prof[comp] - cp[2:])) / (h * h)
+            adv = prof[along] * (cp[2:] - cp[:-2]) / (2 * h)
+            wrong = prof_n[comp] - dt * (rho * adv + diff) / rho
+            assert comp == along or np.abs(wrong - ct).max() > 1e-4 * scale
+
+
 # ---------------------------------------------------------------- pressure RHS and projection (C10)
 def test_pressure_rhs_linear_velocity(orc):
     n, h, dt = 10, 0.1, 0.02
