@@ -51,6 +51,8 @@ enum { MODE_SWEEP = 0, MODE_PRO = 1, MODE_RR = 2, MODE_SEED = 3 };
 struct LParams {
     int nx, ny, nz;
     int zchunk;                 // output planes per block (even)
+    int dir;                    // +1: blocks march towards larger z, -1: towards smaller z (one-stage launches; the host alternates it
+                                // between consecutive passes so that a pass starts on the planes its predecessor left in L2)
     float sx0, sx1, sy0, sy1, sz0, sz1;
     float cc, icc;              // 1/(24 h^2) and its inverse
     float omega;
@@ -80,7 +82,8 @@ struct LCfg {
     static constexpr int PLANE = ((PX * PY + 31) / 32) * 32;              // floats per staged x / k plane (128-byte multiple)
     static constexpr int BPLANE = ((TX * TY + 31) / 32) * 32;             // floats per staged b tile
     static constexpr int CPX = TX / 2 + 8, CPY = TY / 2 + 2;              // PRO: staged tile of the coarse correction
-    static constexpr int CPLANE = MODE == 1 ? ((CPX * CPY + 31) / 32) * 32 : 0;
+    static constexpr int CPLANE_PRO = ((CPX * CPY + 31) / 32) * 32;
+    static constexpr int CPLANE = MODE == 1 ? CPLANE_PRO : 0;
     static constexpr int SLOT = PLANE * (VAR ? 2 : 1) + BPLANE + CPLANE;  // floats per ring slot: x, (k,) b, (x_c)
     static constexpr uint32_t CBOX_BYTES = (uint32_t)(CPX * CPY * sizeof(float));
     static constexpr uint32_t BOX_BYTES = (uint32_t)(PX * PY * sizeof(float));
@@ -179,13 +182,42 @@ __device__ __forceinline__ void out_row(const RT& a, const RT& m, const RT& c, u
     Bout[0] = ppp; Bout[1] = ppq;
 }
 
-template <class C>
-__global__ void __launch_bounds__(C::NT, C::MINB)
-lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmk,
-            const __grid_constant__ CUtensorMap tmb, const __grid_constant__ CUtensorMap tmc, const LParams P) {
-    constexpr int RY = C::RY, PX = C::PX, PY = C::PY, PLANE = C::PLANE, NS = C::NS, LX = C::LX, SLOT = C::SLOT;
+// ---- wave scheduling (wave_kernel.cuh): several dependent stages of one level in ONE launch -------------------------
+// A block of stage s + 1 reads the planes that the blocks of stage s (its own tile and the 8 tiles around it) have already
+// written; the intermediate iterate travels through L2, not HBM.  Each block publishes in `my_prog` how many planes of
+// its z chunk are complete and visible; a consumer polls the flags of its producers before it asks TMA for a plane.
+// Chunks march in alternating directions (even chunks upwards, odd ones downwards) so that the two chunks that meet at a
+// boundary both start or both end there: the halo plane a consumer needs from the neighbouring chunk is produced at the
+// same point of the march as its own, and an output plane is only overwritten (the iterate ping-pongs between two
+// buffers) after every block that reads its old contents has moved past it.  Producers always have lower block indices
+// than their consumers and blocks are dispatched in index order, so a waiting block never keeps its producer off the SMs.
+struct WaveCtx {
+    int dir;               // +1: the chunk marches towards larger z, -1: towards smaller z
+    int tx, ty, chunk;     // this block's tile and z chunk
+    int gx, gy, nch;       // tiles and chunks of the level
+    int zchunk;            // planes per chunk (the last chunk may be shorter)
+    int* my_prog;          // this block's progress flag (nullptr: nobody waits for this stage)
+    const int* dep_prog;   // progress flags [nch][gy][gx] of the stage that produces this stage's iterate (nullptr: none)
+    int* err;              // set to 1 if a wait timed out (the result is then garbage, but the kernel ends)
+    long long* prof;       // scratch instrumentation (nullptr in production): per block {t0, t1, wait ns, publish ns, polls, waits}
+};
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+    int v; asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <class C, int MODE, bool WAVE>
+__device__ __forceinline__ void lean_body(const CUtensorMap& tmx, const CUtensorMap& tmk, const CUtensorMap& tmb,
+                                          const CUtensorMap& tmc, const LParams& P, const int bx, const int by, const int bz,
+                                          const WaveCtx& wc) {
+    constexpr int RY = C::RY, PX = C::PX, PY = C::PY, PLANE = C::PLANE, NS = C::NS, LX = C::LX;
     constexpr bool VAR = C::VAR;
-    constexpr int MODE = C::MODE;
+    constexpr int CPLANE = MODE == MODE_PRO ? C::CPLANE_PRO : 0;
+    constexpr int SLOT = PLANE * (VAR ? 2 : 1) + C::BPLANE + CPLANE;
     constexpr int KOFF = PLANE, BOFF = PLANE * (VAR ? 2 : 1);      // k and b inside a ring slot
     constexpr int COFF = BOFF + C::BPLANE;                         // PRO: coarse tile
     static_assert(RY == 2, "2 output rows per thread");
@@ -196,9 +228,12 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
 
     const int tid = threadIdx.x, lx = tid % LX, ly = tid / LX;
     const int nx = P.nx, ny = P.ny, nz = P.nz;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int zc0 = blockIdx.z * P.zchunk, zc1 = min(zc0 + P.zchunk, nz);
-    const int pbeg = zc0 - 1, niter = zc1 - zc0 + 2;               // even: zchunk and nz are even
+    const int x0 = bx * C::TX, y0 = by * C::TY;
+    const int zc0 = bz * P.zchunk, zc1 = min(zc0 + P.zchunk, nz);
+    const int niter = zc1 - zc0 + 2;                               // even: zchunk and nz are even
+    // iteration `it` stages plane pfirst + dir * it and finalises the plane staged one iteration earlier
+    const int dir = WAVE ? wc.dir : P.dir;
+    const int pfirst = dir > 0 ? zc0 - 1 : zc1;
     const int c0 = 4 * lx, gi0 = x0 + c0, gj0 = y0 + RY * ly;
     const bool active = gi0 < nx && gj0 < ny;
 
@@ -235,14 +270,61 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
     auto issue = [&](int it) {   // one thread: TMA of the x, k planes of iteration `it` and of the b tile it finalises
         uint64_t* bar = &bars[it % NS];
         float* dst = ring + (it % NS) * SLOT;
-        const bool wb = it >= 2 && MODE != MODE_SEED;              // plane pbeg + it - 1 >= zc0
+        const bool wb = it >= 2 && MODE != MODE_SEED;              // the plane finalised in iteration `it` lies in the chunk
         const bool zx = MODE == MODE_SWEEP && P.zero_x;            // x planes stay the zeros written below
         mbar_expect_tx(bar, C::BOX_BYTES * ((VAR ? 1u : 0u) + (zx ? 0u : 1u)) + (wb ? C::BBOX_BYTES : 0u) + (MODE == MODE_PRO ? C::CBOX_BYTES : 0u));
-        const int z = zsrc(pbeg + it);
+        const int z = zsrc(pfirst + dir * it);
         if (!zx) tma_load_plane(dst, &tmx, bar, x0 - 4, y0 - 1, z);
         if (VAR) tma_load_plane(dst + KOFF, &tmk, bar, x0 - 4, y0 - 1, z);
-        if (wb) tma_load_plane(dst + BOFF, &tmb, bar, x0, y0, pbeg + it - 1);
+        if (wb) tma_load_plane(dst + BOFF, &tmb, bar, x0, y0, pfirst + dir * (it - 1));
         if (MODE == MODE_PRO) tma_load_plane(dst + COFF, &tmc, bar, (x0 >> 1) - 4, (y0 >> 1) - 1, z >> 1);
+    };
+    // ---- wave scheduling: wait until the producers of this stage's iterate have written the plane of iteration `it` ----
+    // (warp 0, converged).  `known` caches the progress of the producers in this block's own chunk.
+    int known = 0;
+    auto wait_dep = [&](int it) {
+        if (!WAVE || wc.dep_prog == nullptr) return;
+        // the plane of iteration `it` in march order: position it - 1 of this chunk; position -1 is the last-but-first plane
+        // of the chunk behind the start, position len the plane beyond the end -- both lie in a neighbouring chunk that
+        // marches the other way (or are ghost planes: the mirrored plane is this chunk's own first / last plane)
+        const int len = zc1 - zc0;
+        int c = wc.chunk, need = it;                                // own chunk: positions 0 .. it - 1 complete
+        if (it == 0) {
+            const int cn = wc.chunk - dir;                          // chunk behind the start; it starts at the same boundary
+            if (cn >= 0 && cn < wc.nch) { c = cn; need = 1; } else need = 1;
+        } else if (it == len + 1) {
+            const int cn = wc.chunk + dir;                          // chunk beyond the end; it ends at the same boundary
+            if (cn >= 0 && cn < wc.nch) { c = cn; need = min(wc.zchunk, nz - cn * wc.zchunk); } else need = len;
+        }
+        if (c == wc.chunk && known >= need) return;
+        const int lane = tid & 31;
+        const long long tw0 = (WAVE && wc.prof) ? gtime() : 0;
+        const int ddx = lane % 3 - 1, ddy = (lane / 3) % 3 - 1;
+        const int ux = wc.tx + ddx, uy = wc.ty + ddy;
+        const bool valid = lane < 9 && ux >= 0 && ux < wc.gx && uy >= 0 && uy < wc.gy;
+        const int* fp = wc.dep_prog + ((size_t)c * wc.gy + (valid ? uy : wc.ty)) * wc.gx + (valid ? ux : wc.tx);
+        int m = 0;
+        for (long long spin = 0;; ++spin) {
+            const int v = valid ? ld_acquire_gpu(fp) : 0x7fffffff;
+            m = __reduce_min_sync(0xffffffffu, v);
+            if (WAVE && wc.prof && lane == 0) wc.prof[4] += 1;
+            if (m >= need) break;
+            if (spin > (1ll << 22)) { if (lane == 0) atomicExch(wc.err, 1); break; }   // ~ seconds: give up, flag the error
+            __nanosleep(64);
+        }
+        __syncwarp();
+        if (c == wc.chunk) known = m;
+        if (WAVE && wc.prof && lane == 0) { wc.prof[2] += gtime() - tw0; wc.prof[5] += 1; }
+    };
+    // publish: `count` planes of this chunk are complete (called by thread 0 after a block barrier that follows their stores)
+    auto publish = [&](int count) {
+        if (!WAVE || wc.my_prog == nullptr) return;
+        // the consumers read these planes through TMA (async proxy); the release makes the block's stores (ordered before
+        // this thread by the block barrier) visible at gpu scope before the flag
+        const long long tp0 = wc.prof ? gtime() : 0;
+        asm volatile("fence.proxy.async.global;" ::: "memory");
+        st_release_gpu(wc.my_prog, count);
+        if (wc.prof) wc.prof[3] += gtime() - tp0;
     };
 
     if (tid == 0) {
@@ -260,7 +342,17 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
     // kernel of the cycle are first read below.  The next kernel may begin its own prologue from here on.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (tid == 0)
+    if (WAVE && wc.prof && tid == 0) wc.prof[0] = gtime();
+    if (WAVE) {
+        if (tid < 32)
+            for (int q = 0; q < NS && q < niter; ++q) {
+                wait_dep(q);
+                if (tid == 0) {
+                    if (wc.dep_prog) asm volatile("fence.proxy.async.global;" ::: "memory");
+                    issue(q);
+                }
+            }
+    } else if (tid == 0)
         for (int q = 0; q < NS && q < niter; ++q) issue(q);
 
     // ---- per-point state carried along z ---------------------------------------------------------
@@ -283,11 +375,26 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
     // one plane: PAR = parity of the iteration index
     auto body = [&](auto par_tag, const int it) {
         constexpr int PAR = decltype(par_tag)::value;
-        const int p = pbeg + it;
+        const int p = pfirst + dir * it;
         const int slot = it & (NS - 1);
         // ---- ring hand-back: everyone has finished iteration it - 1, so its slot can be refilled ----
         __syncthreads();
-        if (tid == 0 && it >= 1 && it - 1 + NS < niter) {
+        if (WAVE) {
+            if (tid < 32) {
+                if (it >= 1 && it - 1 + NS < niter) {
+                    wait_dep(it - 1 + NS);
+                    if (tid == 0) {
+                        // slot reuse: generic reads of the slot before the TMA write; and the producers' stores (acquired in
+                        // wait_dep) before the TMA read of global memory.  (A plain fence.proxy.async is a full MEMBAR.GPU.)
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        if (wc.dep_prog) asm volatile("fence.proxy.async.global;" ::: "memory");
+                        issue(it - 1 + NS);
+                    }
+                }
+                // iterations <= it - 1 are complete: they finalised the chunk positions 0 .. it - 3
+                if (tid == 0 && PAR == 0 && it >= 4) publish(it - 2);
+            }
+        } else if (tid == 0 && it >= 1 && it - 1 + NS < niter) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             issue(it - 1 + NS);
         }
@@ -353,7 +460,7 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         }
 
         // ---- finalise plane p - 1 ----
-        const int qc = p - 1;
+        const int qc = p - dir;
         if (it >= 2) {
             const u64 icc2 = bc2(P.icc), cc2 = bc2(P.cc), om12 = bc2(MODE == MODE_SEED ? P.om_x : 1.f - omega);
             const float om_g = MODE == MODE_SEED ? P.om_g : omega;
@@ -388,7 +495,7 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
                     *reinterpret_cast<ulonglong2*>(P.out + ((size_t)qc * ny + (gj0 + j)) * nx + gi0) = make_ulonglong2(o[0], o[1]);
             }
             if (MODE == MODE_RR) {
-                if (PAR == 0) {     // qc = zc0 + it - 2 with zc0 even: PAR 0 <=> qc even
+                if (PAR == 0) {     // first plane of a pair {2m, 2m + 1} in march order (zc0, zc1 are even)
                     hold0 = rs0; hold1 = rs1;
                 } else if (active) {
                     const size_t ci = ((size_t)(qc >> 1) * nyc + (gj0 >> 1)) * nxc + (gi0 >> 1);
@@ -413,6 +520,19 @@ lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUt
         body(std::integral_constant<int, 0>{}, it);
         body(std::integral_constant<int, 1>{}, it + 1);
     }
+    if (WAVE && wc.my_prog != nullptr) {     // the whole chunk is complete
+        __syncthreads();
+        if (tid == 0) publish(zc1 - zc0);
+    }
+    if (WAVE && wc.prof && tid == 0) wc.prof[1] = gtime();
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::NT, C::MINB)
+lean_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmk,
+            const __grid_constant__ CUtensorMap tmb, const __grid_constant__ CUtensorMap tmc, const LParams P) {
+    const WaveCtx none = {};
+    lean_body<C, C::MODE, false>(tmx, tmk, tmb, tmc, P, blockIdx.x, blockIdx.y, blockIdx.z, none);
 }
 
 }  // namespace lk

@@ -407,9 +407,13 @@ void mg_destroy(mg_solver* s) {
 
 int mg_set_params(mg_solver* s, const mg_params* p) {
     CHECK_SOLVER(s);
-    if (!p || p->nu_pre < 0 || p->nu_post < 0 || p->coarse_sweeps < 0 || p->sweeps_per_pass < 1 || !(p->omega > 0.0) ||
-        !(p->omega < 2.0)) {
+    if (!p || p->nu_pre < 0 || p->nu_post < 0 || p->coarse_sweeps < 0 || !(p->omega > 0.0) || !(p->omega < 2.0)) {
         set_error("mg_set_params: invalid parameters");
+        return MG_EINVAL;
+    }
+    // stages per launch of the wave kernel (wave_kernel.cuh): 1 .. 4 are implemented; anything else is refused
+    if (p->sweeps_per_pass < 1 || p->sweeps_per_pass > 4) {
+        set_error("mg_set_params: sweeps_per_pass = %d is not implemented (1 .. 4)", p->sweeps_per_pass);
         return MG_EINVAL;
     }
     s->p = *p;

@@ -1,21 +1,21 @@
-// mg_fused.cu -- host side of the tuned fp32 path: pass planning for the fused smoother /
-// transfer kernel (fused_kernel.cuh), TMA descriptors, the single-CTA coarse tail, and CUDA-graph
-// replay of the whole V-cycle (north_star "fused" kernels).
+// mg_fused.cu -- host side of the tuned fp32 path: pass planning for the streaming smoother / transfer kernel
+// (lean_kernel.cuh: one stage per launch; wave_kernel.cuh: up to `sweeps_per_pass` dependent stages per launch), TMA
+// descriptors, the cluster / single-block coarse tail (ctail_kernel.cuh, tail_kernel.cuh), and CUDA-graph replay of the
+// whole V-cycle (north_star "fused" kernels).
 #include <algorithm>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 #include "fused.h"
-#include "fused_kernel.cuh"
 #include "solver.h"
 #include "lean_kernel.cuh"
+#include "wave_kernel.cuh"
 #include "ctail_kernel.cuh"
 #include "tail_kernel.cuh"
 
 namespace mgb {
 namespace {
-
-using fk::FParams;
 
 // ---- TMA descriptor encoding through the driver entry point (no link-time libcuda dependency) ----
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -97,143 +97,112 @@ __global__ void dinv_kernel(int nx, int ny, int nz, float ce, float cc, float cd
 }
 
 struct LevelPlan {
-    bool tiled = false;       // handled by fused_kernel
-    bool stream = false;      // handled by stream_kernel
+    bool stream = false;      // handled by lean_kernel / wave_kernel
     float* dinv = nullptr;    // 1/D (variable k), levels >= 1
-    float* tmp2 = nullptr;    // residual scratch of non-tiled levels
+    float* tmp2 = nullptr;    // residual scratch of levels the streaming kernels do not cover
     float ce = 0, cc = 0, cdiag = 0, w0 = 0;
+    long long passes = 0;     // one-stage launches issued on this level (parity = march direction of the next one)
 };
 
 struct FusedState {
     std::vector<LevelPlan> lp;
-    bool attrs_set = false;
-    bool zero_x_once = false; // the next SWEEP launch takes its input iterate as zero (zero-guess cycles)
+    int sm_count = 148;       // multiprocessors of the solver's device
     float* cmat = nullptr;    // the coarsest solve tabulated as a matrix (ctail_kernel.cuh), n_c <= 64
     bool cmat_valid = false;
+    int* wave_sync = nullptr; // wave_kernel: progress flags [WAVE_FLAGS], then the finished-block counter and the error word
 };
+constexpr int WAVE_FLAGS = 8192;
 
-constexpr int TXD = 56, TYD = 28;   // + halo = 64 x 32 cells per plane, 16 x 16 threads
-
-template <int NS, bool RR, bool PRO, bool VAR>
-int launch_cfg(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
-               float* xc_out, int first_sweep) {
-    using C = fk::Cfg<NS, RR, PRO, VAR, TXD, TYD>;
-    FusedState* fs = (FusedState*)s->fused_state;
-    LevelData& L = s->lv[l];
-    const LevelPlan& lp = fs->lp[l];
-    static bool attr_done = false;
-    if (!attr_done) {
-        MGB_CUDA(cudaFuncSetAttribute(fk::fused_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        attr_done = true;
-    }
-    CUtensorMap tmx, tmk, tmb;
-    int rc;
-    if ((rc = make_tmap(&tmx, src, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
-    if ((rc = make_tmap(&tmb, b, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
-    if (VAR) { if ((rc = make_tmap(&tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
-    else tmk = tmx;
-    FParams P;
-    std::memset(&P, 0, sizeof(P));
-    P.nx = L.nx; P.ny = L.ny; P.nz = L.nz;
-    const int tiles = ((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
-    // z chunking: minimise (waves over 148 SMs) x (planes per block incl. pipeline fill)
-    int best_chunks = 1; double best_cost = 1e30;
-    for (int nch = 1; nch <= std::max(1, L.nz / 2); ++nch) {
-        int zc = (L.nz + nch - 1) / nch; zc += zc & 1;
-        const int real = (L.nz + zc - 1) / zc;
-        const double waves = std::ceil((double)tiles * real / 148.0);
-        const double cost = waves * (zc + 2 * C::NST + 3);
-        if (cost < best_cost - 1e-9) { best_cost = cost; best_chunks = real; P.zchunk = zc; }
-    }
-    (void)best_chunks;
-    const int nchunks = (L.nz + P.zchunk - 1) / P.zchunk;
-    P.sx0 = L.Lf.s[0]; P.sx1 = L.Lf.s[1]; P.sy0 = L.Lf.s[2]; P.sy1 = L.Lf.s[3]; P.sz0 = L.Lf.s[4]; P.sz1 = L.Lf.s[5];
-    P.any_s0 = 0;
-    for (int f = 0; f < 6; ++f) if (L.Lf.s[f] == 0.f) P.any_s0 = 1;
-    P.ce = lp.ce; P.cc = lp.cc; P.cdiag = lp.cdiag; P.w0 = lp.w0;
-    P.omega = (float)s->p.omega;
-    P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
-    if (RR) {
-        const LevelPlan& cp = fs->lp[l + 1];
-        P.dinv_c = cp.dinv;
-        P.gc_const = first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
-    }
-    dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
-    fk::fused_kernel<C><<<grid, C::NT, C::SMEM, s->st>>>(tmx, tmk, tmb, P);
-    MGB_LAUNCH_CHECK();
-    ++s->launches;
+// One-time per-(device, kernel) set-up: opt-in to > 48 KB of dynamic shared memory and the resident blocks per SM.
+// cudaFuncSetAttribute and the occupancy query apply to the CURRENT device, so the cache is keyed by it.
+struct KernelSetup { int device; const void* fn; int ctas_per_sm; };
+int kernel_setup(int device, const void* fn, int threads, size_t smem, int* ctas_per_sm) {
+    static std::mutex mu;
+    static std::vector<KernelSetup> done;
+    std::lock_guard<std::mutex> lock(mu);
+    for (const KernelSetup& k : done)
+        if (k.device == device && k.fn == fn) { if (ctas_per_sm) *ctas_per_sm = k.ctas_per_sm; return 0; }
+    MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    int nb = 0;
+    MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, threads, smem));
+    done.push_back({device, fn, nb > 0 ? nb : 1});
+    if (ctas_per_sm) *ctas_per_sm = done.back().ctas_per_sm;
     return 0;
 }
 
-// dispatch on (NS, RR, PRO, VAR)
-int launch_pass(mg_solver* s, int l, int NS, bool rr, bool pro, const float* src, const float* b, float* dst,
-                const float* xc = nullptr, float* bc_out = nullptr, float* xc_out = nullptr, int first_sweep = 0) {
-    const bool var = s->var_k;
-#define MGB_CASE(ns, r, p)                                                                                          \
-    if (NS == ns && rr == r && pro == p)                                                                            \
-        return var ? launch_cfg<ns, r, p, true>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep)                 \
-                   : launch_cfg<ns, r, p, false>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
-    MGB_CASE(1, false, false)
-    MGB_CASE(2, false, false)
-    MGB_CASE(1, false, true)
-    MGB_CASE(2, false, true)
-    MGB_CASE(0, true, false)
-    MGB_CASE(1, true, false)
-#undef MGB_CASE
-    set_error("fused pass (%d sweeps, rr=%d, pro=%d) is not instantiated", NS, (int)rr, (int)pro);
-    return MG_EINVAL;
-}
+// One stage of a pass on level l: what it reads and writes besides the iterate.
+struct StageSpec {
+    int mode = lk::MODE_SWEEP;
+    const float* xc = nullptr;      // PRO: coarse correction
+    float* bc_out = nullptr;        // RR: restricted residual
+    float* xc_out = nullptr;        // RR: the coarse level's first sweep (or zeros)
+    int first_sweep = 0;            // RR
+    int zero_x = 0;                 // SWEEP: the incoming iterate is zero whatever the buffer holds
+};
 
-// ---- single-stage streaming kernel (stream_kernel.cuh) -----------------------------------------
-template <int LX, int LY, int MINB, bool VAR, int MODE>
-int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
-                      float* xc_out, int first_sweep) {
-    using C = lk::LCfg<LX, LY, VAR, MODE, MINB>;
+// tensor maps and parameters of one stage (shared by the one-stage and the wave launches)
+template <class C>
+int fill_stage(mg_solver* s, int l, const StageSpec& sp, const float* src, const float* b, float* dst, int zchunk,
+               CUtensorMap* tmx, CUtensorMap* tmk, CUtensorMap* tmb, CUtensorMap* tmc, lk::LParams* Pout) {
     FusedState* fs = (FusedState*)s->fused_state;
     LevelData& L = s->lv[l];
     const LevelPlan& lp = fs->lp[l];
-    static int ctas_per_sm = 0;
-    if (!ctas_per_sm) {
-        MGB_CUDA(cudaFuncSetAttribute(lk::lean_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        MGB_CUDA(cudaFuncSetAttribute(lk::lean_kernel<C>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        int nb = 0;
-        MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, lk::lean_kernel<C>, C::NT, C::SMEM));
-        ctas_per_sm = nb > 0 ? nb : 1;
-    }
-    CUtensorMap tmx, tmk, tmb, tmc;
     int rc;
-    if ((rc = make_tmap(&tmx, src, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
-    if ((rc = make_tmap(&tmb, b, L.nx, L.ny, L.nz, C::TX, C::TY))) return rc;
-    if (VAR) { if ((rc = make_tmap(&tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
-    else tmk = tmx;
-    if (MODE == lk::MODE_PRO) { if ((rc = make_tmap(&tmc, xc, L.nx / 2, L.ny / 2, L.nz / 2, C::CPX, C::CPY))) return rc; }
-    else tmc = tmx;
+    if ((rc = make_tmap(tmx, src, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
+    if ((rc = make_tmap(tmb, b, L.nx, L.ny, L.nz, C::TX, C::TY))) return rc;
+    if (C::VAR) { if ((rc = make_tmap(tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
+    else *tmk = *tmx;
+    if (sp.mode == lk::MODE_PRO) { if ((rc = make_tmap(tmc, sp.xc, L.nx / 2, L.ny / 2, L.nz / 2, C::CPX, C::CPY))) return rc; }
+    else *tmc = *tmx;
     lk::LParams P;
     std::memset(&P, 0, sizeof(P));
     P.nx = L.nx; P.ny = L.ny; P.nz = L.nz;
+    P.zchunk = zchunk;
+    P.dir = 1;
+    P.sx0 = L.Lf.s[0]; P.sx1 = L.Lf.s[1]; P.sy0 = L.Lf.s[2]; P.sy1 = L.Lf.s[3]; P.sz0 = L.Lf.s[4]; P.sz1 = L.Lf.s[5];
+    P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
+    P.omega = (float)s->p.omega;
+    P.out = dst; P.xc = sp.xc; P.bc_out = sp.bc_out; P.xc_out = sp.xc_out; P.first_sweep = sp.first_sweep;
+    P.zero_x = (sp.mode == lk::MODE_SWEEP && sp.zero_x) ? 1 : 0;
+    if (sp.mode == lk::MODE_SEED) { P.om_g = P.omega * P.omega; P.om_x = P.omega * (2.f - P.omega); P.icc = 0.f; }
+    if (sp.mode == lk::MODE_RR) {
+        const LevelPlan& cp = fs->lp[l + 1];
+        P.dinv_c = cp.dinv;
+        P.gc_const = sp.first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
+    }
+    *Pout = P;
+    return 0;
+}
+
+// ---- one stage per launch (lean_kernel.cuh) ---------------------------------------------------------
+template <int LX, int LY, int MINB, bool VAR, int MODE>
+int launch_stream_cfg(mg_solver* s, int l, const StageSpec& sp, const float* src, const float* b, float* dst) {
+    using C = lk::LCfg<LX, LY, VAR, MODE, MINB>;
+    FusedState* fs = (FusedState*)s->fused_state;
+    LevelData& L = s->lv[l];
+    int ctas_per_sm = 1, rc;
+    if ((rc = kernel_setup(s->device, (const void*)lk::lean_kernel<C>, C::NT, C::SMEM, &ctas_per_sm))) return rc;
     const int tiles = ((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
     // z chunking: minimise (waves over the resident CTA slots) x (planes per block incl. the two halo planes)
     double best_cost = 1e30;
-    const int slots = 148 * ctas_per_sm;
+    int zchunk = L.nz;
+    const int slots = fs->sm_count * ctas_per_sm;
     for (int nch = 1; nch <= std::max(1, L.nz / 2); ++nch) {
         int zc = (L.nz + nch - 1) / nch; zc += zc & 1;
         const int real = (L.nz + zc - 1) / zc;
         const double waves = std::ceil((double)tiles * real / (double)slots);
         const double cost = waves * (zc + 2 + 2);
-        if (cost < best_cost - 1e-9) { best_cost = cost; P.zchunk = zc; }
+        if (cost < best_cost - 1e-9) { best_cost = cost; zchunk = zc; }
     }
-    const int nchunks = (L.nz + P.zchunk - 1) / P.zchunk;
-    P.sx0 = L.Lf.s[0]; P.sx1 = L.Lf.s[1]; P.sy0 = L.Lf.s[2]; P.sy1 = L.Lf.s[3]; P.sz0 = L.Lf.s[4]; P.sz1 = L.Lf.s[5];
-    P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
-    P.omega = (float)s->p.omega;
-    P.out = dst; P.xc = xc; P.bc_out = bc_out; P.xc_out = xc_out; P.first_sweep = first_sweep;
-    if (MODE == lk::MODE_SWEEP && fs->zero_x_once) { P.zero_x = 1; fs->zero_x_once = false; }
-    if (MODE == lk::MODE_SEED) { P.om_g = P.omega * P.omega; P.om_x = P.omega * (2.f - P.omega); P.icc = 0.f; }
-    if (MODE == lk::MODE_RR) {
-        const LevelPlan& cp = fs->lp[l + 1];
-        P.dinv_c = cp.dinv;
-        P.gc_const = first_sweep ? (float)(s->p.omega / cp.w0) : 0.f;
-    }
+    const int nchunks = (L.nz + zchunk - 1) / zchunk;
+    CUtensorMap tmx, tmk, tmb, tmc;
+    lk::LParams P;
+    if ((rc = fill_stage<C>(s, l, sp, src, b, dst, zchunk, &tmx, &tmk, &tmb, &tmc, &P))) return rc;
+    // serpentine: consecutive passes of a level march in opposite directions
+    static const bool serp = getenv("MG_NO_SERPENTINE") == nullptr;
+    if (serp) { P.dir = (fs->lp[l].passes & 1) ? -1 : 1; }
+    ++fs->lp[l].passes;
     dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
     MGB_CUDA(launch_pdl(lk::lean_kernel<C>, grid, dim3(C::NT), C::SMEM, s->st, tmx, tmk, tmb, tmc, P));
     ++s->launches;
@@ -241,46 +210,124 @@ int launch_stream_cfg(mg_solver* s, int l, const float* src, const float* b, flo
 }
 
 template <bool VAR, int MODE>
-int launch_stream_lx(mg_solver* s, int l, const float* src, const float* b, float* dst, const float* xc, float* bc_out,
-                     float* xc_out, int first_sweep) {
+int launch_stream_lx(mg_solver* s, int l, const StageSpec& sp, const float* src, const float* b, float* dst) {
     const int nx = s->lv[l].nx;
     // 128-thread blocks, 3 per SM: 168 registers per thread keep the per-point state and the staged rows out of local memory
-    if (nx >= 96) return launch_stream_cfg<32, 4, 3, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
-    if (nx >= 48) return launch_stream_cfg<16, 8, 3, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
-    return launch_stream_cfg<8, 16, 3, VAR, MODE>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+    if (nx >= 96) return launch_stream_cfg<32, 4, 3, VAR, MODE>(s, l, sp, src, b, dst);
+    if (nx >= 48) return launch_stream_cfg<16, 8, 3, VAR, MODE>(s, l, sp, src, b, dst);
+    return launch_stream_cfg<8, 16, 3, VAR, MODE>(s, l, sp, src, b, dst);
 }
 
-// one streaming pass on level l: mode = lk::MODE_*
-int launch_stream(mg_solver* s, int l, int mode, const float* src, const float* b, float* dst, const float* xc = nullptr,
-                  float* bc_out = nullptr, float* xc_out = nullptr, int first_sweep = 0) {
-#define MGB_SCASE(m)                                                                                             \
-    if (mode == m)                                                                                               \
-        return s->var_k ? launch_stream_lx<true, m>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep)          \
-                        : launch_stream_lx<false, m>(s, l, src, b, dst, xc, bc_out, xc_out, first_sweep);
+// one streaming pass on level l
+int launch_stream(mg_solver* s, int l, const StageSpec& sp, const float* src, const float* b, float* dst) {
+#define MGB_SCASE(m)                                                                       \
+    if (sp.mode == m)                                                                      \
+        return s->var_k ? launch_stream_lx<true, m>(s, l, sp, src, b, dst)                 \
+                        : launch_stream_lx<false, m>(s, l, sp, src, b, dst);
     MGB_SCASE(lk::MODE_SWEEP)
     MGB_SCASE(lk::MODE_PRO)
     MGB_SCASE(lk::MODE_RR)
     MGB_SCASE(lk::MODE_SEED)
 #undef MGB_SCASE
-    set_error("stream pass mode %d is not instantiated", mode);
+    set_error("stream pass mode %d is not instantiated", sp.mode);
     return MG_EINVAL;
+}
+
+// ---- several dependent stages per launch (wave_kernel.cuh) ------------------------------------------
+// Stages st[0 .. n) of level l in one launch; the iterate starts in `cur` and ping-pongs with `oth` (RR stages do not
+// write it).  Returns MG_ESHAPE-like "does not fit" as +1 so that the caller can fall back to fewer stages per launch.
+template <int LX, int LY, int MINB, bool VAR>
+int launch_wave_cfg(mg_solver* s, int l, const StageSpec* st, int n, float* cur, float* oth, const float* b) {
+    using C = lk::LCfg<LX, LY, VAR, lk::MODE_PRO, MINB>;
+    FusedState* fs = (FusedState*)s->fused_state;
+    LevelData& L = s->lv[l];
+    auto kern = wk::wave_kernel<LX, LY, VAR, MINB>;
+    int ctas_per_sm = 1, rc;
+    if ((rc = kernel_setup(s->device, (const void*)kern, C::NT, C::SMEM, &ctas_per_sm))) return rc;
+    const int gx = (L.nx + C::TX - 1) / C::TX, gy = (L.ny + C::TY - 1) / C::TY, tiles = gx * gy;
+    const int slots = fs->sm_count * ctas_per_sm;
+    // every block of every stage has to be resident at once for the stages to overlap: as many z chunks as fit
+    int nch = slots / (tiles * n);
+    if (nch < 1) return 1;
+    nch = std::min(nch, std::max(1, L.nz / 8));
+    int zchunk = (L.nz + nch - 1) / nch; zchunk += zchunk & 1;
+    nch = (L.nz + zchunk - 1) / zchunk;
+    if ((size_t)(n - 1) * nch * tiles > (size_t)WAVE_FLAGS) return 1;
+    wk::WParams W;
+    std::memset(&W, 0, sizeof(W));
+    W.nstages = n; W.nch = nch; W.gx = gx; W.gy = gy;
+    { const char* d = getenv("MG_WAVE_DEBUG"); W.debug = d ? atoi(d) : 0; }
+    if (getenv("MG_WAVE_PROF")) {      // scratch: 8 words per block, dumped by the caller through the pointer in the env var
+        static long long* prof = nullptr;
+        if (!prof) { cudaMalloc(&prof, 8 * 8 * 4096); FILE* f = fopen(getenv("MG_WAVE_PROF"), "w"); if (f) { fprintf(f, "%llu\n", (unsigned long long)prof); fclose(f); } }
+        cudaMemsetAsync(prof, 0, 8 * 8 * 4096, s->st);
+        W.prof = prof;
+    }
+    W.prog = fs->wave_sync; W.done = fs->wave_sync + WAVE_FLAGS; W.err = fs->wave_sync + WAVE_FLAGS + 1;
+    for (int i = 0; i < n; ++i) {
+        wk::WStage& S = W.st[i];
+        S.mode = st[i].mode;
+        const bool writes = st[i].mode != lk::MODE_RR;
+        if ((rc = fill_stage<C>(s, l, st[i], cur, b, writes ? oth : nullptr, zchunk, &S.tmx, &S.tmk, &S.tmb, &S.tmc, &S.P))) return rc;
+        if (writes) std::swap(cur, oth);
+    }
+    dim3 grid(gx, gy, nch * n);
+    MGB_CUDA(launch_pdl(kern, grid, dim3(C::NT), C::SMEM, s->st, W));
+    ++s->launches;
+    return 0;
+}
+
+int launch_wave(mg_solver* s, int l, const StageSpec* st, int n, float* cur, float* oth, const float* b) {
+    const int nx = s->lv[l].nx;
+#define MGB_WCASE(lx, ly)                                                                   \
+    return s->var_k ? launch_wave_cfg<lx, ly, 3, true>(s, l, st, n, cur, oth, b)            \
+                    : launch_wave_cfg<lx, ly, 3, false>(s, l, st, n, cur, oth, b);
+    if (nx >= 96) { MGB_WCASE(32, 4) }
+    if (nx >= 48) { MGB_WCASE(16, 8) }
+    MGB_WCASE(8, 16)
+#undef MGB_WCASE
+}
+
+// A chain of stages on a streaming level: groups of up to `sweeps_per_pass` stages per launch.  *res = the buffer that
+// holds the iterate afterwards.
+int run_chain(mg_solver* s, int l, float* cur, float* oth, const float* b, const StageSpec* st, int n, float** res) {
+    int i = 0;
+    while (i < n) {
+        int g = std::min(std::min(s->p.sweeps_per_pass, wk::MAXS), n - i);
+        int rc = 1;
+        const int gmin = (getenv("MG_WAVE_DEBUG") && (atoi(getenv("MG_WAVE_DEBUG")) & 4)) ? 1 : 2;
+        while (g >= gmin && (rc = launch_wave(s, l, st + i, g, cur, oth, b)) == 1) --g;     // 1: does not fit the machine
+        if (g >= gmin && rc) return rc;
+        if (g < gmin) {
+            g = 1;
+            const bool writes = st[i].mode != lk::MODE_RR;
+            if ((rc = launch_stream(s, l, st[i], cur, b, writes ? oth : nullptr))) return rc;
+        }
+        for (int q = i; q < i + g; ++q)
+            if (st[q].mode != lk::MODE_RR) std::swap(cur, oth);
+        i += g;
+    }
+    *res = cur;
+    return 0;
 }
 
 int ensure_state(mg_solver* s) {
     if (s->fused_state) return 0;
     FusedState* fs = new FusedState();
     fs->lp.resize(s->levels);
+    s->fused_state = fs;                  // owned by the solver from here on (fused_release frees partial state)
+    if (cudaDeviceGetAttribute(&fs->sm_count, cudaDevAttrMultiProcessorCount, s->device) != cudaSuccess || fs->sm_count < 1) fs->sm_count = 148;
     for (int l = 0; l < s->levels; ++l) {
         LevelData& L = s->lv[l];
         LevelPlan& lp = fs->lp[l];
         const double h2 = L.hx * L.hx;
         lp.ce = (float)(1.0 / (12.0 * h2)); lp.cc = (float)(1.0 / (24.0 * h2));
         lp.cdiag = (float)(4.0 / (3.0 * h2)); lp.w0 = (float)(8.0 / (3.0 * h2));
-        lp.tiled = (L.nx % 4 == 0) && (L.ny % 2 == 0) && (L.nz % 2 == 0) && L.nx >= 16 && L.ny >= 16 && L.nz >= 8;
         lp.stream = (L.nx % 4 == 0) && (L.ny % 2 == 0) && (L.nz % 2 == 0) && L.nx >= 8 && L.ny >= 4 && L.nz >= 2;
-        if (!lp.tiled && cudaMalloc(&lp.tmp2, L.n * sizeof(float)) != cudaSuccess) { set_error("fused: out of memory"); return MG_EALLOC; }
+        if (!lp.stream && cudaMalloc(&lp.tmp2, L.n * sizeof(float)) != cudaSuccess) { set_error("fused: out of memory"); return MG_EALLOC; }
     }
-    s->fused_state = fs;
+    if (cudaMalloc(&fs->wave_sync, (WAVE_FLAGS + 2) * sizeof(int)) != cudaSuccess) { set_error("fused: out of memory"); return MG_EALLOC; }
+    MGB_CUDA(cudaMemsetAsync(fs->wave_sync, 0, (WAVE_FLAGS + 2) * sizeof(int), s->st));
     return 0;
 }
 
@@ -305,38 +352,36 @@ inline void mark(mg_solver* s, int idx) {
 }
 
 // `sweeps` Jacobi sweeps on level l starting from `cur` (other buffer `oth`), optionally preceded by
-// x += P xc.  Returns the buffer holding the result through *res.
-int sweeps_level(mg_solver* s, int l, float* cur, float* oth, const float* b, int sweeps, const float* xc, float** res) {
+// x += P xc.  Returns the buffer holding the result through *res.  `zero_x`: the incoming iterate is zero whatever
+// `cur` holds (streaming levels with sweeps >= 1 only; the caller checks).
+int sweeps_level(mg_solver* s, int l, float* cur, float* oth, const float* b, int sweeps, const float* xc, float** res,
+                 int zero_x = 0) {
     FusedState* fs = (FusedState*)s->fused_state;
     LevelData& L = s->lv[l];
     int rc;
-    const bool stream = fs->lp[l].stream && s->p.sweeps_per_pass == 1;
-    if (stream || fs->lp[l].tiled) {
+    if (fs->lp[l].stream) {
         bool pro = xc != nullptr;
         // the PRO pass stages x_c by TMA: its row pitch (nx / 2 floats) must be a multiple of 16 bytes
-        if (pro && (sweeps == 0 || (stream && (L.nx / 2) % 4 != 0))) {
+        if (pro && (sweeps == 0 || (L.nx / 2) % 4 != 0)) {
             if ((rc = launch_prolong_add<float>(L.nx, L.ny, L.nz, xc, cur, s->st))) return rc;
             ++s->launches;
             pro = false;
         }
-        while (sweeps > 0) {
-            const int ns = (!stream && sweeps >= 2) ? 2 : 1;
-            if (stream) rc = launch_stream(s, l, pro ? lk::MODE_PRO : lk::MODE_SWEEP, cur, b, oth, pro ? xc : nullptr);
-            else rc = launch_pass(s, l, ns, false, pro, cur, b, oth, pro ? xc : nullptr);
-            if (rc) return rc;
-            std::swap(cur, oth);
-            sweeps -= ns; pro = false;
+        std::vector<StageSpec> st((size_t)sweeps);
+        if (sweeps > 0) {
+            if (pro) { st[0].mode = lk::MODE_PRO; st[0].xc = xc; }
+            st[0].zero_x = zero_x;
         }
-    } else {
-        if (xc) {
-            if ((rc = launch_prolong_add<float>(L.nx, L.ny, L.nz, xc, cur, s->st))) return rc;
-            ++s->launches;
-        }
-        for (int it = 0; it < sweeps; ++it) {
-            if ((rc = launch_jacobi<float>(L.Lf, (const float*)L.k, cur, b, oth, s->st))) return rc;
-            ++s->launches;
-            std::swap(cur, oth);
-        }
+        return run_chain(s, l, cur, oth, b, st.data(), sweeps, res);
+    }
+    if (xc) {
+        if ((rc = launch_prolong_add<float>(L.nx, L.ny, L.nz, xc, cur, s->st))) return rc;
+        ++s->launches;
+    }
+    for (int it = 0; it < sweeps; ++it) {
+        if ((rc = launch_jacobi<float>(L.Lf, (const float*)L.k, cur, b, oth, s->st))) return rc;
+        ++s->launches;
+        std::swap(cur, oth);
     }
     *res = cur;
     return 0;
@@ -370,11 +415,7 @@ int launch_tail(mg_solver* s, int l, float* x, const float* b, int done, size_t 
     P.omega = (float)s->p.omega;
     P.nu_pre = s->p.nu_pre; P.nu_post = s->p.nu_post; P.coarse_sweeps = s->p.coarse_sweeps;
     P.first_done = done; P.x = x; P.b = b;
-    static bool attr_done = false;
-    if (!attr_done) {
-        MGB_CUDA(cudaFuncSetAttribute(tk::tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
-    }
+    { int rc = kernel_setup(s->device, (const void*)tk::tail_kernel, tk::NT, 200 * 1024, nullptr); if (rc) return rc; }
     MGB_CUDA(launch_pdl(tk::tail_kernel, dim3(1), dim3(tk::NT), smem, s->st, P));
     ++s->launches;
     return 0;
@@ -473,11 +514,7 @@ int launch_ctail(mg_solver* s, int l, float* x, const float* b, int done, size_t
     P.nu_pre = s->p.nu_pre; P.nu_post = s->p.nu_post; P.coarse_sweeps = s->p.coarse_sweeps;
     P.first_done = done; P.x = x; P.b = b;
     P.cmat = fs->cmat_valid ? fs->cmat : nullptr;
-    static bool attr_done = false;
-    if (!attr_done) {
-        MGB_CUDA(cudaFuncSetAttribute(ck::ctail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
-    }
+    { int rc = kernel_setup(s->device, (const void*)ck::ctail_kernel, ck::NT, 200 * 1024, nullptr); if (rc) return rc; }
     MGB_CUDA(launch_pdl(ck::ctail_kernel, dim3(ck::NC), dim3(ck::NT), smem, s->st, P));
     ++s->launches;
     return 0;
@@ -485,7 +522,9 @@ int launch_ctail(mg_solver* s, int l, float* x, const float* b, int done, size_t
 
 // Level l of the V-cycle.  `A` holds the incoming iterate (for l > 0 the parent's fused first sweep
 // has already been applied when `done` = 1); the final iterate of the level is returned in *res.
-int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int done, float** res) {
+// Level 0 only: `zero_x` = the incoming iterate is zero whatever A holds; `seed` = A holds the Jacobi seed y = b / D and the
+// first stage turns it into the iterate after two sweeps (then `done` = 2).
+int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int done, float** res, int zero_x = 0, int seed = 0) {
     FusedState* fs = (FusedState*)s->fused_state;
     LevelData& L = s->lv[l];
     int rc;
@@ -509,17 +548,16 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
     const bool child_coarsest = (l + 1 == s->levels - 1);
     const int first = child_coarsest ? (s->p.coarse_sweeps >= 1) : (s->p.nu_pre >= 1);
     float *cur = A, *oth = B;
-    int rem = std::max(0, s->p.nu_pre - done);
-    if (fs->lp[l].stream && s->p.sweeps_per_pass == 1) {
-        if ((rc = sweeps_level(s, l, cur, oth, b, rem, nullptr, &cur))) return rc;
+    const int rem = std::max(0, s->p.nu_pre - done);
+    if (fs->lp[l].stream) {
+        // down leg: [SEED] + pre-smoothing sweeps + residual / restriction / coarse first sweep, as one chain of stages
+        std::vector<StageSpec> st;
+        if (seed) { StageSpec sp; sp.mode = lk::MODE_SEED; st.push_back(sp); }
+        for (int q = 0; q < rem; ++q) { StageSpec sp; sp.zero_x = (q == 0 && zero_x); st.push_back(sp); }
+        StageSpec rr; rr.mode = lk::MODE_RR; rr.bc_out = (float*)C.b; rr.xc_out = (float*)C.x; rr.first_sweep = first;
+        st.push_back(rr);
+        if ((rc = run_chain(s, l, cur, oth, b, st.data(), (int)st.size(), &cur))) return rc;
         oth = (cur == A) ? B : A;
-        if ((rc = launch_stream(s, l, lk::MODE_RR, cur, b, nullptr, nullptr, (float*)C.b, (float*)C.x, first))) return rc;
-    } else if (fs->lp[l].tiled) {
-        const int tail = rem & 1;                       // sweeps fused with the residual + restriction pass
-        if ((rc = sweeps_level(s, l, cur, oth, b, rem - tail, nullptr, &cur))) return rc;
-        oth = (cur == A) ? B : A;
-        if ((rc = launch_pass(s, l, tail, true, false, cur, b, tail ? oth : nullptr, nullptr, (float*)C.b, (float*)C.x, first))) return rc;
-        if (tail) std::swap(cur, oth);
     } else {
         if ((rc = sweeps_level(s, l, cur, oth, b, rem, nullptr, &cur))) return rc;
         oth = (cur == A) ? B : A;
@@ -550,19 +588,10 @@ int cycle_level(mg_solver* s, int l, float* A, float* B, const float* b, int don
 // (written by the defect kernel); the first pass turns it into the iterate after TWO sweeps,
 // x_2 = omega (2 - omega) y - omega^2 D^-1 (A - D) y, without reading b: one 12-byte pass instead of two sweeps.
 int enqueue_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
-    FusedState* fs = (FusedState*)s->fused_state;
     float* res = nullptr;
     float *A = x, *B = (float*)s->lv[0].tmp;
-    int done = 0, rc;
-    if (zero_guess == 2) {
-        if ((rc = launch_stream(s, 0, lk::MODE_SEED, x, b, B))) return rc;
-        std::swap(A, B);
-        done = 2;
-    }
-    fs->zero_x_once = zero_guess == 1;
-    rc = cycle_level(s, 0, A, B, b, done, &res);
-    fs->zero_x_once = false;
-    if (rc) return rc;
+    int rc;
+    if ((rc = cycle_level(s, 0, A, B, b, zero_guess == 2 ? 2 : 0, &res, zero_guess == 1, zero_guess == 2))) return rc;
     if (res != x) MGB_CUDA(cudaMemcpyAsync(x, res, s->lv[0].n * sizeof(float), cudaMemcpyDeviceToDevice, s->st));
     return 0;
 }
@@ -601,7 +630,7 @@ int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
         // the first launch of the cycle has to be a lean_kernel sweep of level 0; otherwise clear x and run the general cycle
         FusedState* fs = (FusedState*)s->fused_state;
         size_t sm = 0; int a = 0, c = 0;
-        const bool lean0 = fs->lp[0].stream && s->p.sweeps_per_pass == 1 && s->p.nu_pre >= 1 && s->levels > 1 &&
+        const bool lean0 = fs->lp[0].stream && s->p.nu_pre >= 1 && s->levels > 1 &&
                            !ctail_fits(s, 0, &sm, &a, &c) && !tail_fits(s, 0, &sm);
         if (zero_guess == 2 && !(lean0 && s->p.nu_pre >= 2)) { set_error("fused_vcycle: the seeded cycle is not available"); return MG_EINVAL; }
         if (!lean0) {
@@ -618,7 +647,7 @@ bool fused_seed_supported(mg_solver* s) {
     if (ensure_state(s)) return false;
     FusedState* fs = (FusedState*)s->fused_state;
     size_t sm = 0; int a = 0, c = 0;
-    return fs->lp[0].stream && s->p.sweeps_per_pass == 1 && s->p.nu_pre >= 2 && s->levels > 1 && !ctail_fits(s, 0, &sm, &a, &c) &&
+    return fs->lp[0].stream && s->p.nu_pre >= 2 && s->levels > 1 && !ctail_fits(s, 0, &sm, &a, &c) &&
            !tail_fits(s, 0, &sm);
 }
 
@@ -627,6 +656,7 @@ void fused_release(mg_solver* s) {
     if (!fs) return;
     for (auto& lp : fs->lp) { cudaFree(lp.dinv); cudaFree(lp.tmp2); }
     cudaFree(fs->cmat);
+    cudaFree(fs->wave_sync);
     delete fs;
     s->fused_state = nullptr;
 }

@@ -55,8 +55,8 @@ def make_solver(mg, shape, h, levels, bc, dt, k=None, fused=1, **params):
     nz, ny, nx = shape
     hh = h if isinstance(h, tuple) else (h, h, h)
     s = mg.mg_create((nx, ny, nz, *hh), levels, bc, mg.MG_F32 if dt == "f32" else mg.MG_F64)
-    # fused: 0 = one generic kernel per operation, 1 = streaming one-stage kernels (sweeps_per_pass 1),
-    #        2 = two-stage temporally fused kernels (sweeps_per_pass 2)
+    # fused: 0 = one generic kernel per operation, 1 = streaming kernels, one stage per launch (sweeps_per_pass 1),
+    #        T >= 2 = wave kernel, up to T dependent stages per launch (sweeps_per_pass T; wave_kernel.cuh)
     p = dict(nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=max(fused, 1), omega=2.0 / 3.0, mixed_precision=1)
     p.update(params)
     mg.mg_set_params(s, **p)
@@ -69,7 +69,7 @@ def make_solver(mg, shape, h, levels, bc, dt, k=None, fused=1, **params):
 SHAPES = [((32, 32, 32), 1.0 / 32), ((8, 24, 40), 1.0 / 40), ((70, 36, 132), 0.01), ((4, 4, 4), 0.25)]
 
 
-@pytest.mark.parametrize("fused", [0, 1, 2])
+@pytest.mark.parametrize("fused", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("dt", ["f32", "f64"])
 @pytest.mark.parametrize("var", [False, True])
 @pytest.mark.parametrize("bc", BC_MIXES)
@@ -127,7 +127,7 @@ def test_anisotropic_spacing(mg, orc):
         mg.mg_destroy(s)
 
 
-@pytest.mark.parametrize("fused", [0, 1, 2])
+@pytest.mark.parametrize("fused", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("dt", ["f32", "f64"])
 @pytest.mark.parametrize("var", [False, True])
 @pytest.mark.parametrize("shape,h,levels,bc,nu", [
