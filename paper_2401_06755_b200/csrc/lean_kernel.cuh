@@ -199,9 +199,7 @@ struct WaveCtx {
     int* my_prog;          // this block's progress flag (nullptr: nobody waits for this stage)
     const int* dep_prog;   // progress flags [nch][gy][gx] of the stage that produces this stage's iterate (nullptr: none)
     int* err;              // set to 1 if a wait timed out (the result is then garbage, but the kernel ends)
-    long long* prof;       // scratch instrumentation (nullptr in production): per block {t0, t1, wait ns, publish ns, polls, waits}
 };
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
 
 __device__ __forceinline__ int ld_acquire_gpu(const int* p) {
     int v; asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
@@ -298,7 +296,6 @@ __device__ __forceinline__ void lean_body(const CUtensorMap& tmx, const CUtensor
         }
         if (c == wc.chunk && known >= need) return;
         const int lane = tid & 31;
-        const long long tw0 = (WAVE && wc.prof) ? gtime() : 0;
         const int ddx = lane % 3 - 1, ddy = (lane / 3) % 3 - 1;
         const int ux = wc.tx + ddx, uy = wc.ty + ddy;
         const bool valid = lane < 9 && ux >= 0 && ux < wc.gx && uy >= 0 && uy < wc.gy;
@@ -307,24 +304,20 @@ __device__ __forceinline__ void lean_body(const CUtensorMap& tmx, const CUtensor
         for (long long spin = 0;; ++spin) {
             const int v = valid ? ld_acquire_gpu(fp) : 0x7fffffff;
             m = __reduce_min_sync(0xffffffffu, v);
-            if (WAVE && wc.prof && lane == 0) wc.prof[4] += 1;
             if (m >= need) break;
             if (spin > (1ll << 22)) { if (lane == 0) atomicExch(wc.err, 1); break; }   // ~ seconds: give up, flag the error
             __nanosleep(64);
         }
         __syncwarp();
         if (c == wc.chunk) known = m;
-        if (WAVE && wc.prof && lane == 0) { wc.prof[2] += gtime() - tw0; wc.prof[5] += 1; }
     };
     // publish: `count` planes of this chunk are complete (called by thread 0 after a block barrier that follows their stores)
     auto publish = [&](int count) {
         if (!WAVE || wc.my_prog == nullptr) return;
         // the consumers read these planes through TMA (async proxy); the release makes the block's stores (ordered before
         // this thread by the block barrier) visible at gpu scope before the flag
-        const long long tp0 = wc.prof ? gtime() : 0;
         asm volatile("fence.proxy.async.global;" ::: "memory");
         st_release_gpu(wc.my_prog, count);
-        if (wc.prof) wc.prof[3] += gtime() - tp0;
     };
 
     if (tid == 0) {
@@ -342,7 +335,6 @@ __device__ __forceinline__ void lean_body(const CUtensorMap& tmx, const CUtensor
     // kernel of the cycle are first read below.  The next kernel may begin its own prologue from here on.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (WAVE && wc.prof && tid == 0) wc.prof[0] = gtime();
     if (WAVE) {
         if (tid < 32)
             for (int q = 0; q < NS && q < niter; ++q) {
@@ -524,7 +516,6 @@ __device__ __forceinline__ void lean_body(const CUtensorMap& tmx, const CUtensor
         __syncthreads();
         if (tid == 0) publish(zc1 - zc0);
     }
-    if (WAVE && wc.prof && tid == 0) wc.prof[1] = gtime();
 }
 
 template <class C>

@@ -256,14 +256,6 @@ int launch_wave_cfg(mg_solver* s, int l, const StageSpec* st, int n, float* cur,
     wk::WParams W;
     std::memset(&W, 0, sizeof(W));
     W.nstages = n; W.nch = nch; W.gx = gx; W.gy = gy;
-    { const char* d = getenv("MG_WAVE_DEBUG"); W.debug = d ? atoi(d) : 0; }
-    if (getenv("MG_WAVE_PROF")) {      // scratch: 8 words per block, dumped by the caller through the pointer in the env var
-        static long long* prof = nullptr;
-        if (!prof) { cudaMalloc(&prof, 8 * 8 * 4096); FILE* f = fopen(getenv("MG_WAVE_PROF"), "w"); if (f) { fprintf(f, "%llu\n", (unsigned long long)prof); fclose(f); } }
-        cudaMemsetAsync(prof, 0, 8 * 8 * 4096, s->st);
-        W.prof = prof;
-    }
-    W.prog = fs->wave_sync; W.done = fs->wave_sync + WAVE_FLAGS; W.err = fs->wave_sync + WAVE_FLAGS + 1;
     for (int i = 0; i < n; ++i) {
         wk::WStage& S = W.st[i];
         S.mode = st[i].mode;
@@ -295,10 +287,9 @@ int run_chain(mg_solver* s, int l, float* cur, float* oth, const float* b, const
     while (i < n) {
         int g = std::min(std::min(s->p.sweeps_per_pass, wk::MAXS), n - i);
         int rc = 1;
-        const int gmin = (getenv("MG_WAVE_DEBUG") && (atoi(getenv("MG_WAVE_DEBUG")) & 4)) ? 1 : 2;
-        while (g >= gmin && (rc = launch_wave(s, l, st + i, g, cur, oth, b)) == 1) --g;     // 1: does not fit the machine
-        if (g >= gmin && rc) return rc;
-        if (g < gmin) {
+        while (g >= 2 && (rc = launch_wave(s, l, st + i, g, cur, oth, b)) == 1) --g;     // 1: does not fit the machine
+        if (g >= 2 && rc) return rc;
+        if (g < 2) {
             g = 1;
             const bool writes = st[i].mode != lk::MODE_RR;
             if ((rc = launch_stream(s, l, st[i], cur, b, writes ? oth : nullptr))) return rc;

@@ -24,11 +24,9 @@ struct WStage {
 
 struct WParams {
     int nstages, nch, gx, gy;
-    int debug;                 // scratch timing knobs: 1 = do not wait, 2 = do not publish
     int* prog;                 // progress flags [nstages][nch][gy][gx], all zero between launches
     int* done;                 // blocks that have finished (the last one clears the flags and this counter)
     int* err;
-    long long* prof;           // scratch instrumentation, 8 words per block (nullptr in production)
     WStage st[MAXS];
 };
 
@@ -42,10 +40,9 @@ __global__ void __launch_bounds__(LX * LY, MINB) wave_kernel(const __grid_consta
     wc.dir = (chunk & 1) ? -1 : 1;
     wc.tx = blockIdx.x; wc.ty = blockIdx.y; wc.chunk = chunk;
     wc.gx = W.gx; wc.gy = W.gy; wc.nch = W.nch; wc.zchunk = S.P.zchunk;
-    wc.my_prog = (stage + 1 < W.nstages && !(W.debug & 2)) ? W.prog + stage * per + ((size_t)chunk * W.gy + blockIdx.y) * W.gx + blockIdx.x : nullptr;
-    wc.dep_prog = (stage > 0 && !(W.debug & 1)) ? W.prog + (stage - 1) * per : nullptr;
+    wc.my_prog = stage + 1 < W.nstages ? W.prog + stage * per + ((size_t)chunk * W.gy + blockIdx.y) * W.gx + blockIdx.x : nullptr;
+    wc.dep_prog = stage > 0 ? W.prog + (stage - 1) * per : nullptr;
     wc.err = W.err;
-    wc.prof = W.prof ? W.prof + 8 * ((size_t)blockIdx.z * W.gy * W.gx + blockIdx.y * W.gx + blockIdx.x) : nullptr;
     switch (S.mode) {
         case lk::MODE_SWEEP: lk::lean_body<C, lk::MODE_SWEEP, true>(S.tmx, S.tmk, S.tmb, S.tmc, S.P, blockIdx.x, blockIdx.y, chunk, wc); break;
         case lk::MODE_PRO: lk::lean_body<C, lk::MODE_PRO, true>(S.tmx, S.tmk, S.tmb, S.tmc, S.P, blockIdx.x, blockIdx.y, chunk, wc); break;
