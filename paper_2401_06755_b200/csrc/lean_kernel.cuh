@@ -51,8 +51,8 @@ enum { MODE_SWEEP = 0, MODE_PRO = 1, MODE_RR = 2, MODE_SEED = 3 };
 struct LParams {
     int nx, ny, nz;
     int zchunk;                 // output planes per block (even)
-    int dir;                    // +1: blocks march towards larger z, -1: towards smaller z (one-stage launches; the host alternates it
-                                // between consecutive passes so that a pass starts on the planes its predecessor left in L2)
+    int dir;                    // +1: blocks march towards larger z, -1: towards smaller z (one-stage launches: +1; alternating the
+                                // direction between consecutive passes was measured: no L2 reuse to be had, 51.3 vs 51.3 us)
     float sx0, sx1, sy0, sy1, sz0, sz1;
     float cc, icc;              // 1/(24 h^2) and its inverse
     float omega;

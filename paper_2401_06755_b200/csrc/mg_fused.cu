@@ -101,7 +101,6 @@ struct LevelPlan {
     float* dinv = nullptr;    // 1/D (variable k), levels >= 1
     float* tmp2 = nullptr;    // residual scratch of levels the streaming kernels do not cover
     float ce = 0, cc = 0, cdiag = 0, w0 = 0;
-    long long passes = 0;     // one-stage launches issued on this level (parity = march direction of the next one)
 };
 
 struct FusedState {
@@ -199,10 +198,6 @@ int launch_stream_cfg(mg_solver* s, int l, const StageSpec& sp, const float* src
     CUtensorMap tmx, tmk, tmb, tmc;
     lk::LParams P;
     if ((rc = fill_stage<C>(s, l, sp, src, b, dst, zchunk, &tmx, &tmk, &tmb, &tmc, &P))) return rc;
-    // serpentine: consecutive passes of a level march in opposite directions
-    static const bool serp = getenv("MG_NO_SERPENTINE") == nullptr;
-    if (serp) { P.dir = (fs->lp[l].passes & 1) ? -1 : 1; }
-    ++fs->lp[l].passes;
     dim3 grid((L.nx + C::TX - 1) / C::TX, (L.ny + C::TY - 1) / C::TY, nchunks);
     MGB_CUDA(launch_pdl(lk::lean_kernel<C>, grid, dim3(C::NT), C::SMEM, s->st, tmx, tmk, tmb, tmc, P));
     ++s->launches;
@@ -256,6 +251,7 @@ int launch_wave_cfg(mg_solver* s, int l, const StageSpec* st, int n, float* cur,
     wk::WParams W;
     std::memset(&W, 0, sizeof(W));
     W.nstages = n; W.nch = nch; W.gx = gx; W.gy = gy;
+    W.prog = fs->wave_sync; W.done = fs->wave_sync + WAVE_FLAGS; W.err = fs->wave_sync + WAVE_FLAGS + 1;
     for (int i = 0; i < n; ++i) {
         wk::WStage& S = W.st[i];
         S.mode = st[i].mode;
