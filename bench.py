@@ -35,9 +35,26 @@ METRIC = "multigrid V-cycles/s at 256^3 fp32 (V(2,2), 7 levels, variable coeffic
 UNIT = "V-cycles/s"
 E2E_CYCLES = 20          # the paper's fixed cycle count per pressure solve
 REF_TIME_BUDGET_S = 150  # wall-clock cap of the oracle arm
-# dram__bytes_read.sum + dram__bytes_write.sum of one fine-level smoother launch, from the ncu --set full
-# capture summarised in profiles/r01_ncu_lean.md (bytes per launch); None until a capture of the current kernel exists
-TRAFFIC_NCU = 252.9e6
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of one fine-level smoother launch, from the ncu --set full
+# capture recorded in TRAFFIC_FILE together with the SHA-256 of the kernel source it was taken from; when the source has
+# changed since, the number is stale and `traffic` is null (the file names the profile summary it belongs to)
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "traffic_lean_sweep.json")
+KERNEL_SOURCE = os.path.join(ROOT, "paper_2401_06755_b200", "csrc", "lean_kernel.cuh")
+
+
+def load_traffic():
+    """(bytes per launch or None, note)"""
+    import hashlib
+    try:
+        with open(TRAFFIC_FILE) as f:
+            d = json.load(f)
+        with open(KERNEL_SOURCE, "rb") as f:
+            sha = hashlib.sha256(f.read()).hexdigest()
+    except (OSError, ValueError) as e:
+        return None, "no traffic record (%s)" % e
+    if d.get("source_sha256") != sha:
+        return None, "stale: %s was captured from another version of lean_kernel.cuh" % d.get("from", TRAFFIC_FILE)
+    return float(d["dram_bytes_per_launch"]), d.get("from", TRAFFIC_FILE)
 
 
 def load_peaks():
@@ -74,35 +91,61 @@ class ClockSampler(threading.Thread):
 
     def run(self):
         try:
-            import pynvml as nv
-            nv.nvmlInit()
-            h = nv.nvmlDeviceGetHandleByIndex(self.index)
-            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
-            names = {
-                getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
-                getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
-                getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
-                getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
-                getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
-            }
-            while not self.stop_flag:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
-                try:
-                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
-                    for bit, name in names.items():
-                        if r & bit:
-                            self.reasons.add(name)
-                except Exception:
-                    pass
-                time.sleep(0.02)
+            self._run_nvml()
         except Exception:
-            self.ok = False
+            try:
+                self._run_smi()
+            except Exception:
+                self.ok = False
+
+    def _run_nvml(self):
+        import pynvml as nv
+        nv.nvmlInit()
+        h = nv.nvmlDeviceGetHandleByIndex(self.index)
+        self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self.stop_flag:
+            self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+            try:
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def _run_smi(self):
+        """No pynvml on this machine: poll nvidia-smi (B200_PROFILING.md's clocks line), one process per sample."""
+        import subprocess
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        self.source = "nvidia-smi"
+        while True:
+            out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
+                                 capture_output=True, text=True, timeout=10).stdout.strip().splitlines()
+            f = [c.strip() for c in out[0].split(",")]
+            self.samples.append(float(f[0]))
+            self.max_mhz = float(f[1])
+            for name, val in zip(names, f[2:]):
+                if val.lower().startswith("active"):
+                    self.reasons.add(name)
+            if self.stop_flag:
+                break
+            time.sleep(0.02)
 
     def summary(self):
         if not self.ok or not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
         return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(self.samples)}
+                "samples": len(self.samples), "source": getattr(self, "source", "nvml")}
 
 
 def max_over_ranks(ms, world, device=None):
@@ -146,6 +189,14 @@ def oracle_rhs(w):
     return oracle.pressure_rhs(g, w.fields["u"], w.fields["v"], w.fields["w"], 1.0).astype(np.float32)
 
 
+def bench_config(w, args, world):
+    """The `config` object of both arms (same keys and values, so that the driver can compare them)."""
+    return {"workload": "config3_rising_bubble_256^3 (BASELINE.json configs[2])", "grid": [w.nx, w.ny, w.nz],
+            "levels": w.levels, "cycle": "V(%d,%d)" % (w.nu_pre, w.nu_post), "omega": w.omega,
+            "coarse_sweeps": w.coarse_sweeps, "bc": "Neumann x5, Dirichlet top", "sweeps_per_pass": args.sweeps_per_pass,
+            "l2_policy": "inputs larger than L2 (x, b, k = 192 MiB > 126 MB)", "parallelism": "replicas x%d" % world}
+
+
 def run_reference(args, rank):
     if rank != 0:
         return
@@ -158,10 +209,10 @@ def run_reference(args, rank):
     sample = "%d V-cycle(s) of config 3 at full size (256^3, 7 levels, V(2,2)), fp64 oracle" % done
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "steps_timed": done, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 / value, "higher_is_better": True,
+        "steps_timed": done, "warmup": args.warmup, "warmup_done": min(args.warmup, 1), "ms_per_step": 1e3 / value,
+        "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config3_rising_bubble_256^3 (BASELINE.json configs[2])", "levels": w.levels,
-                   "cycle": "V(2,2)", "omega": w.omega, "coarse_sweeps": w.coarse_sweeps},
+        "config": bench_config(w, args, args.gpus),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -248,11 +299,12 @@ def run_ours(args, rank, local_rank, world):
         e3.record()
         torch.cuda.synchronize()
         launches_sm = nsw // args.sweeps_per_pass
+        traffic, traffic_src = load_traffic()
         t_ms = e2.elapsed_time(e3) / launches_sm
         nbytes = 16.0 * info[0]
         achieved = nbytes / (t_ms * 1e-3) * 1e-9
         roofline = {"bound": "hbm", "kernel": "fine-level smoother pass (%d sweep(s) per launch)" % args.sweeps_per_pass,
-                    "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": TRAFFIC_NCU,
+                    "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                     "peak_source": peak_src, "alg_bytes_per_launch": nbytes, "ms_per_launch": float(t_ms),
                     "launches_timed": launches_sm}
         del xs
@@ -326,10 +378,7 @@ def run_ours(args, rank, local_rank, world):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "config3_rising_bubble_256^3 (BASELINE.json configs[2])", "grid": [w.nx, w.ny, w.nz],
-                       "levels": w.levels, "cycle": "V(%d,%d)" % (w.nu_pre, w.nu_post), "omega": w.omega,
-                       "coarse_sweeps": w.coarse_sweeps, "bc": "Neumann x5, Dirichlet top", "sweeps_per_pass": args.sweeps_per_pass,
-                       "l2_policy": "inputs larger than L2 (x, b, k = 192 MiB > 126 MB)", "parallelism": "replicas x%d" % world},
+            "config": bench_config(w, args, args.gpus),
             "glups": glups, "lups_per_cycle": lups_per_cycle,
             "alg_bytes_per_cycle": algorithmic_bytes_per_cycle(w, info),
             "effective_gbs": algorithmic_bytes_per_cycle(w, info) * (args.steps / (ms * 1e-3)) * 1e-9,
@@ -350,8 +399,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the config-5 time-step measurement")
-    ap.add_argument("--sweeps-per-pass", type=int, default=1, choices=[1, 2],
-                    help="1: one-stage streaming kernels (default, faster); 2: two-stage temporally fused kernels")
+    ap.add_argument("--sweeps-per-pass", type=int, default=1, choices=[1, 2, 3, 4],
+                    help="stencil stages per launch on a level: 1 = one-stage streaming kernels (default, faster); "
+                         "2-4 = wave kernel (temporal blocking through L2)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -45,8 +45,10 @@ typedef struct { int nx, ny, nz; double hx, hy, hz; } mg_grid;
 /* V-cycle parameters (the paper gives none: P:43, P:47, P:105 name "Jacobi smoothing" only;
  * defaults are BASELINE.json config 1): nu_pre, nu_post weighted-Jacobi sweeps, coarse_sweeps
  * sweeps on the coarsest level from a zero guess, omega the damping.
- * sweeps_per_pass: how many sweeps one kernel pass may fuse temporally (>= 1; results do not
- * depend on it beyond rounding order).  mixed_precision (MG_F32 only): mg_solve keeps the
+ * sweeps_per_pass: how many dependent stencil stages (sweeps, the prolongation + sweep, the residual +
+ * restriction) one kernel launch may carry on a level, 1 .. 4 (wave_kernel.cuh); other values are refused
+ * with MG_EINVAL; a level on which that many stages do not fit the machine at once gets fewer per launch.
+ * Results do not depend on it beyond rounding order.  mixed_precision (MG_F32 only): mg_solve keeps the
  * iterate and the fine-grid residual in fp64 around fp32 V-cycles (reading C6/C8). */
 typedef struct {
     int nu_pre, nu_post, coarse_sweeps, sweeps_per_pass;
@@ -151,7 +153,10 @@ int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const vo
  * P:226-246, 419-427):  n_t = grad C / (1e-7/hx + |grad C|), kappa = -(f(n_tu; w_x) + f(n_tv; w_y) + f(n_tw; w_z)),
  * s_t = sigma_t kappa grad C,  b = f(g rho; w_z) - (f(s_tu; w_x) + f(s_tv; w_y) + f(s_tw; w_z)), plus the contribution of the bottom
  * boundary condition dp_hs/dz = -rho g on the plane z = 0.  Solve A p_hs = b with a constant-coefficient solver and
- * bc = {N, N, N, N, N, D}.  Readings (Eq. 22 / 23 misprints; the signs of Eqs. 5, 43, 44) in DESIGN.md N3.  d_kappa_out may be NULL. */
+ * bc = {N, N, N, N, N, D}.  Readings (Eq. 22 / 23 misprints; the signs of Eqs. 5, 43, 44) in DESIGN.md N3.  d_kappa_out may be NULL.
+ * SIGN: d_kappa_out holds kappa = -div(n_t) and d_st_out s_t = sigma_t kappa grad C with that kappa (reading N3-b: the
+ * continuum-surface-force convention, force towards the centre of curvature, p_hs higher inside a drop).  This is the
+ * OPPOSITE sign of Eq. 5 as printed (kappa = +div n_t); b is numerically the b of Eq. 44 as printed either way. */
 int hydrostatic_rhs(const mg_grid* grid, int dtype, const void* d_C, double rho_l, double rho_g, double g, double sigma_t,
                     void* d_b, void* d_kappa_out, void* cuda_stream);
 /* a10: q <- q - dt k f(p; w_x|y|z), Eq. 54 with Eq. 48; halo of p by bc[6]. */

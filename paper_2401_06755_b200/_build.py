@@ -44,8 +44,19 @@ def _compile(src, force, verbose):
 
 
 def build(force=False, verbose=False):
-    """Compile (if stale) and return the path of libmg_b200.so."""
+    """Compile (if stale) and return the path of libmg_b200.so.  Serialised across processes by a file lock (several
+    ranks or test workers may import the package at once)."""
+    import fcntl
     os.makedirs(OBJ, exist_ok=True)
+    with open(os.path.join(OBJ, ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            return _build_locked(force, verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(force, verbose):
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         results = list(ex.map(lambda s: _compile(s, force, verbose), SOURCES))
     objs = [o for o, _ in results]

@@ -37,6 +37,12 @@ struct Dim3i { int nx, ny, nz; };
 
 inline __host__ __device__ size_t npts(int nx, int ny, int nz) { return (size_t)nx * ny * nz; }
 
+// Per-device facts and one-time kernel set-up (mg_api.cu).  Both are keyed by the CURRENT device and thread-safe:
+// cudaFuncSetAttribute and the occupancy query apply per device, so a process-wide "done" flag would leave a second GPU
+// of the same process without its opt-in to > 48 KB of dynamic shared memory.
+int sm_count();                                                   // multiprocessors of the current device
+int kernel_setup(const void* fn, int threads, size_t smem, int* ctas_per_sm);   // opt-in + resident blocks per SM
+
 // ---- launchers of the generic (any spacing, any BC, one sweep per pass) kernels: mg_generic.cu
 template <typename T> int launch_apply(const Level<T>& L, const T* k, const T* x, T* y, cudaStream_t st);
 template <typename T> int launch_jacobi(const Level<T>& L, const T* k, const T* x, const T* b, T* xnew, cudaStream_t st);

@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(256) axpy_kernel(size_t n, T* __restrict__ y, 
 }
 template <typename T>
 int launch_axpy(size_t n, T* y, const T* x, cudaStream_t st) {
-    axpy_kernel<T><<<(int)std::min<size_t>((n + 255) / 256, 148 * 16), 256, 0, st>>>(n, y, x);
+    axpy_kernel<T><<<(int)std::min<size_t>((n + 255) / 256, (size_t)sm_count() * 16), 256, 0, st>>>(n, y, x);
     MGB_LAUNCH_CHECK();
     return 0;
 }

@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "fused.h"
@@ -17,6 +18,37 @@ void set_error(const char* fmt, ...) {
     va_start(ap, fmt);
     vsnprintf(g_err, sizeof(g_err), fmt, ap);
     va_end(ap);
+}
+
+int sm_count() {
+    static std::mutex mu;
+    static int cache[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!cache[dev] && (cudaDeviceGetAttribute(&cache[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || cache[dev] < 1))
+        cache[dev] = 148;
+    return cache[dev];
+}
+
+int kernel_setup(const void* fn, int threads, size_t smem, int* ctas_per_sm) {
+    struct Entry { int device; const void* fn; int ctas_per_sm; };
+    static std::mutex mu;
+    static std::vector<Entry> done;
+    int dev = 0;
+    MGB_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    for (const Entry& e : done)
+        if (e.device == dev && e.fn == fn) { if (ctas_per_sm) *ctas_per_sm = e.ctas_per_sm; return 0; }
+    if (smem > 48 * 1024) {
+        MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    }
+    int nb = 0;
+    MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, threads, smem));
+    done.push_back({dev, fn, nb > 0 ? nb : 1});
+    if (ctas_per_sm) *ctas_per_sm = done.back().ctas_per_sm;
+    return 0;
 }
 
 // Nodal 27-point filter of -Laplace from the trilinear-FE integrals (reading C1):
@@ -199,7 +231,7 @@ static int solve_plain(mg_solver* s, T* x, const T* b, double tol, int max_cycle
     while (status == MG_NOT_CONVERGED && cycles < max_cycles) {
         if ((rc = vcycle_any<T>(s, x, b))) return rc;
         if ((rc = residual_norm<T>(s, x, b, &nr))) return rc;
-        rel = nr / nb;
+        rel = nb > 0.0 ? nr / nb : 0.0;
         s->history.push_back(rel);
         ++cycles;
         const int u = stop.update(rel);
@@ -285,10 +317,14 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
 }
 
 int ensure_mixed_buffers(mg_solver* s) {
-    if (s->x64) return 0;
+    if (s->x64 && s->k64 && s->r32 && s->e32) return 0;
     const size_t n = s->lv[0].n;
-    if (cudaMalloc(&s->x64, n * 8) != cudaSuccess || cudaMalloc(&s->k64, n * 8) != cudaSuccess ||
-        cudaMalloc(&s->r32, n * 4) != cudaSuccess || cudaMalloc(&s->e32, n * 4) != cudaSuccess) {
+    if ((!s->x64 && cudaMalloc(&s->x64, n * 8) != cudaSuccess) || (!s->k64 && cudaMalloc(&s->k64, n * 8) != cudaSuccess) ||
+        (!s->r32 && cudaMalloc(&s->r32, n * 4) != cudaSuccess) || (!s->e32 && cudaMalloc(&s->e32, n * 4) != cudaSuccess)) {
+        // all or nothing: a later call must not find x64 set and the others NULL
+        cudaFree(s->x64); cudaFree(s->k64); cudaFree(s->r32); cudaFree(s->e32);
+        s->x64 = s->k64 = nullptr; s->r32 = s->e32 = nullptr;
+        cudaGetLastError();
         set_error("mixed-precision buffers: out of device memory");
         return MG_EALLOC;
     }

@@ -5,7 +5,6 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cstring>
-#include <mutex>
 
 #include "fused.h"
 #include "solver.h"
@@ -112,24 +111,6 @@ struct FusedState {
 };
 constexpr int WAVE_FLAGS = 8192;
 
-// One-time per-(device, kernel) set-up: opt-in to > 48 KB of dynamic shared memory and the resident blocks per SM.
-// cudaFuncSetAttribute and the occupancy query apply to the CURRENT device, so the cache is keyed by it.
-struct KernelSetup { int device; const void* fn; int ctas_per_sm; };
-int kernel_setup(int device, const void* fn, int threads, size_t smem, int* ctas_per_sm) {
-    static std::mutex mu;
-    static std::vector<KernelSetup> done;
-    std::lock_guard<std::mutex> lock(mu);
-    for (const KernelSetup& k : done)
-        if (k.device == device && k.fn == fn) { if (ctas_per_sm) *ctas_per_sm = k.ctas_per_sm; return 0; }
-    MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    int nb = 0;
-    MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, threads, smem));
-    done.push_back({device, fn, nb > 0 ? nb : 1});
-    if (ctas_per_sm) *ctas_per_sm = done.back().ctas_per_sm;
-    return 0;
-}
-
 // One stage of a pass on level l: what it reads and writes besides the iterate.
 struct StageSpec {
     int mode = lk::MODE_SWEEP;
@@ -181,7 +162,7 @@ int launch_stream_cfg(mg_solver* s, int l, const StageSpec& sp, const float* src
     FusedState* fs = (FusedState*)s->fused_state;
     LevelData& L = s->lv[l];
     int ctas_per_sm = 1, rc;
-    if ((rc = kernel_setup(s->device, (const void*)lk::lean_kernel<C>, C::NT, C::SMEM, &ctas_per_sm))) return rc;
+    if ((rc = kernel_setup((const void*)lk::lean_kernel<C>, C::NT, C::SMEM, &ctas_per_sm))) return rc;
     const int tiles = ((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
     // z chunking: minimise (waves over the resident CTA slots) x (planes per block incl. the two halo planes)
     double best_cost = 1e30;
@@ -238,7 +219,7 @@ int launch_wave_cfg(mg_solver* s, int l, const StageSpec* st, int n, float* cur,
     LevelData& L = s->lv[l];
     auto kern = wk::wave_kernel<LX, LY, VAR, MINB>;
     int ctas_per_sm = 1, rc;
-    if ((rc = kernel_setup(s->device, (const void*)kern, C::NT, C::SMEM, &ctas_per_sm))) return rc;
+    if ((rc = kernel_setup((const void*)kern, C::NT, C::SMEM, &ctas_per_sm))) return rc;
     const int gx = (L.nx + C::TX - 1) / C::TX, gy = (L.ny + C::TY - 1) / C::TY, tiles = gx * gy;
     const int slots = fs->sm_count * ctas_per_sm;
     // every block of every stage has to be resident at once for the stages to overlap: as many z chunks as fit
@@ -303,7 +284,7 @@ int ensure_state(mg_solver* s) {
     FusedState* fs = new FusedState();
     fs->lp.resize(s->levels);
     s->fused_state = fs;                  // owned by the solver from here on (fused_release frees partial state)
-    if (cudaDeviceGetAttribute(&fs->sm_count, cudaDevAttrMultiProcessorCount, s->device) != cudaSuccess || fs->sm_count < 1) fs->sm_count = 148;
+    fs->sm_count = sm_count();
     for (int l = 0; l < s->levels; ++l) {
         LevelData& L = s->lv[l];
         LevelPlan& lp = fs->lp[l];
@@ -402,7 +383,7 @@ int launch_tail(mg_solver* s, int l, float* x, const float* b, int done, size_t 
     P.omega = (float)s->p.omega;
     P.nu_pre = s->p.nu_pre; P.nu_post = s->p.nu_post; P.coarse_sweeps = s->p.coarse_sweeps;
     P.first_done = done; P.x = x; P.b = b;
-    { int rc = kernel_setup(s->device, (const void*)tk::tail_kernel, tk::NT, 200 * 1024, nullptr); if (rc) return rc; }
+    { int rc = kernel_setup((const void*)tk::tail_kernel, tk::NT, 200 * 1024, nullptr); if (rc) return rc; }
     MGB_CUDA(launch_pdl(tk::tail_kernel, dim3(1), dim3(tk::NT), smem, s->st, P));
     ++s->launches;
     return 0;
@@ -501,7 +482,7 @@ int launch_ctail(mg_solver* s, int l, float* x, const float* b, int done, size_t
     P.nu_pre = s->p.nu_pre; P.nu_post = s->p.nu_post; P.coarse_sweeps = s->p.coarse_sweeps;
     P.first_done = done; P.x = x; P.b = b;
     P.cmat = fs->cmat_valid ? fs->cmat : nullptr;
-    { int rc = kernel_setup(s->device, (const void*)ck::ctail_kernel, ck::NT, 200 * 1024, nullptr); if (rc) return rc; }
+    { int rc = kernel_setup((const void*)ck::ctail_kernel, ck::NT, 200 * 1024, nullptr); if (rc) return rc; }
     MGB_CUDA(launch_pdl(ck::ctail_kernel, dim3(ck::NC), dim3(ck::NT), smem, s->st, P));
     ++s->launches;
     return 0;

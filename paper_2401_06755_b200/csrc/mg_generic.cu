@@ -193,7 +193,8 @@ __global__ void axpy_mixed_kernel(size_t n, double* __restrict__ x, const float*
 
 inline int ew_blocks(size_t n) {
     size_t b = (n + 255) / 256;
-    return (int)(b < 148 * 16 ? (b ? b : 1) : 148 * 16);
+    const size_t cap = (size_t)sm_count() * 16;
+    return (int)(b < cap ? (b ? b : 1) : cap);
 }
 
 }  // namespace

@@ -19,17 +19,12 @@ int launch_march_residual(int nx, int ny, int nz, double h, const double s[6], c
     const int tx = (nx + mk::TX - 1) / mk::TX, ty = (ny + mk::TY - 1) / mk::TY;
     // z chunks: one wave of resident blocks; every chunk pays 2 extra planes
     const size_t smem = (size_t)2 * mk::NSTG * mk::Lay<TXT>::ROW * mk::PYS * sizeof(TXT) + (size_t)mk::NBS * mk::NT * 4 * sizeof(TB);
-    static int per_sm = 0;
-    if (!per_sm) {
-        int nb = 0;
-        MGB_CUDA(cudaFuncSetAttribute(mk::march_residual_kernel<TXT, TB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        MGB_CUDA(cudaFuncSetAttribute(mk::march_residual_kernel<TXT, TB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        MGB_CUDA(cudaFuncSetAttribute(mk::march_residual_kernel<TXT, TB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        MGB_CUDA(cudaFuncSetAttribute(mk::march_residual_kernel<TXT, TB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mk::march_residual_kernel<TXT, TB, true, true>, mk::NT, smem));
-        per_sm = nb > 0 ? nb : 1;
-    }
-    const int want = (148 * per_sm) / (tx * ty);
+    int per_sm = 1, rc0;
+    if ((rc0 = kernel_setup((const void*)mk::march_residual_kernel<TXT, TB, true, true>, mk::NT, smem, &per_sm))) return rc0;
+    if ((rc0 = kernel_setup((const void*)mk::march_residual_kernel<TXT, TB, false, true>, mk::NT, smem, nullptr))) return rc0;
+    if ((rc0 = kernel_setup((const void*)mk::march_residual_kernel<TXT, TB, true, false>, mk::NT, smem, nullptr))) return rc0;
+    if ((rc0 = kernel_setup((const void*)mk::march_residual_kernel<TXT, TB, false, false>, mk::NT, smem, nullptr))) return rc0;
+    const int want = (sm_count() * per_sm) / (tx * ty);
     const int nch = want < 1 ? 1 : (want > nz ? nz : want);
     P.zchunk = (nz + nch - 1) / nch;
     const dim3 grid(tx, ty, (nz + P.zchunk - 1) / P.zchunk);

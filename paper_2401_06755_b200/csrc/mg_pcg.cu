@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(256) cast_kernel2(size_t n, const TA* __restri
     for (size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x) b[c] = (TB)a[c];
 }
 
-inline int blocks_for(size_t n) { return (int)std::min<size_t>((n + 255) / 256, 148 * 16); }
+inline int blocks_for(size_t n) { return (int)std::min<size_t>((n + 255) / 256, (size_t)sm_count() * 16); }
 
 template <typename TZ>   // TZ = float: MG_F32 solver (mixed), double: MG_F64 solver
 int pcg_t(mg_solver* s, void* d_x, const void* d_b, double tol, int max_iter, int* iters_out, double* rel_out) {
