@@ -412,15 +412,19 @@ static double k_abs_pg(const orc_grid* g, double a, double px, double py, double
 }
 
 /* Gradient by the linear-FE filters (Eq. 11 / m_l) and the advection term q . grad(Psi). */
-static void grad_and_adv(const orc_grid* g, const double* psi, const double* u, const double* v, const double* w,
-                         double* px, double* py, double* pz, double* adv) {
+static void grad_and_adv_bc(const orc_grid* g, const int* bc, const double* psi, const double* u, const double* v, const double* w,
+                            double* px, double* py, double* pz, double* adv) {
     const size_t n = (size_t)g->nx * g->ny * g->nz;
     double wx[27], wy[27], wz[27];
     orc_filter(g, 1, wx); orc_filter(g, 2, wy); orc_filter(g, 3, wz);
-    orc_apply_filter(g, BC_COPY, wx, psi, px);
-    orc_apply_filter(g, BC_COPY, wy, psi, py);
-    orc_apply_filter(g, BC_COPY, wz, psi, pz);
+    orc_apply_filter(g, bc, wx, psi, px);
+    orc_apply_filter(g, bc, wy, psi, py);
+    orc_apply_filter(g, bc, wz, psi, pz);
     for (size_t c = 0; c < n; ++c) adv[c] = u[c] * px[c] + v[c] * py[c] + w[c] * pz[c];
+}
+static void grad_and_adv(const orc_grid* g, const double* psi, const double* u, const double* v, const double* w,
+                         double* px, double* py, double* pz, double* adv) {
+    grad_and_adv_bc(g, BC_COPY, psi, u, v, w, px, py, pz, adv);
 }
 
 /* Eq. 29: a = alpha_a f(adv; w_m/m_l - E), alpha_a = 2. */
@@ -500,9 +504,14 @@ void orc_vof_residual(const orc_grid* g, const double* C, const double* u, const
  *   c~ = c_n - dt s~_c / rho (Eq. 45, sigma = 0);  c_half' = (c_n + c~)/2 (Eq. 46).
  * Pressure-gradient and source terms of Eq. 18 are not part of this residual.
  * qh/qn/qt/qhn are arrays of 3 component pointers (u, v, w). */
-void orc_mom_predictor(const orc_grid* g, const double* C, const double* const* qh, const double* const* qn,
-                       double rho_l, double rho_g, double mu_l, double mu_g, double dt,
-                       double* const* qt, double* const* qhn) {
+/* vbc = NULL: every velocity halo is a zero-derivative copy (BASELINE config 5's synthetic benchmark).  Otherwise
+ * vbc[6 * c + f] is the halo code of velocity component c on face f: free-slip walls make the component NORMAL to a
+ * wall odd about it (ghost = -mirror: zero normal velocity on the wall face, the interpolation rule of Fig. 2) and the
+ * tangential components even (zero normal derivative); at an outlet every component is copied.  The halo of a
+ * component enters its gradient (the advection term) and its diffusion; derived fields keep copy halos (reading C9-iv). */
+void orc_mom_predictor_bc(const orc_grid* g, const double* C, const double* const* qh, const double* const* qn, const int* vbc,
+                          double rho_l, double rho_g, double mu_l, double mu_g, double dt,
+                          double* const* qt, double* const* qhn) {
     const size_t n = (size_t)g->nx * g->ny * g->nz;
     double wl[27];
     orc_filter(g, 0, wl);
@@ -511,7 +520,8 @@ void orc_mom_predictor(const orc_grid* g, const double* C, const double* const* 
     double* a = (double*)malloc(n * sizeof(double)); double* kc = (double*)malloc(n * sizeof(double));
     double* diff = (double*)malloc(n * sizeof(double));
     for (int comp = 0; comp < 3; ++comp) {
-        grad_and_adv(g, qh[comp], qh[0], qh[1], qh[2], px, py, pz, adv);
+        const int* cbc = vbc ? vbc + 6 * comp : BC_COPY;
+        grad_and_adv_bc(g, cbc, qh[comp], qh[0], qh[1], qh[2], px, py, pz, adv);
         mixed_mass_residual(g, adv, a);
         for (size_t c = 0; c < n; ++c) {
             const double rho = rho_l * C[c] + rho_g * (1.0 - C[c]);
@@ -520,7 +530,7 @@ void orc_mom_predictor(const orc_grid* g, const double* C, const double* const* 
             const double kabs = k_abs_pg(g, a[c], px[c], py[c], pz[c]);
             kc[c] = rho * fmin(kmax, kabs) + mu;
         }
-        orc_apply_diffusion(g, BC_COPY, wl, kc, qh[comp], diff);
+        orc_apply_diffusion(g, cbc, wl, kc, qh[comp], diff);
         for (size_t c = 0; c < n; ++c) {
             const double rho = rho_l * C[c] + rho_g * (1.0 - C[c]);
             const double s = rho * adv[c] + diff[c];
@@ -532,17 +542,26 @@ void orc_mom_predictor(const orc_grid* g, const double* C, const double* const* 
     free(px); free(py); free(pz); free(adv); free(a); free(kc); free(diff);
 }
 
+void orc_mom_predictor(const orc_grid* g, const double* C, const double* const* qh, const double* const* qn,
+                       double rho_l, double rho_g, double mu_l, double mu_g, double dt,
+                       double* const* qt, double* const* qhn) {
+    orc_mom_predictor_bc(g, C, qh, qn, NULL, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn);
+}
+
 /* Pressure RHS (reading C10; FE divergence structure of Eq. 53):
  * b = -(1/dt) ( f(u~; w_x) + f(v~; w_y) + f(w~; w_z) ), nodal filters, velocity halos copy. */
-void orc_pressure_rhs(const orc_grid* g, const double* u, const double* v, const double* w, double dt, double* b) {
+void orc_pressure_rhs_bc(const orc_grid* g, const double* u, const double* v, const double* w, const int* vbc, double dt, double* b) {
     const size_t n = (size_t)g->nx * g->ny * g->nz;
     double wx[27], wy[27], wz[27];
     orc_filter(g, 1, wx); orc_filter(g, 2, wy); orc_filter(g, 3, wz);
     double* t = (double*)malloc(n * sizeof(double));
-    orc_apply_filter(g, BC_COPY, wx, u, b);
-    orc_apply_filter(g, BC_COPY, wy, v, t); for (size_t c = 0; c < n; ++c) b[c] += t[c];
-    orc_apply_filter(g, BC_COPY, wz, w, t); for (size_t c = 0; c < n; ++c) b[c] = -(b[c] + t[c]) / dt;
+    orc_apply_filter(g, vbc ? vbc : BC_COPY, wx, u, b);
+    orc_apply_filter(g, vbc ? vbc + 6 : BC_COPY, wy, v, t); for (size_t c = 0; c < n; ++c) b[c] += t[c];
+    orc_apply_filter(g, vbc ? vbc + 12 : BC_COPY, wz, w, t); for (size_t c = 0; c < n; ++c) b[c] = -(b[c] + t[c]) / dt;
     free(t);
+}
+void orc_pressure_rhs(const orc_grid* g, const double* u, const double* v, const double* w, double dt, double* b) {
+    orc_pressure_rhs_bc(g, u, v, w, NULL, dt, b);     /* velocity halos: copies */
 }
 
 /* The PAPER'S OWN stage-3 right-hand side, Eqs. 52-53 (SURVEY 8(f) "next 2"): the density stays on the right and

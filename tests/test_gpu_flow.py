@@ -6,6 +6,7 @@ import pytest
 
 from workloads import configs, rng
 from test_gpu_mg import TOL, as_f64, mg, quantise, rel_l2, to_dev  # noqa: F401
+from _parity import assert_close  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 N, D, H0 = configs.BC_NEUMANN, configs.BC_DIRICHLET, configs.BC_DIRICHLET_HALO
@@ -38,8 +39,8 @@ def test_vof_residual_parity(mg, orc, shape, h, dt):
     dC, du, dv, dw = (to_dev(a, dt) for a in (Cf, u, v, w))
     ds, dc = torch.empty_like(dC), torch.empty_like(dC)
     mg.vof_residual(dC, du, dv, dw, hh, tstep, ds, dc)
-    assert rel_l2(as_f64(ds), s_ref) <= 5 * TOL[dt]     # 3 chained passes (adv -> coefficients -> diffusion)
-    assert rel_l2(as_f64(dc), c_ref) <= TOL[dt]
+    assert_close(as_f64(ds), s_ref, 5 * TOL[dt])  # 3 chained passes (adv -> coefficients -> diffusion)
+    assert_close(as_f64(dc), c_ref, TOL[dt])
     # outputs are optional one at a time
     dc2 = torch.empty_like(dC)
     mg.vof_residual(dC, du, dv, dw, hh, tstep, None, dc2)
@@ -77,17 +78,17 @@ def test_momentum_rhs_projection_parity(mg, orc, n, dt):
     dqt = [torch.empty_like(dC) for _ in range(3)]; dqhn = [torch.empty_like(dC) for _ in range(3)]
     mg.mom_predictor(dC, dqh, dqn, w.h, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, dqt, dqhn)
     for c in range(3):
-        assert rel_l2(as_f64(dqt[c]), qt_ref[c]) <= TOL[dt]
-        assert rel_l2(as_f64(dqhn[c]), qhn_ref[c]) <= TOL[dt]
+        assert_close(as_f64(dqt[c]), qt_ref[c], TOL[dt])
+        assert_close(as_f64(dqhn[c]), qhn_ref[c], TOL[dt])
     # pressure RHS
     b_ref = orc.pressure_rhs(g, u, v, ww, w.dt)
     db = torch.empty_like(dC)
     mg.pressure_rhs(dqn[0], dqn[1], dqn[2], w.h, w.dt, db)
-    assert rel_l2(as_f64(db), b_ref) <= TOL[dt] * (50 if dt == "f32" else 1e3)   # divergence of a solenoidal field: cancellation
+    assert_close(as_f64(db), b_ref, TOL[dt] * (50 if dt == "f32" else 1e3))  # divergence of a solenoidal field: cancellation
     ur, vr, wr = (quantise(rng.normal(90 + c, alpha.size).reshape(alpha.shape), dt) for c in range(3))
     b_ref = orc.pressure_rhs(g, ur, vr, wr, w.dt)
     mg.pressure_rhs(to_dev(ur, dt), to_dev(vr, dt), to_dev(wr, dt), w.h, w.dt, db)
-    assert rel_l2(as_f64(db), b_ref) <= TOL[dt]
+    assert_close(as_f64(db), b_ref, TOL[dt])
     # projection with the solver's BC factors on p
     p = quantise(rng.normal(95, alpha.size).reshape(alpha.shape), dt)
     k = quantise(orc.k_from_vof(alpha, w.rho_l, w.rho_g), dt)
@@ -96,7 +97,7 @@ def test_momentum_rhs_projection_parity(mg, orc, n, dt):
         du, dv, dw = to_dev(u, dt), to_dev(v, dt), to_dev(ww, dt)
         mg.project_velocity(to_dev(p, dt), to_dev(k, dt), w.h, bcs, w.dt, du, dv, dw)
         for a, r in ((du, u_ref), (dv, v_ref), (dw, w_ref)):
-            assert rel_l2(as_f64(a), r) <= TOL[dt]
+            assert_close(as_f64(a), r, TOL[dt])
 
 
 @pytest.mark.parametrize("dt", ["f32", "f64"])
@@ -117,9 +118,9 @@ def test_time_step_parity(mg, orc, dt):
         status, cyc, rel = mg.flow_time_step(s, dC, du, dv, dw, dp, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, tol, 200)
         assert status == mg.MG_OK and rel < tol and abs(cyc - cyc_o) <= 2
         lim = (step + 1) * (2e-5 if dt == "f32" else 1e-7)
-        assert rel_l2(as_f64(dp), p) <= lim * 5
+        assert_close(as_f64(dp), p, lim * 5)
         for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
-            assert rel_l2(as_f64(a), r) <= lim
+            assert_close(as_f64(a), r, lim)
     mg.mg_destroy(s)
 
 
@@ -141,9 +142,9 @@ def test_time_step_pcg_parity(mg, orc, dt):
         status, its, rel = mg.flow_time_step_pcg(s, dC, du, dv, dw, dp, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, tol, 200)
         assert status == mg.MG_OK and rel < tol and abs(its - it_o) <= 2
         lim = (step + 1) * (2e-5 if dt == "f32" else 1e-7)
-        assert rel_l2(as_f64(dp), p) <= lim * 5
+        assert_close(as_f64(dp), p, lim * 5)
         for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
-            assert rel_l2(as_f64(a), r) <= lim
+            assert_close(as_f64(a), r, lim)
     mg.mg_destroy(s)
 
 
@@ -162,7 +163,7 @@ def test_pressure_rhs_paper_parity(mg, orc, shape, h, dt):
     db = torch.empty(shape, device="cuda", dtype=torch.float32 if dt == "f32" else torch.float64)
     mg.pressure_rhs_paper(to_dev(Cf, dt), to_dev(u, dt), to_dev(v, dt), to_dev(w, dt), hh, 1000.0, 1.0, 0.01, db)
     # rho q - q rho cancels to rho div q: the same cancellation allowance as the divergence right-hand side
-    assert rel_l2(as_f64(db), b_ref) <= TOL[dt] * (50 if dt == "f32" else 1e3)
+    assert_close(as_f64(db), b_ref, TOL[dt] * (50 if dt == "f32" else 1e3))
 
 
 @pytest.mark.parametrize("dt", ["f32", "f64"])
@@ -181,9 +182,9 @@ def test_time_step_paper_parity(mg, orc, dt):
         rel = mg.flow_time_step_paper(s, dC, du, dv, dw, dp, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, 20, 2)
         lim = (step + 1) * (1e-4 if dt == "f32" else 1e-7)
         assert abs(rel - rel_o) <= 0.05 * rel_o + 1e-12
-        assert rel_l2(as_f64(dp), p) <= lim * 5
+        assert_close(as_f64(dp), p, lim * 5)
         for a, r in ((dC, Cf), (du, u), (dv, v), (dw, ww)):
-            assert rel_l2(as_f64(a), r) <= lim
+            assert_close(as_f64(a), r, lim)
     mg.mg_destroy(s)
 
 
@@ -210,14 +211,14 @@ def test_hydrostatic_rhs_and_solve_parity(mg, orc, dt):
     gx = np.gradient(Cf, h)
     band = np.sqrt(gx[0] ** 2 + gx[1] ** 2 + gx[2] ** 2) > 1.0
     assert band.sum() > 1000
-    assert rel_l2(as_f64(dk)[band], kap_ref[band]) <= (2e-4 if dt == "f32" else 1e-9)
-    assert rel_l2(as_f64(db), b_ref) <= (5 * TOL[dt] if dt == "f32" else 1e-9)
+    assert_close(as_f64(dk)[band], kap_ref[band], (2e-4 if dt == "f32" else 1e-9))
+    assert_close(as_f64(db), b_ref, (5 * TOL[dt] if dt == "f32" else 1e-9))
     bc = (N, N, N, N, N, D)
     s = mg.mg_create((n, n, n, h), levels, bc, mg.MG_F32 if dt == "f32" else mg.MG_F64)
     dp = torch.zeros_like(dC)
     mg.mg_solve(s, dp, db, 0.0, 20)
     p_ref, _, _, _ = orc.solve(g, bc, None, np.zeros(g.shape), b_ref, levels, 0.0, 20)
-    assert rel_l2(as_f64(dp), p_ref) <= (1e-4 if dt == "f32" else 1e-8)
+    assert_close(as_f64(dp), p_ref, (1e-4 if dt == "f32" else 1e-8))
     # physics of the result: hydrostatic at the bottom of the water layer, higher pressure inside the drop
     p = as_f64(dp)
     assert abs((p[0, 4, 4] - p[2, 4, 4]) / (2 * h) - rho_l * grav) <= 0.02 * rho_l * grav
@@ -254,21 +255,23 @@ def test_explicit_kernels_every_pack_width(mg, orc, shape, unaligned, dt):
     s_ref, c_ref = orc.vof_residual(g, Cf, u, v, w, tstep)
     ds, dc = out(), out()
     mg.vof_residual(dC, du, dv, dw, hh, tstep, ds, dc)
-    assert rel_l2(as_f64(ds), s_ref) <= 5 * TOL[dt] and rel_l2(as_f64(dc), c_ref) <= TOL[dt]
+    assert_close(as_f64(ds), s_ref, 5 * TOL[dt])
+    assert_close(as_f64(dc), c_ref, TOL[dt])
     # momentum predictor
     qh = tuple(quantise(0.9 * a + 0.05, dt) for a in (u, v, w))
     qt_ref, qhn_ref = orc.mom_predictor(g, Cf, qh, (u, v, w), 1000.0, 1.0, 1e-3, 1.8e-5, tstep)
     dqt, dqhn = [out() for _ in range(3)], [out() for _ in range(3)]
     mg.mom_predictor(dC, [dev(a) for a in qh], [du, dv, dw], hh, 1000.0, 1.0, 1e-3, 1.8e-5, tstep, dqt, dqhn)
     for c in range(3):
-        assert rel_l2(as_f64(dqt[c]), qt_ref[c]) <= TOL[dt] and rel_l2(as_f64(dqhn[c]), qhn_ref[c]) <= TOL[dt]
+        assert_close(as_f64(dqt[c]), qt_ref[c], TOL[dt])
+        assert_close(as_f64(dqhn[c]), qhn_ref[c], TOL[dt])
     # pressure right-hand sides
     db = out()
     mg.pressure_rhs(du, dv, dw, hh, tstep, db)
-    assert rel_l2(as_f64(db), orc.pressure_rhs(g, u, v, w, tstep)) <= TOL[dt]
+    assert_close(as_f64(db), orc.pressure_rhs(g, u, v, w, tstep), TOL[dt])
     mg.pressure_rhs_paper(dC, du, dv, dw, hh, 1000.0, 1.0, tstep, db)
     # rho q - q rho cancels to rho div q: the cancellation allowance of test_pressure_rhs_paper_parity
-    assert rel_l2(as_f64(db), orc.pressure_rhs_paper(g, Cf, u, v, w, 1000.0, 1.0, tstep)) <= TOL[dt] * (50 if dt == "f32" else 1e3)
+    assert_close(as_f64(db), orc.pressure_rhs_paper(g, Cf, u, v, w, 1000.0, 1.0, tstep), TOL[dt] * (50 if dt == "f32" else 1e3))
     # projection with mixed halo factors
     p = quantise(rng.normal(195, n).reshape(shape), dt)
     k = quantise(orc.k_from_vof(Cf, 1000.0, 1.0), dt)
@@ -277,7 +280,7 @@ def test_explicit_kernels_every_pack_width(mg, orc, shape, unaligned, dt):
     pu, pv, pw = dev(u), dev(v), dev(w)
     mg.project_velocity(dev(p), dev(k), hh, bcs, tstep, pu, pv, pw)
     for a, r in zip((pu, pv, pw), refs):
-        assert rel_l2(as_f64(a), r) <= TOL[dt]
+        assert_close(as_f64(a), r, TOL[dt])
     # stage 1
     b_ref, kap_ref, _ = orc.hydrostatic_rhs(g, Cf, 1000.0, 1.0, 9.81, 0.07)
     dk = out()
@@ -286,5 +289,5 @@ def test_explicit_kernels_every_pack_width(mg, orc, shape, unaligned, dt):
     gr = np.gradient(Cf, hh[0])
     band = np.sqrt(gr[0] ** 2 + gr[1] ** 2 + gr[2] ** 2) > 1.0
     assert band.sum() > 100
-    assert rel_l2(as_f64(dk)[band], kap_ref[band]) <= (2e-4 if dt == "f32" else 1e-9)
-    assert rel_l2(as_f64(db), b_ref) <= (5 * TOL[dt] if dt == "f32" else 1e-9)
+    assert_close(as_f64(dk)[band], kap_ref[band], (2e-4 if dt == "f32" else 1e-9))
+    assert_close(as_f64(db), b_ref, (5 * TOL[dt] if dt == "f32" else 1e-9))

@@ -9,6 +9,7 @@ import pytest
 
 from workloads import configs
 from test_gpu_mg import TOL, as_f64, make_solver, mg, quantise, rel_l2, to_dev  # noqa: F401
+from _parity import assert_close  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 
@@ -26,13 +27,25 @@ def test_config4_full_size(mg, orc):
     x0 = quantise(0.01 * b, "f32")
     dx = to_dev(x0, "f32")
     mg.mg_smooth(s, dx, db, 3)
-    assert rel_l2(as_f64(dx), orc.smooth(g, w.bc, k, x0, b, w.omega, 3)) <= 3 * TOL["f32"]
-    for nu in (1, 2):
-        mg.mg_set_params(s, nu_pre=nu, nu_post=nu, coarse_sweeps=50, sweeps_per_pass=1, omega=w.omega, mixed_precision=1)
-        dx = to_dev(np.zeros(w.shape), "f32")
-        mg.mg_vcycle(s, dx, db)
+    assert_close(as_f64(dx), orc.smooth(g, w.bc, k, x0, b, w.omega, 3), 3 * TOL["f32"])
+    # the sweep of smoothing counts config 4 asks for, each against one oracle cycle; every count also through the wave
+    # kernel ("temporal blocking of 4 sweeps per pass"): on this grid level 0 has more tiles than fit the machine twice
+    # over, so it keeps one stage per launch and the coarser levels carry up to 4
+    for nu in (1, 2, 3, 4):
         x_o = orc.vcycle(g, w.bc, k, np.zeros(w.shape), b, w.levels, nu, nu)
-        assert rel_l2(as_f64(dx), x_o) <= 1e-4, "V(%d,%d)" % (nu, nu)
+        for spp in (1, 4):
+            mg.mg_set_params(s, nu_pre=nu, nu_post=nu, coarse_sweeps=50, sweeps_per_pass=spp, omega=w.omega, mixed_precision=1)
+            dx = to_dev(np.zeros(w.shape), "f32")
+            mg.mg_vcycle(s, dx, db)
+            assert_close(as_f64(dx), x_o, 1e-4, "V(%d,%d) sweeps_per_pass %d" % (nu, nu, spp))
+    # V(1,1) does not converge on this problem (four 1000:1 bubbles, C5): after three cycles the
+    # residual grows by ~2.7 per cycle, and mg_solve has to say so instead of returning MG_NOT_CONVERGED after max_cycles
+    mg.mg_set_params(s, nu_pre=1, nu_post=1, coarse_sweeps=50, sweeps_per_pass=1, omega=w.omega, mixed_precision=1)
+    dx = to_dev(np.zeros(w.shape), "f32")
+    status, cycles, rel = mg.mg_solve(s, dx, db, 1e-6, 10)
+    hist = mg.mg_get_history(s)
+    assert status == mg.MG_STAGNATED and cycles <= 8 and np.isfinite(rel), (status, cycles, rel, hist)
+    assert hist[-1] > 0.95 * hist[-2]
     mg.mg_destroy(s)
 
 
@@ -51,12 +64,14 @@ def test_config5_full_size(mg, orc):
     dqt = [torch.empty_like(dC) for _ in range(3)]; dqh = [torch.empty_like(dC) for _ in range(3)]
     mg.mom_predictor(dC, (du, dv, dw), (du, dv, dw), w.h, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, dqt, dqh)
     for c in range(3):
-        assert rel_l2(as_f64(dqt[c]), qt1[c]) <= TOL["f32"] and rel_l2(as_f64(dqh[c]), qh1[c]) <= TOL["f32"]
+        assert_close(as_f64(dqt[c]), qt1[c], TOL["f32"])
+        assert_close(as_f64(dqh[c]), qh1[c], TOL["f32"])
     # stage 4 kernel on the initial fields
     s_ref, c_ref = orc.vof_residual(g, Cf, u, v, ww, w.dt)
     ds, dcn = torch.empty_like(dC), torch.empty_like(dC)
     mg.vof_residual(dC, du, dv, dw, w.h, w.dt, ds, dcn)
-    assert rel_l2(as_f64(ds), s_ref) <= 5 * TOL["f32"] and rel_l2(as_f64(dcn), c_ref) <= TOL["f32"]
+    assert_close(as_f64(ds), s_ref, 5 * TOL["f32"])
+    assert_close(as_f64(dcn), c_ref, TOL["f32"])
     # the right-hand side the step will solve for, through the same public calls flow_time_step makes (deterministic):
     # the oracle's own b differs from it by the fp32 cancellation error of a divergence (1e-5 relative), which would
     # mask a 1e-6 residual test
@@ -75,9 +90,9 @@ def test_config5_full_size(mg, orc):
     # oracle: second predictor iteration and right-hand side (parity of those stages), then the residual of the GPU's pressure
     qt2, _ = orc.mom_predictor(g, Cf, qh1, qn, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt)
     for c in range(3):
-        assert rel_l2(qt_gpu[c], qt2[c]) <= 2 * TOL["f32"]
+        assert_close(qt_gpu[c], qt2[c], 2 * TOL["f32"])
     k = orc.k_from_vof(Cf, w.rho_l, w.rho_g)
-    assert rel_l2(b_gpu, orc.pressure_rhs(g, qt2[0], qt2[1], qt2[2], w.dt)) <= 50 * TOL["f32"]
+    assert_close(b_gpu, orc.pressure_rhs(g, qt2[0], qt2[1], qt2[2], w.dt), 50 * TOL["f32"])
     p = as_f64(dp)
     r = orc.residual(g, w.bc, k, p, b_gpu)
     # the solver converged its fp64 iterate to rel < 1e-6; what it returns is that iterate rounded to fp32, and the
@@ -85,7 +100,7 @@ def test_config5_full_size(mg, orc):
     assert np.linalg.norm(r) / np.linalg.norm(b_gpu) < 1e-5
     un, vn, wn = orc.project_velocity(g, w.bc, p, k, w.dt, qt_gpu[0], qt_gpu[1], qt_gpu[2])
     for a, ref in ((du, un), (dv, vn), (dw, wn)):
-        assert rel_l2(as_f64(a), ref) <= 2 * TOL["f32"]
+        assert_close(as_f64(a), ref, 2 * TOL["f32"])
     _, Cn = orc.vof_residual(g, Cf, un, vn, wn, w.dt)
-    assert rel_l2(as_f64(dC), Cn) <= 2 * TOL["f32"]
+    assert_close(as_f64(dC), Cn, 2 * TOL["f32"])
     mg.mg_destroy(s)

@@ -6,6 +6,7 @@ import pytest
 
 from workloads import configs, rng
 from test_gpu_mg import TOL, as_f64, make_solver, mg, quantise, rel_l2, to_dev  # noqa: F401
+from _parity import assert_close  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 N, D = configs.BC_NEUMANN, configs.BC_DIRICHLET
@@ -30,14 +31,14 @@ def test_pcg_first_iterations_and_converged_solution(mg, orc, dt):
         st, n, rel = mg.mg_pcg_solve(s, dx, db, 0.0, iters)
         x_o, n_o, rel_o, _ = orc.pcg_solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, 0.0, iters)
         assert n == n_o == iters
-        assert rel_l2(as_f64(dx), x_o) <= (50 * iters * TOL[dt] if dt == "f32" else 1e-9)
+        assert_close(as_f64(dx), x_o, (50 * iters * TOL[dt] if dt == "f32" else 1e-9))
         assert abs(rel - rel_o) <= (2e-3 if dt == "f32" else 1e-8) * rel_o
     dx = to_dev(np.zeros(w.shape), dt)
     st, n, rel = mg.mg_pcg_solve(s, dx, db, 1e-9, 100)
     x_o, n_o, rel_o, hist_o = orc.pcg_solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, 1e-12, 100)
     _, n_tol, _, _ = orc.pcg_solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, 1e-9, 100)
     assert st == mg.MG_OK and rel < 1e-9 and abs(n - n_tol) <= 2
-    assert rel_l2(as_f64(dx), x_o) <= 1e-6
+    assert_close(as_f64(dx), x_o, 1e-6)
     hist = mg.mg_get_history(s)
     assert len(hist) == n
     # the recursively updated residual is the true one (fp64 vectors): check with the oracle's residual of the result
