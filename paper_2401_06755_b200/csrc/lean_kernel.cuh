@@ -63,7 +63,6 @@ struct LParams {
     const float* dinv_c;        // RR, variable k: 1 / D_c on the coarse level
     float gc_const;             // RR, constant k: omega / w0_c
     int first_sweep;            // RR: write x_c = omega b_c / D_c (1) or zeros (0)
-    int bar2;                   // experiment: block barrier every second plane
     int zero_x;                 // SWEEP: the iterate is zero whatever `src` holds: its planes are not read (12 B/point, not 16)
     // MODE_SEED: the first TWO sweeps of a cycle from a zero guess in one pass over y = b / D (written by the defect kernel):
     // x_2 = omega (2 - omega) y + (omega^2 / D) cc (k S(y) + S(k y)) -- the sweep formula x' = om_x x + (om_g / D)(b + cc (..))
@@ -371,17 +370,6 @@ __device__ __forceinline__ void lean_body(const CUtensorMap& tmx, const CUtensor
         const int p = pfirst + dir * it;
         const int slot = it & (NS - 1);
         // ---- ring hand-back: everyone has finished iteration it - 1, so its slot can be refilled ----
-        if (!WAVE && P.bar2) {
-            // one block barrier per TWO planes: at an even iteration the slots of it - 2 and it - 1 are handed back together
-            if (PAR == 0) {
-                __syncthreads();
-                if (tid == 0 && it >= 2) {
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    if (it - 2 + NS < niter) issue(it - 2 + NS);
-                    if (it - 1 + NS < niter) issue(it - 1 + NS);
-                }
-            }
-        } else {
         __syncthreads();
         if (WAVE) {
             if (tid < 32) {
@@ -401,7 +389,6 @@ __device__ __forceinline__ void lean_body(const CUtensorMap& tmx, const CUtensor
         } else if (tid == 0 && it >= 1 && it - 1 + NS < niter) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             issue(it - 1 + NS);
-        }
         }
         mbar_wait(&bars[slot], (uint32_t)((it / NS) & 1));
 
