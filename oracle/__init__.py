@@ -189,21 +189,50 @@ def _ptr3(arrs):
     return (C.c_void_p * 3)(*[a.ctypes.data for a in arrs])
 
 
-def mom_predictor(g, Cf, qh, qn, rho_l, rho_g, mu_l, mu_g, dt):
-    """qh, qn: 3-tuples (u, v, w).  Returns (q_tilde, q_half_new), each a 3-tuple."""
+def mom_predictor(g, Cf, qh, qn, rho_l, rho_g, mu_l, mu_g, dt, vbc=None):
+    """qh, qn: 3-tuples (u, v, w).  vbc as in pressure_rhs().  Returns (q_tilde, q_half_new), each a 3-tuple."""
     Cf = _f64(Cf)
     qh = [_f64(a) for a in qh]; qn = [_f64(a) for a in qn]
     qt = [np.empty(g.shape) for _ in range(3)]; qhn = [np.empty(g.shape) for _ in range(3)]
-    lib().orc_mom_predictor(C.byref(g), _p(Cf), _ptr3(qh), _ptr3(qn), C.c_double(rho_l), C.c_double(rho_g),
-                            C.c_double(mu_l), C.c_double(mu_g), C.c_double(dt), _ptr3(qt), _ptr3(qhn))
+    lib().orc_mom_predictor_bc(C.byref(g), _p(Cf), _ptr3(qh), _ptr3(qn), _vbc(vbc), C.c_double(rho_l), C.c_double(rho_g),
+                               C.c_double(mu_l), C.c_double(mu_g), C.c_double(dt), _ptr3(qt), _ptr3(qhn))
     return tuple(qt), tuple(qhn)
 
 
-def pressure_rhs(g, u, v, w, dt):
+def pressure_rhs(g, u, v, w, dt, vbc=None):
+    """vbc: None (velocity halos are copies) or the 18 halo codes of velocity_bc()."""
     u = _f64(u); v = _f64(v); w = _f64(w)
     b = np.empty(g.shape)
-    lib().orc_pressure_rhs(C.byref(g), _p(u), _p(v), _p(w), C.c_double(dt), _p(b))
+    lib().orc_pressure_rhs_bc(C.byref(g), _p(u), _p(v), _p(w), _vbc(vbc), C.c_double(dt), _p(b))
     return b
+
+
+# halo codes (0 copy, 1 odd about the face, 2 zero) of (u, v, w) on the faces x-, x+, y-, y+, z-, z+
+FREE_SLIP_OPEN_TOP = (1, 1, 0, 0, 0, 0,   0, 0, 1, 1, 0, 0,   0, 0, 0, 0, 1, 0)
+
+
+def velocity_bc(walls=(1, 1, 1, 1, 1, 0)):
+    """Free-slip halo codes: on a wall face the component normal to it is odd about the face (zero normal
+    velocity on the wall), the tangential ones and everything on an open face are copied."""
+    out = []
+    for comp in range(3):
+        out += [1 if walls[f] and f // 2 == comp else 0 for f in range(6)]
+    return tuple(out)
+
+
+def _vbc(vbc):
+    return None if vbc is None else (C.c_int * 18)(*[int(b) for b in vbc])
+
+
+def mom_forcing(g, Cf, p_hs, p_nh, pbc, grav, st, rho_l, rho_g, dt, qt):
+    """q~ <- q~ - (dt / rho) (grad p_hs + grad p~_nh - M (s + s_t))  (Eq. 18's forcing terms).  p_hs, p_nh, st may be None.
+    Returns the new 3-tuple."""
+    Cf = _f64(Cf)
+    qt = [np.array(a, dtype=np.float64, order="C") for a in qt]
+    st = None if st is None else [_f64(a) for a in st]
+    lib().orc_mom_forcing(C.byref(g), _p(Cf), _p(_f64(p_hs)), _p(_f64(p_nh)), _bc(pbc), C.c_double(grav),
+                          None if st is None else _ptr3(st), C.c_double(rho_l), C.c_double(rho_g), C.c_double(dt), _ptr3(qt))
+    return tuple(qt)
 
 
 def pressure_rhs_paper(g, Cf, u, v, w, rho_l, rho_g, dt):
@@ -277,3 +306,36 @@ def time_step_paper(g, bc, Cf, u, v, w, levels, rho_l, rho_g, mu_l, mu_g, dt, cy
         p = p + dp
     _, Cn = vof_residual(g, Cf, un, vn, wn, dt)
     return Cn, un, vn, wn, p, rel
+
+
+BC_PRESSURE = (0, 0, 0, 0, 0, 1)      # p_hs and p_nh: zero derivative on the sides / bottom, zero value on the top face
+
+
+def time_step_full(g, Cf, u, v, w, p_nh, levels, rho_l, rho_g, mu_l, mu_g, grav, sigma_t, dt, tol, max_cycles,
+                   hs_tol=0.0, hs_cycles=20, walls=(1, 1, 1, 1, 1, 0), nu_pre=2, nu_post=2, coarse_sweeps=50, omega=2.0 / 3.0):
+    """One time step of the paper's four-stage method, composed from the oracle's steps:
+      stage 1: b_hs, s_t from C^n (Eqs. 20-23, 43-44); A p_hs = b_hs, constant coefficient, from p_hs = 0,
+                           `hs_cycles` cycles (the paper's fixed 20) or to `hs_tol`
+      stage 2: q_half = q_n; twice: q~ from Eq. 45 with the FULL source of Eq. 18 -- advection + Petrov-Galerkin
+                           diffusion (mom_predictor, free-slip velocity halos P:538), then the pressure gradients of
+                           p_hs and of the previous p_nh and the buoyancy / surface-tension sources (mom_forcing);
+                           q_half = (q_n + q~) / 2 (Eq. 46)
+      stage 3 (P:445-498, reading C10): b = -(1/dt) D.q~ with the wall halos; A(1/rho) dp = b; q = q~ - dt k G dp (Eq. 54);
+                           p_nh += dp
+      stage 4: C_new = C_n - dt s~_C(C_n, q) (Eqs. 16, 55)
+    Returns (C_new, u, v, w, p_hs, p_nh_new, cycles, relres)."""
+    vbc = velocity_bc(walls)
+    b_hs, _, st = hydrostatic_rhs(g, Cf, rho_l, rho_g, grav, sigma_t)
+    p_hs, _, _, _ = solve(g, BC_PRESSURE, None, np.zeros(g.shape), b_hs, levels, hs_tol, hs_cycles, nu_pre, nu_post, coarse_sweeps, omega)
+    qn = (u, v, w)
+    qh = qn
+    for _ in range(2):
+        qt, _ = mom_predictor(g, Cf, qh, qn, rho_l, rho_g, mu_l, mu_g, dt, vbc)
+        qt = mom_forcing(g, Cf, p_hs, p_nh, BC_PRESSURE, grav, st, rho_l, rho_g, dt, qt)
+        qh = tuple(0.5 * (a + b) for a, b in zip(qn, qt))
+    k = k_from_vof(Cf, rho_l, rho_g)
+    b = pressure_rhs(g, qt[0], qt[1], qt[2], dt, vbc)
+    dp, cycles, rel, _ = solve(g, BC_PRESSURE, k, np.zeros(g.shape), b, levels, tol, max_cycles, nu_pre, nu_post, coarse_sweeps, omega)
+    un, vn, wn = project_velocity(g, BC_PRESSURE, dp, k, dt, qt[0], qt[1], qt[2])
+    _, Cn = vof_residual(g, Cf, un, vn, wn, dt)
+    return Cn, un, vn, wn, p_hs, (np.zeros(g.shape) if p_nh is None else _f64(p_nh)) + dp, cycles, rel

@@ -659,6 +659,56 @@ void orc_hydrostatic_rhs(const orc_grid* g, const double* C, double rho_l, doubl
     free(kap); free(t);
 }
 
+/* ------------------------------------------------------------------------------------
+ * Stage 2, the forcing terms of Eq. 18 that the advection-diffusion residual above leaves out (
+ * SURVEY 8(f) next 3):   + f(p_hs + p~_nh; w_x|y|z)  - f(s_c + s_tc; w_m),   nodal.
+ * Eq. 45 is linear in s~, so they are applied to the predicted velocity afterwards:
+ *   q~_c  <-  q~_c - (dt / rho) ( d_c p_hs + d_c p~_nh - M (s_c + s_tc) ),   M = consistent mass filter / m_l,
+ * with s_u = s_v = 0, s_w = -g rho (Eq. 20) and s_t from orc_hydrostatic_rhs (Eq. 21).
+ * Halos: p_hs -- zero derivative on the sides, zero value on the top face (ghost = -mirror), and at the bottom the
+ * extrapolation ghost = mirror + hz g rho(nearest node) that enforces dp_hs/dz = -rho g (the same ghost
+ * orc_hydrostatic_rhs folds into b_hs);  p~_nh -- the factors pbc of its solver;  sources -- copies (reading C9-iv).
+ * p_hs, p_nh, st may be NULL (term absent). */
+static double ghost_phs(const double* p, const double* rho, const orc_grid* g, double grav, int i, int j, int k) {
+    if (i < 0) i = -1 - i; else if (i >= g->nx) i = 2 * g->nx - 1 - i;
+    if (j < 0) j = -1 - j; else if (j >= g->ny) j = 2 * g->ny - 1 - j;
+    if (k < 0) return p[IDX(g, i, j, -1 - k)] + g->hz * grav * rho[IDX(g, i, j, -1 - k)];
+    if (k >= g->nz) return -p[IDX(g, i, j, 2 * g->nz - 1 - k)];
+    return p[IDX(g, i, j, k)];
+}
+void orc_mom_forcing(const orc_grid* g, const double* C, const double* p_hs, const double* p_nh, const int* pbc,
+                     double grav, const double* const* st, double rho_l, double rho_g, double dt, double* const* qt) {
+    const size_t n = (size_t)g->nx * g->ny * g->nz;
+    double wd[27], wm[27];
+    orc_filter(g, 7, wm);
+    double* rho = (double*)malloc(n * sizeof(double));
+    double* src = (double*)malloc(n * sizeof(double));
+    double* t = (double*)malloc(n * sizeof(double));
+    for (size_t c = 0; c < n; ++c) rho[c] = rho_l * C[c] + rho_g * (1.0 - C[c]);
+    for (int d = 0; d < 3; ++d) {
+        orc_filter(g, 1 + d, wd);
+        for (size_t c = 0; c < n; ++c) src[c] = (st && st[d] ? st[d][c] : 0.0) + (d == 2 ? -grav * rho[c] : 0.0);
+        orc_apply_filter(g, BC_COPY, wm, src, t);                                   /* f(s_c + s_tc; w_m) */
+        for (size_t c = 0; c < n; ++c) qt[d][c] += dt * t[c] / rho[c];
+        if (p_nh) {
+            orc_apply_filter(g, pbc, wd, p_nh, t);                                  /* f(p~_nh; w_d) */
+            for (size_t c = 0; c < n; ++c) qt[d][c] -= dt * t[c] / rho[c];
+        }
+        if (p_hs)
+            for (int k = 0; k < g->nz; ++k)
+                for (int j = 0; j < g->ny; ++j)
+                    for (int i = 0; i < g->nx; ++i) {
+                        double a = 0.0;                                             /* f(p_hs; w_d) */
+                        for (int kk = -1; kk <= 1; ++kk)
+                            for (int jj = -1; jj <= 1; ++jj)
+                                for (int ii = -1; ii <= 1; ++ii)
+                                    a += wd[(ii + 1) + 3 * (jj + 1) + 9 * (kk + 1)] * ghost_phs(p_hs, rho, g, grav, i + ii, j + jj, k + kk);
+                        qt[d][IDX(g, i, j, k)] -= dt * a / rho[IDX(g, i, j, k)];
+                    }
+    }
+    free(rho); free(src); free(t);
+}
+
 /* Velocity projection, Eq. 54 with Eq. 48: q = q~ - dt k . f(p; w_x|y|z),
  * k = 1/rho; halo of p by the solver's BC factors.  In place on u, v, w. */
 void orc_project_velocity(const orc_grid* g, const int* bc, const double* p, const double* kcoef, double dt,
