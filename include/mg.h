@@ -141,10 +141,31 @@ int mom_predictor(const mg_grid* grid, int dtype, const void* d_C, const void* c
                   const void* const d_qn[3], double rho_l, double rho_g, double mu_l, double mu_g, double dt,
                   void* const d_qt[3], void* const d_qhn[3], void* cuda_stream);
 
+/* SURVEY 8(f) "next 3": the same predictor with free-slip walls.  vbc[6 c + f] is the halo code (an mg_bc) of velocity
+ * component c = u, v, w on face f: at a wall the component NORMAL to it is odd about the face (MG_BC_DIRICHLET: zero normal
+ * velocity on the wall, the interpolation rule of Fig. 2), the tangential ones and everything on an open face are copied
+ * (MG_BC_NEUMANN).  The halo of a component enters its gradient and its diffusion; derived fields keep copy halos.
+ * vbc = NULL: all copies (= mom_predictor). */
+int mom_predictor_bc(const mg_grid* grid, int dtype, const void* d_C, const void* const d_qh[3], const void* const d_qn[3],
+                     const int vbc[18], double rho_l, double rho_g, double mu_l, double mu_g, double dt, void* const d_qt[3],
+                     void* const d_qhn[3], void* cuda_stream);
+/* SURVEY 8(f) "next 3": the terms of Eq. 18 that the advection-diffusion residual leaves out, applied to the predicted
+ * velocity (Eq. 45 is linear in the source):
+ *   q~_c <- q~_c - (dt / rho) ( f(p_hs + p~_nh; w_c) + f(F_c; w_m) ),   F = -(s + s_t) as written by hydrostatic_rhs_force,
+ * and, if d_qhn != NULL, q_half' = (q_n + q~)/2 (Eq. 46).  Halos: p_hs zero derivative on the sides, zero value on the top face and
+ * the extrapolation ghost mirror + hz g rho below the bottom (dp_hs/dz = -rho g); p~_nh the factors pbc of its solver; F
+ * copies.  d_phs, d_pnh, d_force may be NULL (term absent).  d_qt is updated in place. */
+int mom_forcing(const mg_grid* grid, int dtype, const void* d_C, const void* d_phs, const void* d_pnh, const int pbc[6], double g,
+                const void* const d_force[3], double rho_l, double rho_g, double dt, void* const d_qt[3], const void* const d_qn[3],
+                void* const d_qhn[3], void* cuda_stream);
+
 /* a10: b = -(1/dt) (f(u; w_x) + f(v; w_y) + f(w; w_z)), nodal FE filters of Eq. 11
  * (structure of Eq. 53; reading C10). */
 int pressure_rhs(const mg_grid* grid, int dtype, const void* d_u, const void* d_v, const void* d_w, double dt,
                  void* d_b, void* cuda_stream);
+/* the same with the velocity halo codes vbc of mom_predictor_bc (NULL: copies) */
+int pressure_rhs_bc(const mg_grid* grid, int dtype, const void* d_u, const void* d_v, const void* d_w, const int vbc[18], double dt,
+                    void* d_b, void* cuda_stream);
 /* SURVEY 8(f) "next 2", the paper's own stage-3 right-hand side, Eqs. 52-53: density on the right, constant-
  * coefficient Laplacian:  b = -(1/dt) sum_d f(rho q_d; w_d) + (1/dt) sum_d q_d f(rho; w_d),  rho = rho_l C + rho_g (1 - C). */
 int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w,
@@ -159,6 +180,10 @@ int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const vo
  * OPPOSITE sign of Eq. 5 as printed (kappa = +div n_t); b is numerically the b of Eq. 44 as printed either way. */
 int hydrostatic_rhs(const mg_grid* grid, int dtype, const void* d_C, double rho_l, double rho_g, double g, double sigma_t,
                     void* d_b, void* d_kappa_out, void* cuda_stream);
+/* the same, also writing the force field F = -(s + s_t) = (-s_tu, -s_tv, g rho - s_tw) (Eqs. 20-21) whose FE divergence is b before
+ * the bottom-boundary fold; mom_forcing takes it.  d_force_out[3] may be NULL. */
+int hydrostatic_rhs_force(const mg_grid* grid, int dtype, const void* d_C, double rho_l, double rho_g, double g, double sigma_t,
+                          void* d_b, void* d_kappa_out, void* const d_force_out[3], void* cuda_stream);
 /* a10: q <- q - dt k f(p; w_x|y|z), Eq. 54 with Eq. 48; halo of p by bc[6]. */
 int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void* d_p, const void* d_k,
                      double dt, void* d_u, void* d_v, void* d_w, void* cuda_stream);
@@ -177,6 +202,20 @@ int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, voi
 int flow_time_step_pcg(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l,
                        double rho_g, double mu_l, double mu_g, double dt, double tol, int max_iter,
                        int* iters_out, double* relres_out);
+
+/* SURVEY 8(f) "next 3": the paper's FOUR-stage step on device fields, in place:
+ *   stage 1: hydrostatic_rhs_force(C^n); A p_hs = b_hs with the constant-coefficient solver s_hs from p_hs = 0,
+ *                        hs_cycles cycles (the paper's fixed 20) or until hs_tol;
+ *   stage 2: two predictor iterations with free-slip wall halos (mom_predictor_bc) and the forcing terms of Eq. 18
+ *                        (mom_forcing with p_hs, the incoming d_pnh and the force field);
+ *   stage 3 (reading C10): b = -(1/dt) D.q~ (pressure_rhs_bc); A(1/rho) dp = b with s (mg_solve(tol, max_cycles));
+ *                        q = q~ - dt k G dp; d_pnh += dp;
+ *   stage 4: C <- C - dt s~_C(C^n, q^{n+1}).
+ * walls[6]: 1 = free-slip wall, 0 = open face.  s_hs and s: same grid, dtype, device and stream, bc = {N,N,N,N,N,D}, s_hs
+ * with a constant coefficient.  Returns the status of the stage-3 solve; cycles_out / relres_out refer to it. */
+int flow_time_step_full(mg_solver* s_hs, mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_phs, void* d_pnh,
+                        double rho_l, double rho_g, double mu_l, double mu_g, double g, double sigma_t, double dt, double tol,
+                        int max_cycles, double hs_tol, int hs_cycles, const int walls[6], int* cycles_out, double* relres_out);
 
 /* The same time step with the PAPER'S stage 3 (SURVEY 8(f) "next 2"): constant-coefficient Laplacian with the density on the
  * right (Eqs. 52-53), `cycles` V-cycles per solve from a zero guess (the paper's fixed 20), velocity correction Eq. 54,

@@ -24,6 +24,7 @@ EXPORTS = [
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
     "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_pcg", "flow_time_step_paper", "mg_last_error",
+    "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full",
     "mg_version",
 ]
 
@@ -85,6 +86,13 @@ def _load():
     lib.mom_predictor.argtypes = [C.POINTER(MgGrid), i, vp, C.POINTER(vp), C.POINTER(vp), d, d, d, d, d,
                                   C.POINTER(vp), C.POINTER(vp), vp]
     lib.pressure_rhs.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, d, vp, vp]
+    lib.pressure_rhs_bc.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, pi, d, vp, vp]
+    lib.mom_predictor_bc.argtypes = [C.POINTER(MgGrid), i, vp, C.POINTER(vp), C.POINTER(vp), pi, d, d, d, d, d,
+                                     C.POINTER(vp), C.POINTER(vp), vp]
+    lib.mom_forcing.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, pi, d, C.POINTER(vp), d, d, d, C.POINTER(vp), C.POINTER(vp),
+                                C.POINTER(vp), vp]
+    lib.hydrostatic_rhs_force.argtypes = [C.POINTER(MgGrid), i, vp, d, d, d, d, vp, vp, C.POINTER(vp), vp]
+    lib.flow_time_step_full.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, d, d, i, d, i, pi, pi, pd]
     lib.pressure_rhs_paper.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, d, d, vp, vp]
     lib.flow_time_step_paper.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, i, i, pd]
     lib.hydrostatic_rhs.argtypes = [C.POINTER(MgGrid), i, vp, d, d, d, d, vp, vp, vp]
@@ -300,19 +308,52 @@ def _ptr3(ts, sh, dt_, allow_none=False):
     return (C.c_void_p * 3)(*[_dev(t, sh, dt_).value for t in ts])
 
 
-def mom_predictor(C_, qh, qn, h, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn=None, stream=None):
+def mom_predictor(C_, qh, qn, h, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn=None, stream=None, vbc=None):
     g = _grid_of(C_, h)
     sh, dt_ = tuple(C_.shape), C_.dtype
-    return _check(_lib.mom_predictor(C.byref(g), _dtype_code(C_), _dev(C_), _ptr3(qh, sh, dt_), _ptr3(qn, sh, dt_),
-                                     float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt),
-                                     _ptr3(qt, sh, dt_), _ptr3(qhn, sh, dt_, True), _stream_ptr(stream)))
+    return _check(_lib.mom_predictor_bc(C.byref(g), _dtype_code(C_), _dev(C_), _ptr3(qh, sh, dt_), _ptr3(qn, sh, dt_), _vbc(vbc),
+                                        float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt),
+                                        _ptr3(qt, sh, dt_), _ptr3(qhn, sh, dt_, True), _stream_ptr(stream)))
 
 
-def pressure_rhs(u, v, w, h, dt, b, stream=None):
+def _vbc(vbc):
+    return None if vbc is None else (C.c_int * 18)(*[int(b) for b in vbc])
+
+
+def velocity_bc(walls=(1, 1, 1, 1, 1, 0)):
+    """The 18 halo codes of (u, v, w) for free-slip walls: the wall-normal component is odd about a wall
+    (MG_BC_DIRICHLET), everything else is copied (MG_BC_NEUMANN).  Argument marshalling only."""
+    return tuple(MG_BC_DIRICHLET if walls[f] and f // 2 == comp else MG_BC_NEUMANN for comp in range(3) for f in range(6))
+
+
+def pressure_rhs(u, v, w, h, dt, b, stream=None, vbc=None):
     g = _grid_of(u, h)
     sh, dt_ = tuple(u.shape), u.dtype
-    return _check(_lib.pressure_rhs(C.byref(g), _dtype_code(u), _dev(u), _dev(v, sh, dt_), _dev(w, sh, dt_), float(dt),
-                                    _dev(b, sh, dt_), _stream_ptr(stream)))
+    return _check(_lib.pressure_rhs_bc(C.byref(g), _dtype_code(u), _dev(u), _dev(v, sh, dt_), _dev(w, sh, dt_), _vbc(vbc), float(dt),
+                                       _dev(b, sh, dt_), _stream_ptr(stream)))
+
+
+def mom_forcing(C_, p_hs, p_nh, pbc, h, grav, force, rho_l, rho_g, dt, qt, qn=None, qhn=None, stream=None):
+    """q~ updated in place; p_hs, p_nh, force may be None; qhn (with qn) receives (q_n + q~)/2."""
+    g = _grid_of(C_, h)
+    sh, dt_ = tuple(C_.shape), C_.dtype
+    bcarr = (C.c_int * 6)(*[int(b) for b in pbc])
+    return _check(_lib.mom_forcing(C.byref(g), _dtype_code(C_), _dev(C_), _dev(p_hs, sh, dt_, True), _dev(p_nh, sh, dt_, True), bcarr,
+                                   float(grav), _ptr3(force, sh, dt_, True), float(rho_l), float(rho_g), float(dt), _ptr3(qt, sh, dt_),
+                                   _ptr3(qn, sh, dt_, True), _ptr3(qhn, sh, dt_, True), _stream_ptr(stream)))
+
+
+def flow_time_step_full(s_hs, s, C_, u, v, w, p_hs, p_nh, rho_l, rho_g, mu_l, mu_g, grav, sigma_t, dt, tol, max_cycles,
+                        hs_tol=0.0, hs_cycles=20, walls=(1, 1, 1, 1, 1, 0)):
+    """Returns (status, cycles, relres) of the stage-3 solve."""
+    cyc, rel = C.c_int(0), C.c_double(0.0)
+    sh, dt_ = s.shape, s.torch_dtype
+    wl = (C.c_int * 6)(*[int(b) for b in walls])
+    st = _check(_lib.flow_time_step_full(s_hs.handle, s.handle, _dev(C_, sh, dt_), _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_),
+                                         _dev(p_hs, sh, dt_), _dev(p_nh, sh, dt_), float(rho_l), float(rho_g), float(mu_l), float(mu_g),
+                                         float(grav), float(sigma_t), float(dt), float(tol), int(max_cycles), float(hs_tol),
+                                         int(hs_cycles), wl, C.byref(cyc), C.byref(rel)))
+    return st, cyc.value, rel.value
 
 
 def pressure_rhs_paper(C_, u, v, w, h, rho_l, rho_g, dt, b, stream=None):
@@ -332,11 +373,12 @@ def flow_time_step_paper(s, C_, u, v, w, p, rho_l, rho_g, mu_l, mu_g, dt, cycles
     return rel.value
 
 
-def hydrostatic_rhs(C_, h, rho_l, rho_g, grav, sigma_t, b, kappa_out=None, stream=None):
+def hydrostatic_rhs(C_, h, rho_l, rho_g, grav, sigma_t, b, kappa_out=None, stream=None, force_out=None):
     g = _grid_of(C_, h)
     sh, dt_ = tuple(C_.shape), C_.dtype
-    return _check(_lib.hydrostatic_rhs(C.byref(g), _dtype_code(C_), _dev(C_), float(rho_l), float(rho_g), float(grav), float(sigma_t),
-                                       _dev(b, sh, dt_), _dev(kappa_out, sh, dt_, True), _stream_ptr(stream)))
+    return _check(_lib.hydrostatic_rhs_force(C.byref(g), _dtype_code(C_), _dev(C_), float(rho_l), float(rho_g), float(grav), float(sigma_t),
+                                             _dev(b, sh, dt_), _dev(kappa_out, sh, dt_, True), _ptr3(force_out, sh, dt_, True),
+                                             _stream_ptr(stream)))
 
 
 def project_velocity(p, k, h, bc, dt, u, v, w, stream=None):
@@ -365,3 +407,15 @@ def flow_time_step(s, C_, u, v, w, p, rho_l, rho_g, mu_l, mu_g, dt, tol, max_cyc
                                     _dev(p, sh, dt_), float(rho_l), float(rho_g), float(mu_l), float(mu_g), float(dt),
                                     float(tol), int(max_cycles), C.byref(cyc), C.byref(rel)))
     return st, cyc.value, rel.value
+
+
+def mom_predictor_bc(C_, qh, qn, vbc, h, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn=None, stream=None):
+    return mom_predictor(C_, qh, qn, h, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn, stream, vbc)
+
+
+def pressure_rhs_bc(u, v, w, vbc, h, dt, b, stream=None):
+    return pressure_rhs(u, v, w, h, dt, b, stream, vbc)
+
+
+def hydrostatic_rhs_force(C_, h, rho_l, rho_g, grav, sigma_t, b, kappa_out=None, force_out=None, stream=None):
+    return hydrostatic_rhs(C_, h, rho_l, rho_g, grav, sigma_t, b, kappa_out, stream, force_out)

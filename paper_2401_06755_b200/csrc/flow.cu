@@ -79,6 +79,20 @@ bool can_vec(const mg_grid* g, std::initializer_list<const void*> ptrs) {
         else KERNEL<T, 1><<<march_grid<T, 1>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__);              \
     } while (0)
 #define MGB_MARCH(KERNEL, VEC, G, st, ...) MGB_MARCH_W(KERNEL, vec_w<T>(), VEC, G, st, __VA_ARGS__)
+// the instantiation with halo factors (free-slip walls): the trailing arguments are the Halo6 sets
+#define MGB_MARCH_BC(KERNEL, VEC, G, st, ...)                                                                         \
+    do {                                                                                                              \
+        if (VEC) KERNEL<T, vec_w<T>(), true><<<march_grid<T, vec_w<T>()>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__); \
+        else KERNEL<T, 1, true><<<march_grid<T, 1>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__);                       \
+    } while (0)
+
+// halo factors of a field from mg_bc codes (0 copy: +1, 1 odd about the face: -1, 2 zero halo: 0)
+template <typename T>
+Halo6<T> make_halo(const int* codes) {
+    Halo6<T> H;
+    for (int f = 0; f < 6; ++f) H.s[f] = (T)(codes[f] == MG_BC_NEUMANN ? 1.0 : (codes[f] == MG_BC_DIRICHLET ? -1.0 : 0.0));
+    return H;
+}
 
 template <typename T>
 __global__ void __launch_bounds__(256) axpy_kernel(size_t n, T* __restrict__ y, const T* __restrict__ x) {
@@ -139,7 +153,7 @@ int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T
 }
 
 template <typename T>
-int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T* const qn[3], double rho_l, double rho_g,
+int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T* const qn[3], const int* vbc, double rho_l, double rho_g,
                     double mu_l, double mu_g, double dt, T* const qt[3], T* const qhn[3], cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
     const size_t bytes = npts(g->nx, g->ny, g->nz) * sizeof(T);
@@ -150,6 +164,13 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
     const bool vec = can_vec<T>(g, {C, qh[0], qh[1], qh[2], qn[0], qn[1], qn[2], qt[0], qt[1], qt[2], qhn ? qhn[0] : nullptr,
                                     qhn ? qhn[1] : nullptr, qhn ? qhn[2] : nullptr});
     for (int c = 0; c < 3; ++c) {
+        if (vbc) {      // free-slip walls: the component's own halo factors in its gradient and its diffusion
+            const Halo6<T> H = make_halo<T>(vbc + 6 * c);
+            MGB_MARCH_BC(advection_march, vec, G, st, qh[c], qh[0], qh[1], qh[2], adv, H);
+            MGB_MARCH_BC(mom_coeff_march, vec, G, st, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc, H);
+            MGB_MARCH_BC(mom_update_march, vec, G, st, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c], qhn ? qhn[c] : (T*)nullptr, H);
+            continue;
+        }
         MGB_MARCH(advection_march, vec, G, st, qh[c], qh[0], qh[1], qh[2], adv);
         MGB_MARCH(mom_coeff_march, vec, G, st, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc);
         MGB_MARCH(mom_update_march, vec, G, st, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c], qhn ? qhn[c] : (T*)nullptr);
@@ -159,9 +180,28 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
 }
 
 template <typename T>
-int pressure_rhs_t(const mg_grid* g, const T* u, const T* v, const T* w, double dt, T* b, cudaStream_t st) {
+int pressure_rhs_t(const mg_grid* g, const T* u, const T* v, const T* w, const int* vbc, double dt, T* b, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
-    MGB_MARCH(pressure_rhs_march, can_vec<T>(g, {u, v, w, b}), G, st, u, v, w, (T)(1.0 / dt), b);
+    if (vbc) MGB_MARCH_BC(pressure_rhs_march, can_vec<T>(g, {u, v, w, b}), G, st, u, v, w, (T)(1.0 / dt), b, make_halo<T>(vbc),
+                          make_halo<T>(vbc + 6), make_halo<T>(vbc + 12));
+    else MGB_MARCH(pressure_rhs_march, can_vec<T>(g, {u, v, w, b}), G, st, u, v, w, (T)(1.0 / dt), b);
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
+
+// q~ <- q~ - (dt / rho)(grad(p_hs + p_nh) + M F), q_half' = (q_n + q~)/2 (mom_forcing_march)
+template <typename T>
+int mom_forcing_t(const mg_grid* g, const T* C, const T* phs, const T* pnh, const int* pbc, double grav, const T* const F[3],
+                  double rho_l, double rho_g, double dt, T* const qt[3], const T* const qn[3], T* const qhn[3], cudaStream_t st) {
+    const Geo<T> G = make_geo<T>(g, pbc);
+    const bool vec = can_vec<T>(g, {C, phs, pnh, F ? F[0] : nullptr, F ? F[1] : nullptr, F ? F[2] : nullptr, qt[0], qt[1], qt[2],
+                                    qhn ? qn[0] : nullptr, qhn ? qn[1] : nullptr, qhn ? qn[2] : nullptr, qhn ? qhn[0] : nullptr,
+                                    qhn ? qhn[1] : nullptr, qhn ? qhn[2] : nullptr});
+    // five stencil fields: 2-wide packs keep the rolling sums in registers
+    MGB_MARCH_W(mom_forcing_march, 2, vec, G, st, C, phs, pnh, F ? F[0] : (const T*)nullptr, F ? F[1] : (const T*)nullptr,
+                F ? F[2] : (const T*)nullptr, (T)rho_l, (T)rho_g, (T)grav, (T)dt, qt[0], qt[1], qt[2],
+                qhn ? qn[0] : (const T*)nullptr, qhn ? qn[1] : (const T*)nullptr, qhn ? qn[2] : (const T*)nullptr,
+                qhn ? qhn[0] : (T*)nullptr, qhn ? qhn[1] : (T*)nullptr, qhn ? qhn[2] : (T*)nullptr);
     MGB_LAUNCH_CHECK();
     return 0;
 }
@@ -176,14 +216,16 @@ int pressure_rhs_paper_t(const mg_grid* g, const T* C, const T* u, const T* v, c
 }
 
 template <typename T>
-int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, double grav, double sigma_t, T* b, T* kappa, cudaStream_t st) {
+int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, double grav, double sigma_t, T* b, T* kappa,
+                      T* const force[3], cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
     const size_t bytes = npts(g->nx, g->ny, g->nz) * sizeof(T);
     Scratch ws(st), ws2(st);
     int rc;
-    if ((rc = ws.alloc(3, bytes)) || (rc = ws2.alloc(3, bytes))) return rc;
-    T *n0 = (T*)ws.p[0], *n1 = (T*)ws.p[1], *n2 = (T*)ws.p[2], *f0 = (T*)ws2.p[0], *f1 = (T*)ws2.p[1], *f2 = (T*)ws2.p[2];
-    const bool vec = can_vec<T>(g, {C, b, kappa});
+    if ((rc = ws.alloc(3, bytes)) || (!force && (rc = ws2.alloc(3, bytes)))) return rc;
+    T *n0 = (T*)ws.p[0], *n1 = (T*)ws.p[1], *n2 = (T*)ws.p[2];
+    T *f0 = force ? force[0] : (T*)ws2.p[0], *f1 = force ? force[1] : (T*)ws2.p[1], *f2 = force ? force[2] : (T*)ws2.p[2];
+    const bool vec = can_vec<T>(g, {C, b, kappa, force ? force[0] : nullptr, force ? force[1] : nullptr, force ? force[2] : nullptr});
     MGB_MARCH(normals_march, vec, G, st, C, n0, n1, n2);
     MGB_MARCH(surface_tension_march, vec, G, st, C, n0, n1, n2, (T)rho_l, (T)rho_g, (T)grav, (T)sigma_t, f0, f1, f2, kappa);
     MGB_MARCH(pressure_rhs_march, vec, G, st, f0, f1, f2, T(-1), b);       // b = +(f(fu; w_x) + f(fv; w_y) + f(fw; w_z))
@@ -231,10 +273,22 @@ int vof_residual(const mg_grid* grid, int dtype, const void* d_C, const void* d_
                                   (double*)d_sC_out, (double*)d_Cnew_out, st);
 }
 
+static bool vbc_ok(const int* vbc) {
+    for (int e = 0; vbc && e < 18; ++e)
+        if (vbc[e] < 0 || vbc[e] > 2) { set_error("velocity halo code vbc[%d] = %d is not an mg_bc", e, vbc[e]); return false; }
+    return true;
+}
+
 int mom_predictor(const mg_grid* grid, int dtype, const void* d_C, const void* const d_qh[3], const void* const d_qn[3],
                   double rho_l, double rho_g, double mu_l, double mu_g, double dt, void* const d_qt[3], void* const d_qhn[3],
                   void* cuda_stream) {
-    if (!grid_ok(grid, dtype)) return MG_EINVAL;
+    return mom_predictor_bc(grid, dtype, d_C, d_qh, d_qn, nullptr, rho_l, rho_g, mu_l, mu_g, dt, d_qt, d_qhn, cuda_stream);
+}
+
+int mom_predictor_bc(const mg_grid* grid, int dtype, const void* d_C, const void* const d_qh[3], const void* const d_qn[3],
+                     const int vbc[18], double rho_l, double rho_g, double mu_l, double mu_g, double dt, void* const d_qt[3],
+                     void* const d_qhn[3], void* cuda_stream) {
+    if (!grid_ok(grid, dtype) || !vbc_ok(vbc)) return MG_EINVAL;
     if (!d_C || !d_qh || !d_qn || !d_qt || !(dt > 0.0)) { set_error("mom_predictor: NULL argument or dt <= 0"); return MG_EINVAL; }
     for (int c = 0; c < 3; ++c) {
         if (!d_qh[c] || !d_qn[c] || !d_qt[c] || (d_qhn && !d_qhn[c])) { set_error("mom_predictor: NULL component"); return MG_EINVAL; }
@@ -246,19 +300,44 @@ int mom_predictor(const mg_grid* grid, int dtype, const void* d_C, const void* c
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (dtype == MG_F32)
-        return mom_predictor_t<float>(grid, (const float*)d_C, (const float* const*)d_qh, (const float* const*)d_qn, rho_l, rho_g,
+        return mom_predictor_t<float>(grid, (const float*)d_C, (const float* const*)d_qh, (const float* const*)d_qn, vbc, rho_l, rho_g,
                                       mu_l, mu_g, dt, (float* const*)d_qt, (float* const*)d_qhn, st);
-    return mom_predictor_t<double>(grid, (const double*)d_C, (const double* const*)d_qh, (const double* const*)d_qn, rho_l, rho_g,
+    return mom_predictor_t<double>(grid, (const double*)d_C, (const double* const*)d_qh, (const double* const*)d_qn, vbc, rho_l, rho_g,
                                    mu_l, mu_g, dt, (double* const*)d_qt, (double* const*)d_qhn, st);
+}
+
+int mom_forcing(const mg_grid* grid, int dtype, const void* d_C, const void* d_phs, const void* d_pnh, const int pbc[6], double grav,
+                const void* const d_force[3], double rho_l, double rho_g, double dt, void* const d_qt[3], const void* const d_qn[3],
+                void* const d_qhn[3], void* cuda_stream) {
+    if (!grid_ok(grid, dtype)) return MG_EINVAL;
+    if (!d_C || !d_qt || !d_qt[0] || !d_qt[1] || !d_qt[2] || !(dt > 0.0) || !(rho_l > 0.0) || !(rho_g > 0.0) || (d_pnh && !pbc) ||
+        (d_force && (!d_force[0] || !d_force[1] || !d_force[2])) ||
+        (d_qhn && (!d_qn || !d_qn[0] || !d_qn[1] || !d_qn[2] || !d_qhn[0] || !d_qhn[1] || !d_qhn[2]))) {
+        set_error("mom_forcing: NULL argument, dt <= 0 or density <= 0");
+        return MG_EINVAL;
+    }
+    for (int f = 0; pbc && f < 6; ++f)
+        if (pbc[f] < 0 || pbc[f] > 2) { set_error("mom_forcing: pbc[%d] invalid", f); return MG_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (dtype == MG_F32)
+        return mom_forcing_t<float>(grid, (const float*)d_C, (const float*)d_phs, (const float*)d_pnh, pbc, grav, (const float* const*)d_force,
+                                    rho_l, rho_g, dt, (float* const*)d_qt, (const float* const*)d_qn, (float* const*)d_qhn, st);
+    return mom_forcing_t<double>(grid, (const double*)d_C, (const double*)d_phs, (const double*)d_pnh, pbc, grav, (const double* const*)d_force,
+                                 rho_l, rho_g, dt, (double* const*)d_qt, (const double* const*)d_qn, (double* const*)d_qhn, st);
 }
 
 int pressure_rhs(const mg_grid* grid, int dtype, const void* d_u, const void* d_v, const void* d_w, double dt, void* d_b,
                  void* cuda_stream) {
-    if (!grid_ok(grid, dtype)) return MG_EINVAL;
+    return pressure_rhs_bc(grid, dtype, d_u, d_v, d_w, nullptr, dt, d_b, cuda_stream);
+}
+
+int pressure_rhs_bc(const mg_grid* grid, int dtype, const void* d_u, const void* d_v, const void* d_w, const int vbc[18], double dt,
+                    void* d_b, void* cuda_stream) {
+    if (!grid_ok(grid, dtype) || !vbc_ok(vbc)) return MG_EINVAL;
     if (!d_u || !d_v || !d_w || !d_b || !(dt > 0.0)) { set_error("pressure_rhs: NULL argument or dt <= 0"); return MG_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (dtype == MG_F32) return pressure_rhs_t<float>(grid, (const float*)d_u, (const float*)d_v, (const float*)d_w, dt, (float*)d_b, st);
-    return pressure_rhs_t<double>(grid, (const double*)d_u, (const double*)d_v, (const double*)d_w, dt, (double*)d_b, st);
+    if (dtype == MG_F32) return pressure_rhs_t<float>(grid, (const float*)d_u, (const float*)d_v, (const float*)d_w, vbc, dt, (float*)d_b, st);
+    return pressure_rhs_t<double>(grid, (const double*)d_u, (const double*)d_v, (const double*)d_w, vbc, dt, (double*)d_b, st);
 }
 
 int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double rho_l,
@@ -278,11 +357,22 @@ int pressure_rhs_paper(const mg_grid* grid, int dtype, const void* d_C, const vo
 
 int hydrostatic_rhs(const mg_grid* grid, int dtype, const void* d_C, double rho_l, double rho_g, double grav, double sigma_t, void* d_b,
                     void* d_kappa_out, void* cuda_stream) {
+    return hydrostatic_rhs_force(grid, dtype, d_C, rho_l, rho_g, grav, sigma_t, d_b, d_kappa_out, nullptr, cuda_stream);
+}
+
+int hydrostatic_rhs_force(const mg_grid* grid, int dtype, const void* d_C, double rho_l, double rho_g, double grav, double sigma_t,
+                          void* d_b, void* d_kappa_out, void* const d_force_out[3], void* cuda_stream) {
     if (!grid_ok(grid, dtype)) return MG_EINVAL;
-    if (!d_C || !d_b || !(rho_l > 0.0) || !(rho_g > 0.0)) { set_error("hydrostatic_rhs: NULL argument or density <= 0"); return MG_EINVAL; }
+    if (!d_C || !d_b || !(rho_l > 0.0) || !(rho_g > 0.0) || (d_force_out && (!d_force_out[0] || !d_force_out[1] || !d_force_out[2]))) {
+        set_error("hydrostatic_rhs: NULL argument or density <= 0");
+        return MG_EINVAL;
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (dtype == MG_F32) return hydrostatic_rhs_t<float>(grid, (const float*)d_C, rho_l, rho_g, grav, sigma_t, (float*)d_b, (float*)d_kappa_out, st);
-    return hydrostatic_rhs_t<double>(grid, (const double*)d_C, rho_l, rho_g, grav, sigma_t, (double*)d_b, (double*)d_kappa_out, st);
+    if (dtype == MG_F32)
+        return hydrostatic_rhs_t<float>(grid, (const float*)d_C, rho_l, rho_g, grav, sigma_t, (float*)d_b, (float*)d_kappa_out,
+                                        (float* const*)d_force_out, st);
+    return hydrostatic_rhs_t<double>(grid, (const double*)d_C, rho_l, rho_g, grav, sigma_t, (double*)d_b, (double*)d_kappa_out,
+                                     (double* const*)d_force_out, st);
 }
 
 int project_velocity(const mg_grid* grid, const int bc[6], int dtype, const void* d_p, const void* d_k, double dt, void* d_u,
@@ -353,6 +443,75 @@ int flow_time_step(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, voi
 int flow_time_step_pcg(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_p, double rho_l, double rho_g, double mu_l,
                        double mu_g, double dt, double tol, int max_iter, int* iters_out, double* relres_out) {
     return time_step_impl(s, true, d_C, d_u, d_v, d_w, d_p, rho_l, rho_g, mu_l, mu_g, dt, tol, max_iter, iters_out, relres_out);
+}
+
+// The paper's four-stage step (oracle time_step_full):
+//   stage 1: b_hs and the force field F = -(s + s_t) from C^n (Eqs. 20-23, 43-44); A p_hs = b_hs with the constant-coefficient
+//            solver s_hs from p_hs = 0, hs_cycles cycles (the paper's fixed 20) or to hs_tol
+//   stage 2: q_half = q_n; twice: q~ = predictor(C_n; q_half, q_n) with free-slip wall halos, then the forcing terms of
+//            Eq. 18 (grad p_hs, grad of the previous p_nh, mass-filtered sources); q_half = (q_n + q~)/2   (Eqs. 45-46)
+//   stage 3: k = 1/rho(C_n); b = -(1/dt) D.q~ (wall halos); A(k) dp = b with s_nh; q = q~ - dt k G dp; p_nh += dp   (reading C10)
+//   stage 4: C <- C - dt s~_C(C_n, q)
+// walls[6]: 1 = free-slip wall, 0 = open face (x-, x+, y-, y+, z-, z+).  Both solvers: same grid and dtype, bc {N,N,N,N,N,D}.
+int flow_time_step_full(mg_solver* s_hs, mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_phs, void* d_pnh,
+                        double rho_l, double rho_g, double mu_l, double mu_g, double grav, double sigma_t, double dt, double tol,
+                        int max_cycles, double hs_tol, int hs_cycles, const int walls[6], int* cycles_out, double* relres_out) {
+    if (!s || !s_hs || !d_C || !d_u || !d_v || !d_w || !d_phs || !d_pnh || !walls) { set_error("flow_time_step_full: NULL argument"); return MG_EINVAL; }
+    if (s_hs->dtype != s->dtype || s_hs->grid.nx != s->grid.nx || s_hs->grid.ny != s->grid.ny || s_hs->grid.nz != s->grid.nz ||
+        s_hs->grid.hx != s->grid.hx || s_hs->device != s->device || s_hs->st != s->st || s_hs->var_k) {
+        set_error("flow_time_step_full: the two solvers need the same grid, dtype, device and stream, and s_hs a constant coefficient");
+        return MG_EINVAL;
+    }
+    int vbc[18];
+    for (int c = 0; c < 3; ++c)
+        for (int f = 0; f < 6; ++f) vbc[6 * c + f] = (walls[f] && f / 2 == c) ? MG_BC_DIRICHLET : MG_BC_NEUMANN;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    cudaSetDevice(s->device);
+    const size_t n = s->lv[0].n, es = s->dtype == MG_F64 ? 8 : 4, bytes = n * es;
+    cudaStream_t st = s->st;
+    int rc = 0;
+    {
+        Scratch ws(st), ws2(st), ws3(st);
+        if ((rc = ws.alloc(4, bytes)) || (rc = ws2.alloc(4, bytes)) || (rc = ws3.alloc(3, bytes))) { if (prev >= 0) cudaSetDevice(prev); return rc; }
+        void* qt[3] = {ws.p[0], ws.p[1], ws.p[2]};
+        void* qh[3] = {ws2.p[0], ws2.p[1], ws2.p[2]};
+        void* force[3] = {ws3.p[0], ws3.p[1], ws3.p[2]};
+        void* bbuf = ws.p[3];
+        void* dp = ws2.p[3];
+        const void* qn[3] = {d_u, d_v, d_w};
+        const void* fc[3] = {force[0], force[1], force[2]};
+        int status = 0;
+        // stage 1
+        rc = hydrostatic_rhs_force(&s->grid, s->dtype, d_C, rho_l, rho_g, grav, sigma_t, bbuf, nullptr, force, st);
+        if (!rc) rc = cudaMemsetAsync(d_phs, 0, bytes, st) == cudaSuccess ? 0 : MG_ECUDA;
+        if (!rc) { status = mg_solve(s_hs, d_phs, bbuf, hs_tol, hs_cycles, nullptr, nullptr); if (status < 0) rc = status; }
+        // stage 2
+        if (!rc) rc = mom_predictor_bc(&s->grid, s->dtype, d_C, qn, qn, vbc, rho_l, rho_g, mu_l, mu_g, dt, qt, nullptr, st);
+        if (!rc) rc = mom_forcing(&s->grid, s->dtype, d_C, d_phs, d_pnh, s->bc, grav, fc, rho_l, rho_g, dt, qt, qn, qh, st);
+        if (!rc) { const void* qhc[3] = {qh[0], qh[1], qh[2]}; rc = mom_predictor_bc(&s->grid, s->dtype, d_C, qhc, qn, vbc, rho_l, rho_g, mu_l, mu_g, dt, qt, nullptr, st); }
+        if (!rc) rc = mom_forcing(&s->grid, s->dtype, d_C, d_phs, d_pnh, s->bc, grav, fc, rho_l, rho_g, dt, qt, nullptr, nullptr, st);
+        // stage 3
+        if (!rc) rc = mg_set_coefficient_from_vof(s, d_C, rho_l, rho_g);
+        if (!rc) rc = pressure_rhs_bc(&s->grid, s->dtype, qt[0], qt[1], qt[2], vbc, dt, bbuf, st);
+        if (!rc) rc = cudaMemsetAsync(dp, 0, bytes, st) == cudaSuccess ? 0 : MG_ECUDA;
+        if (!rc) { status = mg_solve(s, dp, bbuf, tol, max_cycles, cycles_out, relres_out); if (status < 0) rc = status; }
+        if (!rc) rc = project_velocity(&s->grid, s->bc, s->dtype, dp, s->lv[0].k, dt, qt[0], qt[1], qt[2], st);
+        if (!rc) rc = s->dtype == MG_F32 ? launch_axpy<float>(n, (float*)d_pnh, (const float*)dp, st)
+                                         : launch_axpy<double>(n, (double*)d_pnh, (const double*)dp, st);
+        // stage 4
+        if (!rc) rc = vof_residual(&s->grid, s->dtype, d_C, qt[0], qt[1], qt[2], dt, nullptr, bbuf, st);
+        if (!rc) {
+            cudaMemcpyAsync(d_C, bbuf, bytes, cudaMemcpyDeviceToDevice, st);
+            cudaMemcpyAsync(d_u, qt[0], bytes, cudaMemcpyDeviceToDevice, st);
+            cudaMemcpyAsync(d_v, qt[1], bytes, cudaMemcpyDeviceToDevice, st);
+            cudaMemcpyAsync(d_w, qt[2], bytes, cudaMemcpyDeviceToDevice, st);
+            if (cudaGetLastError() != cudaSuccess) { set_error("flow_time_step_full: copy failed"); rc = MG_ECUDA; }
+        }
+        if (!rc) rc = status;
+    }
+    if (prev >= 0) cudaSetDevice(prev);
+    return rc;
 }
 
 // Time step with the PAPER'S stage 3 (oracle time_step_paper): constant-coefficient Laplacian, density on the

@@ -149,6 +149,31 @@ __device__ __forceinline__ void load9(const Geo<T>& G, const Col<T, W>& c, const
 template <typename T, int W>
 __device__ __forceinline__ size_t at(const Col<T, W>& c, int q) { return c.nxy * q + c.row[1] + c.i; }
 
+// Halo factors of one field, ghost = s * mirror (the clamped loads of load9 deliver the mirror value).  Used for
+// the pressure in the projection (the solver's factors, reading C10) and for velocity components at free-slip walls
+// (the wall-normal component is odd about the wall, s = -1; everything else is copied, s = +1).
+template <typename T> struct Halo6 { T s[6]; };
+template <typename T>
+struct HaloFac { T fl, fr, fy[3]; };      // z-invariant factors of a thread's 3 x 3 neighbourhood
+template <typename T, int W>
+__device__ __forceinline__ HaloFac<T> halo_fac(const Geo<T>& G, const Col<T, W>& c, const Halo6<T>& H) {
+    HaloFac<T> f;
+    // only the outermost lane of a pack's left / right neighbour can be a ghost
+    f.fl = c.i > 0 ? T(1) : H.s[0]; f.fr = c.i + W < G.nx ? T(1) : H.s[1];
+    f.fy[0] = c.j > 0 ? T(1) : H.s[2]; f.fy[1] = T(1); f.fy[2] = c.j < G.ny - 1 ? T(1) : H.s[3];
+    return f;
+}
+template <typename T, int W>
+__device__ __forceinline__ void halo_scale(const Geo<T>& G, const Halo6<T>& H, const HaloFac<T>& f, int z, Pk<T, W> (&n9)[3][3]) {
+    const T fz = z < 0 ? H.s[4] : (z >= G.nz ? H.s[5] : T(1));
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        n9[b][0][0] *= f.fl; n9[b][2][W - 1] *= f.fr;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] * (fz * f.fy[b]);
+    }
+}
+
 // in-plane tensor-product filters of a 3 x 3 neighbourhood
 template <typename V>
 struct InPlane {
@@ -188,17 +213,21 @@ struct ZAcc {
 template <typename V> __device__ __forceinline__ void push(V (&a)[3], const V& v) { a[0] = a[1]; a[1] = a[2]; a[2] = v; }
 
 // b = -(1/dt) (f(u; w_x) + f(v; w_y) + f(w; w_z))  (reading C10; Eq. 53 structure)
-template <typename T, int W>
+// BC: the three fields carry the halo factors Hu, Hv, Hw (free-slip walls); otherwise their halos are copies
+template <typename T, int W, bool BC = false>
 __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_march(const Geo<T> G, const T* __restrict__ u, const T* __restrict__ v,
-                                                             const T* __restrict__ w, T inv_dt, T* __restrict__ bout) {
+                                                             const T* __restrict__ w, T inv_dt, T* __restrict__ bout,
+                                                             const Halo6<T> Hu = {}, const Halo6<T> Hv = {}, const Halo6<T> Hw = {}) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
+    HaloFac<T> fu = {}, fv = {}, fw = {};
+    if (BC) { fu = halo_fac(G, c, Hu); fv = halo_fac(G, c, Hv); fw = halo_fac(G, c, Hw); }
     ZAcc<V> acc; acc.init();       // Mz (Dx My u + Mx Dy v) + Dz (Mx My w)
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
-        load9(G, c, u, z, n9); const V du = in_plane<T, true, false>(G, n9).dm;
-        load9(G, c, v, z, n9); const V dv = in_plane<T, true, false>(G, n9).md;
-        load9(G, c, w, z, n9); const V mw = in_plane<T, false, false>(G, n9).mm;
+        load9(G, c, u, z, n9); if (BC) halo_scale(G, Hu, fu, z, n9); const V du = in_plane<T, true, false>(G, n9).dm;
+        load9(G, c, v, z, n9); if (BC) halo_scale(G, Hv, fv, z, n9); const V dv = in_plane<T, true, false>(G, n9).md;
+        load9(G, c, w, z, n9); if (BC) halo_scale(G, Hw, fw, z, n9); const V mw = in_plane<T, false, false>(G, n9).mm;
         const V ms = G.M[0] * (du + dv), dw = G.D[2][2] * mw;
         const V div = acc.step(ms + dw, G.M[1] * (du + dv), ms - dw);
         const int q = z - 1;
@@ -222,20 +251,15 @@ __global__ void __launch_bounds__(MBX* MBY) project_march(const Geo<T> G, const 
                                                         T* __restrict__ u, T* __restrict__ v, T* __restrict__ w) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
-    // only the outermost lane of a pack's left / right neighbour can be a ghost
-    const T fl = c.i > 0 ? T(1) : G.s[0], fr = c.i + W < G.nx ? T(1) : G.s[1];
-    const T fy[3] = {c.j > 0 ? T(1) : G.s[2], T(1), c.j < G.ny - 1 ? T(1) : G.s[3]};
+    Halo6<T> H;
+#pragma unroll
+    for (int f = 0; f < 6; ++f) H.s[f] = G.s[f];
+    const HaloFac<T> hf = halo_fac(G, c, H);
     GradRoll<T, V> g; g.init();
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, p, z, n9);
-        const T fz = z < 0 ? G.s[4] : (z >= G.nz ? G.s[5] : T(1));
-#pragma unroll
-        for (int b = 0; b < 3; ++b) {
-            n9[b][0][0] *= fl; n9[b][2][W - 1] *= fr;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] * (fz * fy[b]);
-        }
+        halo_scale(G, H, hf, z, n9);
         g.add(G, in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
@@ -247,16 +271,99 @@ __global__ void __launch_bounds__(MBX* MBY) project_march(const Geo<T> G, const 
     }
 }
 
-// steps 1-2 of reading C9: adv = u psi_x + v psi_y + w psi_z
+// Forcing terms of Eq. 18 applied to the predicted velocity:
+//   q~_d <- q~_d - (dt / rho) ( f(p_hs + p~_nh; w_d) + f(F_d; w_m) ),   F = -(s + s_t)  (hydrostatic_rhs' force field),
+// and optionally q_half' = (q_n + q~) / 2 (Eq. 46).  Halos: p_hs zero derivative on the sides, zero value on the top face,
+// and below the bottom plane mirror + hz g rho(mirror) (dp_hs/dz = -rho g); p~_nh the solver's factors G.s; F copies.
+// Either pressure and F may be absent (NULL).
 template <typename T, int W>
-__global__ void __launch_bounds__(MBX* MBY) advection_march(const Geo<T> G, const T* __restrict__ psi, const T* __restrict__ u,
-                                                          const T* __restrict__ v, const T* __restrict__ w, T* __restrict__ adv) {
+__global__ void __launch_bounds__(MBX* MBY) mom_forcing_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ phs,
+                                                            const T* __restrict__ pnh, const T* __restrict__ F0,
+                                                            const T* __restrict__ F1, const T* __restrict__ F2, T rho_l, T rho_g,
+                                                            T grav, T dt, T* __restrict__ q0, T* __restrict__ q1, T* __restrict__ q2,
+                                                            const T* __restrict__ n0, const T* __restrict__ n1,
+                                                            const T* __restrict__ n2, T* __restrict__ h0, T* __restrict__ h1,
+                                                            T* __restrict__ h2) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
+    Halo6<T> Hn, Hh;
+#pragma unroll
+    for (int f = 0; f < 6; ++f) { Hn.s[f] = G.s[f]; Hh.s[f] = T(1); }
+    Hh.s[5] = T(-1);
+    const HaloFac<T> fn = halo_fac(G, c, Hn), fh = halo_fac(G, c, Hh);
+    GradRoll<T, V> g; g.init();
+    ZAcc<V> m0, m1, m2; m0.init(); m1.init(); m2.init();
+    const bool have_p = phs != nullptr || pnh != nullptr, have_f = F0 != nullptr;
+    for (int z = c.z0 - 1; z <= c.z1; ++z) {
+        V n9[3][3], t9[3][3];
+        if (have_p) {
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) n9[b][a] = V{};
+            if (phs) {
+                load9(G, c, phs, z, t9);
+                halo_scale(G, Hh, fh, z, t9);
+                if (z < 0) {                                   // ghost plane below the bottom: + hz g rho(mirror)
+                    V c9[3][3];
+                    load9(G, c, C, z, c9);
+#pragma unroll
+                    for (int b = 0; b < 3; ++b)
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) t9[b][a] = t9[b][a] + (G.h[2] * grav) * (rho_l * c9[b][a] + rho_g * (T(1) - c9[b][a]));
+                }
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] + t9[b][a];
+            }
+            if (pnh) {
+                load9(G, c, pnh, z, t9);
+                halo_scale(G, Hn, fn, z, t9);
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] + t9[b][a];
+            }
+            g.add(G, in_plane<T, true, false>(G, n9));
+        }
+        V s0 = {}, s1 = {}, s2 = {};
+        if (have_f) {
+            load9(G, c, F0, z, t9); s0 = m0.stepM(G, in_plane<T, false, false>(G, t9).mm);
+            load9(G, c, F1, z, t9); s1 = m1.stepM(G, in_plane<T, false, false>(G, t9).mm);
+            load9(G, c, F2, z, t9); s2 = m2.stepM(G, in_plane<T, false, false>(G, t9).mm);
+        }
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            V gx = {}, gy = {}, gz = {};
+            if (have_p) g.grad(G, gx, gy, gz);
+            const size_t c0 = at(c, q);
+            const V Cc = ldv<T, W>(C + c0);
+            const V f = dt / (rho_l * Cc + rho_g * (T(1) - Cc));
+            const V u = ldv<T, W>(q0 + c0) - f * (gx + s0), v = ldv<T, W>(q1 + c0) - f * (gy + s1), w = ldv<T, W>(q2 + c0) - f * (gz + s2);
+            stv(q0 + c0, u); stv(q1 + c0, v); stv(q2 + c0, w);
+            if (h0) {
+                stv(h0 + c0, T(0.5) * (ldv<T, W>(n0 + c0) + u)); stv(h1 + c0, T(0.5) * (ldv<T, W>(n1 + c0) + v));
+                stv(h2 + c0, T(0.5) * (ldv<T, W>(n2 + c0) + w));
+            }
+        }
+    }
+}
+
+// steps 1-2 of reading C9: adv = u psi_x + v psi_y + w psi_z
+template <typename T, int W, bool BC = false>
+__global__ void __launch_bounds__(MBX* MBY) advection_march(const Geo<T> G, const T* __restrict__ psi, const T* __restrict__ u,
+                                                          const T* __restrict__ v, const T* __restrict__ w, T* __restrict__ adv,
+                                                          const Halo6<T> H = {}) {
+    typedef Pk<T, W> V;
+    const Col<T, W> c = make_col<T, W>(G);
+    HaloFac<T> hf = {};
+    if (BC) hf = halo_fac(G, c, H);
     GradRoll<T, V> g; g.init();
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, psi, z, n9);
+        if (BC) halo_scale(G, H, hf, z, n9);
         g.add(G, in_plane<T, true, false>(G, n9));
         const int q = z - 1;
         if (q >= c.z0 && c.ok) {
@@ -278,19 +385,22 @@ __device__ __forceinline__ Pk<T, W> k_abs_pk(const Geo<T>& G, const Pk<T, W>& a,
 
 // momentum: k_c = rho min{k_max, k_abs(c)} + mu (Eqs. 30-32; k_square of the lost Eq. 28 omitted);
 // k_abs from the gradient of the component and the mixed-mass residual a = 2 (Mx My Mz - E) adv (Eq. 29)
-template <typename T, int W>
+template <typename T, int W, bool BC = false>
 __global__ void __launch_bounds__(MBX* MBY) mom_coeff_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ comp,
                                                           const T* __restrict__ u, const T* __restrict__ v, const T* __restrict__ w,
                                                           const T* __restrict__ adv, T rho_l, T rho_g, T mu_l, T mu_g,
-                                                          T* __restrict__ kc) {
+                                                          T* __restrict__ kc, const Halo6<T> H = {}) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
+    HaloFac<T> hf = {};
+    if (BC) hf = halo_fac(G, c, H);
     GradRoll<T, V> g; g.init();
     ZAcc<V> am; am.init();               // Mz of Mx My adv
     V a0 = {}, a0n = {};                 // adv at the centre of planes q, q + 1
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, comp, z, n9);
+        if (BC) halo_scale(G, H, hf, z, n9);
         g.add(G, in_plane<T, true, false>(G, n9));
         load9(G, c, adv, z, n9);
         const V madv = am.stepM(G, in_plane<T, false, false>(G, n9).mm);
@@ -319,18 +429,21 @@ struct Diff3 {
 
 // s = rho adv + f^lap(c, k_c; w_lap) (Eq. 18 without pressure / source terms), q~ = q_n - dt s / rho (Eq. 45, sigma = 0),
 // q_half' = (q_n + q~)/2 (Eq. 46).  w_lap = (Kx My + Mx Ky) Mz + Mx My Kz.
-template <typename T, int W>
+template <typename T, int W, bool BC = false>
 __global__ void __launch_bounds__(MBX* MBY) mom_update_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ comp,
                                                            const T* __restrict__ kc, const T* __restrict__ adv,
                                                            const T* __restrict__ qn, T rho_l, T rho_g, T dt, T* __restrict__ qt,
-                                                           T* __restrict__ qhn) {
+                                                           T* __restrict__ qhn, const Halo6<T> H = {}) {
     typedef Pk<T, W> V;
     const Col<T, W> c = make_col<T, W>(G);
+    HaloFac<T> hf = {};
+    if (BC) hf = halo_fac(G, c, H);
     Diff3<V> L; L.init();                        // w_lap of x, k, k x: Mz of the in-plane (Kx My + Mx Ky) + Kz of the in-plane Mx My
     V x0 = {}, x0n = {}, k0 = {}, k0n = {};
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V nx9[3][3], nk9[3][3], nz9[3][3];
         load9(G, c, comp, z, nx9);
+        if (BC) halo_scale(G, H, hf, z, nx9);    // the component's halo; k_c keeps its copy halo, so ghost(k c) = s k c (mirror)
         load9(G, c, kc, z, nk9);
 #pragma unroll
         for (int b = 0; b < 3; ++b)
