@@ -39,21 +39,28 @@ REF_TIME_BUDGET_S = 150  # wall-clock cap of the oracle arm
 # capture recorded in TRAFFIC_FILE together with the SHA-256 of the kernel source it was taken from; when the source has
 # changed since, the number is stale and `traffic` is null (the file names the profile summary it belongs to)
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "traffic_lean_sweep.json")
-KERNEL_SOURCE = os.path.join(ROOT, "paper_2401_06755_b200", "csrc", "lean_kernel.cuh")
+KERNEL_SOURCES = [os.path.join(ROOT, "paper_2401_06755_b200", "csrc", f) for f in ("lean_kernel.cuh", "lean_body.inc")]
+
+
+def kernel_source_sha256():
+    import hashlib
+    h = hashlib.sha256()
+    for path in KERNEL_SOURCES:
+        with open(path, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
 
 
 def load_traffic():
     """(bytes per launch or None, note)"""
-    import hashlib
     try:
         with open(TRAFFIC_FILE) as f:
             d = json.load(f)
-        with open(KERNEL_SOURCE, "rb") as f:
-            sha = hashlib.sha256(f.read()).hexdigest()
+        sha = kernel_source_sha256()
     except (OSError, ValueError) as e:
         return None, "no traffic record (%s)" % e
     if d.get("source_sha256") != sha:
-        return None, "stale: %s was captured from another version of lean_kernel.cuh" % d.get("from", TRAFFIC_FILE)
+        return None, "stale: %s was captured from another version of lean_kernel.cuh / lean_body.inc" % d.get("from", TRAFFIC_FILE)
     return float(d["dram_bytes_per_launch"]), d.get("from", TRAFFIC_FILE)
 
 

@@ -26,7 +26,7 @@ def _newest_header():
     t = 0.0
     for root in (CSRC, os.path.join(os.path.dirname(HERE), "include")):
         for f in os.listdir(root):
-            if f.endswith((".h", ".cuh")):
+            if f.endswith((".h", ".cuh", ".inc")):
                 t = max(t, os.path.getmtime(os.path.join(root, f)))
     return t
 

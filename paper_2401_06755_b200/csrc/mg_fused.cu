@@ -139,7 +139,6 @@ int fill_stage(mg_solver* s, int l, const StageSpec& sp, const float* src, const
     std::memset(&P, 0, sizeof(P));
     P.nx = L.nx; P.ny = L.ny; P.nz = L.nz;
     P.zchunk = zchunk;
-    P.dir = 1;
     P.sx0 = L.Lf.s[0]; P.sx1 = L.Lf.s[1]; P.sy0 = L.Lf.s[2]; P.sy1 = L.Lf.s[3]; P.sz0 = L.Lf.s[4]; P.sz1 = L.Lf.s[5];
     P.cc = lp.cc; P.icc = (float)(24.0 * L.hx * L.hx);
     P.omega = (float)s->p.omega;

@@ -134,17 +134,25 @@ def main():
     mg.mg_set_coefficient_from_vof(s, f32(w.fields["alpha"]), w.rho_l, w.rho_g)
     b = rhs_from_velocity(w)
     x = torch.zeros_like(b)
-    print("| nu | us per cycle | V-cycles/s | GLUPS | residual reduction over 10 cycles |\n|---|---|---|---|---|")
+    print("| nu | sweeps_per_pass | us per cycle | V-cycles/s | GLUPS | residual over 10 cycles | mg_solve(1e-6, 10) |\n|---|---|---|---|---|---|---|")
     npts = [mg.mg_level_info(s, l)[0] for l in range(w.levels)]
+    names = {mg.MG_OK: "MG_OK", mg.MG_NOT_CONVERGED: "MG_NOT_CONVERGED", mg.MG_STAGNATED: "MG_STAGNATED"}
     for nu in (1, 2, 3, 4):
-        mg.mg_set_params(s, nu_pre=nu, nu_post=nu, coarse_sweeps=50, sweeps_per_pass=1, omega=w.omega, mixed_precision=1)
-        x.zero_()
-        st, cyc, rel = mg.mg_solve(s, x, b, 0.0, 10)
-        h = mg.mg_get_history(s)
-        msc, _ = timed(lambda: mg.mg_vcycle(s, x, b), 50)
-        lups = sum(n * 2 * nu for n in npts[:-1]) + npts[-1] * 50
-        print("| %d | %.1f | %.0f | %.1f | %.2e -> %.2e |" % (nu, msc * 1e3, 1e3 / msc, lups / msc * 1e-6, h[0], h[-1]))
-    print("\n(one sweep per pass: the two-stage temporally fused kernel is slower, DESIGN.md 5.7)")
+        for spp in (1, 4):
+            mg.mg_set_params(s, nu_pre=nu, nu_post=nu, coarse_sweeps=50, sweeps_per_pass=spp, omega=w.omega, mixed_precision=1)
+            x.zero_()
+            st, cyc, rel = mg.mg_solve(s, x, b, 0.0, 10)
+            h = mg.mg_get_history(s)
+            x.zero_()
+            st2, cyc2, rel2 = mg.mg_solve(s, x, b, 1e-6, 10)
+            msc, _ = timed(lambda: mg.mg_vcycle(s, x, b), 50)
+            lups = sum(n * 2 * nu for n in npts[:-1]) + npts[-1] * 50
+            print("| %d | %d | %.1f | %.0f | %.1f | %.2e -> %.2e | %s after %d cycles |"
+                  % (nu, spp, msc * 1e3, 1e3 / msc, lups / msc * 1e-6, h[0], h[-1], names.get(st2, str(st2)), cyc2))
+    print("\n(V(1,1) DIVERGES on this problem -- four 1000:1 bubbles, piecewise-constant transfers: mg_solve reports MG_STAGNATED;"
+          " V(2,2) and up converge slowly, as on config 3.  sweeps_per_pass = 4 is the wave kernel, wave_kernel.cuh: on this grid"
+          " level 0 has 256 tiles, more than fit the machine twice, so it keeps one stage per launch and the coarser levels carry"
+          " up to 4; it is slower than one stage per launch, DESIGN.md 5.8)")
     mg.mg_destroy(s)
     del x, b
 
@@ -179,6 +187,31 @@ def main():
     print("\nthe same 12 steps with V-cycle-preconditioned CG for the pressure (flow_time_step_pcg, not in the paper): %.2f ms per step = "
           "%.1f time-steps/s; iterations per solve %s; last status %d, relres %.2e" % (ms, 1e3 / ms, its[2:], st, rel))
     mg.mg_destroy(s)
+
+    # ---- the paper's four-stage step ----
+    print("\n### The paper's four-stage step (stage 1 hydrostatic + surface-tension pressure, 20 fixed cycles; free-slip walls; "
+          "forcing terms of Eq. 18; stage 3 to 1e-6), flow_time_step_full, from rest under gravity\n")
+    s_hs = solver_for(w)
+    s_nh = solver_for(w)
+    C = f32(w.fields["alpha"])
+    u, v, ww = (torch.zeros_like(C) for _ in range(3))
+    phs, pnh = torch.zeros_like(C), torch.zeros_like(C)
+    dt_full = 0.1 * w.h / 3.0          # Courant 0.1 at the free-fall speed sqrt(2 g H) ~ 3 m/s of a unit box
+    cycs = []
+    for it in range(7):
+        if it == 2:
+            torch.cuda.synchronize(); e0.record()
+        st, cyc, rel = mg.flow_time_step_full(s_hs, s_nh, C, u, v, ww, phs, pnh, w.rho_l, w.rho_g, w.mu_l, w.mu_g, 9.81, 0.0728,
+                                              dt_full, w.tol, 100, 0.0, 20)
+        cycs.append(cyc)
+    e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 5
+    print("5 steps after 2 warm-up steps: %.2f ms per step = %.1f time-steps/s; stage-3 cycles per solve %s; last status %d, relres %.2e;"
+          " max |q| %.4f m/s after 7 steps of %.2e s (g t = %.4f)"
+          % (ms, 1e3 / ms, cycs[2:], st, rel, float(torch.maximum(torch.maximum(u.abs().max(), v.abs().max()), ww.abs().max())),
+             dt_full, 9.81 * 7 * dt_full))
+    mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)
+    del phs, pnh
 
     print("\n### The same step with the paper's own stage 3 (constant-coefficient Laplacian, density on the right, Eqs. 52-53; "
           "2 passes x 20 fixed cycles, P:429, P:498)\n")
