@@ -177,11 +177,11 @@ def pcg_solve(g, bc, k, x, b, levels, tol, max_iter, nu=2, coarse_sweeps=50, ome
     return x, n, rel.value, hist[:n]
 
 
-def vof_residual(g, Cf, u, v, w, dt):
-    """Returns (sC, Cnew)."""
+def vof_residual(g, Cf, u, v, w, dt, detector=3):
+    """detector: 3 = Eq. 33, 5 = the 5-point oscillation detectors of Eq. 34.  Returns (sC, Cnew)."""
     Cf = _f64(Cf); u = _f64(u); v = _f64(v); w = _f64(w)
     s = np.empty(g.shape); cn = np.empty(g.shape)
-    lib().orc_vof_residual(C.byref(g), _p(Cf), _p(u), _p(v), _p(w), C.c_double(dt), _p(s), _p(cn))
+    lib().orc_vof_residual_ex(C.byref(g), _p(Cf), _p(u), _p(v), _p(w), C.c_double(dt), int(detector), _p(s), _p(cn))
     return s, cn
 
 

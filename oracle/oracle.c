@@ -439,8 +439,12 @@ static void mixed_mass_residual(const orc_grid* g, const double* adv, double* a)
 
 /* vof_residual (reading C9, steps 1-12): sC = nodal s~_C of Eq. 16;
  * Cnew (may be NULL) = C - dt sC, Eq. 55. */
-void orc_vof_residual(const orc_grid* g, const double* C, const double* u, const double* v, const double* w,
-                      double dt, double* sC, double* Cnew) {
+/* detector = 3: Eq. 33 (linear 3 x 3 x 3 filters);  detector = 5: the 5-point oscillation detectors of Eq. 34, the
+ * minimum of the three products of consecutive differences over i-2 .. i+2 ("a much more rigorous approach to detecting an
+ * oscillation") -- SURVEY 8(f) next 4, the part of the higher-order scheme the paper prints in full.  Halo of C: copy,
+ * i.e. reflection about the face for the second ghost layer as well (-1 -> 0, -2 -> 1). */
+void orc_vof_residual_ex(const orc_grid* g, const double* C, const double* u, const double* v, const double* w,
+                         double dt, int detector, double* sC, double* Cnew) {
     const size_t n = (size_t)g->nx * g->ny * g->nz;
     const double Kp = 300.0, Km = 300.0;          /* K+, K-  */
     const double beta = 0.1, eps_x = 1e-4;        /* Eq. 36 */
@@ -468,6 +472,17 @@ void orc_vof_residual(const orc_grid* g, const double* C, const double* u, const
                 S[0] = (C0 - ghost(C, g, BC_COPY, i - 1, j, k)) * (ghost(C, g, BC_COPY, i + 1, j, k) - C0);
                 S[1] = (C0 - ghost(C, g, BC_COPY, i, j - 1, k)) * (ghost(C, g, BC_COPY, i, j + 1, k) - C0);
                 S[2] = (C0 - ghost(C, g, BC_COPY, i, j, k - 1)) * (ghost(C, g, BC_COPY, i, j, k + 1) - C0);
+                if (detector == 5) {                                                 /* Eq. 34 */
+                    const int di[3] = {1, 0, 0}, dj[3] = {0, 1, 0}, dk[3] = {0, 0, 1};
+                    for (int d = 0; d < 3; ++d) {
+                        double cv[5];
+                        for (int m = -2; m <= 2; ++m) cv[m + 2] = ghost(C, g, BC_COPY, i + m * di[d], j + m * dj[d], k + m * dk[d]);
+                        const double p0 = (cv[1] - cv[0]) * (cv[2] - cv[1]);
+                        const double p1 = (cv[2] - cv[1]) * (cv[3] - cv[2]);
+                        const double p2 = (cv[3] - cv[2]) * (cv[4] - cv[3]);
+                        S[d] = fmin(p0, fmin(p1, p2));
+                    }
+                }
                 if (C0 > 0.95 || C0 < 0.05) S[0] = S[1] = S[2] = -1.0;
                 /* step 7: Eq. 37 */
                 const double g2 = Cx[c] * Cx[c] + Cy[c] * Cy[c] + Cz[c] * Cz[c];
@@ -495,6 +510,10 @@ void orc_vof_residual(const orc_grid* g, const double* C, const double* u, const
     if (Cnew) for (size_t c = 0; c < n; ++c) Cnew[c] = C[c] - dt * sC[c];            /* step 12: Eq. 55 */
     free(Cx); free(Cy); free(Cz); free(adv); free(a); free(diff);
     for (int d = 0; d < 3; ++d) free(kd[d]);
+}
+void orc_vof_residual(const orc_grid* g, const double* C, const double* u, const double* v, const double* w,
+                      double dt, double* sC, double* Cnew) {
+    orc_vof_residual_ex(g, C, u, v, w, dt, 3, sC, Cnew);
 }
 
 /* Momentum advection-diffusion residual and predictor (Eqs. 18, 30-32, 45-46; P:198-220,

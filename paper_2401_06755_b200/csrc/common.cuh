@@ -41,7 +41,9 @@ inline __host__ __device__ size_t npts(int nx, int ny, int nz) { return (size_t)
 // cudaFuncSetAttribute and the occupancy query apply per device, so a process-wide "done" flag would leave a second GPU
 // of the same process without its opt-in to > 48 KB of dynamic shared memory.
 int sm_count();                                                   // multiprocessors of the current device
-int kernel_setup(const void* fn, int threads, size_t smem, int* ctas_per_sm);   // opt-in + resident blocks per SM
+// opt-in to `smem` bytes of dynamic shared memory (+ the maximum shared-memory carve-out if asked: the TMA-ring kernels want
+// it, the cp.async marching kernels lose a third of their speed without L1) and the resident blocks per SM
+int kernel_setup(const void* fn, int threads, size_t smem, int* ctas_per_sm, bool max_carveout = false);
 
 // ---- launchers of the generic (any spacing, any BC, one sweep per pass) kernels: mg_generic.cu
 template <typename T> int launch_apply(const Level<T>& L, const T* k, const T* x, T* y, cudaStream_t st);

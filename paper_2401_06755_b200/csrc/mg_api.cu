@@ -31,7 +31,7 @@ int sm_count() {
     return cache[dev];
 }
 
-int kernel_setup(const void* fn, int threads, size_t smem, int* ctas_per_sm) {
+int kernel_setup(const void* fn, int threads, size_t smem, int* ctas_per_sm, bool max_carveout) {
     struct Entry { int device; const void* fn; int ctas_per_sm; };
     static std::mutex mu;
     static std::vector<Entry> done;
@@ -40,10 +40,8 @@ int kernel_setup(const void* fn, int threads, size_t smem, int* ctas_per_sm) {
     std::lock_guard<std::mutex> lock(mu);
     for (const Entry& e : done)
         if (e.device == dev && e.fn == fn) { if (ctas_per_sm) *ctas_per_sm = e.ctas_per_sm; return 0; }
-    if (smem > 48 * 1024) {
-        MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    }
+    if (smem > 48 * 1024) MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (max_carveout) MGB_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     int nb = 0;
     MGB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, threads, smem));
     done.push_back({dev, fn, nb > 0 ? nb : 1});

@@ -161,7 +161,7 @@ int launch_stream_cfg(mg_solver* s, int l, const StageSpec& sp, const float* src
     FusedState* fs = (FusedState*)s->fused_state;
     LevelData& L = s->lv[l];
     int ctas_per_sm = 1, rc;
-    if ((rc = kernel_setup((const void*)lk::lean_kernel<C>, C::NT, C::SMEM, &ctas_per_sm))) return rc;
+    if ((rc = kernel_setup((const void*)lk::lean_kernel<C>, C::NT, C::SMEM, &ctas_per_sm, true))) return rc;
     const int tiles = ((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
     // z chunking: minimise (waves over the resident CTA slots) x (planes per block incl. the two halo planes)
     double best_cost = 1e30;
@@ -218,7 +218,7 @@ int launch_wave_cfg(mg_solver* s, int l, const StageSpec* st, int n, float* cur,
     LevelData& L = s->lv[l];
     auto kern = wk::wave_kernel<LX, LY, VAR, MINB>;
     int ctas_per_sm = 1, rc;
-    if ((rc = kernel_setup((const void*)kern, C::NT, C::SMEM, &ctas_per_sm))) return rc;
+    if ((rc = kernel_setup((const void*)kern, C::NT, C::SMEM, &ctas_per_sm, true))) return rc;
     const int gx = (L.nx + C::TX - 1) / C::TX, gy = (L.ny + C::TY - 1) / C::TY, tiles = gx * gy;
     const int slots = fs->sm_count * ctas_per_sm;
     // every block of every stage has to be resident at once for the stages to overlap: as many z chunks as fit

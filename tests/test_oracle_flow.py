@@ -25,7 +25,7 @@ def _constants():
     return out
 
 
-def _vof_1d(C, u, v, w, h, dt, cst):
+def _vof_1d(C, u, v, w, h, dt, cst, detector=3):
     """The scheme of Eqs. 16, 27, 29, 33, 35-42 reduced BY HAND to fields that vary along x only:
     every 3x3x3 filter collapses to its 1-D factor because the mass factors sum to one, the y/z
     diffusion terms vanish, and S^y = S^z = 0 (or -1 under the override).  Constants are read from
@@ -37,6 +37,11 @@ def _vof_1d(C, u, v, w, h, dt, cst):
     a = cst["alpha_a"] * (ap[:-2] - 2 * adv + ap[2:]) / 6.0
     kabs = cst["alpha_kabs"] * h * np.abs(a) / (cst["eps_k"] + np.abs(Cx) / 3.0)
     S = (C - Cp[:-2]) * (Cp[2:] - C)
+    if detector == 5:                         # Eq. 34: min of the three products over i-2 .. i+2; halo = reflection
+        C2 = np.pad(C, 2, mode="symmetric")
+        d = np.diff(C2)                       # d[m] = C2[m+1] - C2[m]; cell i sits at C2[i+2]
+        n = len(C)
+        S = np.minimum(np.minimum(d[0:n] * d[1:n + 1], d[1:n + 1] * d[2:n + 2]), d[2:n + 2] * d[3:n + 3])
     S = np.where((C > cst["C_hi"]) | (C < cst["C_lo"]), -1.0, S)
     wp = -np.maximum(-1.0, np.minimum(0.0, cst["K_plus"] * S))
     wm = np.minimum(1.0, np.maximum(0.0, cst["K_minus"] * S))
@@ -75,6 +80,55 @@ def test_vof_one_dimensional_profile(orc, axis):
     sC, Cn = orc.vof_residual(g, C3, comps[0], comps[1], comps[2], dt)
     assert np.abs(sC - ref.reshape(bshape)).max() < 1e-11 * np.abs(ref).max()
     assert np.abs(Cn - (C3 - dt * sC)).max() < 1e-15                         # Eq. 55
+
+
+@pytest.mark.parametrize("axis", [2, 1, 0])
+def test_vof_five_point_detectors_eq34(orc, axis):
+    """Eq. 34: the same smeared step with wiggles against the hand-reduced 1-D scheme with the 5-point detector; the
+    profile has extrema one cell away from cells where Eq. 33 sees none, so the two detectors differ there (asserted) --
+    and nowhere in the monotone part of the step."""
+    cst = _constants()
+    n, h, dt = 24, 0.05, 0.004
+    i = np.arange(n)
+    C = 0.5 * (1 + np.tanh((i - 11.3) / 1.7)) + 0.04 * np.sin(1.9 * i)
+    u = 1.0 + 0.3 * np.cos(0.4 * i)
+    v, w = 0.35, -0.2
+    ref5, _, _, _ = _vof_1d(C, u, v, w, h, dt, cst, detector=5)
+    ref3, _, _, _ = _vof_1d(C, u, v, w, h, dt, cst, detector=3)
+    assert np.abs(ref5 - ref3).max() > 1e-3 * np.abs(ref3).max()
+    shape = [5, 5, 5]; shape[axis] = n
+    bshape = [1, 1, 1]; bshape[axis] = n
+    g = orc.grid(shape[2], shape[1], shape[0], h)
+    C3 = np.broadcast_to(C.reshape(bshape), shape).copy()
+    comps = [None, None, None]
+    comps[2 - axis] = np.broadcast_to(u.reshape(bshape), shape).copy()
+    rest = [c for c in range(3) if c != 2 - axis]
+    comps[rest[0]], comps[rest[1]] = np.full(shape, v), np.full(shape, w)
+    s5, _ = orc.vof_residual(g, C3, comps[0], comps[1], comps[2], dt, detector=5)
+    s3, _ = orc.vof_residual(g, C3, comps[0], comps[1], comps[2], dt, detector=3)
+    assert np.abs(s5 - ref5.reshape(bshape)).max() < 1e-11 * np.abs(ref5).max()
+    assert np.abs(s3 - ref3.reshape(bshape)).max() < 1e-11 * np.abs(ref3).max()
+
+
+def test_vof_five_point_detector_special_cases(orc):
+    """A monotone profile has no sign change anywhere: min{...} >= 0, no positive (anti-)diffusion weight w+ beyond what
+    Eq. 33 gives, and where the three products are equal (a linear ramp) both detectors agree exactly.  A single-cell
+    spike is seen by the 5-point detector in the two cells on either side of it, by the 3-point one only in the spike."""
+    n, h, dt = 16, 0.1, 0.01
+    g = orc.grid(n, 4, 4, h)
+    i = np.arange(n)
+    ramp = np.broadcast_to((0.2 + 0.04 * i).reshape(1, 1, n), g.shape).copy()       # inside (0.05, 0.95): no override
+    q = [np.full(g.shape, c) for c in (0.7, 0.0, 0.0)]
+    s5, _ = orc.vof_residual(g, ramp, *q, dt, detector=5)
+    s3, _ = orc.vof_residual(g, ramp, *q, dt, detector=3)
+    assert np.abs(s5 - s3)[:, :, 3:-3].max() < 1e-13        # away from the walls (the reflected halo is an extremum)
+    spike = ramp.copy(); spike[:, :, 8] += 0.1                                      # one-cell extremum at i = 8
+    s5, _ = orc.vof_residual(g, spike, *q, dt, detector=5)
+    s3, _ = orc.vof_residual(g, spike, *q, dt, detector=3)
+    differs = np.abs(s5 - s3)[2, 2] > 1e-9
+    # the detectors disagree at i = 6 and i = 10 (their own 3-point product is positive, a neighbouring one is negative); the
+    # directional coefficients there feed the diffusion stencil of the cells next to them
+    assert differs[6:9].all() and differs[9:12].any() and not differs[3:6].any() and not differs[12:13].any()   # walls apart
 
 
 def test_vof_trivial_cases(orc):
