@@ -132,6 +132,11 @@ int mg_set_fused(mg_solver* s, int fused);
  * s~_C / m_l; d_Cnew_out (may be NULL) receives C - dt * sC, Eq. 55. */
 int vof_residual(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v,
                  const void* d_w, double dt, void* d_sC_out, void* d_Cnew_out, void* cuda_stream);
+/* SURVEY 8(f) "next 4", the part of the higher-order scheme the paper prints in full: the same residual with the oscillation
+ * detectors S^x, S^y, S^z chosen by `detector`: 3 = Eq. 33 (three points per direction, = vof_residual), 5 = Eq. 34 (the
+ * minimum of the three products of consecutive differences over i-2 .. i+2; halo of C by reflection).  Other values: MG_EINVAL. */
+int vof_residual_ex(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double dt,
+                    int detector, void* d_sC_out, void* d_Cnew_out, void* cuda_stream);
 
 /* a9: momentum advection-diffusion residual and predictor, Eqs. 18, 30-32, 45-46 (P:198-220,
  * 309-319, 433-441; reading C9 "Momentum").  d_qh[3] = half-level (u, v, w), d_qn[3] = level-n

@@ -24,7 +24,7 @@ EXPORTS = [
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
     "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_pcg", "flow_time_step_paper", "mg_last_error",
-    "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full",
+    "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full", "vof_residual_ex",
     "mg_version",
 ]
 
@@ -83,6 +83,7 @@ def _load():
     lib.mg_launch_count.argtypes = [vp]; lib.mg_launch_count.restype = C.c_longlong
     lib.mg_set_fused.argtypes = [vp, i]
     lib.vof_residual.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, vp, vp, vp]
+    lib.vof_residual_ex.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, i, vp, vp, vp]
     lib.mom_predictor.argtypes = [C.POINTER(MgGrid), i, vp, C.POINTER(vp), C.POINTER(vp), d, d, d, d, d,
                                   C.POINTER(vp), C.POINTER(vp), vp]
     lib.pressure_rhs.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, d, vp, vp]
@@ -298,6 +299,14 @@ def vof_residual(C_, u, v, w, h, dt, sC_out=None, Cnew_out=None, stream=None):
     return _check(_lib.vof_residual(C.byref(g), _dtype_code(C_), _dev(C_), _dev(u, sh, dt_), _dev(v, sh, dt_),
                                     _dev(w, sh, dt_), float(dt), _dev(sC_out, sh, dt_, True), _dev(Cnew_out, sh, dt_, True),
                                     _stream_ptr(stream)))
+
+
+def vof_residual_ex(C_, u, v, w, h, dt, detector, sC_out=None, Cnew_out=None, stream=None):
+    g = _grid_of(C_, h)
+    sh, dt_ = tuple(C_.shape), C_.dtype
+    return _check(_lib.vof_residual_ex(C.byref(g), _dtype_code(C_), _dev(C_), _dev(u, sh, dt_), _dev(v, sh, dt_),
+                                       _dev(w, sh, dt_), float(dt), int(detector), _dev(sC_out, sh, dt_, True),
+                                       _dev(Cnew_out, sh, dt_, True), _stream_ptr(stream)))
 
 
 def _ptr3(ts, sh, dt_, allow_none=False):

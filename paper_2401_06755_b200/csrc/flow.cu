@@ -134,7 +134,7 @@ struct Scratch {  // stream-ordered scratch fields
 };
 
 template <typename T>
-int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double dt, T* sC, T* Cnew, cudaStream_t st) {
+int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double dt, int detector, T* sC, T* Cnew, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
     const size_t bytes = npts(g->nx, g->ny, g->nz) * sizeof(T);
     Scratch ws(st);
@@ -146,6 +146,10 @@ int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T
     const bool vec = can_vec<T>(g, {C, u, v, w, sC, Cnew});
     MGB_MARCH(advection_march, vec, G, st, C, u, v, w, adv);
     // division-heavy: 4-wide packs cost more in registers than they save in loads (231 vs 248 us at 256^3)
+    if (detector == 5) {       // Eq. 34 (vof_coeff_march<T, W, true>)
+        if (vec) vof_coeff_march<T, 2, true><<<march_grid<T, 2>(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
+        else vof_coeff_march<T, 1, true><<<march_grid<T, 1>(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
+    } else
     MGB_MARCH_W(vof_coeff_march, 2, vec, G, st, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
     MGB_MARCH(vof_diffusion_march, vec, G, st, C, adv, kx, ky, kz, (T)dt, sC, Cnew);
     MGB_LAUNCH_CHECK();
@@ -260,16 +264,22 @@ extern "C" {
 
 int vof_residual(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double dt,
                  void* d_sC_out, void* d_Cnew_out, void* cuda_stream) {
+    return vof_residual_ex(grid, dtype, d_C, d_u, d_v, d_w, dt, 3, d_sC_out, d_Cnew_out, cuda_stream);
+}
+
+int vof_residual_ex(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double dt,
+                    int detector, void* d_sC_out, void* d_Cnew_out, void* cuda_stream) {
     if (!grid_ok(grid, dtype)) return MG_EINVAL;
+    if (detector != 3 && detector != 5) { set_error("vof_residual: detector %d is not 3 (Eq. 33) or 5 (Eq. 34)", detector); return MG_EINVAL; }
     if (!d_C || !d_u || !d_v || !d_w || !(dt > 0.0) || (!d_sC_out && !d_Cnew_out) || d_Cnew_out == d_C || d_sC_out == d_C) {
         set_error("vof_residual: NULL / aliased argument or dt <= 0");
         return MG_EINVAL;
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (dtype == MG_F32)
-        return vof_residual_t<float>(grid, (const float*)d_C, (const float*)d_u, (const float*)d_v, (const float*)d_w, dt,
+        return vof_residual_t<float>(grid, (const float*)d_C, (const float*)d_u, (const float*)d_v, (const float*)d_w, dt, detector,
                                      (float*)d_sC_out, (float*)d_Cnew_out, st);
-    return vof_residual_t<double>(grid, (const double*)d_C, (const double*)d_u, (const double*)d_v, (const double*)d_w, dt,
+    return vof_residual_t<double>(grid, (const double*)d_C, (const double*)d_u, (const double*)d_v, (const double*)d_w, dt, detector,
                                   (double*)d_sC_out, (double*)d_Cnew_out, st);
 }
 

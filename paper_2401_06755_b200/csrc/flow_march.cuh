@@ -472,7 +472,16 @@ __global__ void __launch_bounds__(MBX* MBY) mom_update_march(const Geo<T> G, con
 }
 
 // steps 3-10 of reading C9: directional diffusion coefficients k^x, k^y, k^z of the compressive scheme
-template <typename T, int W>
+// Eq. 34: minimum of the three products of consecutive differences of five values in a line
+template <typename V>
+__device__ __forceinline__ V det5(const V& a0, const V& a1, const V& a2, const V& a3, const V& a4) {
+    const V d0 = a1 - a0, d1 = a2 - a1, d2 = a3 - a2, d3 = a4 - a3;
+    return pmin(pmin(d0 * d1, d1 * d2), d2 * d3);
+}
+__device__ __forceinline__ int reflect(int a, int n) { return a < 0 ? -1 - a : (a >= n ? 2 * n - 1 - a : a); }   // copy halo, any depth
+
+// DET5: the oscillation detectors S^x, S^y, S^z are the 5-point ones of Eq. 34 instead of Eq. 33
+template <typename T, int W, bool DET5 = false>
 __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, const T* __restrict__ C, const T* __restrict__ u,
                                                           const T* __restrict__ v, const T* __restrict__ w,
                                                           const T* __restrict__ adv, T k_min, T k_max, T* __restrict__ kx,
@@ -488,13 +497,36 @@ __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, cons
     V a0 = {}, a0n = {};                                          // adv at the centre of planes q, q + 1
     V Cc[3] = {};                                                 // C at the centre of planes q - 1, q, q + 1
     V Sx = {}, Sxn = {}, Sy = {}, Syn = {};                       // Eq. 33 in-plane products of planes q, q + 1
+    // DET5: C at the centre of plane q - 2 (Cm2) and q + 2 (Cp2); x / y neighbours at distance 2 by reflected indices
+    V Cm2 = {}, Cp2 = {};
+    const int il2 = reflect(c.i - 2, G.nx), ir2 = reflect(c.i + W + 1, G.nx);
+    const size_t rowm2 = (size_t)G.nx * reflect(min(c.j, G.ny - 1) - 2, G.ny), rowp2 = (size_t)G.nx * reflect(min(c.j, G.ny - 1) + 2, G.ny);
+    if (DET5) Cc[2] = ldv<T, W>(C + c.nxy * (size_t)reflect(c.z0 - 2, G.nz) + c.row[1] + c.i);    // plane z0 - 2, pushed down to Cc[0] by the time plane z0 is finalised
     for (int z = c.z0 - 1; z <= c.z1; ++z) {
         V n9[3][3];
         load9(G, c, C, z, n9);
         g.add(G, in_plane<T, true, false>(G, n9));
+        if (DET5) Cm2 = Cc[0];                                    // before the push Cc holds planes (z - 3, z - 2, z - 1): plane q - 2
         push(Cc, n9[1][1]);
-        Sx = Sxn; Sxn = (n9[1][1] - n9[1][0]) * (n9[1][2] - n9[1][1]);
-        Sy = Syn; Syn = (n9[1][1] - n9[0][1]) * (n9[2][1] - n9[1][1]);
+        Sx = Sxn; Sy = Syn;
+        if (DET5) {
+            const T* pl = C + c.nxy * (size_t)min(max(z, 0), G.nz - 1);
+            // x: the W + 4 values l2, l1, own 0 .. W - 1, r1, r2 of the centre row
+            T line[W + 4];
+            line[0] = pl[c.row[1] + il2]; line[1] = n9[1][0][0]; line[W + 2] = n9[1][2][W - 1]; line[W + 3] = pl[c.row[1] + ir2];
+#pragma unroll
+            for (int e = 0; e < W; ++e) line[e + 2] = n9[1][1][e];
+#pragma unroll
+            for (int e = 0; e < W; ++e) {
+                const T d0 = line[e + 1] - line[e], d1 = line[e + 2] - line[e + 1], d2 = line[e + 3] - line[e + 2], d3 = line[e + 4] - line[e + 3];
+                Sxn[e] = tmin(tmin(d0 * d1, d1 * d2), d2 * d3);
+            }
+            Syn = det5(ldv<T, W>(pl + rowm2 + c.i), n9[0][1], n9[1][1], n9[2][1], ldv<T, W>(pl + rowp2 + c.i));
+            Cp2 = ldv<T, W>(C + c.nxy * (size_t)reflect(z + 1, G.nz) + c.row[1] + c.i);        // plane q + 2
+        } else {
+            Sxn = (n9[1][1] - n9[1][0]) * (n9[1][2] - n9[1][1]);
+            Syn = (n9[1][1] - n9[0][1]) * (n9[2][1] - n9[1][1]);
+        }
         load9(G, c, adv, z, n9);
         const V madv = am.stepM(G, in_plane<T, false, false>(G, n9).mm);
         a0 = a0n; a0n = n9[1][1];
@@ -504,7 +536,7 @@ __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, cons
             const V a = T(2) * (madv - a0);                                      // step 3, Eq. 29
             const V kabs = k_abs_pk(G, a, Cx, Cy, Cz);                           // step 4, Eq. 27
             const V C0 = Cc[1];
-            V S[3] = {Sx, Sy, (C0 - Cc[0]) * (Cc[2] - C0)};                      // step 5, Eq. 33
+            V S[3] = {Sx, Sy, DET5 ? det5(Cm2, Cc[0], C0, Cc[2], Cp2) : (C0 - Cc[0]) * (Cc[2] - C0)};   // step 5, Eq. 33 / Eq. 34
 #pragma unroll
             for (int e = 0; e < W; ++e)
                 if (C0[e] > T(0.95) || C0[e] < T(0.05)) S[0][e] = S[1][e] = S[2][e] = T(-1);   // override

@@ -127,6 +127,36 @@ def main():
           " the levels from 16^3 down run as one cluster kernel, timed under level 4)")
     mg.mg_destroy(s)
 
+    # ---- what bounds the smoother: sweep time against the footprint, and the wave kernel ----
+    print("\n### What bounds the fine-level smoother: one sweep on 256 x 256 x nz (x, k, b read + x written = 16 B/point)\n")
+    print("| nz | footprint MB | us per sweep | ps per point | effective GB/s |\n|---|---|---|---|---|")
+    for nz in (32, 64, 96, 128, 192, 256):
+        sp = mg.mg_create((256, 256, nz, 1.0 / 256), 1, w.bc, mg.MG_F32)
+        kk = torch.rand((nz, 256, 256), device="cuda") + 0.5
+        bb = torch.randn((nz, 256, 256), device="cuda")
+        mg.mg_set_coefficient(sp, kk)
+        xs = torch.zeros_like(bb)
+        msp, _ = timed(lambda: mg.mg_smooth(sp, xs, bb, 40), 3)
+        n = nz * 65536
+        print("| %d | %.1f | %.2f | %.2f | %.0f |" % (nz, 16.0 * n / 1e6, msp / 40 * 1e3, msp / 40 * 1e9 / n, 16.0 * n / (msp / 40) * 1e-6))
+        mg.mg_destroy(sp)
+        del kk, bb, xs
+    print("\n(footprints up to ~100 MB stay in the 126 MB L2, yet a point costs the same ~3 ps as at 268 MB, where the fields stream from"
+          " HBM: the kernel is bound inside the SM -- issue slots and shared-memory pipe, profiles/r02_ncu_kernels.md -- not by HBM, so"
+          " keeping an intermediate iterate in L2 cannot make a pass cheaper)")
+    print("\n### Config 3 with the wave kernel: sweeps_per_pass stages of a level per launch (wave_kernel.cuh)\n")
+    print("| sweeps_per_pass | us per V-cycle | V-cycles/s | us per sweep (mg_smooth, 24 sweeps) | launches per cycle |\n|---|---|---|---|---|")
+    s = solver_for(w)
+    mg.mg_set_coefficient_from_vof(s, f32(w.fields["alpha"]), w.rho_l, w.rho_g)
+    for spp in (1, 2, 3, 4):
+        mg.mg_set_params(s, nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=spp, omega=w.omega, mixed_precision=1)
+        x = torch.zeros_like(b)
+        msc, _ = timed(lambda: mg.mg_vcycle(s, x, b), 100)
+        l0 = mg.mg_launch_count(s); mg.mg_vcycle(s, x, b); lc = mg.mg_launch_count(s) - l0
+        mss, _ = timed(lambda: mg.mg_smooth(s, x, b, 24), 3)
+        print("| %d | %.1f | %.0f | %.1f | %d |" % (spp, msc * 1e3, 1e3 / msc, mss / 24 * 1e3, lc))
+    mg.mg_destroy(s)
+
     # ---- config 4 ----
     w = configs.config4()
     print("\n## Config 4: 512x512x256 (3 fields = 0.8 GB), four bubbles, 7 levels, V(nu, nu) for nu = 1..4, 10 cycles each\n")
