@@ -3,6 +3,7 @@
 // One stencil stage per pass, three variants:
 //   MODE_SWEEP   weighted-Jacobi sweep                                   x            -> x'
 //   MODE_PRO     prolongation + correction + sweep                      x + P x_c    -> x'   (x_c tile staged by TMA too)
+//   MODE_RES     residual r = b - A x (or y = A x) at full resolution, optionally with ||r||^2 in fp64    x            -> r
 //   MODE_RR      residual, 8-child-mean restriction and the coarse level's first sweep from a
 //                zero guess                                              x            -> b_c, x_c
 //
@@ -46,7 +47,7 @@
 namespace mgb {
 namespace lk {
 
-enum { MODE_SWEEP = 0, MODE_PRO = 1, MODE_RR = 2, MODE_SEED = 3 };
+enum { MODE_SWEEP = 0, MODE_PRO = 1, MODE_RR = 2, MODE_SEED = 3, MODE_RES = 4 };
 
 struct LParams {
     int nx, ny, nz;
@@ -67,6 +68,11 @@ struct LParams {
     // with om_g = omega^2, om_x = omega (2 - omega) and no b term (the b tiles are not fetched, their ring slots are cleared;
     // 12 B/point).  A mode of its own so that the code of the other modes is untouched.
     float om_g, om_x;
+    // MODE_RES: out = rsign (b - A x) (out may be NULL); zero_b: b is absent (its tiles are not fetched), so with rsign = -1
+    // out = A x; acc (may be NULL): sum of out^2 over the grid, accumulated in fp64, one atomic per block
+    float rsign;
+    int zero_b;
+    double* acc;
 };
 
 template <int LX_, int LY_, bool VAR_, int MODE_, int MINB_>

@@ -192,7 +192,9 @@ static int residual_norm(mg_solver* s, const T* x, const T* b, double* out) {
     LevelData& L = s->lv[0];
     MGB_CUDA(cudaMemsetAsync(s->d_acc, 0, sizeof(double), s->st));
     int rc;
-    if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
+    if (sizeof(T) == 4 && s->fused && fused_residual_supported(s))
+        rc = fused_residual(s, (const float*)x, (const float*)b, nullptr, s->d_acc);
+    else if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
         rc = launch_march_residual<T, T>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, x, (const T*)L.k, b, (T*)nullptr, s->d_acc, s->st);
     else rc = launch_residual_norm<T>(lvl<T>(L), (const T*)L.k, x, b, (T*)nullptr, s->d_acc, s->st);
     if (rc) return rc;
@@ -519,6 +521,8 @@ int mg_apply_operator(mg_solver* s, const void* d_x, void* d_y) {
     CHECK_SOLVER(s);
     if (!d_x || !d_y || d_x == d_y) { set_error("mg_apply_operator: NULL or aliased argument"); return MG_EINVAL; }
     LevelData& L = s->lv[0];
+    if (s->dtype == MG_F32 && s->fused && fused_residual_supported(s))      // fp32 uniform grid: streaming kernel, MODE_RES
+        return fused_residual(s, (const float*)d_x, nullptr, (float*)d_y, nullptr);
     ++s->launches;
     if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz)) {   // uniform grid: z-marching kernel, b = NULL -> y = A x
         if (s->dtype == MG_F32)
@@ -535,6 +539,8 @@ int mg_residual(mg_solver* s, const void* d_x, const void* d_b, void* d_r) {
     CHECK_SOLVER(s);
     if (!d_x || !d_b || !d_r || d_x == d_r) { set_error("mg_residual: NULL or aliased argument"); return MG_EINVAL; }
     LevelData& L = s->lv[0];
+    if (s->dtype == MG_F32 && s->fused && fused_residual_supported(s))
+        return fused_residual(s, (const float*)d_x, (const float*)d_b, (float*)d_r, nullptr);
     ++s->launches;
     if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz)) {
         if (s->dtype == MG_F32)

@@ -119,6 +119,8 @@ struct StageSpec {
     float* xc_out = nullptr;        // RR: the coarse level's first sweep (or zeros)
     int first_sweep = 0;            // RR
     int zero_x = 0;                 // SWEEP: the incoming iterate is zero whatever the buffer holds
+    float rsign = 1.f;              // RES: out = rsign (b - A x)
+    double* acc = nullptr;          // RES: sum of out^2 (fp64, added to *acc)
 };
 
 // tensor maps and parameters of one stage (shared by the one-stage and the wave launches)
@@ -130,7 +132,7 @@ int fill_stage(mg_solver* s, int l, const StageSpec& sp, const float* src, const
     const LevelPlan& lp = fs->lp[l];
     int rc;
     if ((rc = make_tmap(tmx, src, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc;
-    if ((rc = make_tmap(tmb, b, L.nx, L.ny, L.nz, C::TX, C::TY))) return rc;
+    if ((rc = make_tmap(tmb, b ? b : src, L.nx, L.ny, L.nz, C::TX, C::TY))) return rc;     // b == NULL (RES: y = A x): never fetched
     if (C::VAR) { if ((rc = make_tmap(tmk, (const float*)L.k, L.nx, L.ny, L.nz, C::PX, C::PY))) return rc; }
     else *tmk = *tmx;
     if (sp.mode == lk::MODE_PRO) { if ((rc = make_tmap(tmc, sp.xc, L.nx / 2, L.ny / 2, L.nz / 2, C::CPX, C::CPY))) return rc; }
@@ -144,6 +146,7 @@ int fill_stage(mg_solver* s, int l, const StageSpec& sp, const float* src, const
     P.omega = (float)s->p.omega;
     P.out = dst; P.xc = sp.xc; P.bc_out = sp.bc_out; P.xc_out = sp.xc_out; P.first_sweep = sp.first_sweep;
     P.zero_x = (sp.mode == lk::MODE_SWEEP && sp.zero_x) ? 1 : 0;
+    if (sp.mode == lk::MODE_RES) { P.rsign = sp.rsign; P.zero_b = b ? 0 : 1; P.acc = sp.acc; }
     if (sp.mode == lk::MODE_SEED) { P.om_g = P.omega * P.omega; P.om_x = P.omega * (2.f - P.omega); P.icc = 0.f; }
     if (sp.mode == lk::MODE_RR) {
         const LevelPlan& cp = fs->lp[l + 1];
@@ -203,6 +206,7 @@ int launch_stream(mg_solver* s, int l, const StageSpec& sp, const float* src, co
     MGB_SCASE(lk::MODE_PRO)
     MGB_SCASE(lk::MODE_RR)
     MGB_SCASE(lk::MODE_SEED)
+    MGB_SCASE(lk::MODE_RES)
 #undef MGB_SCASE
     set_error("stream pass mode %d is not instantiated", sp.mode);
     return MG_EINVAL;
@@ -585,6 +589,20 @@ int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps) {
     if ((rc = sweeps_level(s, 0, x, (float*)s->lv[0].tmp, b, sweeps, nullptr, &res))) return rc;
     if (res != x) MGB_CUDA(cudaMemcpyAsync(x, res, s->lv[0].n * sizeof(float), cudaMemcpyDeviceToDevice, s->st));
     return 0;
+}
+
+// r = b - A x (b != NULL) or y = A x (b == NULL) on the fine level with the streaming kernel (MODE_RES); r may be NULL;
+// acc (may be NULL): ||out||^2 is ADDED to *acc in fp64
+bool fused_residual_supported(mg_solver* s) {
+    if (!fused_supported(s) || ensure_state(s)) return false;
+    return ((FusedState*)s->fused_state)->lp[0].stream;
+}
+int fused_residual(mg_solver* s, const float* x, const float* b, float* r, double* acc) {
+    int rc = ensure_state(s);
+    if (rc) return rc;
+    StageSpec sp;
+    sp.mode = lk::MODE_RES; sp.rsign = b ? 1.f : -1.f; sp.acc = acc;
+    return launch_stream(s, 0, sp, x, b, r);
 }
 
 int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {

@@ -127,7 +127,7 @@ def main():
           " the levels from 16^3 down run as one cluster kernel, timed under level 4)")
     mg.mg_destroy(s)
 
-    # ---- what bounds the smoother: sweep time against the footprint, and the wave kernel (DESIGN.md 5.2) ----
+    # ---- what bounds the smoother: sweep time against the footprint, and the wave kernel (DESIGN.md 5.1, 5.9) ----
     print("\n### What bounds the fine-level smoother: one sweep on 256 x 256 x nz (x, k, b read + x written = 16 B/point)\n")
     print("| nz | footprint MB | us per sweep | ps per point | effective GB/s |\n|---|---|---|---|---|")
     for nz in (32, 64, 96, 128, 192, 256):
@@ -182,7 +182,7 @@ def main():
     print("\n(V(1,1) DIVERGES on this problem -- four 1000:1 bubbles, piecewise-constant transfers: mg_solve reports MG_STAGNATED;"
           " V(2,2) and up converge slowly, as on config 3.  sweeps_per_pass = 4 is the wave kernel, wave_kernel.cuh: on this grid"
           " level 0 has 256 tiles, more than fit the machine twice, so it keeps one stage per launch and the coarser levels carry"
-          " up to 4; it is slower than one stage per launch, DESIGN.md 5.8)")
+          " up to 4; it is slower than one stage per launch, DESIGN.md 5.9)")
     mg.mg_destroy(s)
     del x, b
 
