@@ -49,11 +49,16 @@ typedef struct { int nx, ny, nz; double hx, hy, hz; } mg_grid;
  * restriction) one kernel launch may carry on a level, 1 .. 4 (wave_kernel.cuh); other values are refused
  * with MG_EINVAL; a level on which that many stages do not fit the machine at once gets fewer per launch.
  * Results do not depend on it beyond rounding order.  mixed_precision (MG_F32 only): mg_solve keeps the
- * iterate and the fine-grid residual in fp64 around fp32 V-cycles (reading C6/C8). */
+ * iterate and the fine-grid residual in fp64 around fp32 V-cycles (reading C6/C8).
+ * cycles_per_defect (mixed precision only): V-cycles applied to one correction equation A e = r before the next fp64 defect is
+ * formed -- the first from a zero guess, the others continue the iteration on e with the same r, so in exact arithmetic the
+ * iterates are those of plain cycles; the residual (stopping test, history) is then evaluated every cycles_per_defect cycles
+ * only, which is what saves the time (the fp64 defect and the fp64 update cost 40 % of a cycle).  Default 1: every cycle. */
 typedef struct {
     int nu_pre, nu_post, coarse_sweeps, sweeps_per_pass;
     double omega;
     int mixed_precision;
+    int cycles_per_defect;   /* 1 .. 8, default 1 */
 } mg_params;
 
 enum {

@@ -36,7 +36,8 @@ class MgGrid(C.Structure):
 
 class MgParams(C.Structure):
     _fields_ = [("nu_pre", C.c_int), ("nu_post", C.c_int), ("coarse_sweeps", C.c_int),
-                ("sweeps_per_pass", C.c_int), ("omega", C.c_double), ("mixed_precision", C.c_int)]
+                ("sweeps_per_pass", C.c_int), ("omega", C.c_double), ("mixed_precision", C.c_int),
+                ("cycles_per_defect", C.c_int)]
 
 
 class MgError(RuntimeError):
@@ -194,8 +195,10 @@ def mg_destroy(s):
     s.close()
 
 
-def mg_set_params(s, nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=1, omega=2.0 / 3.0, mixed_precision=1):
-    p = MgParams(int(nu_pre), int(nu_post), int(coarse_sweeps), int(sweeps_per_pass), float(omega), int(mixed_precision))
+def mg_set_params(s, nu_pre=2, nu_post=2, coarse_sweeps=50, sweeps_per_pass=1, omega=2.0 / 3.0, mixed_precision=1,
+                  cycles_per_defect=1):
+    p = MgParams(int(nu_pre), int(nu_post), int(coarse_sweeps), int(sweeps_per_pass), float(omega), int(mixed_precision),
+                 int(cycles_per_defect))
     return _check(_lib.mg_set_params(s.handle, C.byref(p)))
 
 

@@ -71,6 +71,7 @@ namespace mgb {
 int ensure_mixed_buffers(mg_solver* s);   // x64, k64, r32, e32 of the mixed-precision loops (mg_api.cu)
 int vcycle_zero_guess(mg_solver* s, void* x, const void* b);   // V-cycle from x = 0; x need not be initialised (mg_api.cu)
 int launch_axpy_mixed(size_t n, double* x64, const float* e32, cudaStream_t st);  // x64 += e32
+int launch_record_acc(double* acc0, double* hist, int* ctr, cudaStream_t st);     // hist[(*ctr)++] = *acc0; *acc0 = 0
 int launch_cast_f2d(size_t n, const float* a, double* b, cudaStream_t st);
 int launch_cast_d2f(size_t n, const double* a, float* b, cudaStream_t st);
 int launch_k64_from_vof(size_t n, const float* alpha, double rho_l, double rho_g, double* k64, cudaStream_t st);

@@ -9,6 +9,8 @@ bool fused_supported(const mg_solver* s);
 int fused_prepare(mg_solver* s);
 int fused_smooth(mg_solver* s, float* x, const float* b, int sweeps);
 int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess = 0);   // 1: x = 0 implied; 2: x holds b / D (mg_fused.cu)
+int fused_vcycle_prepare(mg_solver* s);        // state + tabulated coarsest solve: before recording fused_vcycle_enqueue in a graph
+int fused_vcycle_enqueue(mg_solver* s, float* x, const float* b, int zero_guess);   // the cycle's launches on s->st, no graph of its own
 bool fused_seed_supported(mg_solver* s);
 bool fused_residual_supported(mg_solver* s);   // the fine level is a streaming-kernel level
 int fused_residual(mg_solver* s, const float* x, const float* b, float* r, double* acc);   // r = b - A x, or A x if b == NULL; ||.||^2 added to *acc

@@ -208,12 +208,13 @@ static int residual_norm(mg_solver* s, const T* x, const T* b, double* out) {
 // Stopping bookkeeping shared by the solve loops (reading C6; stagnation rule of include/mg.h).
 struct Stop {
     double tol; int stag = 0; double prev;
+    double rate = 0.95;      // "no progress" = the residual fell by less than this factor since the last evaluation
     // returns -1 to continue, else the status
     int update(double rel) {
         if (!std::isfinite(rel)) return MG_STAGNATED;
         if (rel < tol) return MG_OK;
         if (tol == 0.0) return -1;  // fixed cycle count (the paper's mode): no stagnation test
-        stag = (rel > 0.95 * prev) ? stag + 1 : 0;
+        stag = (rel > rate * prev) ? stag + 1 : 0;
         prev = rel;
         return stag >= 3 ? MG_STAGNATED : -1;
     }
@@ -243,7 +244,10 @@ static int solve_plain(mg_solver* s, T* x, const T* b, double tol, int max_cycle
 }
 
 // fp32 solver with the fp64 outer defect-correction loop (reading C6 "fp32 reading", C8):
-//   x64 = x;  repeat { r32 = float(b - A64 x64); stop on ||r||/||b||;  e = Vcycle_fp32(0, r32);  x64 += e }
+//   x64 = x;  repeat { r32 = float(b - A64 x64); stop on ||r||/||b||;  e = m V-cycles on A e = r32 from e = 0;  x64 += e }
+// m = cycles_per_defect (1 by default).  One round of the loop -- the m cycles, the update and the next defect with its norm --
+// is ONE CUDA graph: a one-thread kernel files the squared norm in the residual history on the device, so the launches of a
+// round have no gaps between them and a fixed-count solve (tol = 0, the paper's mode) never waits for the host.
 static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int max_cycles, int* cycles_out,
                        double* rel_out) {
     LevelData& L = s->lv[0];
@@ -251,63 +255,76 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     if ((rc = norm2<float>(s, L.n, b, &nb))) return rc;
     if ((rc = launch_cast_f2d(L.n, x, s->x64, s->st))) return rc;
     ++s->launches;
+    const bool marching = s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz);
     // Seeded correction cycles: the defect kernel also writes y = r32 / D into e32, and the cycle's first pass turns y into the
     // iterate after two sweeps from a zero guess (mg_fused.cu) -- one 12-byte pass instead of a 12-byte and a 16-byte one.
-    const bool seeded = s->fused && fused_supported(s) && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz) && fused_seed_supported(s);
-    auto correction_cycle = [&]() -> int { return seeded ? fused_vcycle(s, s->e32, s->r32, 2) : vcycle_zero_guess(s, s->e32, s->r32); };
-    auto resid_into = [&](double* dacc) -> int {      // r32 = float(b - A64 x64), ||r||^2 into *dacc (no read-back)
-        MGB_CUDA(cudaMemsetAsync(dacc, 0, sizeof(double), s->st));
+    const bool seeded = s->fused && fused_supported(s) && marching && fused_seed_supported(s);
+    auto defect_into = [&](double* dacc) -> int {      // r32 = float(b - A64 x64), ||r||^2 ADDED to *dacc
         int r2;
-        if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
+        if (marching)
             r2 = launch_march_residual<double, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, s->x64, s->var_k ? s->k64 : nullptr, b, s->r32,
                                                       dacc, s->st, 0, seeded ? s->e32 : nullptr);
         else r2 = launch_residual_mixed(L.Ld, s->var_k ? s->k64 : nullptr, s->x64, b, s->r32, dacc, s->st);
         if (!r2) ++s->launches;
         return r2;
     };
-    auto resid = [&](double* rel) -> int {
-        MGB_CUDA(cudaMemsetAsync(s->d_acc, 0, sizeof(double), s->st));
+    MGB_CUDA(cudaMemsetAsync(s->d_acc, 0, sizeof(double), s->st));
+    if ((rc = defect_into(s->d_acc))) return rc;
+    if ((rc = read_acc(s, &sq))) return rc;
+    double rel = nb > 0.0 ? std::sqrt(sq) / nb : 0.0;
+    int cycles = 0, status = (rel < tol) ? MG_OK : MG_NOT_CONVERGED;
+    const int m_max = std::max(1, std::min(s->p.cycles_per_defect, 8));
+    Stop stop{tol, 0, rel};
+    // one round: mm cycles on A e = r32, x64 += e, next defect, its squared norm filed at hist[ctr++]
+    auto round = [&](int mm, bool in_graph) -> int {
         int r2;
-        if (s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz))
-            r2 = launch_march_residual<double, float>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, s->x64, s->var_k ? s->k64 : nullptr, b, s->r32,
-                                                      s->d_acc, s->st, 0, seeded ? s->e32 : nullptr);
-        else r2 = launch_residual_mixed(L.Ld, s->var_k ? s->k64 : nullptr, s->x64, b, s->r32, s->d_acc, s->st);
-        if (r2) return r2;
+        for (int i = 0; i < mm; ++i) {
+            if (in_graph) r2 = fused_vcycle_enqueue(s, s->e32, s->r32, i == 0 ? (seeded ? 2 : 1) : 0);
+            else if (i == 0) r2 = seeded ? fused_vcycle(s, s->e32, s->r32, 2) : vcycle_zero_guess(s, s->e32, s->r32);
+            else r2 = vcycle_any<float>(s, s->e32, s->r32);
+            if (r2) return r2;
+        }
+        if ((r2 = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return r2;
         ++s->launches;
-        if ((r2 = read_acc(s, &sq))) return r2;
-        *rel = nb > 0.0 ? std::sqrt(sq) / nb : 0.0;
+        if ((r2 = defect_into(s->d_acc))) return r2;
+        if ((r2 = launch_record_acc(s->d_acc, s->d_acc + 1, s->d_ctr, s->st))) return r2;
+        ++s->launches;
         return 0;
     };
-    double rel;
-    if ((rc = resid(&rel))) return rc;
-    Stop stop{tol, 0, rel};
-    int cycles = 0, status = (rel < tol) ? MG_OK : MG_NOT_CONVERGED;
-    if (tol == 0.0 && max_cycles > 0 && max_cycles < ACC_N) {     // fixed cycle count: enqueue everything, read the norms once
-        for (int c = 0; c < max_cycles; ++c) {
-            if ((rc = correction_cycle())) return rc;
-            if ((rc = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return rc;
-            ++s->launches;
-            if ((rc = resid_into(s->d_acc + 1 + c))) return rc;
-        }
-        MGB_CUDA(cudaMemcpyAsync(s->h_acc + 1, s->d_acc + 1, max_cycles * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+    MGB_CUDA(cudaMemsetAsync(s->d_acc, 0, sizeof(double), s->st));
+    MGB_CUDA(cudaMemsetAsync(s->d_ctr, 0, sizeof(int), s->st));
+    const bool graphs = seeded && !s->timing;          // the fused cycle can be recorded together with the rest of the round
+    if (graphs && (rc = fused_vcycle_prepare(s))) return rc;
+    int rounds = 0, read = 0;
+    std::vector<int> round_cycles;
+    auto fetch = [&](int upto) -> int {                // history entries [read, upto) from the device
+        if (upto <= read) return 0;
+        MGB_CUDA(cudaMemcpyAsync(s->h_acc + 1 + read, s->d_acc + 1 + read, (upto - read) * sizeof(double), cudaMemcpyDeviceToHost, s->st));
         MGB_CUDA(cudaStreamSynchronize(s->st));
-        for (int c = 0; c < max_cycles; ++c) {
+        for (int c = read; c < upto; ++c) {
             rel = nb > 0.0 ? std::sqrt(s->h_acc[1 + c]) / nb : 0.0;
             s->history.push_back(rel);
             if (!std::isfinite(rel)) status = MG_STAGNATED;
         }
-        cycles = max_cycles;
+        read = upto;
+        return 0;
+    };
+    while (status == MG_NOT_CONVERGED && cycles < max_cycles && rounds < ACC_N - 1) {
+        const int mm = std::min(m_max, max_cycles - cycles);
+        if (graphs) rc = replay_graph(s, s->x64, b, [&]() { return round(mm, true); }, 16 + mm);
+        else rc = round(mm, false);
+        if (rc) return rc;
+        cycles += mm; ++rounds;
+        if (tol > 0.0) {                               // tolerance-driven: the host decides after every round
+            if ((rc = fetch(rounds))) return rc;
+            if (status == MG_NOT_CONVERGED) {
+                stop.rate = std::pow(0.95, mm);
+                const int u = stop.update(rel);
+                if (u >= 0) status = u;
+            }
+        }
     }
-    while (status == MG_NOT_CONVERGED && cycles < max_cycles) {
-        if ((rc = correction_cycle())) return rc;
-        if ((rc = launch_axpy_mixed(L.n, s->x64, s->e32, s->st))) return rc;
-        ++s->launches;
-        if ((rc = resid(&rel))) return rc;
-        s->history.push_back(rel);
-        ++cycles;
-        const int u = stop.update(rel);
-        if (u >= 0) status = u;
-    }
+    if ((rc = fetch(rounds))) return rc;               // fixed cycle count: all norms at once
     if ((rc = launch_cast_d2f(L.n, s->x64, x, s->st))) return rc;
     ++s->launches;
     MGB_CUDA(cudaStreamSynchronize(s->st));
@@ -352,8 +369,11 @@ static int alloc_k(mg_solver* s) {
 }
 
 static void invalidate_graph(mg_solver* s) {
-    if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
-    s->graph_x = s->graph_b = nullptr;
+    for (auto& g : s->graphs) {
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+        g = mg_solver::GraphSlot();
+    }
+    ++s->epoch;
 }
 
 }  // namespace mgb
@@ -409,6 +429,7 @@ int mg_create(mg_solver** out, const mg_grid* grid, int levels, const int bc[6],
         if (l > 0) ok = ok && cudaMalloc(&L.x, L.n * es) == cudaSuccess && cudaMalloc(&L.b, L.n * es) == cudaSuccess;
     }
     ok = ok && cudaMalloc(&s->d_acc, ACC_N * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&s->d_ctr, sizeof(int)) == cudaSuccess;
     ok = ok && cudaMallocHost(&s->h_acc, ACC_N * sizeof(double)) == cudaSuccess;
     if (!ok) {
         set_error("mg_create: allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -436,7 +457,7 @@ void mg_destroy(mg_solver* s) {
     for (double* v : s->pcg_v) cudaFree(v);
     cudaFree(s->pcg_s);
     cudaFree(s->hx_dev); cudaFree(s->hb_dev);
-    cudaFree(s->d_acc);
+    cudaFree(s->d_acc); cudaFree(s->d_ctr);
     if (s->h_acc) cudaFreeHost(s->h_acc);
     delete s;
 }
@@ -445,6 +466,10 @@ int mg_set_params(mg_solver* s, const mg_params* p) {
     CHECK_SOLVER(s);
     if (!p || p->nu_pre < 0 || p->nu_post < 0 || p->coarse_sweeps < 0 || !(p->omega > 0.0) || !(p->omega < 2.0)) {
         set_error("mg_set_params: invalid parameters");
+        return MG_EINVAL;
+    }
+    if (p->cycles_per_defect < 1 || p->cycles_per_defect > 8) {
+        set_error("mg_set_params: cycles_per_defect = %d is out of range (1 .. 8)", p->cycles_per_defect);
         return MG_EINVAL;
     }
     // stages per launch of the wave kernel (wave_kernel.cuh): 1 .. 4 are implemented; anything else is refused

@@ -107,6 +107,7 @@ struct FusedState {
     int sm_count = 148;       // multiprocessors of the solver's device
     float* cmat = nullptr;    // the coarsest solve tabulated as a matrix (ctail_kernel.cuh), n_c <= 64
     bool cmat_valid = false;
+    long long cmat_epoch = -1;  // mg_solver::epoch the table was built in (a parameter change bumps it)
     int* wave_sync = nullptr; // wave_kernel: progress flags [WAVE_FLAGS], then the finished-block counter and the error word
 };
 constexpr int WAVE_FLAGS = 8192;
@@ -467,6 +468,14 @@ int refresh_cmat(mg_solver* s) {
     return 0;
 }
 
+// the tabulated coarsest solve follows the coefficient (fused_prepare clears the flag) and the parameters (the solver's epoch)
+int ensure_cmat(mg_solver* s) {
+    FusedState* fs = (FusedState*)s->fused_state;
+    if (fs->cmat_valid && fs->cmat_epoch == s->epoch) return 0;
+    fs->cmat_epoch = s->epoch;
+    return refresh_cmat(s);
+}
+
 int launch_ctail(mg_solver* s, int l, float* x, const float* b, int done, size_t smem, int nd, int ns) {
     FusedState* fs = (FusedState*)s->fused_state;
     ck::CParams P;
@@ -605,12 +614,17 @@ int fused_residual(mg_solver* s, const float* x, const float* b, float* r, doubl
     return launch_stream(s, 0, sp, x, b, r);
 }
 
-int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
+// Everything a cycle needs that must NOT be recorded with it (state, the tabulated coarsest solve): call before
+// fused_vcycle_enqueue when the enqueue happens inside a graph capture.
+int fused_vcycle_prepare(mg_solver* s) {
     int rc = ensure_state(s);
     if (rc) return rc;
-    // the tabulated coarsest solve follows the coefficient (fused_prepare clears the flag) and the parameters (a parameter
-    // change drops the recorded graph)
-    if ((!((FusedState*)s->fused_state)->cmat_valid || !s->graph_exec) && (rc = refresh_cmat(s))) return rc;
+    // the tabulated coarsest solve follows the coefficient (fused_prepare clears the flag) and the parameters (the epoch)
+    return ensure_cmat(s);
+}
+
+// Launch the kernels of one cycle on s->st (no graph of its own: the caller may be recording one).
+int fused_vcycle_enqueue(mg_solver* s, float* x, const float* b, int zero_guess) {
     if (zero_guess) {
         // the first launch of the cycle has to be a lean_kernel sweep of level 0; otherwise clear x and run the general cycle
         FusedState* fs = (FusedState*)s->fused_state;
@@ -623,8 +637,14 @@ int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
             zero_guess = 0;
         }
     }
-    if (s->timing) return enqueue_vcycle(s, x, b, zero_guess);
-    return replay_graph(s, x, b, [&]() { return enqueue_vcycle(s, x, b, zero_guess); }, zero_guess);
+    return enqueue_vcycle(s, x, b, zero_guess);
+}
+
+int fused_vcycle(mg_solver* s, float* x, const float* b, int zero_guess) {
+    int rc = fused_vcycle_prepare(s);
+    if (rc) return rc;
+    if (s->timing) return fused_vcycle_enqueue(s, x, b, zero_guess);
+    return replay_graph(s, x, b, [&]() { return fused_vcycle_enqueue(s, x, b, zero_guess); }, zero_guess);
 }
 
 // the seeded cycle (zero_guess 2) needs a lean_kernel sweep as the first launch of level 0 and two pre-smoothing sweeps

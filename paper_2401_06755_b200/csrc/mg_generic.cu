@@ -275,6 +275,18 @@ int launch_sumsq(size_t n, const T* v, double* d_acc, cudaStream_t st) {
     return 0;
 }
 
+namespace {
+__global__ void record_acc_kernel(double* acc0, double* hist, int* ctr) {
+    hist[*ctr] = *acc0;
+    *acc0 = 0.0;
+    *ctr += 1;
+}
+}  // namespace
+int launch_record_acc(double* acc0, double* hist, int* ctr, cudaStream_t st) {
+    record_acc_kernel<<<1, 1, 0, st>>>(acc0, hist, ctr);
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
 int launch_axpy_mixed(size_t n, double* x64, const float* e32, cudaStream_t st) {
     axpy_mixed_kernel<<<ew_blocks(n), 256, 0, st>>>(n, x64, e32);
     MGB_LAUNCH_CHECK();

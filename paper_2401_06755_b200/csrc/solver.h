@@ -28,7 +28,7 @@ struct mg_solver {
     int dtype = MG_F32;
     int device = 0;
     cudaStream_t st = nullptr;
-    mg_params p{2, 2, 50, 1, 2.0 / 3.0, 1};
+    mg_params p{2, 2, 50, 1, 2.0 / 3.0, 1, 1};
     bool var_k = false;
     int fused = 1;
     std::vector<mgb::LevelData> lv;
@@ -45,19 +45,28 @@ struct mg_solver {
     void* hb_dev = nullptr;
     // norms
     double* d_acc = nullptr;
+    int* d_ctr = nullptr;     // device-side index of the next residual-history slot (solve-cycle graph)
     double* h_acc = nullptr;  // pinned
     std::vector<double> history;
     long long launches = 0;
     // per-level instrumentation of mg_vcycle_timed
     bool timing = false;
     std::vector<cudaEvent_t> ev;
-    // CUDA-graph replay of the fused V-cycle, keyed by the (x, b) pointers it was captured with
-    cudaGraphExec_t graph_exec = nullptr;
-    cudaStream_t cap_st = nullptr;  // private stream used only to record the graph
-    const void* graph_x = nullptr;
-    const void* graph_b = nullptr;
-    int graph_flavour = 0;            // 0: general initial guess, 1: zero initial guess (first fine sweep x = omega b / D)
-    long long graph_launches = 0;  // kernels inside one replay
+    // CUDA-graph replay of recorded launch sequences (a V-cycle, a zero-guess cycle, a whole solve cycle), keyed by the (x, b)
+    // pointers and the flavour they were captured with; a small cache, least recently used slot replaced
+    struct GraphSlot {
+        cudaGraphExec_t exec = nullptr;
+        const void* x = nullptr;
+        const void* b = nullptr;
+        int flavour = 0;
+        long long launches = 0;    // kernels inside one replay
+        long long used = 0;        // stamp of the last replay
+    };
+    static constexpr int GRAPH_SLOTS = 4;
+    GraphSlot graphs[GRAPH_SLOTS];
+    long long graph_clock = 0;
+    long long epoch = 0;              // bumped whenever the recorded graphs are dropped (parameters, coefficient kind, fused switch)
+    cudaStream_t cap_st = nullptr;    // private stream used only to record graphs
     void* fused_state = nullptr;   // owned by mg_fused.cu
 };
 
@@ -68,8 +77,16 @@ namespace mgb {
 // on the caller's stream.  mg_set_params / mg_set_coefficient / mg_set_fused drop the recorded graph.
 template <class F>
 int replay_graph(mg_solver* s, const void* x, const void* b, F&& enqueue, int flavour = 0) {
-    if (!s->graph_exec || s->graph_x != x || s->graph_b != b || s->graph_flavour != flavour) {
-        if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+    mg_solver::GraphSlot* slot = nullptr;
+    for (auto& g : s->graphs)
+        if (g.exec && g.x == x && g.b == b && g.flavour == flavour) { slot = &g; break; }
+    if (!slot) {
+        slot = &s->graphs[0];
+        for (auto& g : s->graphs) {
+            if (!g.exec) { slot = &g; break; }
+            if (g.used < slot->used) slot = &g;
+        }
+        if (slot->exec) { cudaGraphExecDestroy(slot->exec); slot->exec = nullptr; }
         const long long before = s->launches;
         cudaGraph_t graph = nullptr;
         if (!s->cap_st) MGB_CUDA(cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking));
@@ -79,17 +96,18 @@ int replay_graph(mg_solver* s, const void* x, const void* b, F&& enqueue, int fl
         const int rc = enqueue();
         s->st = user_st;
         const cudaError_t e = cudaStreamEndCapture(s->cap_st, &graph);
-        s->graph_launches = s->launches - before;
+        slot->launches = s->launches - before;
         s->launches = before;
         if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
         if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); return MG_ECUDA; }
-        const cudaError_t e2 = cudaGraphInstantiate(&s->graph_exec, graph, 0);
+        const cudaError_t e2 = cudaGraphInstantiate(&slot->exec, graph, 0);
         cudaGraphDestroy(graph);
-        if (e2 != cudaSuccess) { s->graph_exec = nullptr; set_error("graph instantiate failed: %s", cudaGetErrorString(e2)); return MG_ECUDA; }
-        s->graph_x = x; s->graph_b = b; s->graph_flavour = flavour;
+        if (e2 != cudaSuccess) { slot->exec = nullptr; set_error("graph instantiate failed: %s", cudaGetErrorString(e2)); return MG_ECUDA; }
+        slot->x = x; slot->b = b; slot->flavour = flavour;
     }
-    MGB_CUDA(cudaGraphLaunch(s->graph_exec, s->st));
-    s->launches += s->graph_launches;
+    slot->used = ++s->graph_clock;
+    MGB_CUDA(cudaGraphLaunch(slot->exec, s->st));
+    s->launches += slot->launches;
     return 0;
 }
 

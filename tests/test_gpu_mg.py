@@ -176,6 +176,35 @@ def test_config1_solve(mg, orc, dt):
     mg.mg_destroy(s)
 
 
+@pytest.mark.parametrize("m", [2, 3])
+def test_cycles_per_defect(mg, orc, m):
+    """cycles_per_defect = m: m V-cycles on one correction equation between two fp64 defects.  In exact arithmetic the iterates
+    are those of plain cycles, so the residual history (one entry per defect) must follow the oracle's at the cycles m, 2m, ...,
+    the converged solution must be the oracle's, and a fixed cycle count that is not a multiple of m ends with a shorter round."""
+    w = configs.config1()
+    g = orc.grid(w.nx, w.ny, w.nz, w.h)
+    b = quantise(w.fields["b"], "f32")
+    x_ref, _, _, hist_o = orc.solve(g, w.bc, None, np.zeros(w.shape), b, w.levels, 1e-12, 100)
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32", cycles_per_defect=m)
+    assert mg.mg_get_params(s)["cycles_per_defect"] == m
+    dx, db = to_dev(np.zeros(w.shape), "f32"), to_dev(b, "f32")
+    status, cycles, rel = mg.mg_solve(s, dx, db, 1e-9, 100)
+    hist = mg.mg_get_history(s)
+    assert status == mg.MG_OK and rel < 1e-9 and cycles % m == 0 and len(hist) == cycles // m
+    assert np.allclose(hist[:3], hist_o[m - 1::m][:3], rtol=1e-3), (hist, hist_o)
+    assert_close(as_f64(dx), x_ref, 1e-6)
+    # 7 fixed cycles: rounds of m, m, ... and a shorter last one; same iterate as with a defect after every cycle
+    dx7 = to_dev(np.zeros(w.shape), "f32")
+    status, cycles, rel = mg.mg_solve(s, dx7, db, 0.0, 7)
+    assert cycles == 7 and len(mg.mg_get_history(s)) == -(-7 // m)
+    x7, _, _, h7 = orc.solve(g, w.bc, None, np.zeros(w.shape), b, w.levels, 0.0, 7)
+    assert abs(rel - h7[-1]) <= 1e-3 * h7[-1]
+    assert_close(as_f64(dx7), x7, 1e-5)
+    with pytest.raises(mg.MgError):
+        mg.mg_set_params(s, cycles_per_defect=0)
+    mg.mg_destroy(s)
+
+
 def test_pure_fp32_solve_stagnates_cleanly(mg, orc):
     w = configs.config1()
     b = quantise(w.fields["b"], "f32")
