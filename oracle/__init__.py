@@ -31,11 +31,18 @@ def grid(nx, ny, nz, hx, hy=None, hz=None):
     return Grid(nx, ny, nz, hx, hx if hy is None else hy, hx if hz is None else hz)
 
 
+# ORACLE_SANITIZE=1: the pins run against a build with AddressSanitizer + UndefinedBehaviorSanitizer (no OpenMP, -O1);
+# the interpreter must then be started with LD_PRELOAD=$(gcc -print-file-name=libasan.so) (profiles/r02_oracle_sanitizers.md)
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") == "1"
+if _SANITIZE:
+    _LIB = os.path.join(_HERE, "liboracle_san.so")
+
+
 def build(force=False):
     """Compile oracle.c with gcc (plain C99, -O2, OpenMP on the outer z loops)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall",
-                               "-o", _LIB, _SRC, "-lm"])
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if _SANITIZE else ["-O2", "-fopenmp"]
+        subprocess.check_call(["gcc", *flags, "-fPIC", "-shared", "-std=c99", "-Wall", "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 
