@@ -125,6 +125,12 @@ def main():
         print("| %d | %dx%dx%d | %d | %.1f | %.1f | %.1f |" % (l, nx, ny, nz, n, dn[l] * 1e3, up[l] * 1e3, n * 77.5e-6))
     print("\n(per-level times are taken outside the graph, with events between the launches: their sum exceeds the graph's cycle time;"
           " the levels from 16^3 down run as one cluster kernel, timed under level 4)")
+    r3 = torch.empty_like(b)
+    msr, _ = timed(lambda: mg.mg_residual(s, x, b, r3), 50)
+    msa, _ = timed(lambda: mg.mg_apply_operator(s, x, r3), 50)
+    print("\nmg_residual (r = b - A x, 16 B/point): %.1f us = %.0f GB/s; mg_apply_operator (y = A x, 12 B/point): %.1f us = %.0f GB/s"
+          " (streaming kernel, MODE_RES)" % (msr * 1e3, 16.0 * w.n / msr * 1e-6, msa * 1e3, 12.0 * w.n / msa * 1e-6))
+    del r3
     mg.mg_destroy(s)
 
     # ---- what bounds the smoother: sweep time against the footprint, and the wave kernel ----
