@@ -112,6 +112,11 @@ int mg_pcg_solve(mg_solver* s, void* d_x, const void* d_b, double tol, int max_i
 /* Same with HOST buffers: copies h_b and the guess h_x to the device, solves, copies x back. */
 int mg_solve_host(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out,
                   double* relres_out);
+/* Same from a ZERO initial guess (the pressure correction of a time step starts from zero): h_x is output only
+ * and is not read; the guess is set on the device, so the call moves one field in (h_b) and one out (h_x).  The iterates
+ * are those of mg_solve_host called with h_x = 0, bit for bit. */
+int mg_solve_host_zero(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out,
+                       double* relres_out);
 /* Relative residual after every cycle of the last mg_solve (up to n entries); returns count. */
 int mg_get_history(const mg_solver* s, double* h_history, int n);
 

@@ -22,7 +22,7 @@ MG_EINVAL, MG_ESHAPE, MG_ECUDA, MG_EALLOC = -1, -2, -3, -4
 EXPORTS = [
     "mg_create", "mg_destroy", "mg_set_params", "mg_get_params", "mg_set_coefficient",
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
-    "mg_solve_host", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
+    "mg_solve_host", "mg_solve_host_zero", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
     "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_pcg", "flow_time_step_paper", "mg_last_error",
     "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full", "vof_residual_ex",
     "mg_version",
@@ -77,6 +77,7 @@ def _load():
     lib.mg_vcycle.argtypes = [vp, vp, vp]
     lib.mg_solve.argtypes = [vp, vp, vp, d, i, pi, pd]
     lib.mg_solve_host.argtypes = [vp, vp, vp, d, i, pi, pd]
+    lib.mg_solve_host_zero.argtypes = [vp, vp, vp, d, i, pi, pd]
     lib.mg_pcg_solve.argtypes = [vp, vp, vp, d, i, pi, pd]
     lib.mg_get_history.argtypes = [vp, pd, i]
     lib.mg_level_info.argtypes = [vp, i, pi, pi, pi]; lib.mg_level_info.restype = C.c_longlong
@@ -253,15 +254,24 @@ def mg_pcg_solve(s, x, b, tol, max_iter):
     return st, it.value, rel.value
 
 
-def mg_solve_host(s, x_host, b_host, tol, max_cycles):
-    """x_host, b_host: contiguous CPU tensors (pinned or not).  Returns (status, cycles, relres)."""
+def _solve_host(fn, s, x_host, b_host, tol, max_cycles):
     for t in (x_host, b_host):
         if t.is_cuda or not t.is_contiguous() or t.dtype != s.torch_dtype or tuple(t.shape) != s.shape:
             raise ValueError("expected contiguous CPU tensors of the solver's shape and dtype")
     cyc, rel = C.c_int(0), C.c_double(0.0)
-    st = _check(_lib.mg_solve_host(s.handle, C.c_void_p(x_host.data_ptr()), C.c_void_p(b_host.data_ptr()), float(tol),
-                                   int(max_cycles), C.byref(cyc), C.byref(rel)))
+    st = _check(fn(s.handle, C.c_void_p(x_host.data_ptr()), C.c_void_p(b_host.data_ptr()), float(tol), int(max_cycles),
+                   C.byref(cyc), C.byref(rel)))
     return st, cyc.value, rel.value
+
+
+def mg_solve_host(s, x_host, b_host, tol, max_cycles):
+    """x_host (guess in, solution out), b_host: contiguous CPU tensors (pinned or not).  Returns (status, cycles, relres)."""
+    return _solve_host(_lib.mg_solve_host, s, x_host, b_host, tol, max_cycles)
+
+
+def mg_solve_host_zero(s, x_host, b_host, tol, max_cycles):
+    """As mg_solve_host from a zero guess: x_host is output only (not read, not copied to the device)."""
+    return _solve_host(_lib.mg_solve_host_zero, s, x_host, b_host, tol, max_cycles)
 
 
 def mg_get_history(s):

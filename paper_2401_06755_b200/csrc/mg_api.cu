@@ -607,8 +607,8 @@ int mg_solve(mg_solver* s, void* d_x, const void* d_b, double tol, int max_cycle
     return solve_mixed(s, (float*)d_x, (const float*)d_b, tol, max_cycles, cycles_out, relres_out);
 }
 
-int mg_solve_host(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out,
-                  double* relres_out) {
+static int solve_host(mg_solver* s, void* h_x, const void* h_b, bool zero_guess, double tol, int max_cycles, int* cycles_out,
+                      double* relres_out) {
     CHECK_SOLVER(s);
     if (!h_x || !h_b) { set_error("mg_solve_host: NULL argument"); return MG_EINVAL; }
     const size_t bytes = s->lv[0].n * esize(s);
@@ -616,13 +616,22 @@ int mg_solve_host(mg_solver* s, void* h_x, const void* h_b, double tol, int max_
         set_error("mg_solve_host: out of device memory");
         return MG_EALLOC;
     }
-    MGB_CUDA(cudaMemcpyAsync(s->hx_dev, h_x, bytes, cudaMemcpyHostToDevice, s->st));
+    if (zero_guess) MGB_CUDA(cudaMemsetAsync(s->hx_dev, 0, bytes, s->st));         // all-zero bytes = +0.0 in fp32 and fp64
+    else MGB_CUDA(cudaMemcpyAsync(s->hx_dev, h_x, bytes, cudaMemcpyHostToDevice, s->st));
     MGB_CUDA(cudaMemcpyAsync(s->hb_dev, h_b, bytes, cudaMemcpyHostToDevice, s->st));
     const int status = mg_solve(s, s->hx_dev, s->hb_dev, tol, max_cycles, cycles_out, relres_out);
     if (status < 0) return status;
     MGB_CUDA(cudaMemcpyAsync(h_x, s->hx_dev, bytes, cudaMemcpyDeviceToHost, s->st));
     MGB_CUDA(cudaStreamSynchronize(s->st));
     return status;
+}
+
+int mg_solve_host(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out, double* relres_out) {
+    return solve_host(s, h_x, h_b, false, tol, max_cycles, cycles_out, relres_out);
+}
+
+int mg_solve_host_zero(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out, double* relres_out) {
+    return solve_host(s, h_x, h_b, true, tol, max_cycles, cycles_out, relres_out);
 }
 
 int mg_get_history(const mg_solver* s, double* h_history, int n) {

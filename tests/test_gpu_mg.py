@@ -253,6 +253,11 @@ def test_mg_solve_host_matches_the_oracle(mg, orc):
     x5, _, _, hist_o = orc.solve(g, w.bc, None, np.zeros(w.shape), b, w.levels, 0.0, 5)
     assert cycles == 5 and np.allclose(mg.mg_get_history(s), hist_o, rtol=1e-3)
     assert_close(hx.double().numpy(), x5, 1e-5)
+    # zero-guess entry point: the output buffer is not read (fill it with NaN), the iterates are the same bit for bit
+    hz = torch.full(w.shape, float("nan"), dtype=torch.float32).pin_memory()
+    status, cycles, rel = mg.mg_solve_host_zero(s, hz, hb, 0.0, 5)
+    assert cycles == 5 and np.array_equal(hz.numpy(), hx.numpy())
+    assert_close(hz.double().numpy(), x5, 1e-5)
     mg.mg_destroy(s)
 
 
