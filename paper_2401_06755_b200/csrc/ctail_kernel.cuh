@@ -130,6 +130,10 @@ __device__ __forceinline__ void exchange(cg::cluster_group& cl, const Slab& L, i
     cl.sync();
 }
 
+__device__ __forceinline__ void cpa4(float* dst, const float* src) {      // 4-byte asynchronous copy global -> shared
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+
 __device__ __forceinline__ void swap_xy(Slab& L) { float* t = L.X; L.X = L.Y; L.Y = t; }
 
 __global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(NT, 1) ctail_kernel(const CParams P) {
@@ -166,6 +170,8 @@ __global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(NT, 1) ctail_kernel
     float* sres = p;                                                  // block 0: result of the solo cycle (lv[0].n floats)
 
     // ---- static data: coefficient slabs with copy halos, 1/D; solo levels in block 0 ----
+    // All of it by asynchronous copies (cp.async, 4 bytes each) with ONE wait at the end: as plain loads the five loops below were five
+    // dependent round trips to L2 / HBM (4.4 us, most of it exposed: the predecessor in the stream is a 3 us kernel).
 #pragma unroll
     for (int t = 0; t < MAXD; ++t) {
         if (t >= nd) break;
@@ -174,10 +180,11 @@ __global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(NT, 1) ctail_kernel
         for (int e = tid; e < (L.nzl + 2) * L.ps; e += NT) {
             const int zl = e / L.ps, r = e - zl * L.ps;
             const int zg = min(max(rank * L.nzl + zl - 1, 0), nzg - 1);
-            L.K[e] = P.k[t] ? P.k[t][(size_t)zg * L.ps + r] : 1.f;
+            if (P.k[t]) cpa4(L.K + e, P.k[t] + (size_t)zg * L.ps + r); else L.K[e] = 1.f;
         }
-        for (int e = tid; e < L.nzl * L.ps; e += NT)
-            L.DI[e] = P.dinv[t] ? P.dinv[t][(size_t)rank * L.nzl * L.ps + e] : P.dinv_const[t];
+        for (int e = tid; e < L.nzl * L.ps; e += NT) {
+            if (P.dinv[t]) cpa4(L.DI + e, P.dinv[t] + (size_t)rank * L.nzl * L.ps + e); else L.DI[e] = P.dinv_const[t];
+        }
     }
     if (rank == 0) {
 #pragma unroll
@@ -185,8 +192,8 @@ __global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(NT, 1) ctail_kernel
             if (u >= ns) break;
             const tk::Lv& L = lv[u];
             for (int idx = tid; idx < L.n; idx += NT) {
-                L.K[idx] = P.k[nd + u] ? P.k[nd + u][idx] : 1.f;
-                L.DI[idx] = P.dinv[nd + u] ? P.dinv[nd + u][idx] : P.dinv_const[nd + u];
+                if (P.k[nd + u]) cpa4(L.K + idx, P.k[nd + u] + idx); else L.K[idx] = 1.f;
+                if (P.dinv[nd + u]) cpa4(L.DI + idx, P.dinv[nd + u] + idx); else L.DI[idx] = P.dinv_const[nd + u];
             }
         }
     }
@@ -199,12 +206,12 @@ __global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(NT, 1) ctail_kernel
         for (int e = tid; e < (L.nzl + 2) * L.ps; e += NT) {          // x with its halo planes straight from global memory
             const int zl = e / L.ps, r = e - zl * L.ps;
             const int z = rank * L.nzl + zl - 1;
-            const float f = z < 0 ? P.s[4] : (z >= nzg ? P.s[5] : 1.f);
-            const int zg = z < 0 ? 0 : (z >= nzg ? nzg - 1 : z);
-            L.X[e] = f * P.x[(size_t)zg * L.ps + r];
+            if (z >= 0 && z < nzg) cpa4(L.X + e, P.x + (size_t)z * L.ps + r);
+            else L.X[e] = (z < 0 ? P.s[4] : P.s[5]) * P.x[(size_t)(z < 0 ? 0 : nzg - 1) * L.ps + r];      // ghost plane = s * mirror
         }
-        for (int e = tid; e < L.nzl * L.ps; e += NT) L.B[e] = P.b[(size_t)rank * L.nzl * L.ps + e];
+        for (int e = tid; e < L.nzl * L.ps; e += NT) cpa4(L.B + e, P.b + (size_t)rank * L.nzl * L.ps + e);
     }
+    asm volatile("cp.async.wait_all;" ::: "memory");
     cl.sync();       // every block of the cluster is running and has its data: distributed shared memory may be used from here
 
     const float omega = P.omega;
