@@ -10,8 +10,8 @@ and synthetic (workloads/configs.py); they stand in for the paper's rising-bubbl
 
 One step = one V-cycle (rows a1-a6 of the hot path) on device-resident fields, launched through
 the C ABI (mg_vcycle).  `value` = V-cycles/s over all ranks (replicas only: the path does not
-shard); `e2e` = the same metric through mg_solve_host with HOST buffers
-(H2D of x and b, 20 cycles -- the paper's fixed count, P:429 -- D2H of x inside the timed region).
+shard); `e2e` = the same metric through mg_solve_host_zero with HOST buffers
+(H2D of b, zero guess, 20 cycles -- the paper's fixed count, P:429 -- D2H of x inside the timed region).
 `roofline` is for the dominant kernel, timed live with CUDA events by mg_vcycle_timed on the
 solver's stream.  `cpu_baseline` is the fp64 oracle (oracle/oracle.c), as it stands, on the host
 cores.  `--impl reference` times that oracle alone (rank 0 only).

@@ -66,7 +66,7 @@ enum {
     MG_NOT_CONVERGED = 1, /* mg_solve stopped on max_cycles */
     MG_STAGNATED = 2,     /* residual ratio > 0.95 for 3 consecutive cycles, or non-finite */
     MG_EINVAL = -1,       /* NULL or out-of-range argument */
-    MG_ESHAPE = -2,       /* a dimension not divisible by 2^(levels-1), or coarsest dimension < 2 */
+    MG_ESHAPE = -2,       /* a dimension not divisible by 2^(levels-1), coarsest dimension < 2, or more than 2^31 - 1 points */
     MG_ECUDA = -3,        /* a CUDA call failed (no device, launch error, ...) */
     MG_EALLOC = -4        /* device or host allocation failed */
 };
@@ -75,7 +75,8 @@ enum {
  * (Eqs. 8, 11-13; readings C1, C2) on `grid`, with `levels` grids
  * coarsened 2:1 (n_{l+1} = n_l/2, h_{l+1} = 2 h_l, operator rediscretised, reading C5) and the
  * boundary factors bc[6] = {x-, x+, y-, y+, z-, z+}.  The solver owns its level hierarchy,
- * scratch, CUDA graph and pinned host words.  Coefficient starts as k = 1 (constant). */
+ * scratch, CUDA graph and pinned host words.  Coefficient starts as k = 1 (constant).  Size: nx ny nz <= 2^31 - 1 (MG_ESHAPE
+ * otherwise); 1024 x 1024 x 512 (2 GiB per fp32 field) is the largest grid under test (tests/test_gpu_maxsize.py). */
 int mg_create(mg_solver** out, const mg_grid* grid, int levels, const int bc[6], int dtype, void* cuda_stream);
 void mg_destroy(mg_solver* s);
 

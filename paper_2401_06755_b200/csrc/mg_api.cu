@@ -406,6 +406,10 @@ int mg_create(mg_solver** out, const mg_grid* grid, int levels, const int bc[6],
                   grid->ny, grid->nz, levels);
         return MG_ESHAPE;
     }
+    if ((long long)grid->nx * grid->ny * grid->nz > 2147483647LL) {           // element indices of a level are 32-bit in places
+        set_error("mg_create: %dx%dx%d has more than 2^31 - 1 points", grid->nx, grid->ny, grid->nz);
+        return MG_ESHAPE;
+    }
     int dev = 0;
     MGB_CUDA(cudaGetDevice(&dev));
     mg_solver* s = new (std::nothrow) mg_solver();

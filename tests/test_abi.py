@@ -43,6 +43,8 @@ def test_compute_calls_fail_loudly_without_gpu():
     rc = lib.mg_create(ctypes.byref(h), ctypes.byref(G(8, 8, 8, .1, .1, .1)), 2, bc, 0, None)
     assert rc == -3 and not h.value and lib.mg_last_error()          # MG_ECUDA, no CPU fallback
     assert lib.mg_create(ctypes.byref(h), ctypes.byref(G(9, 8, 8, .1, .1, .1)), 2, bc, 0, None) == -2   # MG_ESHAPE
+    assert lib.mg_create(ctypes.byref(h), ctypes.byref(G(2048, 1024, 1024, .1, .1, .1)), 2, bc, 0, None) == -2   # > 2^31 - 1 points
+    assert b"2^31" in lib.mg_last_error()
     with pytest.raises(Exception):
         import paper_2401_06755_b200 as m
         m.mg_create((8, 8, 8, 0.1), 2, (1,) * 6)
