@@ -76,7 +76,7 @@ enum {
  * coarsened 2:1 (n_{l+1} = n_l/2, h_{l+1} = 2 h_l, operator rediscretised, reading C5) and the
  * boundary factors bc[6] = {x-, x+, y-, y+, z-, z+}.  The solver owns its level hierarchy,
  * scratch, CUDA graph and pinned host words.  Coefficient starts as k = 1 (constant).  Size: nx ny nz <= 2^31 - 1 (MG_ESHAPE
- * otherwise); 1024 x 1024 x 512 (2 GiB per fp32 field) is the largest grid under test (tests/test_gpu_maxsize.py). */
+ * otherwise); 2048 x 1024 x 512 (2^30 points, 4 GiB per fp32 field) is the largest grid under test (tests/test_gpu_maxsize.py). */
 int mg_create(mg_solver** out, const mg_grid* grid, int levels, const int bc[6], int dtype, void* cuda_stream);
 void mg_destroy(mg_solver* s);
 

@@ -1,11 +1,11 @@
-"""GPU parity beyond BASELINE.json's sizes: 1024 x 1024 x 512 (5.4e8 points, 2 GiB per fp32 field, so byte offsets pass 2^31 and
-element offsets 2^29) -- a size the oracle cannot run in a test -- checked on EVERY point through a reflection identity.
+"""GPU parity beyond BASELINE.json's sizes: 2048 x 1024 x 512 (2^30 points, 4 GiB per fp32 field, so byte offsets pass 2^31 and
+reach 2^32) -- a size the oracle cannot run in a test -- checked on EVERY point through a reflection identity.
 
 Mirroring a problem across a Neumann face (ghost = mirror value) gives a problem on the doubled domain whose operator,
 Jacobi sweep, restriction, prolongation and coarsest sweeps all commute with the reflection: every point of the mirrored grid sees
 exactly the neighbour values its mirror image sees.  So with the same number of levels (the big grid's coarsest level is the small
 one's mirrored too) the V-cycle of the mirrored problem is the mirrored V-cycle of the small problem, and the oracle's 256^3
-result checks the 1024 x 1024 x 512 GPU result block by block (16 x and y blocks, 2 z blocks, each plain or flipped).  Across the
+result checks the 2048 x 1024 x 512 GPU result block by block (8 x 4 blocks in x and y, 2 in z, each plain or flipped).  Across the
 bottom face the mirror turns the z pair (Neumann, Dirichlet) into (Dirichlet, Dirichlet).  In fp32 the two differ only by the
 order in which a point adds its left / right neighbours."""
 import numpy as np
@@ -17,7 +17,7 @@ from _parity import MAXABS_FACTOR
 
 pytestmark = pytest.mark.gpu
 N, D = configs.BC_NEUMANN, configs.BC_DIRICHLET
-MX, MY = 4, 4          # copies along x and y (plain, flipped, plain, flipped); along z: (flipped, plain)
+MX, MY = 8, 4          # copies along x and y (plain, flipped, plain, flipped); along z: (flipped, plain)
 
 
 def _mirror_dev(a):
@@ -32,28 +32,28 @@ def _mirror_dev(a):
 
 
 def _check_blocks(dev, ref, tol, what, factor=MAXABS_FACTOR):
-    """every block of the device field against the small reference (fp64), with the bounds of tests/_parity.py"""
+    """every block of the device field against the small reference (fp64), with the bounds of tests/_parity.py; the differences are
+    formed on the device in fp64 (test plumbing: 64 blocks of 1.7e7 points)"""
+    import torch
     nz, ny, nx = ref.shape
-    host = dev.cpu().numpy()
-    assert host.shape == (2 * nz, MY * ny, MX * nx)
-    num = 0.0
-    worst = 0.0
+    assert tuple(dev.shape) == (2 * nz, MY * ny, MX * nx)
+    r = torch.from_numpy(np.ascontiguousarray(ref)).cuda()
+    num, worst = 0.0, 0.0
     for bz in range(2):
         for by in range(MY):
             for bx in range(MX):
-                blk = host[bz * nz:(bz + 1) * nz, by * ny:(by + 1) * ny, bx * nx:(bx + 1) * nx].astype(np.float64)
-                if bz == 0: blk = blk[::-1]
-                if by % 2: blk = blk[:, ::-1]
-                if bx % 2: blk = blk[:, :, ::-1]
-                d = blk - ref
+                blk = dev[bz * nz:(bz + 1) * nz, by * ny:(by + 1) * ny, bx * nx:(bx + 1) * nx].double()
+                flips = [ax for ax, f in ((0, bz == 0), (1, by % 2 == 1), (2, bx % 2 == 1)) if f]
+                if flips: blk = blk.flip(flips)
+                d = blk - r
                 num += float((d * d).sum())
-                worst = max(worst, float(np.abs(d).max()))
+                worst = max(worst, float(d.abs().max()))
     den = 2 * MY * MX * float((ref * ref).sum())
     rel, mx = np.sqrt(num / den), worst / np.abs(ref).max()
     assert rel <= tol and mx <= factor * tol, "%s: rel L2 %.3e (bound %.1e), max-abs %.3e (bound %.1e)" % (what, rel, tol, mx, factor * tol)
 
 
-def test_mirrored_rising_bubble_1024x1024x512(mg, orc):
+def test_mirrored_rising_bubble_2048x1024x512(mg, orc):
     import torch
     w = configs.config3()                                   # 256^3, 7 levels, faces (N, N, N, N, N, D)
     g = orc.grid(w.nx, w.ny, w.nz, w.h)
@@ -62,7 +62,7 @@ def test_mirrored_rising_bubble_1024x1024x512(mg, orc):
     k = orc.k_from_vof(alpha, w.rho_l, w.rho_g)
     x0 = quantise(0.01 * b, "f32")
     shape = (2 * w.nz, MY * w.ny, MX * w.nx)
-    assert np.prod(shape) * 4 >= 2 ** 31
+    assert np.prod(shape) * 4 == 2 ** 32
     s = make_solver(mg, shape, w.h, w.levels, (N, N, N, N, D, D), "f32")
     d_alpha = _mirror_dev(alpha)
     mg.mg_set_coefficient_from_vof(s, d_alpha, w.rho_l, w.rho_g)
@@ -96,3 +96,83 @@ def test_mirrored_rising_bubble_1024x1024x512(mg, orc):
     _check_blocks(dx, as_f64(dxs), 2e-5, "reflection identity, cycle 2")
     mg.mg_destroy(s_small)
     mg.mg_destroy(s)
+
+
+# ---- explicit stages at the same size: sampled sub-boxes against the oracle ------------------------------------------
+# The explicit kernels are local (radius <= 3 cells per stage chain), so a box cut out of the big input, handed to the oracle
+# as a grid of its own, reproduces the big grid's result everywhere except within RIM cells of a cut face (where the oracle
+# applies a boundary rule the big grid does not have there).  Faces of a box that lie ON the domain boundary are real boundary
+# faces on both sides and are compared up to the edge.
+BASE = 128
+RIM = 6       # vof_residual: advection (1) + coefficients (1, or 2 with Eq. 34) + diffusion (1); momentum 3; kept generous
+
+
+def _fold(i):
+    """index into the 128-cell base field of the mirrored tiling (period 256: plain, flipped)"""
+    m = np.asarray(i) % (2 * BASE)
+    return np.where(m < BASE, m, 2 * BASE - 1 - m)
+
+
+def _tile_dev(a, shape):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    for ax in range(3):
+        pair = torch.cat([t, t.flip(ax)], ax)
+        t = torch.cat([pair] * (shape[ax] // (2 * BASE)), ax)
+    return t.contiguous()
+
+
+def _cut(a, box):
+    (z0, z1), (y0, y1), (x0, x1) = box
+    return np.ascontiguousarray(a[np.ix_(_fold(np.arange(z0, z1)), _fold(np.arange(y0, y1)), _fold(np.arange(x0, x1)))])
+
+
+def _inner(box, shape):
+    """slices of the box interior that the cut faces do not reach, and the same region in the big grid"""
+    loc, glob = [], []
+    for (a0, a1), n in zip(box, shape):
+        lo = 0 if a0 == 0 else RIM
+        hi = (a1 - a0) if a1 == n else (a1 - a0) - RIM
+        loc.append(slice(lo, hi)); glob.append(slice(a0 + lo, a0 + hi))
+    return tuple(loc), tuple(glob)
+
+
+def test_explicit_stages_2048x1024x512(mg, orc):
+    import torch
+    from _parity import assert_close
+    shape = (512, 1024, 2048)
+    nz, ny, nx = shape
+    w = configs.config5(BASE, 5)
+    h, dt = w.h, w.dt
+    base = {q: quantise(w.fields[q], "f32") for q in ("alpha", "u", "v", "w")}
+    dC, du, dv, dw = (_tile_dev(base[q], shape) for q in ("alpha", "u", "v", "w"))
+    # every box holds a piece of the interface (base x = 32: the water column), so the residuals in it are not rounding only
+    boxes = [((nz - 40, nz), (ny - 36, ny), (nx - 48, nx)),                  # the last addresses of the fields, three real faces
+             ((0, 36), (0, 40), (0, 44)),                                    # the first ones
+             ((236, 276), (500, 540), (976, 1040)),                          # interior, across tile seams, byte offsets around 2^31
+             ((nz - 36, nz), (100, 140), (976, 1040))]                       # top face only
+    for box in boxes:
+        xs = _fold(np.arange(*box[2])); zs = _fold(np.arange(*box[0]))
+        assert xs.min() < 32 <= xs.max() and zs.min() < 64
+    ds, dcn = torch.empty_like(dC), torch.empty_like(dC)
+    mg.vof_residual(dC, du, dv, dw, h, dt, ds, dcn)
+    db = torch.empty_like(dC)
+    mg.pressure_rhs(du, dv, dw, h, dt, db)
+    dqt = [torch.empty_like(dC) for _ in range(3)]
+    dqh = [torch.empty_like(dC) for _ in range(3)]
+    mg.mom_predictor(dC, (du, dv, dw), (du, dv, dw), h, w.rho_l, w.rho_g, w.mu_l, w.mu_g, dt, dqt, dqh)
+    for box in boxes:
+        sub = {q: _cut(base[q], box) for q in base}
+        bz, by, bx = (b1 - b0 for b0, b1 in box)
+        g = orc.grid(bx, by, bz, h)
+        loc, glob = _inner(box, shape)
+        take = lambda t: t[glob].double().cpu().numpy()
+        s_ref, c_ref = orc.vof_residual(g, sub["alpha"], sub["u"], sub["v"], sub["w"], dt)
+        assert_close(take(ds), s_ref[loc], 5 * TOL["f32"], "s_C %s" % (box,))
+        assert_close(take(dcn), c_ref[loc], TOL["f32"], "C_new %s" % (box,))
+        assert_close(take(db), orc.pressure_rhs(g, sub["u"], sub["v"], sub["w"], dt)[loc], 50 * TOL["f32"], "b %s" % (box,))
+        qn = (sub["u"], sub["v"], sub["w"])
+        qt_ref, qh_ref = orc.mom_predictor(g, sub["alpha"], qn, qn, w.rho_l, w.rho_g, w.mu_l, w.mu_g, dt)
+        for c in range(3):
+            assert_close(take(dqt[c]), qt_ref[c][loc], TOL["f32"], "q~[%d] %s" % (c, box))
+            assert_close(take(dqh[c]), qh_ref[c][loc], TOL["f32"], "q_half[%d] %s" % (c, box))
