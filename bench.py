@@ -337,8 +337,8 @@ def run_ours(args, rank, local_rank, world):
     ms_e2e = max_over_ranks(ms_e2e, world, dev)
     e2e = {"value": world * calls * E2E_CYCLES / (ms_e2e * 1e-3), "unit": UNIT,
            "h2d_bytes_per_step": hb.numel() * 4, "d2h_bytes_per_step": hx.numel() * 4,
-           "step": "one mg_solve_host_zero call = %d V-cycles from a zero guess, fp64 defect and residual norm every %d cycle(s)"
-                   % (E2E_CYCLES, args.cycles_per_defect),
+           "step": "one mg_solve_host_zero call = %d V-cycles from a zero guess, fp64 defect and residual norm every %s cycle(s)"
+                   % (E2E_CYCLES, "4 (cycles_per_defect 0 = adaptive; fixed count)" if args.cycles_per_defect == 0 else str(args.cycles_per_defect)),
            "calls": calls}
 
     # config 5 (BASELINE.json configs[4]): full time step on 256^3 (momentum predictor x2, pressure RHS, mixed-precision
@@ -413,8 +413,9 @@ def main():
     ap.add_argument("--sweeps-per-pass", type=int, default=1, choices=[1, 2, 3, 4],
                     help="stencil stages per launch on a level: 1 = one-stage streaming kernels (default, faster); "
                          "2-4 = wave kernel (temporal blocking through L2)")
-    ap.add_argument("--cycles-per-defect", type=int, default=2,
-                    help="mixed-precision solves (e2e, time step): V-cycles per fp64 defect / residual check (mg_params.cycles_per_defect)")
+    ap.add_argument("--cycles-per-defect", type=int, default=0,
+                    help="mixed-precision solves (e2e, time step): V-cycles per fp64 defect / residual check (mg_params.cycles_per_defect); "
+                         "0 (default) = adaptive: chosen by the solve loop from the contraction it observes, 4 for a fixed cycle count")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

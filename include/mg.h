@@ -53,12 +53,17 @@ typedef struct { int nx, ny, nz; double hx, hy, hz; } mg_grid;
  * cycles_per_defect (mixed precision only): V-cycles applied to one correction equation A e = r before the next fp64 defect is
  * formed -- the first from a zero guess, the others continue the iteration on e with the same r, so in exact arithmetic the
  * iterates are those of plain cycles; the residual (stopping test, history) is then evaluated every cycles_per_defect cycles
- * only, which is what saves the time (the fp64 defect and the fp64 update cost 40 % of a cycle).  Default 1: every cycle. */
+ * only, which is what saves the time (the fp64 defect and the fp64 update cost 40 % of a cycle).  Default 1: every cycle.
+ * 0 = adaptive: a tolerance-driven solve starts with one cycle per defect and then takes, round by round, as many cycles as the
+ * contraction observed in the last round says are still needed to reach tol, at most 8 and no more than keep the round's
+ * contraction above 1e-5 (what fp32 resolves of a correction), rounded down to 1, 2, 4 or 8; a fixed-count solve (tol = 0)
+ * takes 4 (then 2, 1 for what is left).
+ * mg_get_history_cycles tells after how many cycles each history entry was taken. */
 typedef struct {
     int nu_pre, nu_post, coarse_sweeps, sweeps_per_pass;
     double omega;
     int mixed_precision;
-    int cycles_per_defect;   /* 1 .. 8, default 1 */
+    int cycles_per_defect;   /* 1 .. 8, default 1; 0 = adaptive */
 } mg_params;
 
 enum {
@@ -120,6 +125,9 @@ int mg_solve_host_zero(mg_solver* s, void* h_x, const void* h_b, double tol, int
                        double* relres_out);
 /* Relative residual after every cycle of the last mg_solve (up to n entries); returns count. */
 int mg_get_history(const mg_solver* s, double* h_history, int n);
+/* The number of V-cycles (mg_pcg_solve: iterations) completed when each of those entries was taken: 1, 2, 3, ... unless
+ * cycles_per_defect != 1 (up to n entries; returns count, the same as mg_get_history). */
+int mg_get_history_cycles(const mg_solver* s, int* h_cycles, int n);
 
 /* Measurement helpers.  mg_level_info: points of level l (returns < 0 if l is out of range).
  * mg_vcycle_timed: one V-cycle with CUDA events around every level's down leg and up leg;

@@ -22,7 +22,7 @@ MG_EINVAL, MG_ESHAPE, MG_ECUDA, MG_EALLOC = -1, -2, -3, -4
 EXPORTS = [
     "mg_create", "mg_destroy", "mg_set_params", "mg_get_params", "mg_set_coefficient",
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
-    "mg_solve_host", "mg_solve_host_zero", "mg_get_history", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
+    "mg_solve_host", "mg_solve_host_zero", "mg_get_history", "mg_get_history_cycles", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
     "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_pcg", "flow_time_step_paper", "mg_last_error",
     "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full", "vof_residual_ex",
     "mg_version",
@@ -80,6 +80,7 @@ def _load():
     lib.mg_solve_host_zero.argtypes = [vp, vp, vp, d, i, pi, pd]
     lib.mg_pcg_solve.argtypes = [vp, vp, vp, d, i, pi, pd]
     lib.mg_get_history.argtypes = [vp, pd, i]
+    lib.mg_get_history_cycles.argtypes = [vp, pi, i]
     lib.mg_level_info.argtypes = [vp, i, pi, pi, pi]; lib.mg_level_info.restype = C.c_longlong
     lib.mg_vcycle_timed.argtypes = [vp, vp, vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     lib.mg_launch_count.argtypes = [vp]; lib.mg_launch_count.restype = C.c_longlong
@@ -278,6 +279,14 @@ def mg_get_history(s):
     n = _lib.mg_get_history(s.handle, None, 0)
     buf = (C.c_double * max(n, 1))()
     _lib.mg_get_history(s.handle, buf, n)
+    return list(buf[:n])
+
+
+def mg_get_history_cycles(s):
+    """cycles completed when each entry of mg_get_history was taken"""
+    n = _lib.mg_get_history_cycles(s.handle, None, 0)
+    buf = (C.c_int * max(n, 1))()
+    _lib.mg_get_history_cycles(s.handle, buf, n)
     return list(buf[:n])
 
 

@@ -235,6 +235,7 @@ static int solve_plain(mg_solver* s, T* x, const T* b, double tol, int max_cycle
         rel = nb > 0.0 ? nr / nb : 0.0;
         s->history.push_back(rel);
         ++cycles;
+        s->history_cycles.push_back(cycles);
         const int u = stop.update(rel);
         if (u >= 0) status = u;
     }
@@ -273,7 +274,12 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     if ((rc = read_acc(s, &sq))) return rc;
     double rel = nb > 0.0 ? std::sqrt(sq) / nb : 0.0;
     int cycles = 0, status = (rel < tol) ? MG_OK : MG_NOT_CONVERGED;
-    const int m_max = std::max(1, std::min(s->p.cycles_per_defect, 8));
+    // cycles per round: the parameter, or (cycles_per_defect = 0) chosen round by round: as many cycles as the observed contraction
+    // says are still needed, at most M_AUTO -- defects cost time, cycles beyond the tolerance cost more
+    constexpr int M_AUTO = 4, M_AUTO_TOL = 8;     // fixed-count solves; tolerance-driven solves (bounded by the contraction, below)
+    const bool adaptive = s->p.cycles_per_defect == 0;
+    const int m_max = adaptive ? M_AUTO : std::max(1, std::min(s->p.cycles_per_defect, 8));
+    int m_next = adaptive && tol > 0.0 ? 1 : m_max;
     Stop stop{tol, 0, rel};
     // one round: mm cycles on A e = r32, x64 += e, next defect, its squared norm filed at hist[ctr++]
     auto round = [&](int mm, bool in_graph) -> int {
@@ -304,23 +310,43 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
         for (int c = read; c < upto; ++c) {
             rel = nb > 0.0 ? std::sqrt(s->h_acc[1 + c]) / nb : 0.0;
             s->history.push_back(rel);
+            s->history_cycles.push_back(round_cycles[c]);
             if (!std::isfinite(rel)) status = MG_STAGNATED;
         }
         read = upto;
         return 0;
     };
     while (status == MG_NOT_CONVERGED && cycles < max_cycles && rounds < ACC_N - 1) {
-        const int mm = std::min(m_max, max_cycles - cycles);
+        int mm = std::min(m_next, max_cycles - cycles);
+        if (adaptive) {                                // round lengths 1, 2, 4, 8 only: every length is a recorded graph of its own
+            int p2 = 1;
+            while (2 * p2 <= mm) p2 *= 2;
+            mm = p2;
+        }
         if (graphs) rc = replay_graph(s, s->x64, b, [&]() { return round(mm, true); }, 16 + mm);
         else rc = round(mm, false);
         if (rc) return rc;
         cycles += mm; ++rounds;
+        round_cycles.push_back(cycles);
         if (tol > 0.0) {                               // tolerance-driven: the host decides after every round
+            const double before = rel;
             if ((rc = fetch(rounds))) return rc;
             if (status == MG_NOT_CONVERGED) {
                 stop.rate = std::pow(0.95, mm);
                 const int u = stop.update(rel);
                 if (u >= 0) status = u;
+            }
+            if (adaptive && status == MG_NOT_CONVERGED) {
+                // per-cycle contraction of the last round -> cycles still needed.  Early cycles contract faster than late ones, so
+                // this errs towards too few cycles per round (one more defect), not towards cycles past the tolerance.
+                // A round must not contract the correction below what fp32 resolves of it: rho^m >= 1e-5.
+                const double rho = before > 0.0 ? std::pow(rel / before, 1.0 / mm) : 1.0;
+                double need = M_AUTO, cap = M_AUTO;
+                if (rho > 0.0 && rho < 1.0 && rel > tol) {
+                    need = std::ceil(std::log(tol / rel) / std::log(rho));
+                    cap = std::min((double)M_AUTO_TOL, std::floor(std::log(1e-5) / std::log(rho)));
+                }
+                m_next = (int)std::max(1.0, std::min(cap, need));
             }
         }
     }
@@ -472,8 +498,8 @@ int mg_set_params(mg_solver* s, const mg_params* p) {
         set_error("mg_set_params: invalid parameters");
         return MG_EINVAL;
     }
-    if (p->cycles_per_defect < 1 || p->cycles_per_defect > 8) {
-        set_error("mg_set_params: cycles_per_defect = %d is out of range (1 .. 8)", p->cycles_per_defect);
+    if (p->cycles_per_defect < 0 || p->cycles_per_defect > 8) {
+        set_error("mg_set_params: cycles_per_defect = %d is out of range (0 = adaptive, 1 .. 8)", p->cycles_per_defect);
         return MG_EINVAL;
     }
     // stages per launch of the wave kernel (wave_kernel.cuh): 1 .. 4 are implemented; anything else is refused
@@ -603,7 +629,7 @@ int mg_vcycle(mg_solver* s, void* d_x, const void* d_b) {
 int mg_solve(mg_solver* s, void* d_x, const void* d_b, double tol, int max_cycles, int* cycles_out, double* relres_out) {
     CHECK_SOLVER(s);
     if (!d_x || !d_b || max_cycles < 0 || !(tol >= 0.0)) { set_error("mg_solve: invalid argument"); return MG_EINVAL; }
-    s->history.clear();
+    s->history.clear(); s->history_cycles.clear();
     if (s->dtype == MG_F64) return solve_plain<double>(s, (double*)d_x, (const double*)d_b, tol, max_cycles, cycles_out, relres_out);
     if (!s->p.mixed_precision) return solve_plain<float>(s, (float*)d_x, (const float*)d_b, tol, max_cycles, cycles_out, relres_out);
     int rc = ensure_mixed_buffers(s);
@@ -636,6 +662,13 @@ int mg_solve_host(mg_solver* s, void* h_x, const void* h_b, double tol, int max_
 
 int mg_solve_host_zero(mg_solver* s, void* h_x, const void* h_b, double tol, int max_cycles, int* cycles_out, double* relres_out) {
     return solve_host(s, h_x, h_b, true, tol, max_cycles, cycles_out, relres_out);
+}
+
+int mg_get_history_cycles(const mg_solver* s, int* h_cycles, int n) {
+    if (!s) { set_error("NULL solver"); return MG_EINVAL; }
+    const int m = (int)s->history_cycles.size();
+    for (int c = 0; c < m && c < n && h_cycles; ++c) h_cycles[c] = s->history_cycles[c];
+    return m;
 }
 
 int mg_get_history(const mg_solver* s, double* h_history, int n) {

@@ -143,6 +143,7 @@ int pcg_t(mg_solver* s, void* d_x, const void* d_b, double tol, int max_iter, in
             if ((rc = read(S_RR, &rr))) return rc;
             rel = std::sqrt(rr) / nbn;
             s->history.push_back(rel);
+            s->history_cycles.push_back((int)s->history.size());
             ++it;
             if (!std::isfinite(rel)) { status = MG_STAGNATED; break; }
             if (rel < tol) { status = MG_OK; break; }
@@ -181,7 +182,7 @@ extern "C" int mg_pcg_solve(mg_solver* s, void* d_x, const void* d_b, double tol
     int prev = -1;
     cudaGetDevice(&prev);
     cudaSetDevice(s->device);
-    s->history.clear();
+    s->history.clear(); s->history_cycles.clear();
     const int rc = s->dtype == MG_F32 ? pcg_t<float>(s, d_x, d_b, tol, max_iter, iters_out, relres_out)
                                       : pcg_t<double>(s, d_x, d_b, tol, max_iter, iters_out, relres_out);
     if (prev >= 0) cudaSetDevice(prev);

@@ -48,6 +48,7 @@ struct mg_solver {
     int* d_ctr = nullptr;     // device-side index of the next residual-history slot (solve-cycle graph)
     double* h_acc = nullptr;  // pinned
     std::vector<double> history;
+    std::vector<int> history_cycles;   // V-cycles (iterations) completed when history[i] was taken
     long long launches = 0;
     // per-level instrumentation of mg_vcycle_timed
     bool timing = false;
@@ -62,7 +63,7 @@ struct mg_solver {
         long long launches = 0;    // kernels inside one replay
         long long used = 0;        // stamp of the last replay
     };
-    static constexpr int GRAPH_SLOTS = 4;
+    static constexpr int GRAPH_SLOTS = 6;
     GraphSlot graphs[GRAPH_SLOTS];
     long long graph_clock = 0;
     long long epoch = 0;              // bumped whenever the recorded graphs are dropped (parameters, coefficient kind, fused switch)

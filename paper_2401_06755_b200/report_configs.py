@@ -105,6 +105,13 @@ def main():
     ms, (st, cyc, rel) = timed(run3, 3)
     print("20 cycles with fp64 residuals: %.3f ms (%.1f V-cycles/s); final relative residual %.2e\n" % (ms, 20e3 / ms, rel))
     print("history: " + ", ".join("%.2e" % h for h in mg.mg_get_history(s)) + "\n")
+    mg.mg_set_params(s, nu_pre=w.nu_pre, nu_post=w.nu_post, coarse_sweeps=w.coarse_sweeps, sweeps_per_pass=1, omega=w.omega,
+                     mixed_precision=1, cycles_per_defect=0)
+    ms, (st, cyc, rel) = timed(run3, 3)
+    print("the same with cycles_per_defect = 0 (fp64 defects after cycles %s): %.3f ms (%.1f V-cycles/s); final relative residual %.2e\n"
+          % (mg.mg_get_history_cycles(s), ms, 20e3 / ms, rel))
+    mg.mg_set_params(s, nu_pre=w.nu_pre, nu_post=w.nu_post, coarse_sweeps=w.coarse_sweeps, sweeps_per_pass=1, omega=w.omega,
+                     mixed_precision=1, cycles_per_defect=1)
     def run3p():
         x.zero_()
         return mg.mg_pcg_solve(s, x, b, 1e-7, 100)
@@ -195,21 +202,27 @@ def main():
     # ---- config 5 ----
     w = configs.config5()
     print("\n## Config 5: full time step on 256^3 (momentum x2, pressure RHS, solve to 1e-6, projection, VoF)\n")
-    s = solver_for(w)
-    C, u, v, ww = (f32(w.fields[q]) for q in ("alpha", "u", "v", "w"))
-    p = torch.empty_like(C)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    cycs = []
-    for it in range(12):
-        if it == 2:
-            torch.cuda.synchronize(); e0.record()
-        st, cyc, rel = mg.flow_time_step(s, C, u, v, ww, p, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, w.tol, 100)
-        cycs.append(cyc)
-    e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 10
-    print("10 steps after 2 warm-up steps: %.2f ms per step = %.1f time-steps/s; cycles per solve %s; last status %d, relres %.2e"
-          % (ms, 1e3 / ms, cycs[2:], st, rel))
-    print("\nvolume fraction after 12 steps: min %.4f max %.4f; max |q| %.4f" % (float(C.min()), float(C.max()),
+    # cycles_per_defect: 1 = an fp64 defect (residual check) after every cycle, the library's default; 0 = the solve loop picks the
+    # cycles of every round from the contraction it observes (what bench.py uses)
+    for cpd in (1, 0):
+        s = solver_for(w, cycles_per_defect=cpd)
+        C, u, v, ww = (f32(w.fields[q]) for q in ("alpha", "u", "v", "w"))
+        p = torch.empty_like(C)
+        cycs = []
+        for it in range(12):
+            if it == 2:
+                torch.cuda.synchronize(); e0.record()
+            st, cyc, rel = mg.flow_time_step(s, C, u, v, ww, p, w.rho_l, w.rho_g, w.mu_l, w.mu_g, w.dt, w.tol, 100)
+            cycs.append(cyc)
+        e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 10
+        print("cycles_per_defect %d: 10 steps after 2 warm-up steps: %.2f ms per step = %.1f time-steps/s; cycles per solve %s (residual "
+              "checks of the last solve after cycles %s); last status %d, relres %.2e\n"
+              % (cpd, ms, 1e3 / ms, cycs[2:], mg.mg_get_history_cycles(s), st, rel))
+        if cpd == 1:
+            mg.mg_destroy(s)
+    print("volume fraction after 12 steps: min %.4f max %.4f; max |q| %.4f" % (float(C.min()), float(C.max()),
           float(torch.maximum(torch.maximum(u.abs().max(), v.abs().max()), ww.abs().max()))))
     C, u, v, ww = (f32(w.fields[q]) for q in ("alpha", "u", "v", "w"))
     its = []
@@ -227,27 +240,28 @@ def main():
     # ---- the paper's four-stage step ----
     print("\n### The paper's four-stage step (stage 1 hydrostatic + surface-tension pressure, 20 fixed cycles; free-slip walls; "
           "forcing terms of Eq. 18; stage 3 to 1e-6), flow_time_step_full, from rest under gravity\n")
-    s_hs = solver_for(w)
-    s_nh = solver_for(w)
-    C = f32(w.fields["alpha"])
-    u, v, ww = (torch.zeros_like(C) for _ in range(3))
-    phs, pnh = torch.zeros_like(C), torch.zeros_like(C)
     dt_full = 0.1 * w.h / 3.0          # Courant 0.1 at the free-fall speed sqrt(2 g H) ~ 3 m/s of a unit box
-    cycs = []
-    for it in range(7):
-        if it == 2:
-            torch.cuda.synchronize(); e0.record()
-        st, cyc, rel = mg.flow_time_step_full(s_hs, s_nh, C, u, v, ww, phs, pnh, w.rho_l, w.rho_g, w.mu_l, w.mu_g, 9.81, 0.0728,
-                                              dt_full, w.tol, 100, 0.0, 20)
-        cycs.append(cyc)
-    e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 5
-    print("5 steps after 2 warm-up steps: %.2f ms per step = %.1f time-steps/s; stage-3 cycles per solve %s; last status %d, relres %.2e;"
-          " max |q| %.4f m/s after 7 steps of %.2e s (g t = %.4f)"
-          % (ms, 1e3 / ms, cycs[2:], st, rel, float(torch.maximum(torch.maximum(u.abs().max(), v.abs().max()), ww.abs().max())),
-             dt_full, 9.81 * 7 * dt_full))
-    mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)
-    del phs, pnh
+    for cpd in (1, 0):
+        s_hs = solver_for(w, cycles_per_defect=cpd)
+        s_nh = solver_for(w, cycles_per_defect=cpd)
+        C = f32(w.fields["alpha"])
+        u, v, ww = (torch.zeros_like(C) for _ in range(3))
+        phs, pnh = torch.zeros_like(C), torch.zeros_like(C)
+        cycs = []
+        for it in range(7):
+            if it == 2:
+                torch.cuda.synchronize(); e0.record()
+            st, cyc, rel = mg.flow_time_step_full(s_hs, s_nh, C, u, v, ww, phs, pnh, w.rho_l, w.rho_g, w.mu_l, w.mu_g, 9.81, 0.0728,
+                                                  dt_full, w.tol, 100, 0.0, 20)
+            cycs.append(cyc)
+        e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 5
+        print("cycles_per_defect %d: 5 steps after 2 warm-up steps: %.2f ms per step = %.1f time-steps/s; stage-3 cycles per solve %s; last "
+              "status %d, relres %.2e; max |q| %.4f m/s after 7 steps of %.2e s (g t = %.4f)\n"
+              % (cpd, ms, 1e3 / ms, cycs[2:], st, rel, float(torch.maximum(torch.maximum(u.abs().max(), v.abs().max()), ww.abs().max())),
+                 dt_full, 9.81 * 7 * dt_full))
+        mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)
+        del phs, pnh
 
     print("\n### The same step with the paper's own stage 3 (constant-coefficient Laplacian, density on the right, Eqs. 52-53; "
           "2 passes x 20 fixed cycles, P:429, P:498)\n")

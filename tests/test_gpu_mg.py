@@ -200,8 +200,39 @@ def test_cycles_per_defect(mg, orc, m):
     x7, _, _, h7 = orc.solve(g, w.bc, None, np.zeros(w.shape), b, w.levels, 0.0, 7)
     assert abs(rel - h7[-1]) <= 1e-3 * h7[-1]
     assert_close(as_f64(dx7), x7, 1e-5)
+    assert mg.mg_get_history_cycles(s) == [min(m * (i + 1), 7) for i in range(-(-7 // m))]
     with pytest.raises(mg.MgError):
-        mg.mg_set_params(s, cycles_per_defect=0)
+        mg.mg_set_params(s, cycles_per_defect=9)
+    mg.mg_destroy(s)
+
+
+def test_adaptive_cycles_per_defect(mg, orc):
+    """cycles_per_defect = 0: the solve loop picks the cycles of every round from the contraction it has seen.  Whatever it picks,
+    each history entry must be the oracle's residual after the reported number of cycles, the solve must not run more than one
+    round past the oracle's cycle count, and a fixed-count solve must do exactly the cycles asked for."""
+    w = configs.config2(64, 5)
+    g = orc.grid(w.nx, w.ny, w.nz, w.h)
+    alpha = quantise(w.fields["alpha"], "f32")
+    b = quantise(orc.pressure_rhs(g, w.fields["u"], w.fields["v"], w.fields["w"], 1.0), "f32")
+    k = orc.k_from_vof(alpha, w.rho_l, w.rho_g)
+    _, n_o, _, hist_o = orc.solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, 1e-7, 200)
+    s = make_solver(mg, w.shape, w.h, w.levels, w.bc, "f32", cycles_per_defect=0)
+    mg.mg_set_coefficient_from_vof(s, to_dev(alpha, "f32"), w.rho_l, w.rho_g)
+    assert mg.mg_get_params(s)["cycles_per_defect"] == 0
+    dx, db = to_dev(np.zeros(w.shape), "f32"), to_dev(b, "f32")
+    status, cycles, rel = mg.mg_solve(s, dx, db, 1e-7, 200)
+    hist, at = mg.mg_get_history(s), mg.mg_get_history_cycles(s)
+    assert status == mg.MG_OK and rel < 1e-7 and at[-1] == cycles and len(hist) == len(at)
+    assert n_o <= cycles <= n_o + 3, (cycles, n_o, at)
+    assert at[0] == 1 and all(b_ - a_ in (1, 2, 4, 8) for a_, b_ in zip(at, at[1:])) and len(at) < cycles      # fewer defects than cycles
+    ho = orc.solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, 0.0, cycles)[3]
+    assert np.allclose(hist, [ho[c - 1] for c in at], rtol=2e-2), (hist, at, ho)
+    # fixed count: rounds of 4 and a shorter last one
+    dx.zero_()
+    status, cycles, rel = mg.mg_solve(s, dx, db, 0.0, 10)
+    assert cycles == 10 and mg.mg_get_history_cycles(s) == [4, 8, 10]        # rounds of 4, 4, 2
+    x10 = orc.solve(g, w.bc, k, np.zeros(w.shape), b, w.levels, 0.0, 10)[0]
+    assert_close(as_f64(dx), x10, 1e-4)
     mg.mg_destroy(s)
 
 
