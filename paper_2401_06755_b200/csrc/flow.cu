@@ -86,6 +86,12 @@ bool can_vec(const mg_grid* g, std::initializer_list<const void*> ptrs) {
         else KERNEL<T, 1, true><<<march_grid<T, 1>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__);                       \
     } while (0)
 
+#define MGB_MARCH_BC_W(KERNEL, WV, VEC, G, st, ...)                                                     \
+    do {                                                                                                \
+        if (VEC) KERNEL<T, WV, true><<<march_grid<T, WV>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__);  \
+        else KERNEL<T, 1, true><<<march_grid<T, 1>(G), dim3(MBX, MBY), 0, st>>>(G, __VA_ARGS__);        \
+    } while (0)
+
 // halo factors of a field from mg_bc codes (0 copy: +1, 1 odd about the face: -1, 2 zero halo: 0)
 template <typename T>
 Halo6<T> make_halo(const int* codes) {
@@ -162,22 +168,25 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
     const Geo<T> G = make_geo<T>(g, nullptr);
     const size_t bytes = npts(g->nx, g->ny, g->nz) * sizeof(T);
     Scratch ws(st);
-    int rc = ws.alloc(2, bytes);
+    int rc = ws.alloc(4, bytes);
     if (rc) return rc;
-    T *adv = (T*)ws.p[0], *kc = (T*)ws.p[1];
+    T *adv[3] = {(T*)ws.p[0], (T*)ws.p[1], (T*)ws.p[2]}, *kc = (T*)ws.p[3];
     const bool vec = can_vec<T>(g, {C, qh[0], qh[1], qh[2], qn[0], qn[1], qn[2], qt[0], qt[1], qt[2], qhn ? qhn[0] : nullptr,
                                     qhn ? qhn[1] : nullptr, qhn ? qhn[2] : nullptr});
+    // the advection terms of all three components in one pass (each velocity field is read once), then coefficient and update per
+    // component.  2-wide packs: three rolling gradients do not fit the registers of a 4-wide one.
+    if (vbc) MGB_MARCH_BC_W(advection3_march, 2, vec, G, st, qh[0], qh[1], qh[2], adv[0], adv[1], adv[2], make_halo<T>(vbc),
+                            make_halo<T>(vbc + 6), make_halo<T>(vbc + 12));
+    else MGB_MARCH_W(advection3_march, 2, vec, G, st, qh[0], qh[1], qh[2], adv[0], adv[1], adv[2]);
     for (int c = 0; c < 3; ++c) {
         if (vbc) {      // free-slip walls: the component's own halo factors in its gradient and its diffusion
             const Halo6<T> H = make_halo<T>(vbc + 6 * c);
-            MGB_MARCH_BC(advection_march, vec, G, st, qh[c], qh[0], qh[1], qh[2], adv, H);
-            MGB_MARCH_BC(mom_coeff_march, vec, G, st, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc, H);
-            MGB_MARCH_BC(mom_update_march, vec, G, st, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c], qhn ? qhn[c] : (T*)nullptr, H);
+            MGB_MARCH_BC(mom_coeff_march, vec, G, st, C, qh[c], qh[0], qh[1], qh[2], adv[c], (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc, H);
+            MGB_MARCH_BC(mom_update_march, vec, G, st, C, qh[c], kc, adv[c], qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c], qhn ? qhn[c] : (T*)nullptr, H);
             continue;
         }
-        MGB_MARCH(advection_march, vec, G, st, qh[c], qh[0], qh[1], qh[2], adv);
-        MGB_MARCH(mom_coeff_march, vec, G, st, C, qh[c], qh[0], qh[1], qh[2], adv, (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc);
-        MGB_MARCH(mom_update_march, vec, G, st, C, qh[c], kc, adv, qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c], qhn ? qhn[c] : (T*)nullptr);
+        MGB_MARCH(mom_coeff_march, vec, G, st, C, qh[c], qh[0], qh[1], qh[2], adv[c], (T)rho_l, (T)rho_g, (T)mu_l, (T)mu_g, kc);
+        MGB_MARCH(mom_update_march, vec, G, st, C, qh[c], kc, adv[c], qn[c], (T)rho_l, (T)rho_g, (T)dt, qt[c], qhn ? qhn[c] : (T*)nullptr);
     }
     MGB_LAUNCH_CHECK();
     return 0;
