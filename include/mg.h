@@ -156,6 +156,18 @@ int vof_residual(const mg_grid* grid, int dtype, const void* d_C, const void* d_
  * minimum of the three products of consecutive differences over i-2 .. i+2; halo of C by reflection).  Other values: MG_EINVAL. */
 int vof_residual_ex(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double dt,
                     int detector, void* d_sC_out, void* d_Cnew_out, void* cuda_stream);
+/* The same residual for callers that must not allocate (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no cudaMalloc / cudaMallocAsync / cudaFree and no allocating library routine is called.  The four intermediate fields
+ * (adv, k^x, k^y, k^z) live in a static device array of VOF_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds until
+ * the process exits; inputs and outputs are the caller's, as in vof_residual_ex, and the results are bit-identical to it.
+ * Limit: 4 * roundup(nx ny nz * sizeof(element), 256) <= VOF_NOALLOC_SCRATCH_BYTES, i.e. up to 524288 points in fp32 (64 x 64 x 128)
+ * and 262144 in fp64 (64^3); larger grids are refused with MG_EINVAL and a message that names both sizes (use vof_residual_ex).
+ * Every call on a device shares that one array: calls that overlap on the GPU (different streams, or graphs replayed concurrently)
+ * race on it -- keep them on one stream or order them with events.  The array keeps the last call's contents; nothing in it has
+ * to start at zero (every field is fully written before it is read), so no clearing is needed between calls. */
+#define VOF_NOALLOC_SCRATCH_BYTES (8u << 20)
+int vof_residual_noalloc(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double dt,
+                         int detector, void* d_sC_out, void* d_Cnew_out, void* cuda_stream);
 
 /* a9: momentum advection-diffusion residual and predictor, Eqs. 18, 30-32, 45-46 (P:198-220,
  * 309-319, 433-441; reading C9 "Momentum").  d_qh[3] = half-level (u, v, w), d_qn[3] = level-n

@@ -24,7 +24,7 @@ EXPORTS = [
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_solve_host_zero", "mg_get_history", "mg_get_history_cycles", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
     "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_pcg", "flow_time_step_paper", "mg_last_error",
-    "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full", "vof_residual_ex",
+    "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full", "vof_residual_ex", "vof_residual_noalloc",
     "mg_version",
 ]
 
@@ -87,6 +87,7 @@ def _load():
     lib.mg_set_fused.argtypes = [vp, i]
     lib.vof_residual.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, vp, vp, vp]
     lib.vof_residual_ex.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, i, vp, vp, vp]
+    lib.vof_residual_noalloc.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, i, vp, vp, vp]
     lib.mom_predictor.argtypes = [C.POINTER(MgGrid), i, vp, C.POINTER(vp), C.POINTER(vp), d, d, d, d, d,
                                   C.POINTER(vp), C.POINTER(vp), vp]
     lib.pressure_rhs.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, d, vp, vp]
@@ -329,6 +330,16 @@ def vof_residual_ex(C_, u, v, w, h, dt, detector, sC_out=None, Cnew_out=None, st
     return _check(_lib.vof_residual_ex(C.byref(g), _dtype_code(C_), _dev(C_), _dev(u, sh, dt_), _dev(v, sh, dt_),
                                        _dev(w, sh, dt_), float(dt), int(detector), _dev(sC_out, sh, dt_, True),
                                        _dev(Cnew_out, sh, dt_, True), _stream_ptr(stream)))
+
+
+def vof_residual_noalloc(C_, u, v, w, h, dt, detector=3, sC_out=None, Cnew_out=None, stream=None):
+    """vof_residual_ex without any allocation by the library (static device scratch; size limit VOF_NOALLOC_SCRATCH_BYTES of
+    include/mg.h, MgError(MG_EINVAL) beyond it).  Calls that overlap on the GPU race on the shared scratch."""
+    g = _grid_of(C_, h)
+    sh, dt_ = tuple(C_.shape), C_.dtype
+    return _check(_lib.vof_residual_noalloc(C.byref(g), _dtype_code(C_), _dev(C_), _dev(u, sh, dt_), _dev(v, sh, dt_),
+                                            _dev(w, sh, dt_), float(dt), int(detector), _dev(sC_out, sh, dt_, True),
+                                            _dev(Cnew_out, sh, dt_, True), _stream_ptr(stream)))
 
 
 def _ptr3(ts, sh, dt_, allow_none=False):

@@ -13,6 +13,7 @@
 #include <cmath>
 #include <cstdint>
 #include <initializer_list>
+#include <mutex>
 
 #include "solver.h"
 
@@ -162,6 +163,25 @@ int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T
     return 0;
 }
 
+// vof_residual_t with the four scratch fields given by the caller (vof_residual_noalloc); nothing is allocated or freed
+template <typename T>
+int vof_residual_scratch_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double dt, int detector, T* sC, T* Cnew,
+                           T* adv, T* kx, T* ky, T* kz, cudaStream_t st) {
+    const Geo<T> G = make_geo<T>(g, nullptr);
+    const double hmax = fmax(g->hx, fmax(g->hy, g->hz)), hmin = fmin(g->hx, fmin(g->hy, g->hz));
+    const double k_min = 1e-4 / dt * hmax * hmax, k_max = 0.05 / dt * hmin * hmin;   // Eq. 42
+    const bool vec = can_vec<T>(g, {C, u, v, w, sC, Cnew});
+    MGB_MARCH(advection_march, vec, G, st, C, u, v, w, adv);
+    if (detector == 5) {       // Eq. 34
+        if (vec) vof_coeff_march<T, 2, true><<<march_grid<T, 2>(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
+        else vof_coeff_march<T, 1, true><<<march_grid<T, 1>(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
+    } else
+    MGB_MARCH_W(vof_coeff_march, 2, vec, G, st, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);
+    MGB_MARCH(vof_diffusion_march, vec, G, st, C, adv, kx, ky, kz, (T)dt, sC, Cnew);
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
+
 template <typename T>
 int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T* const qn[3], const int* vbc, double rho_l, double rho_g,
                     double mu_l, double mu_g, double dt, T* const qt[3], T* const qhn[3], cudaStream_t st) {
@@ -269,6 +289,28 @@ bool grid_ok(const mg_grid* g, int dtype) {
 
 using namespace mgb;
 
+// ---- vof_residual_noalloc: scratch that exists without any allocation call ----------------------------------------------------
+// The four intermediate fields of the VoF residual (adv, k^x, k^y, k^z) in a file-scope device array: VOF_NOALLOC_SCRATCH_BYTES
+// (include/mg.h, 8 MiB) on every GPU that loads the library, until the process exits.  In HOST code `g_vof_scratch` is only a
+// stand-in for the symbol, not a device address: the address is asked for once per device, with that device current
+// (cudaGetSymbolAddress), and that pointer is what the kernels get.
+static __device__ __align__(256) unsigned char g_vof_scratch[VOF_NOALLOC_SCRATCH_BYTES];
+
+static int vof_scratch_address(unsigned char** out) {
+    static std::mutex mu;
+    static unsigned char* addr[64] = {nullptr};
+    int dev = -1;
+    MGB_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && addr[dev]) { *out = addr[dev]; return 0; }
+    unsigned char* p = nullptr;
+    MGB_CUDA(cudaGetSymbolAddress((void**)&p, g_vof_scratch));
+    if (!p) { set_error("vof_residual_noalloc: no device address for the scratch array"); return MG_ECUDA; }
+    if (dev >= 0 && dev < 64) addr[dev] = p;
+    *out = p;
+    return 0;
+}
+
 extern "C" {
 
 int vof_residual(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double dt,
@@ -290,6 +332,37 @@ int vof_residual_ex(const mg_grid* grid, int dtype, const void* d_C, const void*
                                      (float*)d_sC_out, (float*)d_Cnew_out, st);
     return vof_residual_t<double>(grid, (const double*)d_C, (const double*)d_u, (const double*)d_v, (const double*)d_w, dt, detector,
                                   (double*)d_sC_out, (double*)d_Cnew_out, st);
+}
+
+int vof_residual_noalloc(const mg_grid* grid, int dtype, const void* d_C, const void* d_u, const void* d_v, const void* d_w, double dt,
+                         int detector, void* d_sC_out, void* d_Cnew_out, void* cuda_stream) {
+    if (!grid_ok(grid, dtype)) return MG_EINVAL;
+    if (detector != 3 && detector != 5) { set_error("vof_residual_noalloc: detector %d is not 3 (Eq. 33) or 5 (Eq. 34)", detector); return MG_EINVAL; }
+    if (!d_C || !d_u || !d_v || !d_w || !(dt > 0.0) || (!d_sC_out && !d_Cnew_out) || d_Cnew_out == d_C || d_sC_out == d_C) {
+        set_error("vof_residual_noalloc: NULL / aliased argument or dt <= 0");
+        return MG_EINVAL;
+    }
+    const size_t esz = dtype == MG_F32 ? 4 : 8;
+    const size_t field = (npts(grid->nx, grid->ny, grid->nz) * esz + 255) / 256 * 256;      // every field starts 256-byte aligned
+    if (4 * field > (size_t)VOF_NOALLOC_SCRATCH_BYTES) {
+        set_error("vof_residual_noalloc: %dx%dx%d %s needs %zu bytes of scratch, the static array holds %zu (VOF_NOALLOC_SCRATCH_BYTES); "
+                  "use vof_residual_ex", grid->nx, grid->ny, grid->nz, dtype == MG_F32 ? "fp32" : "fp64", 4 * field,
+                  (size_t)VOF_NOALLOC_SCRATCH_BYTES);
+        return MG_EINVAL;
+    }
+    unsigned char* base = nullptr;
+    int rc = vof_scratch_address(&base);
+    if (rc) return rc;
+    // nothing in the scratch has to start at zero: the first kernel writes every point of adv, the second every point of k^x, k^y,
+    // k^z, before the kernel that reads them -- whatever an earlier call left there is overwritten
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (dtype == MG_F32)
+        return vof_residual_scratch_t<float>(grid, (const float*)d_C, (const float*)d_u, (const float*)d_v, (const float*)d_w, dt, detector,
+                                             (float*)d_sC_out, (float*)d_Cnew_out, (float*)base, (float*)(base + field),
+                                             (float*)(base + 2 * field), (float*)(base + 3 * field), st);
+    return vof_residual_scratch_t<double>(grid, (const double*)d_C, (const double*)d_u, (const double*)d_v, (const double*)d_w, dt, detector,
+                                          (double*)d_sC_out, (double*)d_Cnew_out, (double*)base, (double*)(base + field),
+                                          (double*)(base + 2 * field), (double*)(base + 3 * field), st);
 }
 
 static bool vbc_ok(const int* vbc) {
