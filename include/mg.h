@@ -91,7 +91,9 @@ int mg_get_params(const mg_solver* s, mg_params* p);
 /* Coefficient k (a7).  d_k: nx*ny*nz values of k > 0, or NULL for constant k = 1.  The field is
  * copied; coarse levels get the arithmetic mean of the 8 children (reading C5). */
 int mg_set_coefficient(mg_solver* s, const void* d_k);
-/* k = 1 / (rho_l alpha + rho_g (1 - alpha)), Eqs. 2 and 19; no clipping (C7). */
+/* k = 1 / (rho_l a + rho_g (1 - a)), Eqs. 2 and 19, with a = alpha limited to [0, 1] (reading C7: the paper does not
+ * clip, but an undershoot of alpha below -rho_g / (rho_l - rho_g) = -0.001 would make the density negative and the operator
+ * indefinite; the explicit stages form rho and mu the same way). */
 int mg_set_coefficient_from_vof(mg_solver* s, const void* d_alpha, double rho_l, double rho_g);
 
 /* a1: y = A x on the fine level.  d_y must not alias d_x. */
@@ -252,6 +254,12 @@ int flow_time_step_pcg(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w,
 int flow_time_step_full(mg_solver* s_hs, mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_phs, void* d_pnh,
                         double rho_l, double rho_g, double mu_l, double mu_g, double g, double sigma_t, double dt, double tol,
                         int max_cycles, double hs_tol, int hs_cycles, const int walls[6], int* cycles_out, double* relres_out);
+/* The same step with the stage-3 solver chosen by pressure_solver: 0 = mg_solve (plain cycles, the paper's; = flow_time_step_full),
+ * 1 = mg_pcg_solve (tol, max_cycles iterations; its requirements apply).  Other values: MG_EINVAL. */
+int flow_time_step_full_ex(mg_solver* s_hs, mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_phs, void* d_pnh,
+                           double rho_l, double rho_g, double mu_l, double mu_g, double g, double sigma_t, double dt, double tol,
+                           int max_cycles, double hs_tol, int hs_cycles, const int walls[6], int pressure_solver, int* cycles_out,
+                           double* relres_out);
 
 /* The same time step with the PAPER'S stage 3 (SURVEY 8(f) "next 2"): constant-coefficient Laplacian with the density on the
  * right (Eqs. 52-53), `cycles` V-cycles per solve from a zero guess (the paper's fixed 20), velocity correction Eq. 54,

@@ -19,6 +19,8 @@
  * (both branches of min{k_max, k_abs} of Eqs. 30-32 under varying rho and mu), and -- for the step composition in
  * oracle/__init__.py -- the stages chained by hand, the potential-flow property of stage 4 (Eq. 16 advects with
  * u^{n+1}) and the second-order accuracy of the two predictor iterations (tests/test_oracle_step.py).
+ * The limit of the volume fraction in the material mixtures (reading C7, mix01 below): closed-form k values, bit-identity of
+ * every rho / mu consumer under limiting, and the scaling law that shows the surface-tension terms are NOT limited.
  * PARITY UNPINNED against the paper (no worked example exists in its text): the transfer
  * operators / coarse operator (Fig. 5 is an image), the momentum residual without the
  * missing Eq. 28, and vof_residual beyond its hand-computable special cases.
@@ -273,9 +275,19 @@ void orc_prolong_add(const orc_grid* gf, const double* xc, double* xf) {
                 xf[IDX(gf, i, j, k)] += xc[IDX(&gc, i / 2, j / 2, k / 2)];
 }
 
-/* k = 1 / (rho_l alpha + rho_g (1 - alpha)), Eqs. 2 and 19; no clipping (C7). */
+/* Material property of the one-fluid model, Eqs. 2 and 19: a = a_l C + a_g (1 - C), with C limited to [0, 1]
+ * first (reading C7, revised in round 2: the paper does not clip, and says of its scheme only that it "reduces the
+ * likelihood" of C leaving [0, 1]; an undershoot C = -0.003 gives rho < 0 at rho_g / rho_l = 1e-3 and the pressure
+ * operator loses definiteness).  Only the mixtures rho and mu see the limited value; gradients, curvature and the VoF scheme
+ * use C as it is. */
+static inline double mix01(double al, double ag, double C) {
+    const double c = C < 0.0 ? 0.0 : (C > 1.0 ? 1.0 : C);
+    return al * c + ag * (1.0 - c);
+}
+
+/* k = 1 / rho(alpha), Eqs. 2 and 19, alpha limited to [0, 1] (C7). */
 void orc_k_from_vof(size_t n, const double* alpha, double rho_l, double rho_g, double* kcoef) {
-    for (size_t c = 0; c < n; ++c) kcoef[c] = 1.0 / (rho_l * alpha[c] + rho_g * (1.0 - alpha[c]));
+    for (size_t c = 0; c < n; ++c) kcoef[c] = 1.0 / mix01(rho_l, rho_g, alpha[c]);
 }
 
 /* ------------------------------------------------------------------------------------
@@ -543,15 +555,15 @@ void orc_mom_predictor_bc(const orc_grid* g, const double* C, const double* cons
         grad_and_adv_bc(g, cbc, qh[comp], qh[0], qh[1], qh[2], px, py, pz, adv);
         mixed_mass_residual(g, adv, a);
         for (size_t c = 0; c < n; ++c) {
-            const double rho = rho_l * C[c] + rho_g * (1.0 - C[c]);
-            const double mu = mu_l * C[c] + mu_g * (1.0 - C[c]);
+            const double rho = mix01(rho_l, rho_g, C[c]);
+            const double mu = mix01(mu_l, mu_g, C[c]);
             const double kmax = g->hx * fabs(qh[0][c]) + g->hy * fabs(qh[1][c]) + g->hz * fabs(qh[2][c]);
             const double kabs = k_abs_pg(g, a[c], px[c], py[c], pz[c]);
             kc[c] = rho * fmin(kmax, kabs) + mu;
         }
         orc_apply_diffusion(g, cbc, wl, kc, qh[comp], diff);
         for (size_t c = 0; c < n; ++c) {
-            const double rho = rho_l * C[c] + rho_g * (1.0 - C[c]);
+            const double rho = mix01(rho_l, rho_g, C[c]);
             const double s = rho * adv[c] + diff[c];
             const double t = qn[comp][c] - dt * s / rho;
             qt[comp][c] = t;
@@ -597,7 +609,7 @@ void orc_pressure_rhs_paper(const orc_grid* g, const double* C, const double* u,
     double* rho = (double*)malloc(n * sizeof(double));
     double* m = (double*)malloc(n * sizeof(double));
     double* t = (double*)malloc(n * sizeof(double));
-    for (size_t c = 0; c < n; ++c) { rho[c] = rho_l * C[c] + rho_g * (1.0 - C[c]); b[c] = 0.0; }
+    for (size_t c = 0; c < n; ++c) { rho[c] = mix01(rho_l, rho_g, C[c]); b[c] = 0.0; }
     const double* vel[3] = {u, v, w};
     const double* flt[3] = {wx, wy, wz};
     for (int d = 0; d < 3; ++d) {
@@ -655,7 +667,7 @@ void orc_hydrostatic_rhs(const orc_grid* g, const double* C, double rho_l, doubl
     for (size_t c = 0; c < n; ++c)
         for (int d = 0; d < 3; ++d) st[d][c] = sigma_t * kap[c] * gc[d][c];
     /* b = f(g rho; w_z) - div(s_t)   (Eq. 43) */
-    for (size_t c = 0; c < n; ++c) nt[0][c] = grav * (rho_l * C[c] + rho_g * (1.0 - C[c]));      /* reuse: g rho */
+    for (size_t c = 0; c < n; ++c) nt[0][c] = grav * mix01(rho_l, rho_g, C[c]);      /* reuse: g rho */
     orc_apply_filter(g, BC_COPY, wz, nt[0], b);
     for (int d = 0; d < 3; ++d) {
         orc_apply_filter(g, BC_COPY, flt[d], st[d], t);
@@ -703,7 +715,7 @@ void orc_mom_forcing(const orc_grid* g, const double* C, const double* p_hs, con
     double* rho = (double*)malloc(n * sizeof(double));
     double* src = (double*)malloc(n * sizeof(double));
     double* t = (double*)malloc(n * sizeof(double));
-    for (size_t c = 0; c < n; ++c) rho[c] = rho_l * C[c] + rho_g * (1.0 - C[c]);
+    for (size_t c = 0; c < n; ++c) rho[c] = mix01(rho_l, rho_g, C[c]);
     for (int d = 0; d < 3; ++d) {
         orc_filter(g, 1 + d, wd);
         for (size_t c = 0; c < n; ++c) src[c] = (st && st[d] ? st[d][c] : 0.0) + (d == 2 ? -grav * rho[c] : 0.0);

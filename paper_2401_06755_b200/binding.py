@@ -24,7 +24,7 @@ EXPORTS = [
     "mg_set_coefficient_from_vof", "mg_apply_operator", "mg_smooth", "mg_residual", "mg_vcycle", "mg_solve", "mg_pcg_solve",
     "mg_solve_host", "mg_solve_host_zero", "mg_get_history", "mg_get_history_cycles", "mg_level_info", "mg_vcycle_timed", "mg_launch_count", "mg_set_fused",
     "vof_residual", "mom_predictor", "pressure_rhs", "pressure_rhs_paper", "hydrostatic_rhs", "project_velocity", "flow_time_step", "flow_time_step_pcg", "flow_time_step_paper", "mg_last_error",
-    "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full", "vof_residual_ex", "vof_residual_noalloc",
+    "mom_predictor_bc", "pressure_rhs_bc", "mom_forcing", "hydrostatic_rhs_force", "flow_time_step_full", "flow_time_step_full_ex", "vof_residual_ex", "vof_residual_noalloc",
     "mg_version",
 ]
 
@@ -98,6 +98,7 @@ def _load():
                                 C.POINTER(vp), vp]
     lib.hydrostatic_rhs_force.argtypes = [C.POINTER(MgGrid), i, vp, d, d, d, d, vp, vp, C.POINTER(vp), vp]
     lib.flow_time_step_full.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, d, d, i, d, i, pi, pi, pd]
+    lib.flow_time_step_full_ex.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, d, d, d, d, d, d, d, d, i, d, i, pi, i, pi, pd]
     lib.pressure_rhs_paper.argtypes = [C.POINTER(MgGrid), i, vp, vp, vp, vp, d, d, d, vp, vp]
     lib.flow_time_step_paper.argtypes = [vp, vp, vp, vp, vp, vp, d, d, d, d, d, i, i, pd]
     lib.hydrostatic_rhs.argtypes = [C.POINTER(MgGrid), i, vp, d, d, d, d, vp, vp, vp]
@@ -395,6 +396,19 @@ def flow_time_step_full(s_hs, s, C_, u, v, w, p_hs, p_nh, rho_l, rho_g, mu_l, mu
                                          _dev(p_hs, sh, dt_), _dev(p_nh, sh, dt_), float(rho_l), float(rho_g), float(mu_l), float(mu_g),
                                          float(grav), float(sigma_t), float(dt), float(tol), int(max_cycles), float(hs_tol),
                                          int(hs_cycles), wl, C.byref(cyc), C.byref(rel)))
+    return st, cyc.value, rel.value
+
+
+def flow_time_step_full_ex(s_hs, s, C_, u, v, w, p_hs, p_nh, rho_l, rho_g, mu_l, mu_g, grav, sigma_t, dt, tol, max_cycles,
+                           hs_tol=0.0, hs_cycles=20, walls=(1, 1, 1, 1, 1, 0), pressure_solver=0):
+    """flow_time_step_full with the stage-3 solver chosen: 0 = plain cycles, 1 = V-cycle-preconditioned CG."""
+    cyc, rel = C.c_int(0), C.c_double(0.0)
+    sh, dt_ = s.shape, s.torch_dtype
+    wl = (C.c_int * 6)(*[int(b) for b in walls])
+    st = _check(_lib.flow_time_step_full_ex(s_hs.handle, s.handle, _dev(C_, sh, dt_), _dev(u, sh, dt_), _dev(v, sh, dt_), _dev(w, sh, dt_),
+                                            _dev(p_hs, sh, dt_), _dev(p_nh, sh, dt_), float(rho_l), float(rho_g), float(mu_l), float(mu_g),
+                                            float(grav), float(sigma_t), float(dt), float(tol), int(max_cycles), float(hs_tol),
+                                            int(hs_cycles), wl, int(pressure_solver), C.byref(cyc), C.byref(rel)))
     return st, cyc.value, rel.value
 
 

@@ -548,6 +548,15 @@ int flow_time_step_pcg(mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w,
 int flow_time_step_full(mg_solver* s_hs, mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_phs, void* d_pnh,
                         double rho_l, double rho_g, double mu_l, double mu_g, double grav, double sigma_t, double dt, double tol,
                         int max_cycles, double hs_tol, int hs_cycles, const int walls[6], int* cycles_out, double* relres_out) {
+    return flow_time_step_full_ex(s_hs, s, d_C, d_u, d_v, d_w, d_phs, d_pnh, rho_l, rho_g, mu_l, mu_g, grav, sigma_t, dt, tol, max_cycles,
+                                  hs_tol, hs_cycles, walls, 0, cycles_out, relres_out);
+}
+
+int flow_time_step_full_ex(mg_solver* s_hs, mg_solver* s, void* d_C, void* d_u, void* d_v, void* d_w, void* d_phs, void* d_pnh,
+                           double rho_l, double rho_g, double mu_l, double mu_g, double grav, double sigma_t, double dt, double tol,
+                           int max_cycles, double hs_tol, int hs_cycles, const int walls[6], int pressure_solver, int* cycles_out,
+                           double* relres_out) {
+    if (pressure_solver != 0 && pressure_solver != 1) { set_error("flow_time_step_full_ex: pressure_solver %d is not 0 (cycles) or 1 (PCG)", pressure_solver); return MG_EINVAL; }
     if (!s || !s_hs || !d_C || !d_u || !d_v || !d_w || !d_phs || !d_pnh || !walls) { set_error("flow_time_step_full: NULL argument"); return MG_EINVAL; }
     if (s_hs->dtype != s->dtype || s_hs->grid.nx != s->grid.nx || s_hs->grid.ny != s->grid.ny || s_hs->grid.nz != s->grid.nz ||
         s_hs->grid.hx != s->grid.hx || s_hs->device != s->device || s_hs->st != s->st || s_hs->var_k) {
@@ -587,7 +596,11 @@ int flow_time_step_full(mg_solver* s_hs, mg_solver* s, void* d_C, void* d_u, voi
         if (!rc) rc = mg_set_coefficient_from_vof(s, d_C, rho_l, rho_g);
         if (!rc) rc = pressure_rhs_bc(&s->grid, s->dtype, qt[0], qt[1], qt[2], vbc, dt, bbuf, st);
         if (!rc) rc = cudaMemsetAsync(dp, 0, bytes, st) == cudaSuccess ? 0 : MG_ECUDA;
-        if (!rc) { status = mg_solve(s, dp, bbuf, tol, max_cycles, cycles_out, relres_out); if (status < 0) rc = status; }
+        if (!rc) {
+            status = pressure_solver == 1 ? mg_pcg_solve(s, dp, bbuf, tol, max_cycles, cycles_out, relres_out)
+                                          : mg_solve(s, dp, bbuf, tol, max_cycles, cycles_out, relres_out);
+            if (status < 0) rc = status;
+        }
         if (!rc) rc = project_velocity(&s->grid, s->bc, s->dtype, dp, s->lv[0].k, dt, qt[0], qt[1], qt[2], st);
         if (!rc) rc = s->dtype == MG_F32 ? launch_axpy<float>(n, (float*)d_pnh, (const float*)dp, st)
                                          : launch_axpy<double>(n, (double*)d_pnh, (const double*)dp, st);

@@ -80,6 +80,18 @@ template <typename T, int W> __device__ __forceinline__ Pk<T, W> pmax(const Pk<T
 template <typename T, int W> __device__ __forceinline__ Pk<T, W> pmin(T a, const Pk<T, W>& b) { return pmin(splat<T, W>(a), b); }
 template <typename T, int W> __device__ __forceinline__ Pk<T, W> pmax(T a, const Pk<T, W>& b) { return pmax(splat<T, W>(a), b); }
 
+// Material property of the one-fluid model, Eqs. 2 / 19: a = a_l C + a_g (1 - C) with C limited to [0, 1] first
+// (reading C11: the paper does not clip, but an undershoot C = -0.003 -- which its scheme only makes "less likely", P:359 --
+// gives rho < 0 at rho_g / rho_l = 1e-3, an indefinite pressure operator and a blow-up of the collapsing column)
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> mix01(T al, T ag, const Pk<T, W>& C) {
+    const Pk<T, W> c = pmax(T(0), pmin(T(1), C));
+    return al * c + ag * (T(1) - c);
+}
+template <typename T> __device__ __forceinline__ T mix01(T al, T ag, T C) {
+    const T c = tmax(T(0), tmin(T(1), C));
+    return al * c + ag * (T(1) - c);
+}
+
 // aligned vector load / store of a pack (W sizeof(T) = 4, 8, 16 or 32 bytes)
 template <typename T, int W>
 __device__ __forceinline__ Pk<T, W> ldv(const T* __restrict__ p) {
@@ -310,7 +322,7 @@ __global__ void __launch_bounds__(MBX* MBY) mom_forcing_march(const Geo<T> G, co
 #pragma unroll
                     for (int b = 0; b < 3; ++b)
 #pragma unroll
-                        for (int a = 0; a < 3; ++a) t9[b][a] = t9[b][a] + (G.h[2] * grav) * (rho_l * c9[b][a] + rho_g * (T(1) - c9[b][a]));
+                        for (int a = 0; a < 3; ++a) t9[b][a] = t9[b][a] + (G.h[2] * grav) * mix01(rho_l, rho_g, c9[b][a]);
                 }
 #pragma unroll
                 for (int b = 0; b < 3; ++b)
@@ -339,7 +351,7 @@ __global__ void __launch_bounds__(MBX* MBY) mom_forcing_march(const Geo<T> G, co
             if (have_p) g.grad(G, gx, gy, gz);
             const size_t c0 = at(c, q);
             const V Cc = ldv<T, W>(C + c0);
-            const V f = dt / (rho_l * Cc + rho_g * (T(1) - Cc));
+            const V f = dt / mix01(rho_l, rho_g, Cc);
             const V u = ldv<T, W>(q0 + c0) - f * (gx + s0), v = ldv<T, W>(q1 + c0) - f * (gy + s1), w = ldv<T, W>(q2 + c0) - f * (gz + s2);
             stv(q0 + c0, u); stv(q1 + c0, v); stv(q2 + c0, w);
             if (h0) {
@@ -451,8 +463,8 @@ __global__ void __launch_bounds__(MBX* MBY) mom_coeff_march(const Geo<T> G, cons
             const V a = T(2) * (madv - a0);
             const size_t c0 = at(c, q);
             const V Cc = ldv<T, W>(C + c0);
-            const V rho = rho_l * Cc + rho_g * (T(1) - Cc);
-            const V mu = mu_l * Cc + mu_g * (T(1) - Cc);
+            const V rho = mix01(rho_l, rho_g, Cc);
+            const V mu = mix01(mu_l, mu_g, Cc);
             const V kmax = G.h[0] * pabs(ldv<T, W>(u + c0)) + G.h[1] * pabs(ldv<T, W>(v + c0)) + G.h[2] * pabs(ldv<T, W>(w + c0));   // Eq. 30
             stv(kc + c0, rho * pmin(kmax, k_abs_pk(G, a, px, py, pz)) + mu);
         }
@@ -501,7 +513,7 @@ __global__ void __launch_bounds__(MBX* MBY) mom_update_march(const Geo<T> G, con
             const V diff = T(0.5) * (Lz + k0 * Lx - x0 * Lk);
             const size_t c0 = at(c, q);
             const V Cc = ldv<T, W>(C + c0);
-            const V rho = rho_l * Cc + rho_g * (T(1) - Cc);
+            const V rho = mix01(rho_l, rho_g, Cc);
             const V s = rho * ldv<T, W>(adv + c0) + diff;
             const V qv = ldv<T, W>(qn + c0);
             const V t = qv - dt * s / rho;
@@ -666,7 +678,7 @@ __global__ void __launch_bounds__(MBX* MBY) pressure_rhs_paper_march(const Geo<T
 #pragma unroll
         for (int b = 0; b < 3; ++b)
 #pragma unroll
-            for (int a = 0; a < 3; ++a) r9[b][a] = rho_l * r9[b][a] + rho_g * (T(1) - r9[b][a]);
+            for (int a = 0; a < 3; ++a) r9[b][a] = mix01(rho_l, rho_g, r9[b][a]);
         gr.add(G, in_plane<T, true, false>(G, r9));
         const T* const vel[3] = {u, v, w};
         V part[3];
@@ -743,7 +755,7 @@ __global__ void __launch_bounds__(MBX* MBY) surface_tension_march(const Geo<T> G
             const size_t c0 = at(c, q);
             const V sk = -sigma_t * kap;                        // -s_t = sk grad C
             stv(fu + c0, sk * gx); stv(fv + c0, sk * gy);
-            stv(fw + c0, sk * gz + grav * (rho_l * C0 + rho_g * (T(1) - C0)));
+            stv(fw + c0, sk * gz + grav * mix01(rho_l, rho_g, C0));
             if (kappa) stv(kappa + c0, kap);
         }
     }
@@ -763,7 +775,7 @@ __global__ void bottom_fold_kernel(const Geo<T> G, const T* __restrict__ C, T rh
             const int ii = min(max(i + a - 1, 0), G.nx - 1), jj = min(max(j + bb - 1, 0), G.ny - 1);
             const T Cv = C[(size_t)jj * G.nx + ii];
             const T wl = (G.K[0][a] * G.M[bb] + G.M[a] * G.K[1][bb]) * G.M[0] + G.M[a] * G.M[bb] * G.K[2][0];
-            add -= wl * G.h[2] * grav * (rho_l * Cv + rho_g * (T(1) - Cv));
+            add -= wl * G.h[2] * grav * mix01(rho_l, rho_g, Cv);
         }
     b[(size_t)j * G.nx + i] += add;
 }

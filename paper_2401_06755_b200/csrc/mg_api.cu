@@ -1,6 +1,7 @@
 // mg_api.cu -- the C ABI of include/mg.h: solver object, level hierarchy, V-cycle and solve
 // loops.  Kernels live in mg_generic.cu (any grid / dtype) and mg_fused.cu (tuned fp32 path).
 #include <cmath>
+#include <limits>
 #include <cstdarg>
 #include <cstring>
 #include <mutex>
@@ -220,11 +221,20 @@ struct Stop {
     }
 };
 
+// a right-hand side with NaN / Inf in it (a time step that has blown up): say so instead of reporting ||r|| / ||b|| = 0
+static int nonfinite_rhs(int* cycles_out, double* rel_out) {
+    set_error("mg_solve: the right-hand side is not finite");
+    if (cycles_out) *cycles_out = 0;
+    if (rel_out) *rel_out = std::numeric_limits<double>::quiet_NaN();
+    return MG_STAGNATED;
+}
+
 template <typename T>
 static int solve_plain(mg_solver* s, T* x, const T* b, double tol, int max_cycles, int* cycles_out, double* rel_out) {
     LevelData& L = s->lv[0];
     int rc; double nb, nr;
     if ((rc = norm2<T>(s, L.n, b, &nb))) return rc;
+    if (!std::isfinite(nb)) return nonfinite_rhs(cycles_out, rel_out);
     if ((rc = residual_norm<T>(s, x, b, &nr))) return rc;
     double rel = nb > 0.0 ? nr / nb : 0.0;
     Stop stop{tol, 0, rel};
@@ -254,6 +264,7 @@ static int solve_mixed(mg_solver* s, float* x, const float* b, double tol, int m
     LevelData& L = s->lv[0];
     int rc; double nb, sq;
     if ((rc = norm2<float>(s, L.n, b, &nb))) return rc;
+    if (!std::isfinite(nb)) return nonfinite_rhs(cycles_out, rel_out);
     if ((rc = launch_cast_f2d(L.n, x, s->x64, s->st))) return rc;
     ++s->launches;
     const bool marching = s->fused && march_supported(L.nx, L.ny, L.nz, L.hx, L.hy, L.hz);

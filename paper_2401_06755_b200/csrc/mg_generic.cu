@@ -164,7 +164,8 @@ __global__ void prolong_add_kernel(int nxf, int nyf, int nzf, const T* __restric
 template <typename TA, typename TK>
 __global__ void k_from_vof_kernel(size_t n, const TA* __restrict__ alpha, double rho_l, double rho_g, TK* __restrict__ k) {
     for (size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x) {
-        const TK a = (TK)alpha[c];
+        TK a = (TK)alpha[c];
+        a = a < TK(0) ? TK(0) : (a > TK(1) ? TK(1) : a);          // reading C11: rho from the volume fraction limited to [0, 1]
         k[c] = TK(1) / ((TK)rho_l * a + (TK)rho_g * (TK(1) - a));
     }
 }

@@ -121,6 +121,12 @@ int pcg_t(mg_solver* s, void* d_x, const void* d_b, double tol, int max_iter, in
     MGB_CUDA(cudaMemsetAsync(sc, 0, S_N * sizeof(double), st));
     if ((rc = launch_sumsq<double>(n, b, sc + S_PQ, st))) return rc;
     if ((rc = read(S_PQ, &bb))) return rc;
+    if (!std::isfinite(bb)) {          // a right-hand side with NaN / Inf in it: say so instead of reporting a zero residual
+        set_error("mg_pcg_solve: the right-hand side is not finite");
+        if (iters_out) *iters_out = 0;
+        if (rel_out) *rel_out = std::nan("");
+        return MG_STAGNATED;
+    }
     if ((rc = launch_march_residual<double, double>(L.nx, L.ny, L.nz, L.hx, L.Ld.s, x, k, b, r, sc + S_RR, st))) return rc;
     s->launches += 2;
     if ((rc = read(S_RR, &rr))) return rc;

@@ -53,6 +53,48 @@ def solver_for(w, dtype=None, **params):
     return s
 
 
+def collapsing_column(n=64):
+    """SURVEY 8(f) next 3, "a real collapsing-column run can be sanity-checked qualitatively": the four-stage step on a water column
+    (a = 0.25 wide, H = 0.5 high, unit box, free-slip walls, open top) released from rest, to T* = t sqrt(2 g / a) = 3.5."""
+    import time
+    levels = int(np.log2(n)) - 1
+    w = configs.config5(n, levels)
+    h, grav, sig, a, H = w.h, 9.81, 0.0728, 0.25, 0.5
+    dt = 0.1 * h / 3.0
+    xs = (np.arange(n) + 0.5) * h
+    print("\n### A collapsing water column with the four-stage step (%d^3, %d levels, dt = %.2e s = Courant 0.1 at 3 m/s; a = %.2f, H = %.2f; "
+          "sqrt(g H) = %.2f, sqrt(2 g H) = %.2f m/s)\n" % (n, levels, dt, a, H, np.sqrt(grav * H), np.sqrt(2 * grav * H)))
+    for ps, name in ((0, "plain V(2,2) cycles (mg_solve)"), (1, "V-cycle-preconditioned CG (mg_pcg_solve)")):
+        s_hs, s_nh = solver_for(w, cycles_per_defect=0), solver_for(w, cycles_per_defect=0)
+        C = f32(w.fields["alpha"])
+        u, v, ww = (torch.zeros_like(C) for _ in range(3))
+        phs, pnh = torch.zeros_like(C), torch.zeros_like(C)
+        vol0 = float(C.double().sum())
+        t, step, cycles, nxt, worst = 0.0, 0, 0, 0.5, 0
+        print("stage 3 by %s:\n" % name)
+        print("| T* | t s | front x/a | column height / H | liquid volume drift | min C | max C | max liquid speed m/s | max speed m/s | cycles per step |")
+        print("|---|---|---|---|---|---|---|---|---|---|")
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        while t * np.sqrt(2 * grav / a) < 3.5:
+            st, cyc, rel = mg.flow_time_step_full_ex(s_hs, s_nh, C, u, v, ww, phs, pnh, w.rho_l, w.rho_g, w.mu_l, w.mu_g, grav, sig, dt,
+                                                     1e-6, 100, 0.0, 20, (1, 1, 1, 1, 1, 0), ps)
+            t += dt; step += 1; cycles += cyc; worst = max(worst, st)
+            ts = t * np.sqrt(2 * grav / a)
+            if ts >= nxt:
+                Cb, Cw = C[0, n // 2, :].cpu().numpy(), C[:, n // 2, 0].cpu().numpy()
+                wet, col = np.where(Cb > 0.5)[0], np.where(Cw > 0.5)[0]
+                sp = torch.sqrt(u * u + v * v + ww * ww)
+                print("| %.2f | %.4f | %.2f | %.2f | %+.1e | %.3f | %.3f | %.2f | %.2f | %.1f |" % (
+                    ts, t, xs[wet.max()] / a if wet.size else 0.0, xs[col.max()] / H if col.size else 0.0,
+                    float(C.double().sum()) / vol0 - 1, float(C.min()), float(C.max()), float((sp * (C > 0.5)).max()), float(sp.max()),
+                    cycles / step))
+                nxt += 0.5
+        torch.cuda.synchronize()
+        print("\n%d steps, %.2f ms per step (wall clock, host loop included), worst stage-3 status %d\n" % (step, (time.perf_counter() - t0) / step * 1e3, worst))
+        mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)
+    print("Without the limit on C in the material mixtures (DESIGN.md reading C7) the same run ends at T* = 0.7 (at 32^3: 0.9): C undershoots to -0.003 in the thin tongue at the front, rho = 1000 C + (1 - C) turns negative there, the stage-3 operator loses definiteness and both solvers diverge within twenty steps.")
+
+
 def main():
     torch.cuda.set_device(0)
     print("# The five BASELINE.json configurations on one B200 (%s)\n" % mg.mg_version())
@@ -262,6 +304,8 @@ def main():
                  dt_full, 9.81 * 7 * dt_full))
         mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)
         del phs, pnh
+
+    collapsing_column(64)
 
     print("\n### The same step with the paper's own stage 3 (constant-coefficient Laplacian, density on the right, Eqs. 52-53; "
           "2 passes x 20 fixed cycles, P:429, P:498)\n")

@@ -154,3 +154,126 @@ def test_four_stage_step_parity(mg, orc, dt):
     # the column has started to fall: the step is not a no-op
     assert np.abs(ww).max() > 0.5 * grav * tstep
     mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_material_mixtures_with_out_of_range_volume_fraction(mg, orc, dt):
+    """Reading C7 (revised): rho and mu from C limited to [0, 1], everything else from C as it is.  C runs from -0.2 to 1.25 here
+    (rho would be negative without the limit), through every entry point that forms a mixture."""
+    import torch
+    shape, h = (12, 16, 20), 0.05
+    nz, ny, nx = shape
+    n = nx * ny * nz
+    g = orc.grid(nx, ny, nz, h)
+    x, y, z = configs.centres(nx, ny, nz, 1.0)
+    d = (0.7 * x / nx + 0.4 * y / ny + 0.6 * z / nz) - 0.8
+    Cf = quantise(1.45 * (0.5 * (1 + np.tanh(d * 5.0)) + 0.0 * (x + y + z)) - 0.2 + 0.02 * rng.normal(3, n).reshape(shape), dt)
+    assert Cf.min() < -0.1 and Cf.max() > 1.1
+    q = tuple(quantise(0.3 * rng.normal(40 + c, n).reshape(shape) + 0.2, dt) for c in range(3))
+    rho_l, rho_g, mu_l, mu_g, tstep, grav = 1000.0, 1.0, 1e-3, 1e-5, 0.1 * h, 9.81
+    dC = to_dev(Cf, dt)
+    dq = [to_dev(a, dt) for a in q]
+    # k = 1 / rho in the solver: the operator built from it against the oracle's
+    code = mg.MG_F32 if dt == "f32" else mg.MG_F64
+    s = mg.mg_create((nx, ny, nz, h), 2, BCP, code)
+    mg.mg_set_coefficient_from_vof(s, dC, rho_l, rho_g)
+    dy = torch.empty_like(dC)
+    mg.mg_apply_operator(s, dq[0], dy)
+    assert_close(as_f64(dy), orc.apply_operator(g, BCP, orc.k_from_vof(Cf, rho_l, rho_g), q[0]), TOL[dt])
+    mg.mg_destroy(s)
+    # momentum predictor, forcing terms, hydrostatic right-hand side, the paper's stage-3 right-hand side
+    vbc = orc.velocity_bc()
+    qt_ref, qh_ref = orc.mom_predictor(g, Cf, q, q, rho_l, rho_g, mu_l, mu_g, tstep, vbc)
+    dqt, dqh = [torch.empty_like(dC) for _ in range(3)], [torch.empty_like(dC) for _ in range(3)]
+    mg.mom_predictor_bc(dC, dq, dq, vbc, h, rho_l, rho_g, mu_l, mu_g, tstep, dqt, dqh)
+    for c in range(3):
+        assert_close(as_f64(dqt[c]), qt_ref[c], TOL[dt])
+        assert_close(as_f64(dqh[c]), qh_ref[c], TOL[dt])
+    p_hs = quantise(1e3 * rng.normal(51, n).reshape(shape), dt)
+    pbc = (N, D, N, N, N, D)
+    rho = rho_l * np.clip(Cf, 0, 1) + rho_g * (1 - np.clip(Cf, 0, 1))
+    z0 = np.zeros(shape)
+    ref = orc.mom_forcing(g, Cf, p_hs, None, pbc, grav, (z0, z0, grav * rho), rho_l, rho_g, tstep, q)
+    dq2 = [to_dev(a, dt) for a in q]
+    mg.mom_forcing(dC, to_dev(p_hs, dt), None, pbc, h, grav, None, rho_l, rho_g, tstep, dq2)
+    for c in range(3):
+        assert_close(as_f64(dq2[c]) - q[c], ref[c] - q[c], (20 if dt == "f32" else 1e3) * TOL[dt])
+    b_ref, _, _ = orc.hydrostatic_rhs(g, Cf, rho_l, rho_g, grav, 0.0)
+    db = torch.empty_like(dC)
+    mg.hydrostatic_rhs(dC, h, rho_l, rho_g, grav, 0.0, db)
+    assert_close(as_f64(db), b_ref, 5 * TOL[dt] if dt == "f32" else 1e-9)
+    mg.pressure_rhs_paper(dC, dq[0], dq[1], dq[2], h, rho_l, rho_g, tstep, db)
+    assert_close(as_f64(db), orc.pressure_rhs_paper(g, Cf, q[0], q[1], q[2], rho_l, rho_g, tstep), 50 * TOL[dt])
+
+
+def test_non_finite_right_hand_side_is_reported(mg):
+    """A step that has blown up hands NaN to the solver: mg_solve and mg_pcg_solve must say MG_STAGNATED with a NaN residual, not
+    MG_OK with residual 0 (||b|| = NaN fails every comparison)."""
+    import torch
+    n = 32
+    for mixed in (1, 0):
+        s = mg.mg_create((n, n, n, 1.0 / n), 3, BCP, mg.MG_F32)
+        mg.mg_set_params(s, mixed_precision=mixed)
+        b = torch.randn(n, n, n, device="cuda")
+        b[3, 4, 5] = float("nan")
+        x = torch.zeros_like(b)
+        status, cycles, rel = mg.mg_solve(s, x, b, 1e-6, 10)
+        assert status == mg.MG_STAGNATED and cycles == 0 and np.isnan(rel)
+        status, its, rel = mg.mg_pcg_solve(s, x, b, 1e-6, 10)
+        assert status == mg.MG_STAGNATED and its == 0 and np.isnan(rel)
+        b[3, 4, 5] = float("inf")
+        status, cycles, rel = mg.mg_solve(s, x, b, 0.0, 3)
+        assert status == mg.MG_STAGNATED and np.isnan(rel)
+        mg.mg_destroy(s)
+
+
+@pytest.mark.parametrize("pressure_solver", [0, 1])
+def test_collapsing_column_runs_and_behaves(mg, pressure_solver):
+    """Qualitative check of the whole four-stage step ("a real collapsing-column run can be sanity-checked
+    qualitatively"): a water column (width a = 0.25, height H = 0.5, 1000:1 density, free-slip box, 32^3) released from rest, 330
+    steps to T* = t sqrt(2 g / a) = 3.  Not a parity test -- the oracle would need minutes -- but physics any correct
+    implementation shows: the run stays finite (it does NOT without the limit of reading C7: rho < 0 at step 100), liquid volume
+    is conserved to 0.1 %, the column height falls and the front advances monotonically, the front has crossed x = 3 a by
+    T* = 3 at a speed between sqrt(g H) and Ritter's dam-break bound 2 sqrt(g H), and the liquid never moves faster than
+    free fall from the column top allows, sqrt(2 g H), by more than 15 %.  Both stage-3 solvers (plain cycles, PCG) must do it."""
+    import torch
+    n, levels = 32, 4
+    w = configs.config5(n, levels)
+    h, grav, sig, a, H = w.h, 9.81, 0.0728, 0.25, 0.5
+    s_hs = mg.mg_create((n, n, n, h), levels, BCP, mg.MG_F32)
+    s_nh = mg.mg_create((n, n, n, h), levels, BCP, mg.MG_F32)
+    for s in (s_hs, s_nh):
+        mg.mg_set_params(s, cycles_per_defect=0)
+    C = to_dev(w.fields["alpha"], "f32")
+    u, v, ww = (torch.zeros_like(C) for _ in range(3))
+    phs, pnh = torch.zeros_like(C), torch.zeros_like(C)
+    tstep = 0.1 * h / 3.0
+    vol0 = float(C.double().sum())
+    xs = (np.arange(n) + 0.5) * h
+    tstar = lambda t: t * np.sqrt(2 * grav / a)
+    fronts, heights, t = [], [], 0.0
+    while tstar(t) < 3.0:
+        status, cyc, rel = mg.flow_time_step_full_ex(s_hs, s_nh, C, u, v, ww, phs, pnh, w.rho_l, w.rho_g, w.mu_l, w.mu_g, grav, sig, tstep,
+                                                     1e-6, 100, 0.0, 20, (1, 1, 1, 1, 1, 0), pressure_solver)
+        t += tstep
+        assert status == mg.MG_OK and rel < 1e-6, (t, status, cyc, rel)
+        if len(fronts) % 10 == 0 or tstar(t) >= 3.0:
+            Cb, Cw = C[0, n // 2, :].cpu().numpy(), C[:, n // 2, 0].cpu().numpy()
+            wet, col = np.where(Cb > 0.5)[0], np.where(Cw > 0.5)[0]
+            assert wet.size and col.size
+            speed = torch.sqrt(u * u + v * v + ww * ww)
+            assert float((speed * (C > 0.5)).max()) <= 1.15 * np.sqrt(2 * grav * H)
+            fronts.append((tstar(t), xs[wet.max()])); heights.append(xs[col.max()])
+        else:
+            fronts.append(None)
+    fr = [f for f in fronts if f is not None]
+    assert all(np.isfinite(float(q.abs().max())) for q in (C, u, v, ww))
+    assert abs(float(C.double().sum()) / vol0 - 1) < 1e-3
+    assert float(C.min()) > -0.15 and float(C.max()) < 1.15
+    assert all(b[1] >= a_[1] - 1e-12 for a_, b in zip(fr, fr[1:])) and all(b <= a_ + 1e-12 for a_, b in zip(heights, heights[1:]))
+    assert fr[-1][1] > 3.0 * a and heights[-1] < 0.6 * H
+    # front speed over 1.2 <= T* <= 2.8 (after the initial acceleration, before the far wall)
+    mid = [f for f in fr if 1.2 <= f[0] <= 2.8]
+    vfront = (mid[-1][1] - mid[0][1]) / ((mid[-1][0] - mid[0][0]) / np.sqrt(2 * grav / a))
+    assert np.sqrt(grav * H) < vfront < 2 * np.sqrt(grav * H), vfront
+    mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)

@@ -8,6 +8,8 @@ import os
 import numpy as np
 import pytest
 
+from workloads import configs
+
 N, D = 0, 1
 HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -509,3 +511,64 @@ def test_curvature_of_a_sphere(orc):
     p_in = x[n // 2, n // 2, n // 2]
     p_out = x[n // 2, n // 2, 3]
     assert abs((p_in - p_out) - 2.0 / R) <= 0.1 * 2.0 / R
+
+
+# ---- reading C7 (revised): rho and mu from the volume fraction limited to [0, 1]; everything else sees C as it is ----------
+def _out_of_range_vof(shape, seed):
+    """a smooth interface with undershoots to -0.2 and overshoots to 1.25 on both sides of it"""
+    nz, ny, nx = shape
+    x, y, z = configs.centres(nx, ny, nz, 1.0)
+    d = (0.7 * x / nx + 0.4 * y / ny + 0.6 * z / nz) - 0.8
+    Cin = 0.5 * (1 + np.tanh(d * 5.0)) + 0.0 * (x + y + z)
+    return 1.45 * Cin - 0.2 + 0.02 * _rand(shape, seed)
+
+
+def test_material_mixtures_limit_the_volume_fraction(orc):
+    """Eqs. 2 / 19 with C limited to [0, 1]: closed-form values of k = 1 / rho; and every routine that sees C only through rho
+    and mu gives, for an out-of-range C, exactly what it gives for the limited field (dropping the limit anywhere breaks one
+    of the equalities; the inputs make rho NEGATIVE without it: 1000 * (-0.2) + 1.2)."""
+    rho_l, rho_g, mu_l, mu_g = 1000.0, 1.0, 1e-3, 1e-5
+    a = np.array([-0.2, -1e-3, 0.0, 0.3, 1.0, 1.4])
+    assert np.allclose(orc.k_from_vof(a, rho_l, rho_g), [1.0, 1.0, 1.0, 1.0 / (300.0 + 0.7), 1e-3, 1e-3], rtol=1e-15)
+    shape, h, dt = (10, 12, 14), 0.1, 0.01
+    g = orc.grid(shape[2], shape[1], shape[0], h)
+    C = _out_of_range_vof(shape, 7)
+    Cl = np.clip(C, 0.0, 1.0)
+    assert C.min() < -0.1 and C.max() > 1.1 and (rho_l * C + rho_g * (1 - C)).min() < 0
+    q = tuple(0.3 * _rand(shape, 20 + c) + 0.2 for c in range(3))
+    for vbc in (None, orc.velocity_bc()):
+        for r, rl in zip(orc.mom_predictor(g, C, q, q, rho_l, rho_g, mu_l, mu_g, dt, vbc), orc.mom_predictor(g, Cl, q, q, rho_l, rho_g, mu_l, mu_g, dt, vbc)):
+            for c in range(3):
+                assert np.array_equal(r[c], rl[c]) and np.isfinite(r[c]).all()
+    assert np.array_equal(orc.pressure_rhs_paper(g, C, q[0], q[1], q[2], rho_l, rho_g, dt), orc.pressure_rhs_paper(g, Cl, q[0], q[1], q[2], rho_l, rho_g, dt))
+    p_hs, p_nh = 1e3 * _rand(shape, 31), 1e3 * _rand(shape, 32)
+    st = tuple(1e3 * _rand(shape, 33 + c) for c in range(3))
+    pbc = (0, 1, 0, 0, 0, 1)
+    f, fl = (orc.mom_forcing(g, c_, p_hs, p_nh, pbc, 9.81, st, rho_l, rho_g, dt, q) for c_ in (C, Cl))
+    for c in range(3):
+        assert np.array_equal(f[c], fl[c])
+
+
+def test_only_the_mixtures_are_limited_not_the_interface_terms(orc):
+    """hydrostatic_rhs = gravity part (through rho: limited) + surface-tension part (through grad C and the curvature: NOT
+    limited).  sigma = 0: equal to the limited field's, bit for bit.  g = 0: C' = 1.45 C - 0.2 has the same normals and
+    curvature as C and 1.45 times its gradient, so b(C') = 1.45 b(C) (up to the epsilon of the normalisation) -- a limit on C in
+    the curvature or in grad C would flatten C' and break this by O(1)."""
+    n, h = 16, 1.0 / 16
+    g = orc.grid(n, n, n, h)
+    c = (np.arange(n) + 0.5) * h
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    r = np.sqrt((X - 0.5) ** 2 + (Y - 0.45) ** 2 + (Z - 0.55) ** 2)
+    C0 = 0.5 * (1 - np.tanh((r - 0.25) / (1.5 * h)))
+    C1 = 1.45 * C0 - 0.2
+    assert C1.min() < -0.19 and C1.max() > 1.2
+    b_g, _, _ = orc.hydrostatic_rhs(g, C1, 1000.0, 1.0, 9.81, 0.0)
+    b_gl, _, _ = orc.hydrostatic_rhs(g, np.clip(C1, 0, 1), 1000.0, 1.0, 9.81, 0.0)
+    assert np.array_equal(b_g, b_gl) and np.abs(b_g).max() > 0
+    b_s0, kap0, st0 = orc.hydrostatic_rhs(g, C0, 1000.0, 1.0, 0.0, 0.0728)
+    b_s1, kap1, st1 = orc.hydrostatic_rhs(g, C1, 1000.0, 1.0, 0.0, 0.0728)
+    band = np.abs(C0 - 0.5) < 0.4                                   # where the gradient is well above the normalisation's epsilon
+    assert np.abs(b_s0[band]).max() > 0
+    assert np.abs(b_s1 - 1.45 * b_s0)[band].max() < 2e-3 * np.abs(b_s0[band]).max()
+    b_cl, _, _ = orc.hydrostatic_rhs(g, np.clip(C1, 0, 1), 1000.0, 1.0, 0.0, 0.0728)
+    assert np.abs(b_cl - 1.45 * b_s0)[band].max() > 0.05 * np.abs(b_s0[band]).max()      # the limited field is a different problem
