@@ -15,7 +15,9 @@
 #include <initializer_list>
 #include <mutex>
 
+#include "fused.h"
 #include "solver.h"
+#include "lean_kernel.cuh"
 
 namespace mgb {
 namespace {
@@ -49,20 +51,26 @@ Geo<T> make_geo(const mg_grid* g, const int* bc) {
 
 // Eqs. 26/27: alpha_kabs = 1/16 (p = 1), eps_k = 1e-7; Eq. 27 on
 // uniform spacing, Eq. 26 otherwise (reading C9-ii).
+// a / b: fp32 by the approximate reciprocal (2 ulp; the true division costs ~12 instructions and a branch, and the coefficient
+// kernels, which are bound by instruction issue, do three per point), fp64 exactly
+__device__ __forceinline__ float fdiv(float a, float b) { return __fdividef(a, b); }
+__device__ __forceinline__ double fdiv(double a, double b) { return a / b; }
+
 template <typename T>
 __device__ __forceinline__ T k_abs_pg(const Geo<T>& G, T a, T px, T py, T pz) {
     const T alpha_kabs = T(1.0 / 16.0), eps_k = T(1e-7);
     const T ax = fabs(px), ay = fabs(py), az = fabs(pz);
     const T s = ax + ay + az;
     const T third = T(1.0 / 3.0);       // a multiplication, not a second division per point
-    if (G.uniform) return alpha_kabs * G.h[0] * fabs(a) / (eps_k + s * third);
-    return alpha_kabs * fabs(a) * (G.h[0] * ax + G.h[1] * ay + G.h[2] * az) / (eps_k + s * s * third);
+    if (G.uniform) return fdiv(alpha_kabs * G.h[0] * fabs(a), eps_k + s * third);
+    return fdiv(alpha_kabs * fabs(a) * (G.h[0] * ax + G.h[1] * ay + G.h[2] * az), eps_k + s * s * third);
 }
 
 template <typename T> __device__ __forceinline__ T tmin(T a, T b) { return a < b ? a : b; }
 template <typename T> __device__ __forceinline__ T tmax(T a, T b) { return a > b ? a : b; }
 
 #include "flow_march.cuh"
+#include "flow_tma.cuh"
 
 // W-wide kernels need nx % W == 0 and 16-byte aligned fields (vector loads); otherwise the W = 1 instantiation runs
 template <typename T> constexpr int vec_w() { return sizeof(T) == 4 ? 4 : 2; }
@@ -140,6 +148,19 @@ struct Scratch {  // stream-ordered scratch fields
     ~Scratch() { for (int q = 0; q < n; ++q) cudaFreeAsync(p[q], st); }
 };
 
+// ---- TMA-staged variants (flow_tma.cuh): fp32, vector path ------------------------------------------------------------
+inline bool tma_path() { static const bool off = getenv("MG_NO_FLOW_TMA") != nullptr; return !off; }
+// descriptors of `ns` stencil fields followed by `nc` centre fields
+inline int fill_maps(ft::Maps* M, const mg_grid* g, std::initializer_list<const float*> stencil, std::initializer_list<const float*> centre) {
+    int f = 0, rc;
+    for (const float* p : stencil) if ((rc = make_tmap_f32(&M->m[f++], p, g->nx, g->ny, g->nz, ft::PX, ft::PY))) return rc;
+    for (const float* p : centre) if ((rc = make_tmap_f32(&M->m[f++], p, g->nx, g->ny, g->nz, ft::TX, ft::TY))) return rc;
+    for (; f < ft::MAXF; ++f) M->m[f] = M->m[0];
+    return 0;
+}
+template <int NSF, int NCF, typename K>
+int setup_tma_kernel(K kernel) { return kernel_setup((const void*)kernel, ft::NT, ft::Ring<NSF, NCF>::SMEM, nullptr, true); }
+
 template <typename T>
 int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double dt, int detector, T* sC, T* Cnew, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
@@ -151,7 +172,31 @@ int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T
     const double hmax = fmax(g->hx, fmax(g->hy, g->hz)), hmin = fmin(g->hx, fmin(g->hy, g->hz));
     const double k_min = 1e-4 / dt * hmax * hmax, k_max = 0.05 / dt * hmin * hmin;   // Eq. 42
     const bool vec = can_vec<T>(g, {C, u, v, w, sC, Cnew});
-    MGB_MARCH(advection_march, vec, G, st, C, u, v, w, adv);
+    bool staged = false;
+    if constexpr (sizeof(T) == 4) {
+        if (vec && tma_path()) {
+            ft::Maps M;
+            if ((rc = fill_maps(&M, g, {(const float*)C}, {(const float*)u, (const float*)v, (const float*)w}))) return rc;
+            if ((rc = setup_tma_kernel<1, 3>(ft::advection_tma))) return rc;
+            ft::advection_tma<<<march_grid<float, 4>(G), dim3(MBX, MBY), ft::Ring<1, 3>::SMEM, st>>>(M, G, (float*)adv);
+            staged = true;
+        }
+    }
+    if (!staged) MGB_MARCH(advection_march, vec, G, st, C, u, v, w, adv);
+    if constexpr (sizeof(T) == 4) {
+        if (staged && detector != 5) {       // Eq. 33 detectors: coefficient and diffusion kernels staged by TMA as well
+            ft::Maps M;
+            if ((rc = fill_maps(&M, g, {(const float*)C, (const float*)adv}, {(const float*)u, (const float*)v, (const float*)w}))) return rc;
+            if ((rc = setup_tma_kernel<2, 3>(ft::vof_coeff_tma))) return rc;
+            ft::vof_coeff_tma<<<march_grid<float, 4>(G), dim3(MBX, MBY), ft::Ring<2, 3>::SMEM, st>>>(M, G, (float)k_min, (float)k_max, (float*)kx,
+                                                                                                  (float*)ky, (float*)kz);
+            if ((rc = fill_maps(&M, g, {(const float*)C, (const float*)kx, (const float*)ky, (const float*)kz}, {(const float*)adv}))) return rc;
+            if ((rc = setup_tma_kernel<4, 1>(ft::vof_diffusion_tma))) return rc;
+            ft::vof_diffusion_tma<<<march_grid<float, 4>(G), dim3(MBX, MBY), ft::Ring<4, 1>::SMEM, st>>>(M, G, (float)dt, (float*)sC, (float*)Cnew);
+            MGB_LAUNCH_CHECK();
+            return 0;
+        }
+    }
     // division-heavy: 4-wide packs cost more in registers than they save in loads (231 vs 248 us at 256^3)
     if (detector == 5) {       // Eq. 34 (vof_coeff_march<T, W, true>)
         if (vec) vof_coeff_march<T, 2, true><<<march_grid<T, 2>(G), dim3(MBX, MBY), 0, st>>>(G, C, u, v, w, adv, (T)k_min, (T)k_max, kx, ky, kz);

@@ -47,6 +47,12 @@ template <typename T, int W> __device__ __forceinline__ Pk<T, W> operator-(const
     for (int e = 0; e < W; ++e) r.v[e] = -a.v[e];
     return r;
 }
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pdiv(const Pk<T, W>& a, const Pk<T, W>& b) {      // fdiv lane by lane
+    Pk<T, W> r;
+#pragma unroll
+    for (int e = 0; e < W; ++e) r.v[e] = fdiv(a.v[e], b.v[e]);
+    return r;
+}
 template <typename T, int W> __device__ __forceinline__ Pk<T, W> splat(T a) {
     Pk<T, W> r;
 #pragma unroll
@@ -595,10 +601,10 @@ __global__ void __launch_bounds__(MBX* MBY) vof_coeff_march(const Geo<T> G, cons
             const size_t c0 = at(c, q);
             const V uu = ldv<T, W>(u + c0), vv = ldv<T, W>(v + c0), ww = ldv<T, W>(w + c0);
             const V g2 = Cx * Cx + Cy * Cy + Cz * Cz;
-            const V gq = (uu * Cx + vv * Cy + ww * Cz) / (eps_x + g2);           // step 7, Eq. 37
+            const V gq = pdiv(uu * Cx + vv * Cy + ww * Cz, eps_x + g2);           // step 7, Eq. 37
             const V us = gq * Cx, vs = gq * Cy, ws = gq * Cz;
-            const V kneg = -beta * (uu * uu + vv * vv + ww * ww) /               // step 8, Eq. 36
-                           (eps_x + g2 * (pabs(us) + pabs(vs) + pabs(ws)) * T(1.0 / 3.0));
+            const V kneg = pdiv(-beta * (uu * uu + vv * vv + ww * ww),           // step 8, Eq. 36
+                                eps_x + g2 * (pabs(us) + pabs(vs) + pabs(ws)) * T(1.0 / 3.0));
             T* const out[3] = {kx, ky, kz};
 #pragma unroll
             for (int d = 0; d < 3; ++d) {

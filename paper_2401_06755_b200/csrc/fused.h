@@ -15,4 +15,6 @@ bool fused_seed_supported(mg_solver* s);
 bool fused_residual_supported(mg_solver* s);   // the fine level is a streaming-kernel level
 int fused_residual(mg_solver* s, const float* x, const float* b, float* r, double* acc);   // r = b - A x, or A x if b == NULL; ||.||^2 added to *acc
 void fused_release(mg_solver* s);
+// TMA descriptor of a 3-D fp32 field, box = px x py cells of one z plane, out-of-bounds cells read as 0 (tm: CUtensorMap*)
+int make_tmap_f32(void* tm, const float* ptr, int nx, int ny, int nz, int px, int py);
 }  // namespace mgb

@@ -61,6 +61,11 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+}  // namespace
+// the same encoder for the explicit kernels (flow.cu, flow_tma.cuh); tm points to a CUtensorMap
+int make_tmap_f32(void* tm, const float* ptr, int nx, int ny, int nz, int px, int py) { return make_tmap((CUtensorMap*)tm, ptr, nx, ny, nz, px, py); }
+namespace {
+
 // ---- small helper kernels for levels below the tile size ------------------------------------
 __global__ void first_sweep_kernel(size_t n, const float* __restrict__ bc, const float* __restrict__ dinv, float g,
                                    float* __restrict__ xc) {
