@@ -158,8 +158,8 @@ inline int fill_maps(ft::Maps* M, const mg_grid* g, std::initializer_list<const 
     for (; f < ft::MAXF; ++f) M->m[f] = M->m[0];
     return 0;
 }
-template <int NSF, int NCF, typename K>
-int setup_tma_kernel(K kernel) { return kernel_setup((const void*)kernel, ft::NT, ft::Ring<NSF, NCF>::SMEM, nullptr, true); }
+template <int NSF, int NCF, int ND = ft::NS, typename K>
+int setup_tma_kernel(K kernel) { return kernel_setup((const void*)kernel, ft::NT, ft::Ring<NSF, NCF, ND>::SMEM, nullptr, true); }
 
 template <typename T>
 int vof_residual_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double dt, int detector, T* sC, T* Cnew, cudaStream_t st) {
@@ -227,6 +227,36 @@ int vof_residual_scratch_t(const mg_grid* g, const T* C, const T* u, const T* v,
     return 0;
 }
 
+// mom_predictor_t with the TMA-staged kernels (fp32 vector path): same launches, same arithmetic
+template <bool BC>
+int mom_predictor_tma_bc(const mg_grid* g, const Geo<float>& G, const float* C, const float* const qh[3], const float* const qn[3], const int* vbc,
+                         double rho_l, double rho_g, double mu_l, double mu_g, double dt, float* const qt[3], float* const qhn[3],
+                         float* const adv[3], float* kc, cudaStream_t st) {
+    int rc;
+    ft::Maps M;
+    const dim3 grid = march_grid<float, 4>(G), block(MBX, MBY);
+    Halo6<float> H[3] = {};
+    for (int c = 0; c < 3; ++c) H[c] = BC ? make_halo<float>(vbc + 6 * c) : Halo6<float>{};
+    if ((rc = fill_maps(&M, g, {qh[0], qh[1], qh[2]}, {}))) return rc;
+    if ((rc = setup_tma_kernel<3, 0>(ft::advection3_tma<BC>))) return rc;
+    ft::advection3_tma<BC><<<grid, block, ft::Ring<3, 0>::SMEM, st>>>(M, G, adv[0], adv[1], adv[2], H[0], H[1], H[2]);
+    if ((rc = setup_tma_kernel<2, 4, 3>(ft::mom_coeff_tma<BC>)) || (rc = setup_tma_kernel<2, 3, 3>(ft::mom_update_tma<BC>))) return rc;
+    for (int c = 0; c < 3; ++c) {
+        if ((rc = fill_maps(&M, g, {qh[c], adv[c]}, {C, qh[0], qh[1], qh[2]}))) return rc;
+        ft::mom_coeff_tma<BC><<<grid, block, ft::Ring<2, 4, 3>::SMEM, st>>>(M, G, (float)rho_l, (float)rho_g, (float)mu_l, (float)mu_g, kc, H[c]);
+        if ((rc = fill_maps(&M, g, {qh[c], kc}, {C, adv[c], qn[c]}))) return rc;
+        ft::mom_update_tma<BC><<<grid, block, ft::Ring<2, 3, 3>::SMEM, st>>>(M, G, (float)rho_l, (float)rho_g, (float)dt, qt[c], qhn ? qhn[c] : nullptr, H[c]);
+    }
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
+inline int mom_predictor_tma(const mg_grid* g, const Geo<float>& G, const float* C, const float* const qh[3], const float* const qn[3], const int* vbc,
+                             double rho_l, double rho_g, double mu_l, double mu_g, double dt, float* const qt[3], float* const qhn[3],
+                             float* const adv[3], float* kc, cudaStream_t st) {
+    return vbc ? mom_predictor_tma_bc<true>(g, G, C, qh, qn, vbc, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn, adv, kc, st)
+               : mom_predictor_tma_bc<false>(g, G, C, qh, qn, vbc, rho_l, rho_g, mu_l, mu_g, dt, qt, qhn, adv, kc, st);
+}
+
 template <typename T>
 int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T* const qn[3], const int* vbc, double rho_l, double rho_g,
                     double mu_l, double mu_g, double dt, T* const qt[3], T* const qhn[3], cudaStream_t st) {
@@ -238,6 +268,10 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
     T *adv[3] = {(T*)ws.p[0], (T*)ws.p[1], (T*)ws.p[2]}, *kc = (T*)ws.p[3];
     const bool vec = can_vec<T>(g, {C, qh[0], qh[1], qh[2], qn[0], qn[1], qn[2], qt[0], qt[1], qt[2], qhn ? qhn[0] : nullptr,
                                     qhn ? qhn[1] : nullptr, qhn ? qhn[2] : nullptr});
+    if constexpr (sizeof(T) == 4) {
+        if (vec && tma_path()) return mom_predictor_tma(g, G, (const float*)C, (const float* const*)qh, (const float* const*)qn, vbc, rho_l, rho_g,
+                                                        mu_l, mu_g, dt, (float* const*)qt, (float* const*)qhn, (float* const*)adv, (float*)kc, st);
+    }
     // the advection terms of all three components in one pass (each velocity field is read once), then coefficient and update per
     // component.  2-wide packs: three rolling gradients do not fit the registers of a 4-wide one.
     if (vbc) MGB_MARCH_BC_W(advection3_march, 2, vec, G, st, qh[0], qh[1], qh[2], adv[0], adv[1], adv[2], make_halo<T>(vbc),
@@ -257,9 +291,30 @@ int mom_predictor_t(const mg_grid* g, const T* C, const T* const qh[3], const T*
     return 0;
 }
 
+inline int pressure_rhs_tma_launch(const mg_grid* g, const Geo<float>& G, const float* u, const float* v, const float* w, const int* vbc,
+                                   float inv_dt, float* b, cudaStream_t st) {
+    int rc;
+    ft::Maps M;
+    if ((rc = fill_maps(&M, g, {u, v, w}, {}))) return rc;
+    const dim3 grid = march_grid<float, 4>(G), block(MBX, MBY);
+    if (vbc) {
+        if ((rc = setup_tma_kernel<3, 0>(ft::pressure_rhs_tma<true>))) return rc;
+        ft::pressure_rhs_tma<true><<<grid, block, ft::Ring<3, 0>::SMEM, st>>>(M, G, inv_dt, b, make_halo<float>(vbc), make_halo<float>(vbc + 6),
+                                                                                make_halo<float>(vbc + 12));
+    } else {
+        if ((rc = setup_tma_kernel<3, 0>(ft::pressure_rhs_tma<false>))) return rc;
+        ft::pressure_rhs_tma<false><<<grid, block, ft::Ring<3, 0>::SMEM, st>>>(M, G, inv_dt, b, Halo6<float>{}, Halo6<float>{}, Halo6<float>{});
+    }
+    MGB_LAUNCH_CHECK();
+    return 0;
+}
+
 template <typename T>
 int pressure_rhs_t(const mg_grid* g, const T* u, const T* v, const T* w, const int* vbc, double dt, T* b, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
+    if constexpr (sizeof(T) == 4) {
+        if (can_vec<T>(g, {u, v, w, b}) && tma_path()) return pressure_rhs_tma_launch(g, G, u, v, w, vbc, (float)(1.0 / dt), b, st);
+    }
     if (vbc) MGB_MARCH_BC(pressure_rhs_march, can_vec<T>(g, {u, v, w, b}), G, st, u, v, w, (T)(1.0 / dt), b, make_halo<T>(vbc),
                           make_halo<T>(vbc + 6), make_halo<T>(vbc + 12));
     else MGB_MARCH(pressure_rhs_march, can_vec<T>(g, {u, v, w, b}), G, st, u, v, w, (T)(1.0 / dt), b);
@@ -306,7 +361,11 @@ int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, 
     const bool vec = can_vec<T>(g, {C, b, kappa, force ? force[0] : nullptr, force ? force[1] : nullptr, force ? force[2] : nullptr});
     MGB_MARCH(normals_march, vec, G, st, C, n0, n1, n2);
     MGB_MARCH(surface_tension_march, vec, G, st, C, n0, n1, n2, (T)rho_l, (T)rho_g, (T)grav, (T)sigma_t, f0, f1, f2, kappa);
-    MGB_MARCH(pressure_rhs_march, vec, G, st, f0, f1, f2, T(-1), b);       // b = +(f(fu; w_x) + f(fv; w_y) + f(fw; w_z))
+    bool staged = false;
+    if constexpr (sizeof(T) == 4) {
+        if (vec && tma_path()) { if ((rc = pressure_rhs_tma_launch(g, G, f0, f1, f2, nullptr, -1.f, b, st))) return rc; staged = true; }
+    }
+    if (!staged) MGB_MARCH(pressure_rhs_march, vec, G, st, f0, f1, f2, T(-1), b);       // b = +(f(fu; w_x) + f(fv; w_y) + f(fw; w_z))
     bottom_fold_kernel<T><<<dim3((g->nx + 31) / 32, (g->ny + 7) / 8), dim3(32, 8), 0, st>>>(G, C, (T)rho_l, (T)rho_g, (T)grav, b);
     MGB_LAUNCH_CHECK();
     return 0;
@@ -315,6 +374,17 @@ int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, 
 template <typename T>
 int project_t(const mg_grid* g, const int* bc, const T* p, const T* k, double dt, T* u, T* v, T* w, cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, bc);
+    if constexpr (sizeof(T) == 4) {
+        if (can_vec<T>(g, {p, k, u, v, w}) && tma_path()) {
+            int rc;
+            ft::Maps M;
+            if ((rc = fill_maps(&M, g, {p}, {k, u, v, w}))) return rc;
+            if ((rc = setup_tma_kernel<1, 4>(ft::project_tma))) return rc;
+            ft::project_tma<<<march_grid<float, 4>(G), dim3(MBX, MBY), ft::Ring<1, 4>::SMEM, st>>>(M, G, (float)dt, u, v, w);
+            MGB_LAUNCH_CHECK();
+            return 0;
+        }
+    }
     MGB_MARCH(project_march, can_vec<T>(g, {p, k, u, v, w}), G, st, p, k, (T)dt, u, v, w);
     MGB_LAUNCH_CHECK();
     return 0;

@@ -18,16 +18,16 @@ constexpr int W = 4, TX = W * MBX, TY = MBY, NT = MBX * MBY;
 constexpr int PX = TX + 8, PY = TY + 2;
 constexpr int SPLANE = ((PX * PY + 31) / 32) * 32;        // floats per staged stencil plane
 constexpr int CPLANE = TX * TY;                            // floats per staged centre tile
-constexpr int NS = 4;                                      // ring depth
+constexpr int NS = 4;                                      // default ring depth (3 where the slots are large: blocks per SM matter more)
 constexpr int MAXF = 6;
 constexpr uint32_t SBYTES = PX * PY * 4, CBYTES = TX * TY * 4;
 
 struct alignas(64) Maps { CUtensorMap m[MAXF]; };          // stencil fields first, then centre fields
 
-template <int NSF, int NCF>
+template <int NSF, int NCF, int ND = NS>
 struct Ring {
     static constexpr int SLOT = NSF * SPLANE + NCF * CPLANE;
-    static constexpr size_t SMEM = (size_t)(32 + NS * SLOT) * sizeof(float);
+    static constexpr size_t SMEM = (size_t)(32 + ND * SLOT) * sizeof(float);
 };
 
 typedef Pk<float, W> V4;
@@ -76,16 +76,16 @@ __device__ __forceinline__ V4 ldc(uint32_t a, const View& vw) {
 
 // The staging pipeline of one block.  Iteration `it` (0 .. niter - 1) works on stencil plane z0 - 1 + it and finalises output
 // plane q = z0 - 2 + it, whose centre tiles arrive in the same slot.
-template <int NSF, int NCF>
+template <int NSF, int NCF, int ND = NS>
 struct Pipe {
-    typedef Ring<NSF, NCF> R;
+    typedef Ring<NSF, NCF, ND> R;
     uint64_t* bars; float* ring; uint32_t ring_a;
     const Maps* maps;
     int x0, y0, z0, nz, niter;
 
     __device__ __forceinline__ void issue(int it) const {            // one thread
-        uint64_t* bar = &bars[it % NS];
-        float* dst = ring + (it % NS) * R::SLOT;
+        uint64_t* bar = &bars[it % ND];
+        float* dst = ring + (it % ND) * R::SLOT;
         const int z = min(max(z0 - 1 + it, 0), nz - 1), q = z0 - 2 + it;
         const bool wc = NCF > 0 && it >= 2;                            // q lies in the chunk
         lk::mbar_expect_tx(bar, NSF * SBYTES + (wc ? NCF * CBYTES : 0u));
@@ -104,24 +104,24 @@ struct Pipe {
 #pragma unroll
             for (int f = 0; f < NSF + NCF; ++f) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&M.m[f])) : "memory");
 #pragma unroll
-            for (int s = 0; s < NS; ++s) lk::mbar_init(&bars[s], 1);
+            for (int s = 0; s < ND; ++s) lk::mbar_init(&bars[s], 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         }
         __syncthreads();
         if (threadIdx.x == 0 && threadIdx.y == 0)
-            for (int s = 0; s < NS && s < niter; ++s) issue(s);
+            for (int s = 0; s < ND && s < niter; ++s) issue(s);
     }
     // top of iteration `it`: hand the slot of iteration it - 1 back to TMA, wait for this iteration's planes;
     // returns the shared address of the slot
     __device__ __forceinline__ uint32_t acquire(int it) const {
         __syncthreads();
-        if (threadIdx.x == 0 && threadIdx.y == 0 && it >= 1 && it - 1 + NS < niter) {
+        if (threadIdx.x == 0 && threadIdx.y == 0 && it >= 1 && it - 1 + ND < niter) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            issue(it - 1 + NS);
+            issue(it - 1 + ND);
         }
-        lk::mbar_wait(&bars[it % NS], (uint32_t)((it / NS) & 1));
-        return ring_a + 4u * (uint32_t)((it % NS) * R::SLOT);
+        lk::mbar_wait(&bars[it % ND], (uint32_t)((it / ND) & 1));
+        return ring_a + 4u * (uint32_t)((it % ND) * R::SLOT);
     }
     __device__ __forceinline__ uint32_t sfield(uint32_t slot, int f) const { return slot + 4u * (uint32_t)(f * SPLANE); }
     __device__ __forceinline__ uint32_t cfield(uint32_t slot, int f) const { return slot + 4u * (uint32_t)(NSF * SPLANE + f * CPLANE); }
@@ -249,6 +249,188 @@ __global__ void __launch_bounds__(NT) vof_coeff_tma(const __grid_constant__ Maps
                 const V kk = wp * (Kcal * kabs) + wm * (kneg * ih[d]);
                 stv(out[d] + c0, pmax(-k_min, pmin(k_max, kk)));
             }
+        }
+    }
+}
+
+// The advection terms of the three momentum components in one pass (advection3_march)      (maps: u, v, w | -)
+template <bool BC>
+__global__ void __launch_bounds__(NT) advection3_tma(const __grid_constant__ Maps M, const Geo<float> G, float* __restrict__ au,
+                                                     float* __restrict__ av, float* __restrict__ aw, const Halo6<float> Hu,
+                                                     const Halo6<float> Hv, const Halo6<float> Hw) {
+    typedef V4 V;
+    Pipe<3, 0> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    HaloFac<float> hu = {}, hv = {}, hw = {};
+    if (BC) { hu = halo_fac(G, c, Hu); hv = halo_fac(G, c, Hv); hw = halo_fac(G, c, Hw); }
+    GradRoll<float, V> gu, gv, gw; gu.init(); gv.init(); gw.init();
+    V cu = {}, cv = {}, cw = {};
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        const int z = c.z0 - 1 + it;
+        V n9[3][3];
+        load9s(P.sfield(slot, 0), vw, n9);
+        if (BC) halo_scale(G, Hu, hu, z, n9);
+        gu.add(G, in_plane<float, true, false>(G, n9));
+        const V nu = n9[1][1];
+        load9s(P.sfield(slot, 1), vw, n9);
+        if (BC) halo_scale(G, Hv, hv, z, n9);
+        gv.add(G, in_plane<float, true, false>(G, n9));
+        const V nv = n9[1][1];
+        load9s(P.sfield(slot, 2), vw, n9);
+        if (BC) halo_scale(G, Hw, hw, z, n9);
+        gw.add(G, in_plane<float, true, false>(G, n9));
+        const V nw = n9[1][1];
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            const size_t c0 = at(c, q);
+            V gx, gy, gz;
+            gu.grad(G, gx, gy, gz); stv(au + c0, cu * gx + cv * gy + cw * gz);
+            gv.grad(G, gx, gy, gz); stv(av + c0, cu * gx + cv * gy + cw * gz);
+            gw.grad(G, gx, gy, gz); stv(aw + c0, cu * gx + cv * gy + cw * gz);
+        }
+        cu = nu; cv = nv; cw = nw;
+    }
+}
+
+// k_c = rho min{k_max, k_abs(c)} + mu (mom_coeff_march)      (maps: comp, adv | C, u, v, w)
+template <bool BC>
+__global__ void __launch_bounds__(NT) mom_coeff_tma(const __grid_constant__ Maps M, const Geo<float> G, float rho_l, float rho_g, float mu_l,
+                                                    float mu_g, float* __restrict__ kc, const Halo6<float> H) {
+    typedef V4 V;
+    typedef float T;
+    Pipe<2, 4, 3> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    HaloFac<T> hf = {};
+    if (BC) hf = halo_fac(G, c, H);
+    GradRoll<T, V> g; g.init();
+    ZAcc<V> am; am.init();
+    V a0 = {}, a0n = {};
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        const int z = c.z0 - 1 + it;
+        V n9[3][3];
+        load9s(P.sfield(slot, 0), vw, n9);
+        if (BC) halo_scale(G, H, hf, z, n9);
+        g.add(G, in_plane<T, true, false>(G, n9));
+        load9s(P.sfield(slot, 1), vw, n9);
+        const V madv = am.stepM(G, in_plane<T, false, false>(G, n9).mm);
+        a0 = a0n; a0n = n9[1][1];
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            V px, py, pz; g.grad(G, px, py, pz);
+            const V a = T(2) * (madv - a0);
+            const V Cc = ldc(P.cfield(slot, 0), vw);
+            const V rho = mix01(rho_l, rho_g, Cc);
+            const V mu = mix01(mu_l, mu_g, Cc);
+            const V kmax = G.h[0] * pabs(ldc(P.cfield(slot, 1), vw)) + G.h[1] * pabs(ldc(P.cfield(slot, 2), vw)) + G.h[2] * pabs(ldc(P.cfield(slot, 3), vw));
+            stv(kc + at(c, q), rho * pmin(kmax, k_abs_pk(G, a, px, py, pz)) + mu);
+        }
+    }
+}
+
+// s = rho adv + f^lap(c, k_c), q~ = q_n - dt s / rho, q_half' = (q_n + q~) / 2 (mom_update_march)      (maps: comp, k_c | C, adv, q_n)
+template <bool BC>
+__global__ void __launch_bounds__(NT) mom_update_tma(const __grid_constant__ Maps M, const Geo<float> G, float rho_l, float rho_g, float dt,
+                                                     float* __restrict__ qt, float* __restrict__ qhn, const Halo6<float> H) {
+    typedef V4 V;
+    typedef float T;
+    Pipe<2, 3, 3> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    HaloFac<T> hf = {};
+    if (BC) hf = halo_fac(G, c, H);
+    Diff3<V> L; L.init();
+    V x0 = {}, x0n = {}, k0 = {}, k0n = {};
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        const int z = c.z0 - 1 + it;
+        V nx9[3][3], nk9[3][3], nz9[3][3];
+        load9s(P.sfield(slot, 0), vw, nx9);
+        if (BC) halo_scale(G, H, hf, z, nx9);
+        load9s(P.sfield(slot, 1), vw, nk9);
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) nz9[b][a] = nk9[b][a] * nx9[b][a];
+        const InPlane<V> rx = in_plane<T, false, true>(G, nx9), rk = in_plane<T, false, true>(G, nk9), rz = in_plane<T, false, true>(G, nz9);
+        auto lap = [&](ZAcc<V>& a, const InPlane<V>& r) {
+            const V p1 = r.km + r.mk, t = G.M[0] * p1 + G.K[2][0] * r.mm;
+            return a.step(t, G.M[1] * p1 + G.K[2][1] * r.mm, t);
+        };
+        const V Lx = lap(L.f, rx), Lk = lap(L.k, rk), Lz = lap(L.z, rz);
+        x0 = x0n; x0n = nx9[1][1]; k0 = k0n; k0n = nk9[1][1];
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            const V diff = T(0.5) * (Lz + k0 * Lx - x0 * Lk);
+            const size_t c0 = at(c, q);
+            const V rho = mix01(rho_l, rho_g, ldc(P.cfield(slot, 0), vw));
+            const V sv = rho * ldc(P.cfield(slot, 1), vw) + diff;
+            const V qv = ldc(P.cfield(slot, 2), vw);
+            const V t = qv - dt * sv / rho;
+            stv(qt + c0, t);
+            if (qhn) stv(qhn + c0, T(0.5) * (qv + t));
+        }
+    }
+}
+
+// b = -(1/dt) (f(u; w_x) + f(v; w_y) + f(w; w_z)) (pressure_rhs_march)      (maps: u, v, w | -)
+template <bool BC>
+__global__ void __launch_bounds__(NT) pressure_rhs_tma(const __grid_constant__ Maps M, const Geo<float> G, float inv_dt, float* __restrict__ bout,
+                                                       const Halo6<float> Hu, const Halo6<float> Hv, const Halo6<float> Hw) {
+    typedef V4 V;
+    Pipe<3, 0> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    HaloFac<float> fu = {}, fv = {}, fw = {};
+    if (BC) { fu = halo_fac(G, c, Hu); fv = halo_fac(G, c, Hv); fw = halo_fac(G, c, Hw); }
+    ZAcc<V> acc; acc.init();
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        const int z = c.z0 - 1 + it;
+        V n9[3][3];
+        load9s(P.sfield(slot, 0), vw, n9); if (BC) halo_scale(G, Hu, fu, z, n9); const V du = in_plane<float, true, false>(G, n9).dm;
+        load9s(P.sfield(slot, 1), vw, n9); if (BC) halo_scale(G, Hv, fv, z, n9); const V dv = in_plane<float, true, false>(G, n9).md;
+        load9s(P.sfield(slot, 2), vw, n9); if (BC) halo_scale(G, Hw, fw, z, n9); const V mw = in_plane<float, false, false>(G, n9).mm;
+        const V ms = G.M[0] * (du + dv), dw = G.D[2][2] * mw;
+        const V div = acc.step(ms + dw, G.M[1] * (du + dv), ms - dw);
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) stv(bout + at(c, q), -div * inv_dt);
+    }
+}
+
+// q <- q - dt k f(p; w_x|y|z) (project_march); the pressure halo carries the solver's factors G.s      (maps: p | k, u, v, w)
+__global__ void __launch_bounds__(NT) project_tma(const __grid_constant__ Maps M, const Geo<float> G, float dt, float* __restrict__ u,
+                                                  float* __restrict__ v, float* __restrict__ w) {
+    typedef V4 V;
+    Pipe<1, 4> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    Halo6<float> H;
+#pragma unroll
+    for (int f = 0; f < 6; ++f) H.s[f] = G.s[f];
+    const HaloFac<float> hf = halo_fac(G, c, H);
+    GradRoll<float, V> g; g.init();
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        const int z = c.z0 - 1 + it;
+        V n9[3][3];
+        load9s(P.sfield(slot, 0), vw, n9);
+        halo_scale(G, H, hf, z, n9);
+        g.add(G, in_plane<float, true, false>(G, n9));
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const size_t c0 = at(c, q);
+            const V f = dt * ldc(P.cfield(slot, 0), vw);
+            stv(u + c0, ldc(P.cfield(slot, 1), vw) - f * gx); stv(v + c0, ldc(P.cfield(slot, 2), vw) - f * gy); stv(w + c0, ldc(P.cfield(slot, 3), vw) - f * gz);
         }
     }
 }
