@@ -298,12 +298,12 @@ inline int pressure_rhs_tma_launch(const mg_grid* g, const Geo<float>& G, const 
     if ((rc = fill_maps(&M, g, {u, v, w}, {}))) return rc;
     const dim3 grid = march_grid<float, 4>(G), block(MBX, MBY);
     if (vbc) {
-        if ((rc = setup_tma_kernel<3, 0>(ft::pressure_rhs_tma<true>))) return rc;
-        ft::pressure_rhs_tma<true><<<grid, block, ft::Ring<3, 0>::SMEM, st>>>(M, G, inv_dt, b, make_halo<float>(vbc), make_halo<float>(vbc + 6),
+        if ((rc = setup_tma_kernel<3, 0, 3>(ft::pressure_rhs_tma<true>))) return rc;
+        ft::pressure_rhs_tma<true><<<grid, block, ft::Ring<3, 0, 3>::SMEM, st>>>(M, G, inv_dt, b, make_halo<float>(vbc), make_halo<float>(vbc + 6),
                                                                                 make_halo<float>(vbc + 12));
     } else {
-        if ((rc = setup_tma_kernel<3, 0>(ft::pressure_rhs_tma<false>))) return rc;
-        ft::pressure_rhs_tma<false><<<grid, block, ft::Ring<3, 0>::SMEM, st>>>(M, G, inv_dt, b, Halo6<float>{}, Halo6<float>{}, Halo6<float>{});
+        if ((rc = setup_tma_kernel<3, 0, 3>(ft::pressure_rhs_tma<false>))) return rc;
+        ft::pressure_rhs_tma<false><<<grid, block, ft::Ring<3, 0, 3>::SMEM, st>>>(M, G, inv_dt, b, Halo6<float>{}, Halo6<float>{}, Halo6<float>{});
     }
     MGB_LAUNCH_CHECK();
     return 0;

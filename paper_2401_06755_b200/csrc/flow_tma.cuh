@@ -384,7 +384,7 @@ template <bool BC>
 __global__ void __launch_bounds__(NT) pressure_rhs_tma(const __grid_constant__ Maps M, const Geo<float> G, float inv_dt, float* __restrict__ bout,
                                                        const Halo6<float> Hu, const Halo6<float> Hv, const Halo6<float> Hw) {
     typedef V4 V;
-    Pipe<3, 0> P;
+    Pipe<3, 0, 3> P;
     const Col<float, W> c = make_col<float, W>(G);
     P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
     const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
