@@ -359,11 +359,24 @@ int hydrostatic_rhs_t(const mg_grid* g, const T* C, double rho_l, double rho_g, 
     T *n0 = (T*)ws.p[0], *n1 = (T*)ws.p[1], *n2 = (T*)ws.p[2];
     T *f0 = force ? force[0] : (T*)ws2.p[0], *f1 = force ? force[1] : (T*)ws2.p[1], *f2 = force ? force[2] : (T*)ws2.p[2];
     const bool vec = can_vec<T>(g, {C, b, kappa, force ? force[0] : nullptr, force ? force[1] : nullptr, force ? force[2] : nullptr});
-    MGB_MARCH(normals_march, vec, G, st, C, n0, n1, n2);
-    MGB_MARCH(surface_tension_march, vec, G, st, C, n0, n1, n2, (T)rho_l, (T)rho_g, (T)grav, (T)sigma_t, f0, f1, f2, kappa);
     bool staged = false;
     if constexpr (sizeof(T) == 4) {
-        if (vec && tma_path()) { if ((rc = pressure_rhs_tma_launch(g, G, f0, f1, f2, nullptr, -1.f, b, st))) return rc; staged = true; }
+        if (vec && tma_path()) {
+            ft::Maps M;
+            const dim3 grid = march_grid<float, 4>(G), block(MBX, MBY);
+            if ((rc = fill_maps(&M, g, {(const float*)C}, {})) || (rc = setup_tma_kernel<1, 0>(ft::normals_tma))) return rc;
+            ft::normals_tma<<<grid, block, ft::Ring<1, 0>::SMEM, st>>>(M, G, (float*)n0, (float*)n1, (float*)n2);
+            if ((rc = fill_maps(&M, g, {(const float*)C, (const float*)n0, (const float*)n1, (const float*)n2}, {})) ||
+                (rc = setup_tma_kernel<4, 0>(ft::surface_tension_tma))) return rc;
+            ft::surface_tension_tma<<<grid, block, ft::Ring<4, 0>::SMEM, st>>>(M, G, (float)rho_l, (float)rho_g, (float)grav, (float)sigma_t, (float*)f0,
+                                                                                (float*)f1, (float*)f2, (float*)kappa);
+            if ((rc = pressure_rhs_tma_launch(g, G, f0, f1, f2, nullptr, -1.f, b, st))) return rc;
+            staged = true;
+        }
+    }
+    if (!staged) {
+        MGB_MARCH(normals_march, vec, G, st, C, n0, n1, n2);
+        MGB_MARCH(surface_tension_march, vec, G, st, C, n0, n1, n2, (T)rho_l, (T)rho_g, (T)grav, (T)sigma_t, f0, f1, f2, kappa);
     }
     if (!staged) MGB_MARCH(pressure_rhs_march, vec, G, st, f0, f1, f2, T(-1), b);       // b = +(f(fu; w_x) + f(fv; w_y) + f(fw; w_z))
     bottom_fold_kernel<T><<<dim3((g->nx + 31) / 32, (g->ny + 7) / 8), dim3(32, 8), 0, st>>>(G, C, (T)rho_l, (T)rho_g, (T)grav, b);

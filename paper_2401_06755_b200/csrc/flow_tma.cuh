@@ -435,4 +435,65 @@ __global__ void __launch_bounds__(NT) project_tma(const __grid_constant__ Maps M
     }
 }
 
+// n_t = grad C / (eps_t + |grad C|) (normals_march)      (maps: C | -)
+__global__ void __launch_bounds__(NT) normals_tma(const __grid_constant__ Maps M, const Geo<float> G, float* __restrict__ nx_,
+                                                  float* __restrict__ ny_, float* __restrict__ nz_) {
+    typedef V4 V;
+    Pipe<1, 0> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    const float eps_t = 1e-7f / G.h[0];
+    GradRoll<float, V> g; g.init();
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        V n9[3][3];
+        load9s(P.sfield(slot, 0), vw, n9);
+        g.add(G, in_plane<float, true, false>(G, n9));
+        const int q = c.z0 - 2 + it;
+        if (q >= c.z0 && c.ok) {
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const V inv = 1.f / (eps_t + psqrt(gx * gx + gy * gy + gz * gz));
+            const size_t c0 = at(c, q);
+            stv(nx_ + c0, gx * inv); stv(ny_ + c0, gy * inv); stv(nz_ + c0, gz * inv);
+        }
+    }
+}
+
+// force field F = -(s + s_t) and the curvature (surface_tension_march)      (maps: C, n_x, n_y, n_z | -)
+__global__ void __launch_bounds__(NT) surface_tension_tma(const __grid_constant__ Maps M, const Geo<float> G, float rho_l, float rho_g,
+                                                          float grav, float sigma_t, float* __restrict__ fu, float* __restrict__ fv,
+                                                          float* __restrict__ fw, float* __restrict__ kappa) {
+    typedef V4 V;
+    Pipe<4, 0> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    GradRoll<float, V> g; g.init();
+    ZAcc<V> acc; acc.init();
+    V C0 = {}, C0n = {};
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        V n9[3][3];
+        load9s(P.sfield(slot, 0), vw, n9);
+        g.add(G, in_plane<float, true, false>(G, n9));
+        C0 = C0n; C0n = n9[1][1];
+        load9s(P.sfield(slot, 1), vw, n9); const V dx = in_plane<float, true, false>(G, n9).dm;
+        load9s(P.sfield(slot, 2), vw, n9); const V dy = in_plane<float, true, false>(G, n9).md;
+        load9s(P.sfield(slot, 3), vw, n9); const V mz = in_plane<float, false, false>(G, n9).mm;
+        const V ms = G.M[0] * (dx + dy), dn = G.D[2][2] * mz;
+        const V divn = acc.step(ms + dn, G.M[1] * (dx + dy), ms - dn);
+        const int q = c.z0 - 2 + it;
+        if (q >= c.z0 && c.ok) {
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const V kap = -divn;
+            const size_t c0 = at(c, q);
+            const V sk = -sigma_t * kap;
+            stv(fu + c0, sk * gx); stv(fv + c0, sk * gy);
+            stv(fw + c0, sk * gz + grav * mix01(rho_l, rho_g, C0));
+            if (kappa) stv(kappa + c0, kap);
+        }
+    }
+}
+
 }  // namespace ft

@@ -28,8 +28,11 @@ for si, shape in enumerate(shapes):
     b2 = torch.empty_like(C); mg.pressure_rhs_bc(u, v, w, vbc, h, dt, b2)
     pu, pv, pw = u.clone(), v.clone(), w.clone()
     mg.project_velocity(p, k, h, (0, 1, 0, 0, 2, 1), dt, pu, pv, pw)
+    bh, kap = torch.empty_like(C), torch.empty_like(C)
+    F = [torch.empty_like(C) for _ in range(3)]
+    mg.hydrostatic_rhs_force(C, h, 1000.0, 1.0, 9.81, 0.0728, bh, kap, F)
     torch.cuda.synchronize()
-    for name, t in [("sC", sC), ("Cn", Cn), ("b", b), ("b2", b2), ("pu", pu), ("pv", pv), ("pw", pw)] + [("qt%d" % c, qt[c]) for c in range(3)] + [("qh%d" % c, qh[c]) for c in range(3)] + [("qtb%d" % c, qt2[c]) for c in range(3)]:
+    for name, t in [("sC", sC), ("Cn", Cn), ("b", b), ("b2", b2), ("pu", pu), ("pv", pv), ("pw", pw)] + [("qt%d" % c, qt[c]) for c in range(3)] + [("qh%d" % c, qh[c]) for c in range(3)] + [("qtb%d" % c, qt2[c]) for c in range(3)] + [("bh", bh), ("kap", kap)] + [("F%d" % c, F[c]) for c in range(3)]:
         out["%d_%s" % (si, name)] = t.cpu().numpy()
 np.savez(sys.argv[1], **out)
 print("wrote", sys.argv[1], len(out), "arrays;", len(shapes), "shapes")
