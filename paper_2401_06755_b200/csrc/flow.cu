@@ -330,6 +330,21 @@ int mom_forcing_t(const mg_grid* g, const T* C, const T* phs, const T* pnh, cons
     const bool vec = can_vec<T>(g, {C, phs, pnh, F ? F[0] : nullptr, F ? F[1] : nullptr, F ? F[2] : nullptr, qt[0], qt[1], qt[2],
                                     qhn ? qn[0] : nullptr, qhn ? qn[1] : nullptr, qhn ? qn[2] : nullptr, qhn ? qhn[0] : nullptr,
                                     qhn ? qhn[1] : nullptr, qhn ? qhn[2] : nullptr});
+    if constexpr (sizeof(T) == 4) {
+        if (vec && tma_path() && phs && pnh && F) {          // the configuration of the four-stage step: every term present
+            const Geo<float> Gf = G;
+            ft::Maps M;
+            int rc;
+            if ((rc = fill_maps(&M, g, {(const float*)phs, (const float*)pnh, (const float*)F[0], (const float*)F[1], (const float*)F[2]}, {})) ||
+                (rc = setup_tma_kernel<5, 0, 3>(ft::mom_forcing_tma))) return rc;
+            ft::mom_forcing_tma<<<march_grid<float, 4>(Gf), dim3(MBX, MBY), ft::Ring<5, 0, 3>::SMEM, st>>>(
+                M, Gf, (const float*)C, (float)rho_l, (float)rho_g, (float)grav, (float)dt, (float*)qt[0], (float*)qt[1], (float*)qt[2],
+                qhn ? (const float*)qn[0] : nullptr, qhn ? (const float*)qn[1] : nullptr, qhn ? (const float*)qn[2] : nullptr,
+                qhn ? (float*)qhn[0] : nullptr, qhn ? (float*)qhn[1] : nullptr, qhn ? (float*)qhn[2] : nullptr);
+            MGB_LAUNCH_CHECK();
+            return 0;
+        }
+    }
     // five stencil fields: 2-wide packs keep the rolling sums in registers
     MGB_MARCH_W(mom_forcing_march, 2, vec, G, st, C, phs, pnh, F ? F[0] : (const T*)nullptr, F ? F[1] : (const T*)nullptr,
                 F ? F[2] : (const T*)nullptr, (T)rho_l, (T)rho_g, (T)grav, (T)dt, qt[0], qt[1], qt[2],

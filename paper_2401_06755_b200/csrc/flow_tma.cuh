@@ -496,4 +496,69 @@ __global__ void __launch_bounds__(NT) surface_tension_tma(const __grid_constant_
     }
 }
 
+// Forcing terms of Eq. 18 with both pressures and the force field present (mom_forcing_march)      (maps: p_hs, p_nh, F0, F1, F2 | -)
+// C, q~ and q_n are read at the centre only, by plain loads; the bottom ghost plane of p_hs (mirror + h_z g rho) needs the 3 x 3
+// neighbourhood of C in plane 0, read once by the blocks of the lowest chunk.
+__global__ void __launch_bounds__(NT) mom_forcing_tma(const __grid_constant__ Maps M, const Geo<float> G, const float* __restrict__ C, float rho_l,
+                                                      float rho_g, float grav, float dt, float* __restrict__ q0, float* __restrict__ q1,
+                                                      float* __restrict__ q2, const float* __restrict__ n0, const float* __restrict__ n1,
+                                                      const float* __restrict__ n2, float* __restrict__ h0, float* __restrict__ h1,
+                                                      float* __restrict__ h2) {
+    typedef V4 V;
+    typedef float T;
+    Pipe<5, 0, 3> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    Halo6<T> Hn, Hh;
+#pragma unroll
+    for (int f = 0; f < 6; ++f) { Hn.s[f] = G.s[f]; Hh.s[f] = T(1); }
+    Hh.s[5] = T(-1);
+    const HaloFac<T> fn = halo_fac(G, c, Hn), fh = halo_fac(G, c, Hh);
+    GradRoll<T, V> g; g.init();
+    ZAcc<V> m0, m1, m2; m0.init(); m1.init(); m2.init();
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        const int z = c.z0 - 1 + it;
+        V n9[3][3], t9[3][3];
+        load9s(P.sfield(slot, 0), vw, t9);
+        halo_scale(G, Hh, fh, z, t9);
+        if (z < 0) {
+            V c9[3][3];
+            load9(G, c, C, z, c9);
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) t9[b][a] = t9[b][a] + (G.h[2] * grav) * mix01(rho_l, rho_g, c9[b][a]);
+        }
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) n9[b][a] = V{} + t9[b][a];
+        load9s(P.sfield(slot, 1), vw, t9);
+        halo_scale(G, Hn, fn, z, t9);
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] + t9[b][a];
+        g.add(G, in_plane<T, true, false>(G, n9));
+        load9s(P.sfield(slot, 2), vw, t9); const V s0 = m0.stepM(G, in_plane<T, false, false>(G, t9).mm);
+        load9s(P.sfield(slot, 3), vw, t9); const V s1 = m1.stepM(G, in_plane<T, false, false>(G, t9).mm);
+        load9s(P.sfield(slot, 4), vw, t9); const V s2 = m2.stepM(G, in_plane<T, false, false>(G, t9).mm);
+        const int q = z - 1;
+        if (q >= c.z0 && c.ok) {
+            V gx, gy, gz; g.grad(G, gx, gy, gz);
+            const size_t c0 = at(c, q);
+            const V Cc = ldv<T, W>(C + c0);
+            const V f = dt / mix01(rho_l, rho_g, Cc);
+            const V u = ldv<T, W>(q0 + c0) - f * (gx + s0), v = ldv<T, W>(q1 + c0) - f * (gy + s1), w = ldv<T, W>(q2 + c0) - f * (gz + s2);
+            stv(q0 + c0, u); stv(q1 + c0, v); stv(q2 + c0, w);
+            if (h0) {
+                stv(h0 + c0, T(0.5) * (ldv<T, W>(n0 + c0) + u)); stv(h1 + c0, T(0.5) * (ldv<T, W>(n1 + c0) + v));
+                stv(h2 + c0, T(0.5) * (ldv<T, W>(n2 + c0) + w));
+            }
+        }
+    }
+}
+
 }  // namespace ft
