@@ -358,6 +358,17 @@ template <typename T>
 int pressure_rhs_paper_t(const mg_grid* g, const T* C, const T* u, const T* v, const T* w, double rho_l, double rho_g, double dt, T* b,
                          cudaStream_t st) {
     const Geo<T> G = make_geo<T>(g, nullptr);
+    if constexpr (sizeof(T) == 4) {
+        if (can_vec<T>(g, {C, u, v, w, b}) && tma_path()) {
+            ft::Maps M;
+            int rc;
+            if ((rc = fill_maps(&M, g, {C, u, v, w}, {})) || (rc = setup_tma_kernel<4, 0, 3>(ft::pressure_rhs_paper_tma))) return rc;
+            ft::pressure_rhs_paper_tma<<<march_grid<float, 4>(G), dim3(MBX, MBY), ft::Ring<4, 0, 3>::SMEM, st>>>(M, G, (float)rho_l, (float)rho_g,
+                                                                                                         (float)(1.0 / dt), b);
+            MGB_LAUNCH_CHECK();
+            return 0;
+        }
+    }
     MGB_MARCH(pressure_rhs_paper_march, can_vec<T>(g, {C, u, v, w, b}), G, st, C, u, v, w, (T)rho_l, (T)rho_g, (T)(1.0 / dt), b);
     MGB_LAUNCH_CHECK();
     return 0;

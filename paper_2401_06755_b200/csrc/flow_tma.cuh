@@ -561,4 +561,47 @@ __global__ void __launch_bounds__(NT) mom_forcing_tma(const __grid_constant__ Ma
     }
 }
 
+// the paper's stage-3 right-hand side, Eq. 53 (pressure_rhs_paper_march)      (maps: C, u, v, w | -)
+__global__ void __launch_bounds__(NT) pressure_rhs_paper_tma(const __grid_constant__ Maps M, const Geo<float> G, float rho_l, float rho_g,
+                                                             float inv_dt, float* __restrict__ bout) {
+    typedef V4 V;
+    typedef float T;
+    Pipe<4, 0, 3> P;
+    const Col<float, W> c = make_col<float, W>(G);
+    P.start(M, blockIdx.x, blockIdx.y, blockIdx.z, G.nz, c.z1);
+    const View vw = make_view(G, P.x0, P.y0, threadIdx.x, threadIdx.y);
+    ZAcc<V> acc; acc.init();
+    GradRoll<T, V> gr; gr.init();
+    V q0[3] = {}, q0n[3] = {};
+    for (int it = 0; it < P.niter; ++it) {
+        const uint32_t slot = P.acquire(it);
+        V r9[3][3], n9[3][3];
+        load9s(P.sfield(slot, 0), vw, r9);
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) r9[b][a] = mix01(rho_l, rho_g, r9[b][a]);
+        gr.add(G, in_plane<T, true, false>(G, r9));
+        V part[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            load9s(P.sfield(slot, 1 + d), vw, n9);
+            q0[d] = q0n[d]; q0n[d] = n9[1][1];
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) n9[b][a] = n9[b][a] * r9[b][a];
+            if (d == 2) part[d] = in_plane<T, false, false>(G, n9).mm;
+            else { const InPlane<V> r = in_plane<T, true, false>(G, n9); part[d] = d == 0 ? r.dm : r.md; }
+        }
+        const V ms = G.M[0] * (part[0] + part[1]), dw = G.D[2][2] * part[2];
+        const V div = acc.step(ms + dw, G.M[1] * (part[0] + part[1]), ms - dw);
+        const int q = c.z0 - 2 + it;
+        if (q >= c.z0 && c.ok) {
+            V gx, gy, gz; gr.grad(G, gx, gy, gz);
+            stv(bout + at(c, q), (-div + (q0[0] * gx + q0[1] * gy + q0[2] * gz)) * inv_dt);
+        }
+    }
+}
+
 }  // namespace ft

@@ -33,8 +33,9 @@ for si, shape in enumerate(shapes):
     mg.hydrostatic_rhs_force(C, h, 1000.0, 1.0, 9.81, 0.0728, bh, kap, F)
     fq = [u.clone(), v.clone(), w.clone()]; fh = [torch.empty_like(C) for _ in range(3)]
     mg.mom_forcing(C, p, bh * 0.01, (0, 1, 0, 0, 0, 1), h, 9.81, F, 1000.0, 1.0, dt, fq, (u, v, w), fh)
+    bp = torch.empty_like(C); mg.pressure_rhs_paper(C, u, v, w, h, 1000.0, 1.0, dt, bp)
     torch.cuda.synchronize()
-    for name, t in [("sC", sC), ("Cn", Cn), ("b", b), ("b2", b2), ("pu", pu), ("pv", pv), ("pw", pw)] + [("qt%d" % c, qt[c]) for c in range(3)] + [("qh%d" % c, qh[c]) for c in range(3)] + [("qtb%d" % c, qt2[c]) for c in range(3)] + [("bh", bh), ("kap", kap)] + [("F%d" % c, F[c]) for c in range(3)] + [("fq%d" % c, fq[c]) for c in range(3)] + [("fh%d" % c, fh[c]) for c in range(3)]:
+    for name, t in [("sC", sC), ("Cn", Cn), ("b", b), ("b2", b2), ("pu", pu), ("pv", pv), ("pw", pw)] + [("qt%d" % c, qt[c]) for c in range(3)] + [("qh%d" % c, qh[c]) for c in range(3)] + [("qtb%d" % c, qt2[c]) for c in range(3)] + [("bh", bh), ("kap", kap)] + [("F%d" % c, F[c]) for c in range(3)] + [("fq%d" % c, fq[c]) for c in range(3)] + [("fh%d" % c, fh[c]) for c in range(3)] + [("bp", bp)]:
         out["%d_%s" % (si, name)] = t.cpu().numpy()
 np.savez(sys.argv[1], **out)
 print("wrote", sys.argv[1], len(out), "arrays;", len(shapes), "shapes")

@@ -25,7 +25,7 @@ def test_staged_and_plain_load_kernels_agree_bit_for_bit(tmp_path):
         assert r.returncode == 0, r.stderr[-2000:]
         files.append(np.load(f))
     a, b = files
-    assert len(a.files) == len(b.files) == 36 * 27
+    assert len(a.files) == len(b.files) == 36 * 28
     for k in a.files:
         assert np.isfinite(a[k]).all(), k
         assert np.array_equal(a[k], b[k]), k
