@@ -41,6 +41,75 @@ MGB_PK_BIN(-)
 MGB_PK_BIN(*)
 MGB_PK_BIN(/)
 #undef MGB_PK_BIN
+// fp32 packs of even width: two lanes per instruction on the packed fp32 pipe of sm_100a (add / sub / mul .f32x2)
+typedef unsigned long long pk64;
+__device__ __forceinline__ pk64 pk_join(float lo, float hi) { pk64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void pk_split(pk64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ pk64 pk_add(pk64 a, pk64 b) { pk64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ pk64 pk_sub(pk64 a, pk64 b) { pk64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ pk64 pk_mul(pk64 a, pk64 b) { pk64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+#define MGB_PK_F32(OP, FN)                                                                                              \
+    template <int W> __device__ __forceinline__ Pk<float, W> operator OP(const Pk<float, W>& a, const Pk<float, W>& b) { \
+        Pk<float, W> r;                                                                                                 \
+        if constexpr (W % 2 == 0) {                                                                                     \
+            _Pragma("unroll") for (int e = 0; e < W; e += 2)                                                            \
+                pk_split(FN(pk_join(a.v[e], a.v[e + 1]), pk_join(b.v[e], b.v[e + 1])), r.v[e], r.v[e + 1]);             \
+        } else {                                                                                                        \
+            _Pragma("unroll") for (int e = 0; e < W; ++e) r.v[e] = a.v[e] OP b.v[e];                                    \
+        }                                                                                                               \
+        return r;                                                                                                       \
+    }                                                                                                                   \
+    template <int W> __device__ __forceinline__ Pk<float, W> operator OP(const Pk<float, W>& a, float b) {               \
+        Pk<float, W> r;                                                                                                 \
+        if constexpr (W % 2 == 0) {                                                                                     \
+            const pk64 bb = pk_join(b, b);                                                                              \
+            _Pragma("unroll") for (int e = 0; e < W; e += 2) pk_split(FN(pk_join(a.v[e], a.v[e + 1]), bb), r.v[e], r.v[e + 1]); \
+        } else {                                                                                                        \
+            _Pragma("unroll") for (int e = 0; e < W; ++e) r.v[e] = a.v[e] OP b;                                         \
+        }                                                                                                               \
+        return r;                                                                                                       \
+    }                                                                                                                   \
+    template <int W> __device__ __forceinline__ Pk<float, W> operator OP(float a, const Pk<float, W>& b) {               \
+        Pk<float, W> r;                                                                                                 \
+        if constexpr (W % 2 == 0) {                                                                                     \
+            const pk64 aa = pk_join(a, a);                                                                              \
+            _Pragma("unroll") for (int e = 0; e < W; e += 2) pk_split(FN(aa, pk_join(b.v[e], b.v[e + 1])), r.v[e], r.v[e + 1]); \
+        } else {                                                                                                        \
+            _Pragma("unroll") for (int e = 0; e < W; ++e) r.v[e] = a OP b.v[e];                                         \
+        }                                                                                                               \
+        return r;                                                                                                       \
+    }
+MGB_PK_F32(+, pk_add)
+MGB_PK_F32(-, pk_sub)
+MGB_PK_F32(*, pk_mul)
+#undef MGB_PK_F32
+__device__ __forceinline__ pk64 pk_fma(pk64 a, pk64 b, pk64 c) { pk64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+// s * a + b with one rounding (what contraction gives scalar code; the packed operators above are opaque to it)
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pfma(T s, const Pk<T, W>& a, const Pk<T, W>& b) {
+    Pk<T, W> r;
+    if constexpr (sizeof(T) == 4 && W % 2 == 0) {
+        const pk64 ss = pk_join(s, s);
+#pragma unroll
+        for (int e = 0; e < W; e += 2) pk_split(pk_fma(ss, pk_join(a.v[e], a.v[e + 1]), pk_join(b.v[e], b.v[e + 1])), r.v[e], r.v[e + 1]);
+    } else {
+#pragma unroll
+        for (int e = 0; e < W; ++e) r.v[e] = fma(s, a.v[e], b.v[e]);
+    }
+    return r;
+}
+template <typename T, int W> __device__ __forceinline__ Pk<T, W> pfma(const Pk<T, W>& s, const Pk<T, W>& a, const Pk<T, W>& b) {
+    Pk<T, W> r;
+    if constexpr (sizeof(T) == 4 && W % 2 == 0) {
+#pragma unroll
+        for (int e = 0; e < W; e += 2)
+            pk_split(pk_fma(pk_join(s.v[e], s.v[e + 1]), pk_join(a.v[e], a.v[e + 1]), pk_join(b.v[e], b.v[e + 1])), r.v[e], r.v[e + 1]);
+    } else {
+#pragma unroll
+        for (int e = 0; e < W; ++e) r.v[e] = fma(s.v[e], a.v[e], b.v[e]);
+    }
+    return r;
+}
+
 template <typename T, int W> __device__ __forceinline__ Pk<T, W> operator-(const Pk<T, W>& a) {
     Pk<T, W> r;
 #pragma unroll
@@ -207,16 +276,16 @@ __device__ __forceinline__ InPlane<V> in_plane(const Geo<T>& G, const V (&v)[3][
 #pragma unroll
     for (int b = 0; b < 3; ++b) {
         const V e = v[b][0] + v[b][2];
-        sm[b] = T(4) * v[b][1] + e;
+        sm[b] = pfma(T(4), v[b][1], e);
         if (NEED_D) sd[b] = v[b][2] - v[b][0];
-        if (NEED_K) sk[b] = e - T(2) * v[b][1];
+        if (NEED_K) sk[b] = pfma(T(-2), v[b][1], e);
     }
     InPlane<V> r;
     const V smo = sm[0] + sm[2];
-    r.mm = (m * m) * (T(4) * sm[1] + smo);
+    r.mm = (m * m) * pfma(T(4), sm[1], smo);
     r.dm = r.md = r.km = r.mk = V{};
-    if (NEED_D) { r.dm = (m * G.D[0][2]) * (T(4) * sd[1] + (sd[0] + sd[2])); r.md = (m * G.D[1][2]) * (sm[2] - sm[0]); }
-    if (NEED_K) { r.km = (m * G.K[0][0]) * (T(4) * sk[1] + (sk[0] + sk[2])); r.mk = (m * G.K[1][0]) * (smo - T(2) * sm[1]); }
+    if (NEED_D) { r.dm = (m * G.D[0][2]) * pfma(T(4), sd[1], sd[0] + sd[2]); r.md = (m * G.D[1][2]) * (sm[2] - sm[0]); }
+    if (NEED_K) { r.km = (m * G.K[0][0]) * pfma(T(4), sk[1], sk[0] + sk[2]); r.mk = (m * G.K[1][0]) * pfma(T(-2), sm[1], smo); }
     return r;
 }
 
@@ -228,8 +297,8 @@ struct ZAcc {
     V A, B;       // partial outputs of planes z - 1 and z before plane z has arrived
     __device__ __forceinline__ void init() { A = V{}; B = V{}; }
     __device__ __forceinline__ V step(const V& up, const V& mid, const V& dn) { const V done = A + up; A = B + mid; B = dn; return done; }
-    template <typename T> __device__ __forceinline__ V stepM(const Geo<T>& G, const V& v) { const V t = G.M[0] * v; const V done = A + t; A = T(4) * t + B; B = t; return done; }   // Mz = [1, 4, 1] / 6
-    template <typename T> __device__ __forceinline__ V stepK(const Geo<T>& G, const V& v) { const V t = G.K[2][0] * v; const V done = A + t; A = B - T(2) * t; B = t; return done; }   // Kz = [-1, 2, -1] / d^2
+    template <typename T> __device__ __forceinline__ V stepM(const Geo<T>& G, const V& v) { const V t = G.M[0] * v; const V done = A + t; A = pfma(T(4), t, B); B = t; return done; }   // Mz = [1, 4, 1] / 6
+    template <typename T> __device__ __forceinline__ V stepK(const Geo<T>& G, const V& v) { const V t = G.K[2][0] * v; const V done = A + t; A = pfma(T(-2), t, B); B = t; return done; }   // Kz = [-1, 2, -1] / d^2
     template <typename T> __device__ __forceinline__ V stepD(const Geo<T>& G, const V& v) { const V t = G.D[2][2] * v; const V done = A + t; A = B; B = -t; return done; }   // Dz
 };
 template <typename V> __device__ __forceinline__ void push(V (&a)[3], const V& v) { a[0] = a[1]; a[1] = a[2]; a[2] = v; }
