@@ -277,3 +277,20 @@ def test_collapsing_column_runs_and_behaves(mg, pressure_solver):
     vfront = (mid[-1][1] - mid[0][1]) / ((mid[-1][0] - mid[0][0]) / np.sqrt(2 * grav / a))
     assert np.sqrt(grav * H) < vfront < 2 * np.sqrt(grav * H), vfront
     mg.mg_destroy(s_hs); mg.mg_destroy(s_nh)
+
+
+def test_full_step_argument_errors(mg):
+    import torch
+    n = 16
+    s_hs = mg.mg_create((n, n, n, 1.0 / n), 2, BCP, mg.MG_F32)
+    s_nh = mg.mg_create((n, n, n, 1.0 / n), 2, BCP, mg.MG_F32)
+    f = [torch.zeros(n, n, n, device="cuda") for _ in range(6)]
+    with pytest.raises(mg.MgError) as e:
+        mg.flow_time_step_full_ex(s_hs, s_nh, *f, 1000.0, 1.0, 1e-3, 1e-5, 9.81, 0.07, 1e-3, 1e-6, 10, 0.0, 5, (1, 1, 1, 1, 1, 0), 2)
+    assert e.value.code == mg.MG_EINVAL and "pressure_solver" in str(e.value)
+    s_other = mg.mg_create((2 * n, n, n, 1.0 / n), 2, BCP, mg.MG_F32)
+    with pytest.raises(mg.MgError) as e:
+        mg.flow_time_step_full(s_other, s_nh, *f, 1000.0, 1.0, 1e-3, 1e-5, 9.81, 0.07, 1e-3, 1e-6, 10, 0.0, 5)
+    assert e.value.code == mg.MG_EINVAL
+    for s in (s_hs, s_nh, s_other):
+        mg.mg_destroy(s)
